@@ -1,0 +1,334 @@
+/*
+ * blink_oracle.c -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * Plain, slow, obviously-correct CPU statement of what libblinkimg computes: nearest-cell
+ * gridding of visibilities (+ Hermitian conjugates) and the centred inverse 2D DFT that turns a
+ * grid into a dirty image (eq. 5, L190-194 section 6.2.4).  Only tests/,
+ * __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may call it.
+ * It shares no code, header, table or constant generator with paper_2505_15204_b200/csrc.
+ *
+ * Precision: visibilities and uvw arrive as float32 ("32 bit floating point");
+ * the CELL INDEX is decided in float32 exactly as DESIGN.md reading R2 states (one fp32 multiply,
+ * round-to-nearest-even) because floating point decides an integer there; everything else
+ * (accumulation, DFT) is float64.
+ *
+ * Pins (tests/test_oracle_pins.py, all run without a GPU):
+ *   oracle_scale / oracle_cell    : exact on-grid inputs, mirror invariant r+r'=N, brute-force
+ *                                   float64 evaluation away from half-cell boundaries
+ *   oracle_grid_one               : W = 2*B_in = sum(cnt); sum(G) = sum 2 Re V; Hermitian grid;
+ *                                   3-antenna hand case
+ *   oracle_idft2_direct           : single-cell closed form cos(2 pi (ku x + kv y)/N + arg V)
+ *   oracle_ifft2_radix2           : == oracle_idft2_direct on 32x32 (north_star check 4),
+ *                                   == numpy.fft.ifft2 with shifts, Parseval, linearity
+ *   oracle_sparse_image           : == radix-2 image on a full-size image
+ *   oracle_image_one              : unit source at phase centre -> 1.0 at [h][h]; on-grid offset
+ *                                   source peaks at its pixel with value 1.0; |Im| < 1e-6 peak
+ * Nothing here is "parity unpinned".
+ *
+ * Build: gcc -O2 -ffp-contract=off -fPIC -shared -pthread -o liboracle.so blink_oracle.c -lm
+ */
+#include <math.h>
+#include <fenv.h>
+#include <pthread.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+#define ORACLE_C0 299792458.0
+#define ORACLE_PI 3.14159265358979323846264338327950288
+
+/* ------------------------------------------------------------------------------------------
+ * a0. cells per metre for channel frequency f (reading R3):
+ *     u in wavelengths is u_m f / c, the uv cell is 1/(N pixscale) wavelengths,
+ *     so cells = u_m * f * N * pixscale / c.  Evaluated left to right in double, rounded ONCE
+ *     to float.
+ * ---------------------------------------------------------------------------------------- */
+float oracle_scale(double f_hz, int n_pix, double pixscale_rad)
+{
+    double s = f_hz * (double)n_pix;
+    s = s * pixscale_rad;
+    s = s / ORACLE_C0;
+    return (float)s;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * a1. nearest cell of one baseline ("placed ... based on the (u, v) coordinates";
+ *     readings R2 (round half to even), R4 (drop when |iu| or |iv| > h-1), w ignored (L114)).
+ *     Returns the centred linear cell (iv+h)*N + (iu+h), or -1 when dropped.
+ * ---------------------------------------------------------------------------------------- */
+int32_t oracle_cell(float u_m, float v_m, float s, int n_pix)
+{
+    const int h = n_pix / 2;
+    volatile float x = u_m * s;            /* one IEEE fp32 multiply, no contraction */
+    volatile float y = v_m * s;
+    float xr = nearbyintf(x);              /* FE_TONEAREST: ties to even */
+    float yr = nearbyintf(y);
+    const float lim = (float)(h - 1);
+    if (!(fabsf(xr) <= lim && fabsf(yr) <= lim)) return -1;    /* NaN fails -> dropped */
+    int iu = (int)xr, iv = (int)yr;
+    return (int32_t)((iv + h) * n_pix + (iu + h));
+}
+
+/* cell of the Hermitian conjugate sample at (-u,-v): (h-iv)*N + (h-iu)  (reading R1) */
+static int32_t mirror_cell(int32_t cell, int n_pix)
+{
+    const int h = n_pix / 2;
+    int r = cell / n_pix, q = cell % n_pix;
+    int iv = r - h, iu = q - h;
+    return (int32_t)((h - iv) * n_pix + (h - iu));
+}
+int32_t oracle_mirror_cell(int32_t cell, int n_pix) { return mirror_cell(cell, n_pix); }
+
+/* all (t, c, b) indices of a batch: cell_idx[T][C][B] */
+void oracle_cells(const float *uvw_m, const double *freqs_hz, int T, int C, int B,
+                  int n_pix, double pixscale_rad, int32_t *cell_idx)
+{
+    fesetround(FE_TONEAREST);
+    for (int t = 0; t < T; ++t)
+        for (int c = 0; c < C; ++c) {
+            float s = oracle_scale(freqs_hz[c], n_pix, pixscale_rad);
+            for (int b = 0; b < B; ++b) {
+                const float *p = uvw_m + ((size_t)t * B + b) * 3;
+                cell_idx[((size_t)t * C + c) * B + b] = oracle_cell(p[0], p[1], s, n_pix);
+            }
+        }
+}
+
+/* ------------------------------------------------------------------------------------------
+ * a2 + a3. grid ONE image (natural weighting is the paper's default,
+ *     uniform weighting is BASELINE.json's, reading R9).
+ *   vis      [B] complex64 as float pairs, uvw_t [B][3] metres
+ *   grid     [N][N] complex128 as double pairs, centred (DC at [h][h]); zeroed here
+ *   cnt      [N][N] samples per cell (vis + conjugates); zeroed here
+ *   cell_idx [B] (may be NULL)
+ *   returns W: natural = sum(cnt) = 2 B_in ; uniform = number of occupied cells
+ * ---------------------------------------------------------------------------------------- */
+double oracle_grid_one(const float *vis, const float *uvw_t, double f_hz, int B, int n_pix,
+                       double pixscale_rad, int weighting, double *grid, uint32_t *cnt,
+                       int32_t *cell_idx)
+{
+    const size_t n2 = (size_t)n_pix * n_pix;
+    fesetround(FE_TONEAREST);
+    memset(grid, 0, n2 * 2 * sizeof(double));
+    memset(cnt, 0, n2 * sizeof(uint32_t));
+    float s = oracle_scale(f_hz, n_pix, pixscale_rad);
+    for (int b = 0; b < B; ++b) {                                  /* baseline order */
+        int32_t cell = oracle_cell(uvw_t[3 * b], uvw_t[3 * b + 1], s, n_pix);
+        if (cell_idx) cell_idx[b] = cell;
+        if (cell < 0) continue;
+        int32_t cellc = mirror_cell(cell, n_pix);
+        double re = (double)vis[2 * b], im = (double)vis[2 * b + 1];
+        grid[2 * (size_t)cell] += re;   grid[2 * (size_t)cell + 1] += im;      /* G[cell]  += V       */
+        grid[2 * (size_t)cellc] += re;  grid[2 * (size_t)cellc + 1] -= im;     /* G[cell'] += conj(V) */
+        cnt[cell] += 1;  cnt[cellc] += 1;
+    }
+    double W = 0.0;
+    if (weighting == 0) {
+        for (size_t k = 0; k < n2; ++k) W += (double)cnt[k];
+    } else {
+        for (size_t k = 0; k < n2; ++k)
+            if (cnt[k] > 0) {
+                grid[2 * k] /= (double)cnt[k];
+                grid[2 * k + 1] /= (double)cnt[k];
+                W += 1.0;
+            }
+    }
+    return W;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * a4 + a5, THE DEFINITION (sign + because eq. 4 L104 has e^{-i2pi(ul+vm)} in V;
+ * unnormalised; centred on both sides, reading R7: DC cell [h][h] <-> phase-centre pixel [h][h]):
+ *     out[y][x] = sum_{r,q} G[r][q] exp(+2 pi i ((q-h)(x-h) + (r-h)(y-h)) / N)
+ * O(N^4): for N <= 64 only.  out is complex [N][N] as double pairs.
+ * ---------------------------------------------------------------------------------------- */
+void oracle_idft2_direct(const double *grid, int n, double *out)
+{
+    const int h = n / 2;
+    for (int y = 0; y < n; ++y)
+        for (int x = 0; x < n; ++x) {
+            double sr = 0.0, si = 0.0;
+            for (int r = 0; r < n; ++r)
+                for (int q = 0; q < n; ++q) {
+                    double gr = grid[2 * ((size_t)r * n + q)], gi = grid[2 * ((size_t)r * n + q) + 1];
+                    if (gr == 0.0 && gi == 0.0) continue;
+                    /* reduce the integer phase mod N before the trig call: exact */
+                    long long k = (long long)(q - h) * (x - h) + (long long)(r - h) * (y - h);
+                    k %= n; if (k < 0) k += n;
+                    double a = 2.0 * ORACLE_PI * (double)k / (double)n;
+                    double cr = cos(a), ci = sin(a);
+                    sr += gr * cr - gi * ci;
+                    si += gr * ci + gi * cr;
+                }
+            out[2 * ((size_t)y * n + x)] = sr;
+            out[2 * ((size_t)y * n + x) + 1] = si;
+        }
+}
+
+/* same definition, looping over OCCUPIED cells only and over all pixels: O(nnz N^2).
+ * img[y][x] = (1/W) Re(...), imag part optionally to img_im. */
+void oracle_sparse_image(const double *grid, int n, double W, double *img, double *img_im)
+{
+    const int h = n / 2;
+    const size_t n2 = (size_t)n * n;
+    /* table of the N distinct phases, exact argument reduction by integer arithmetic */
+    double *ct = (double *)malloc(sizeof(double) * n), *st = (double *)malloc(sizeof(double) * n);
+    for (int k = 0; k < n; ++k) { ct[k] = cos(2.0 * ORACLE_PI * k / n); st[k] = sin(2.0 * ORACLE_PI * k / n); }
+    for (size_t p = 0; p < n2; ++p) { img[p] = 0.0; if (img_im) img_im[p] = 0.0; }
+    for (int r = 0; r < n; ++r)
+        for (int q = 0; q < n; ++q) {
+            double gr = grid[2 * ((size_t)r * n + q)], gi = grid[2 * ((size_t)r * n + q) + 1];
+            if (gr == 0.0 && gi == 0.0) continue;
+            for (int y = 0; y < n; ++y)
+                for (int x = 0; x < n; ++x) {
+                    long long k = (long long)(q - h) * (x - h) + (long long)(r - h) * (y - h);
+                    k %= n; if (k < 0) k += n;
+                    img[(size_t)y * n + x] += gr * ct[k] - gi * st[k];
+                    if (img_im) img_im[(size_t)y * n + x] += gr * st[k] + gi * ct[k];
+                }
+        }
+    double inv = (W > 0.0) ? 1.0 / W : 0.0;
+    for (size_t p = 0; p < n2; ++p) { img[p] *= inv; if (img_im) img_im[p] *= inv; }
+    free(ct); free(st);
+}
+
+/* ------------------------------------------------------------------------------------------
+ * The FAST route to the same numbers: textbook iterative radix-2 decimation-in-time FFT
+ * (bit reversal, log2 n butterfly levels), sign +, unnormalised, in double; applied to rows
+ * then columns.  The centring is done by index arithmetic exactly as the definition reads:
+ * frequency index k = (q - h) mod N on input, pixel x = (j + h) mod N on output, where the
+ * plain transform is X[j] = sum_k x[k] e^{+2 pi i j k / N}.
+ * ---------------------------------------------------------------------------------------- */
+static void fft1d_radix2_inverse(double *re, double *im, int n)
+{
+    /* bit-reversal permutation */
+    for (int i = 1, j = 0; i < n; ++i) {
+        int bit = n >> 1;
+        for (; j & bit; bit >>= 1) j ^= bit;
+        j ^= bit;
+        if (i < j) { double t = re[i]; re[i] = re[j]; re[j] = t; t = im[i]; im[i] = im[j]; im[j] = t; }
+    }
+    for (int len = 2; len <= n; len <<= 1) {
+        int half = len >> 1;
+        for (int i = 0; i < n; i += len)
+            for (int k = 0; k < half; ++k) {
+                double a = 2.0 * ORACLE_PI * (double)k / (double)len;     /* + sign: inverse */
+                double wr = cos(a), wi = sin(a);
+                double xr = re[i + k + half] * wr - im[i + k + half] * wi;
+                double xi = re[i + k + half] * wi + im[i + k + half] * wr;
+                re[i + k + half] = re[i + k] - xr;  im[i + k + half] = im[i + k] - xi;
+                re[i + k] += xr;                    im[i + k] += xi;
+            }
+    }
+}
+
+/* out[y][x] (complex, double pairs) = centred unnormalised inverse 2D DFT of grid[r][q] */
+void oracle_ifft2_radix2(const double *grid, int n, double *out)
+{
+    const int h = n / 2;
+    double *re = (double *)malloc(sizeof(double) * n), *im = (double *)malloc(sizeof(double) * n);
+    double *tmp = (double *)malloc(sizeof(double) * 2 * (size_t)n * n);
+    /* rows: u -> x */
+    for (int r = 0; r < n; ++r) {
+        for (int q = 0; q < n; ++q) {
+            int k = ((q - h) % n + n) % n;
+            re[k] = grid[2 * ((size_t)r * n + q)];
+            im[k] = grid[2 * ((size_t)r * n + q) + 1];
+        }
+        fft1d_radix2_inverse(re, im, n);
+        for (int j = 0; j < n; ++j) {
+            int x = (j + h) % n;
+            tmp[2 * ((size_t)r * n + x)] = re[j];
+            tmp[2 * ((size_t)r * n + x) + 1] = im[j];
+        }
+    }
+    /* columns: v -> y */
+    for (int x = 0; x < n; ++x) {
+        for (int r = 0; r < n; ++r) {
+            int k = ((r - h) % n + n) % n;
+            re[k] = tmp[2 * ((size_t)r * n + x)];
+            im[k] = tmp[2 * ((size_t)r * n + x) + 1];
+        }
+        fft1d_radix2_inverse(re, im, n);
+        for (int j = 0; j < n; ++j) {
+            int y = (j + h) % n;
+            out[2 * ((size_t)y * n + x)] = re[j];
+            out[2 * ((size_t)y * n + x) + 1] = im[j];
+        }
+    }
+    free(re); free(im); free(tmp);
+}
+
+/* ------------------------------------------------------------------------------------------
+ * One dirty image, start to end (a0..a5): grid, weight, transform, divide by W, real part.
+ *   image [N][N] double; image_im (may be NULL) the imaginary part, also / W
+ *   grid_out (may be NULL) [N][N] complex128; cnt_out (may be NULL); cell_idx (may be NULL)
+ *   returns W.  W == 0 -> all-zero image.
+ * ---------------------------------------------------------------------------------------- */
+double oracle_image_one(const float *vis, const float *uvw_t, double f_hz, int B, int n_pix,
+                        double pixscale_rad, int weighting, double *image, double *image_im,
+                        double *grid_out, uint32_t *cnt_out, int32_t *cell_idx)
+{
+    const size_t n2 = (size_t)n_pix * n_pix;
+    double *grid = grid_out ? grid_out : (double *)malloc(sizeof(double) * 2 * n2);
+    uint32_t *cnt = cnt_out ? cnt_out : (uint32_t *)malloc(sizeof(uint32_t) * n2);
+    double *cimg = (double *)malloc(sizeof(double) * 2 * n2);
+    double W = oracle_grid_one(vis, uvw_t, f_hz, B, n_pix, pixscale_rad, weighting, grid, cnt, cell_idx);
+    oracle_ifft2_radix2(grid, n_pix, cimg);
+    double inv = (W > 0.0) ? 1.0 / W : 0.0;
+    for (size_t p = 0; p < n2; ++p) {
+        image[p] = cimg[2 * p] * inv;
+        if (image_im) image_im[p] = cimg[2 * p + 1] * inv;
+    }
+    free(cimg);
+    if (!grid_out) free(grid);
+    if (!cnt_out) free(cnt);
+    return W;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * Batch driver: images img_ids[0..n_ids) of a [T][C][P][B] visibility set, one image per task,
+ * nthreads POSIX threads.  images [n_ids][N][N] double, wsum [n_ids] double.
+ * Image index i = (t*C + c)*P + p.
+ * ---------------------------------------------------------------------------------------- */
+typedef struct {
+    const float *vis, *uvw_m; const double *freqs_hz;
+    int T, C, P, B, n_pix, weighting; double pixscale_rad;
+    const int64_t *img_ids; int n_ids; double *images; double *wsum;
+    int tid, nthreads;
+} batch_job_t;
+
+static void *batch_worker(void *arg)
+{
+    batch_job_t *j = (batch_job_t *)arg;
+    const size_t n2 = (size_t)j->n_pix * j->n_pix;
+    for (int k = j->tid; k < j->n_ids; k += j->nthreads) {
+        int64_t i = j->img_ids[k];
+        int p = (int)(i % j->P);
+        int c = (int)((i / j->P) % j->C);
+        int t = (int)(i / ((int64_t)j->P * j->C));
+        const float *v = j->vis + 2 * ((((size_t)t * j->C + c) * j->P + p) * (size_t)j->B);
+        const float *uvw = j->uvw_m + (size_t)t * j->B * 3;
+        j->wsum[k] = oracle_image_one(v, uvw, j->freqs_hz[c], j->B, j->n_pix, j->pixscale_rad,
+                                      j->weighting, j->images + (size_t)k * n2, NULL, NULL, NULL, NULL);
+    }
+    return NULL;
+}
+
+int oracle_image_batch(const float *vis, const float *uvw_m, const double *freqs_hz,
+                       int T, int C, int P, int B, int n_pix, double pixscale_rad, int weighting,
+                       const int64_t *img_ids, int n_ids, double *images, double *wsum, int nthreads)
+{
+    if (nthreads < 1) nthreads = 1;
+    if (nthreads > 256) nthreads = 256;
+    pthread_t th[256];
+    batch_job_t jobs[256];
+    for (int k = 0; k < nthreads; ++k) {
+        batch_job_t jb = { vis, uvw_m, freqs_hz, T, C, P, B, n_pix, weighting, pixscale_rad,
+                           img_ids, n_ids, images, wsum, k, nthreads };
+        jobs[k] = jb;
+        if (pthread_create(&th[k], NULL, batch_worker, &jobs[k]) != 0) return -1;
+    }
+    for (int k = 0; k < nthreads; ++k) pthread_join(th[k], NULL);
+    return 0;
+}
