@@ -1,0 +1,136 @@
+/*
+ * blinkimg.h -- C ABI of libblinkimg: batched dirty imaging on one NVIDIA B200 (sm_100a).
+ *
+ * The hot path of the BLINK high-time-resolution imager (arXiv 2505.15204; PAPER.md in the
+ * reference folder): for every (timestep t, fine channel c, polarisation p)
+ *   a0  cells per metre  s_c = float(f_c * N * pixscale / c0)          (u in wavelengths;
+ *                                                                       DESIGN.md reading R3)
+ *   a1  nearest uv cell  iu = rint(u_m * s_c), iv = rint(v_m * s_c)     ("placed ... based on
+ *                                                                       the (u,v) coordinates"; R2, R4)
+ *   a2  accumulate       G[cell] += V, G[cell'] += conj(V)              (no gridding
+ *                                                                       kernel; conjugate at (-u,-v): R1)
+ *   a3  weighting        natural (default) or uniform (BASELINE.json; R9), weight sum W
+ *   a4  inverse FFT along u (rows)      \  PAPER.md L108-110 eq. 5: "2D inverse FFT",
+ *   a5  inverse FFT along v (columns)   /  batched over all grids; sign +, unnormalised (R5)
+ *       + fftshift (L194), * 1/W (R6), real part  ->  float32 dirty image (L150: fp32 throughout)
+ *
+ * Image index i = (t*C + c)*P + p, n_img = T*C*P.  N = n_pix, h = N/2.  All arrays are dense,
+ * row-major, last index fastest.  "centred" means the DC cell / phase-centre pixel is [h][h];
+ * column index = u / l axis, row index = v / m axis (R7, R8).
+ *
+ * Pointers are DEVICE pointers owned by the caller unless marked HOST.  Complex numbers are
+ * interleaved float pairs (re, im) = CUDA float2 = torch.complex64.  Every call is asynchronous
+ * on `stream` (a cudaStream_t passed as void*; NULL = the legacy default stream), allocates and
+ * frees nothing, never writes to its inputs (one documented exception: blink_fft2d_inverse may
+ * clobber `grid`), fully overwrites its outputs, and returns BLINK_OK or a negative error code.
+ * No exceptions, no stderr output, no exit().  Concurrent calls on different streams with
+ * disjoint workspaces and outputs are allowed.  There is no CPU fallback: on a machine without
+ * an sm_100 device every compute call returns BLINK_ERR_CUDA.
+ */
+#ifndef BLINKIMG_H
+#define BLINKIMG_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct blink_c64 { float re, im; } blink_c64;       /* == float2 == complex64 */
+
+enum { BLINK_W_NATURAL = 0, BLINK_W_UNIFORM = 1 };
+enum { BLINK_OP_GRID = 0, BLINK_OP_FFT2D = 1, BLINK_OP_IMAGE = 2, BLINK_OP_IMAGE_HOST = 3 };
+enum {
+    BLINK_OK = 0,
+    BLINK_ERR_INVALID_ARG = -1,   /* NULL / misaligned pointer, non-positive size, bad enum          */
+    BLINK_ERR_UNSUPPORTED = -2,   /* n_pix not a power of two in [32, 4096]; B too large (> 2^18-1)   */
+    BLINK_ERR_WORKSPACE   = -3,   /* workspace smaller than blink_workspace_bytes() reports           */
+    BLINK_ERR_CUDA        = -4    /* a CUDA runtime/driver call failed: see blink_last_cuda_error()   */
+};
+
+/* Options for blink_set_option (process-wide tuning / test switches; defaults in brackets). */
+enum {
+    BLINK_OPT_IMAGE_PATH = 0,     /* [0] 0 = auto, 1 = force unfused (grid -> rows -> columns), 2 = force fused */
+    BLINK_OPT_FUSED_CTAS = 1,     /* [0] 0 = auto (one persistent CTA per SM), else CTAs for the fused kernel  */
+    BLINK_OPT_GRID_CHUNK_B = 2    /* [0] 0 = auto, else baselines per gridder chunk (tests the spill path)     */
+};
+
+const char *blink_strerror(int code);
+const char *blink_last_cuda_error(void);          /* text of the last CUDA failure on this thread, or "" */
+int blink_set_option(int key, int value);
+int blink_get_option(int key, int *value);
+/* Number of kernels this library has launched in this process so far (all threads). */
+unsigned long long blink_kernel_launches(void);
+
+/*
+ * Workspace a call needs for the given problem (bytes; may be 0).  For BLINK_OP_IMAGE this is the
+ * RECOMMENDED size; blink_image accepts anything >= the minimum it reports via *min_bytes (may be
+ * NULL) and chunks the batch to fit.  For BLINK_OP_FFT2D pass the batch as T (C = P = 1, B = 0).
+ */
+int blink_workspace_bytes(int op, int T, int C, int P, int B, int n_pix, int weighting,
+                          size_t *bytes, size_t *min_bytes);
+
+/*
+ * Steps a0-a3: grid every image of the batch.
+ *   vis       in  [T][C][P][B] complex64, baseline fastest, cross-correlations only (R10)
+ *   uvw_m     in  [T][B][3] float32 metres (u, v, w); w is read-compatible but unused
+ *   freqs_hz  in  HOST [C] double
+ *   grid      out [T*C*P][N][N] complex64, centred
+ *   wsum      out [T*C] float32: natural = 2*B_in (samples placed incl. conjugates); uniform = number
+ *                 of occupied cells.  Shared by the P polarisations of a (t,c).
+ *   cell_idx  out OPTIONAL (NULL ok) [T][C][B] int32: centred linear cell (iv+h)*N + (iu+h), -1 if dropped
+ *   counts    out OPTIONAL (NULL ok) [T*C][N][N] uint32 samples per cell (vis + conjugates)
+ * Samples with |iu| > h-1 or |iv| > h-1 (or non-finite uvw) are dropped with their conjugate (R4).
+ * Uniform weighting divides each occupied cell by its count.  A (t,c) with W = 0 gives a zero grid.
+ * Visibilities are binned by uv row-band tile and accumulated in shared memory; when the binned
+ * list of a (t,c) does not fit on chip the baselines are processed in chunks and every chunk after
+ * the first is added to the grid with global atomics (the spill path).
+ */
+int blink_grid(const blink_c64 *vis, const float *uvw_m, const double *freqs_hz,
+               int T, int C, int P, int B, int n_pix, double pixscale_rad, int weighting,
+               blink_c64 *grid, float *wsum, int32_t *cell_idx, uint32_t *counts,
+               void *workspace, size_t workspace_bytes, void *stream);
+
+/*
+ * Steps a4-a5 on arbitrary complex grids (Hermitian or not):
+ *   image[i][y][x] = (1/scale) * Re sum_{r,q} grid[i][r][q] * exp(+2 pi i ((q-h)(x-h) + (r-h)(y-h)) / N)
+ *   grid        in  [batch][N][N] complex64, centred.  CLOBBERED (used as the row-pass output).
+ *   scale       in  OPTIONAL [ceil(batch / scale_stride_div)] float32; image i is multiplied by
+ *                   1/scale[i / scale_stride_div]; an entry of 0 gives a zero image; NULL = unscaled
+ *   image       out [batch][N][N] float32, centred
+ *   image_imag  out OPTIONAL [batch][N][N] float32: the imaginary part, same scaling (debug / tests)
+ * Row pass in shared memory, then a column pass whose tiles are staged by TMA with the fftshift,
+ * the 1/W normalisation and the real-part extraction fused into its store.
+ */
+int blink_fft2d_inverse(blink_c64 *grid, int n_pix, int batch,
+                        const float *scale, int scale_stride_div,
+                        float *image, float *image_imag,
+                        void *workspace, size_t workspace_bytes, void *stream);
+
+/*
+ * Steps a0-a5 fused: visibilities in, dirty images out; the uv grids are never materialised in
+ * full.  Arguments as blink_grid, plus
+ *   image     out [T*C*P][N][N] float32, centred, = Re(...) / W ; W = 0 gives a zero image
+ * The batch is processed in chunks that fit `workspace`.
+ */
+int blink_image(const blink_c64 *vis, const float *uvw_m, const double *freqs_hz,
+                int T, int C, int P, int B, int n_pix, double pixscale_rad, int weighting,
+                float *image, float *wsum, int32_t *cell_idx, uint32_t *counts,
+                void *workspace, size_t workspace_bytes, void *stream);
+
+/*
+ * blink_image with HOST buffers (vis, uvw_m, image, wsum are HOST pointers, ideally pinned):
+ * copies inputs to the device, images, copies the images back, pipelined per timestep on internal
+ * streams.  `workspace` is a DEVICE buffer of at least blink_workspace_bytes(BLINK_OP_IMAGE_HOST)
+ * that also holds the device staging copies.  Synchronous: returns when `image` is complete.
+ */
+int blink_image_host(const blink_c64 *vis_host, const float *uvw_m_host, const double *freqs_hz,
+                     int T, int C, int P, int B, int n_pix, double pixscale_rad, int weighting,
+                     float *image_host, float *wsum_host,
+                     void *workspace, size_t workspace_bytes);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BLINKIMG_H */

@@ -1,0 +1,187 @@
+"""Thin ctypes binding of libblinkimg (include/blinkimg.h): argument marshalling only.
+
+PyTorch is used for device memory and streams; every step of the path runs in the library's CUDA
+kernels.  There is no fallback: if the shared library is missing or a call fails, this raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional
+
+import numpy as np
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SO = os.path.join(_HERE, "libblinkimg.so")
+_lib = None
+
+W_NATURAL, W_UNIFORM = 0, 1
+OP_GRID, OP_FFT2D, OP_IMAGE, OP_IMAGE_HOST = 0, 1, 2, 3
+OPT_IMAGE_PATH, OPT_FUSED_CTAS, OPT_GRID_CHUNK_B = 0, 1, 2
+
+EXPORTS = ["blink_strerror", "blink_last_cuda_error", "blink_set_option", "blink_get_option",
+           "blink_kernel_launches", "blink_workspace_bytes", "blink_grid", "blink_fft2d_inverse",
+           "blink_image", "blink_image_host"]
+
+
+class BlinkError(RuntimeError):
+    pass
+
+
+def lib_path() -> str:
+    return _SO
+
+
+def lib():
+    """Loads libblinkimg.so (built in-tree by paper_2505_15204_b200/build.py).  Fails loudly if absent."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_SO):
+            raise BlinkError(f"{_SO} not found: run `python -m paper_2505_15204_b200.build` (needs nvcc); "
+                             "there is no CPU fallback")
+        L = ctypes.CDLL(_SO)
+        vp, i, d, sz = ctypes.c_void_p, ctypes.c_int, ctypes.c_double, ctypes.c_size_t
+        L.blink_strerror.restype = ctypes.c_char_p
+        L.blink_strerror.argtypes = [i]
+        L.blink_last_cuda_error.restype = ctypes.c_char_p
+        L.blink_last_cuda_error.argtypes = []
+        L.blink_set_option.restype = i
+        L.blink_set_option.argtypes = [i, i]
+        L.blink_get_option.restype = i
+        L.blink_get_option.argtypes = [i, ctypes.POINTER(i)]
+        L.blink_kernel_launches.restype = ctypes.c_ulonglong
+        L.blink_kernel_launches.argtypes = []
+        L.blink_workspace_bytes.restype = i
+        L.blink_workspace_bytes.argtypes = [i, i, i, i, i, i, i, ctypes.POINTER(sz), ctypes.POINTER(sz)]
+        L.blink_grid.restype = i
+        L.blink_grid.argtypes = [vp, vp, vp, i, i, i, i, i, d, i, vp, vp, vp, vp, vp, sz, vp]
+        L.blink_fft2d_inverse.restype = i
+        L.blink_fft2d_inverse.argtypes = [vp, i, i, vp, i, vp, vp, vp, sz, vp]
+        L.blink_image.restype = i
+        L.blink_image.argtypes = [vp, vp, vp, i, i, i, i, i, d, i, vp, vp, vp, vp, vp, sz, vp]
+        L.blink_image_host.restype = i
+        L.blink_image_host.argtypes = [vp, vp, vp, i, i, i, i, i, d, i, vp, vp, vp, sz]
+        _lib = L
+    return _lib
+
+
+def _check(rc: int, what: str) -> None:
+    if rc != 0:
+        L = lib()
+        msg = L.blink_strerror(rc).decode()
+        extra = L.blink_last_cuda_error().decode()
+        raise BlinkError(f"{what} failed: {msg} ({rc})" + (f": {extra}" if extra else ""))
+
+
+def _ptr(t: Optional[torch.Tensor]):
+    return None if t is None else ctypes.c_void_p(t.data_ptr())
+
+
+def _stream(device) -> ctypes.c_void_p:
+    return ctypes.c_void_p(torch.cuda.current_stream(device).cuda_stream)
+
+
+def _dev(t: torch.Tensor, dtype, name: str) -> torch.Tensor:
+    if not t.is_cuda or t.dtype != dtype or not t.is_contiguous():
+        raise BlinkError(f"{name} must be a contiguous CUDA tensor of dtype {dtype}")
+    return t
+
+
+def set_option(key: int, value: int) -> None:
+    _check(lib().blink_set_option(int(key), int(value)), "blink_set_option")
+
+
+def kernel_launches() -> int:
+    return int(lib().blink_kernel_launches())
+
+
+def blink_workspace_bytes(op: int, T: int, C: int, P: int, B: int, n_pix: int, weighting: int):
+    """-> (recommended_bytes, min_bytes)"""
+    rec, mn = ctypes.c_size_t(0), ctypes.c_size_t(0)
+    _check(lib().blink_workspace_bytes(op, T, C, P, B, n_pix, weighting, ctypes.byref(rec), ctypes.byref(mn)),
+           "blink_workspace_bytes")
+    return int(rec.value), int(mn.value)
+
+
+def _freqs(freqs_hz) -> np.ndarray:
+    return np.ascontiguousarray(np.asarray(freqs_hz, dtype=np.float64))
+
+
+def blink_grid(vis: torch.Tensor, uvw_m: torch.Tensor, freqs_hz, n_pix: int, pixscale_rad: float, weighting: int = 0,
+               want_cell_idx: bool = False, want_counts: bool = False, grid: Optional[torch.Tensor] = None):
+    """vis [T][C][P][B] complex64, uvw_m [T][B][3] float32 (CUDA) -> dict(grid, wsum, cell_idx?, counts?)"""
+    _dev(vis, torch.complex64, "vis"); _dev(uvw_m, torch.float32, "uvw_m")
+    T, C, P, B = vis.shape
+    fr = _freqs(freqs_hz)
+    dev = vis.device
+    if grid is None:
+        grid = torch.empty((T * C * P, n_pix, n_pix), dtype=torch.complex64, device=dev)
+    wsum = torch.empty(T * C, dtype=torch.float32, device=dev)
+    cell_idx = torch.empty((T, C, B), dtype=torch.int32, device=dev) if want_cell_idx else None
+    counts = torch.empty((T * C, n_pix, n_pix), dtype=torch.int32, device=dev) if want_counts else None
+    rec, _ = blink_workspace_bytes(OP_GRID, T, C, P, B, n_pix, weighting)
+    ws = torch.empty(max(rec, 16), dtype=torch.uint8, device=dev)
+    rc = lib().blink_grid(_ptr(vis), _ptr(uvw_m), fr.ctypes.data_as(ctypes.c_void_p), T, C, P, B, n_pix,
+                          float(pixscale_rad), int(weighting), _ptr(grid), _ptr(wsum), _ptr(cell_idx), _ptr(counts),
+                          _ptr(ws), ws.numel(), _stream(dev))
+    _check(rc, "blink_grid")
+    return dict(grid=grid, wsum=wsum, cell_idx=cell_idx, counts=counts)
+
+
+def blink_fft2d_inverse(grid: torch.Tensor, scale: Optional[torch.Tensor] = None, scale_stride_div: int = 1,
+                        want_imag: bool = False, image: Optional[torch.Tensor] = None):
+    """grid [batch][N][N] complex64 (CUDA, CLOBBERED) -> dict(image float32, imag?)"""
+    _dev(grid, torch.complex64, "grid")
+    batch, n, n2 = grid.shape
+    assert n == n2
+    dev = grid.device
+    if image is None:
+        image = torch.empty((batch, n, n), dtype=torch.float32, device=dev)
+    imag = torch.empty((batch, n, n), dtype=torch.float32, device=dev) if want_imag else None
+    if scale is not None:
+        _dev(scale, torch.float32, "scale")
+    rc = lib().blink_fft2d_inverse(_ptr(grid), n, batch, _ptr(scale), int(scale_stride_div), _ptr(image), _ptr(imag),
+                                   None, 0, _stream(dev))
+    _check(rc, "blink_fft2d_inverse")
+    return dict(image=image, imag=imag)
+
+
+def blink_image(vis: torch.Tensor, uvw_m: torch.Tensor, freqs_hz, n_pix: int, pixscale_rad: float, weighting: int = 0,
+                want_cell_idx: bool = False, want_counts: bool = False, image: Optional[torch.Tensor] = None,
+                workspace: Optional[torch.Tensor] = None, wsum: Optional[torch.Tensor] = None):
+    """vis [T][C][P][B] complex64, uvw_m [T][B][3] float32 (CUDA) -> dict(image [T*C*P][N][N] float32, wsum, ...)"""
+    _dev(vis, torch.complex64, "vis"); _dev(uvw_m, torch.float32, "uvw_m")
+    T, C, P, B = vis.shape
+    fr = _freqs(freqs_hz)
+    dev = vis.device
+    if image is None:
+        image = torch.empty((T * C * P, n_pix, n_pix), dtype=torch.float32, device=dev)
+    if wsum is None:
+        wsum = torch.empty(T * C, dtype=torch.float32, device=dev)
+    cell_idx = torch.empty((T, C, B), dtype=torch.int32, device=dev) if want_cell_idx else None
+    counts = torch.empty((T * C, n_pix, n_pix), dtype=torch.int32, device=dev) if want_counts else None
+    if workspace is None:
+        rec, _ = blink_workspace_bytes(OP_IMAGE, T, C, P, B, n_pix, weighting)
+        workspace = torch.empty(max(rec, 16), dtype=torch.uint8, device=dev)
+    rc = lib().blink_image(_ptr(vis), _ptr(uvw_m), fr.ctypes.data_as(ctypes.c_void_p), T, C, P, B, n_pix,
+                           float(pixscale_rad), int(weighting), _ptr(image), _ptr(wsum), _ptr(cell_idx), _ptr(counts),
+                           _ptr(workspace), workspace.numel(), _stream(dev))
+    _check(rc, "blink_image")
+    return dict(image=image, wsum=wsum, cell_idx=cell_idx, counts=counts)
+
+
+def blink_image_host(vis_host: torch.Tensor, uvw_host: torch.Tensor, freqs_hz, n_pix: int, pixscale_rad: float,
+                     weighting: int, image_host: torch.Tensor, wsum_host: torch.Tensor, workspace: torch.Tensor):
+    """Host-buffer variant: vis_host / uvw_host / image_host / wsum_host are (pinned) CPU tensors."""
+    T, C, P, B = vis_host.shape
+    fr = _freqs(freqs_hz)
+    for t, dt, nm in ((vis_host, torch.complex64, "vis_host"), (uvw_host, torch.float32, "uvw_host"),
+                      (image_host, torch.float32, "image_host"), (wsum_host, torch.float32, "wsum_host")):
+        if t.is_cuda or t.dtype != dt or not t.is_contiguous():
+            raise BlinkError(f"{nm} must be a contiguous CPU tensor of dtype {dt}")
+    rc = lib().blink_image_host(_ptr(vis_host), _ptr(uvw_host), fr.ctypes.data_as(ctypes.c_void_p), T, C, P, B, n_pix,
+                                float(pixscale_rad), int(weighting), _ptr(image_host), _ptr(wsum_host),
+                                _ptr(workspace), workspace.numel())
+    _check(rc, "blink_image_host")
+    return dict(image=image_host, wsum=wsum_host)

@@ -1,0 +1,62 @@
+// Internal helpers shared by the libblinkimg translation units (not part of the C ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stddef.h>
+#include "../../include/blinkimg.h"
+
+namespace blink {
+
+// --- error plumbing ---------------------------------------------------------------------------
+void set_cuda_error(cudaError_t e, const char *where);          // records text for blink_last_cuda_error()
+void set_error_text(const char *text);
+void count_launch(unsigned n = 1);
+
+#define BLINK_CUDA_TRY(expr)                                                     \
+    do {                                                                         \
+        cudaError_t _e = (expr);                                                 \
+        if (_e != cudaSuccess) { ::blink::set_cuda_error(_e, #expr); return BLINK_ERR_CUDA; } \
+    } while (0)
+
+#define BLINK_LAUNCH_CHECK(name)                                                 \
+    do {                                                                         \
+        cudaError_t _e = cudaGetLastError();                                     \
+        if (_e != cudaSuccess) { ::blink::set_cuda_error(_e, name); return BLINK_ERR_CUDA; } \
+        ::blink::count_launch();                                                 \
+    } while (0)
+
+int  option(int key);
+int  ensure_device();             // checks for an sm_100 device, uploads the twiddle table once per device
+int  sm_count();
+
+static inline bool is_pow2(int n) { return n > 0 && (n & (n - 1)) == 0; }
+static inline bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+static inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+// step a0 (R3): cells per metre, double left to right, rounded once to float
+static inline float scale_for(double f_hz, int n_pix, double pixscale_rad)
+{
+    double s = f_hz * (double)n_pix;
+    s = s * pixscale_rad;
+    s = s / 299792458.0;
+    return (float)s;
+}
+
+constexpr int kMaxChannels = 4096;      // per-channel scales are passed to kernels through a device array
+constexpr int kMaxBaselines = (1 << 18) - 1;
+
+// device twiddle table W[m] = exp(+2 pi i m / 4096), m in [0, 4096), built in double on the host
+constexpr int kTwiddleN = 4096;
+const float2 *twiddle_table();          // device pointer (after ensure_device())
+
+// --- internal entry points used across translation units ---------------------------------------
+// gridder over the flattened (t,c) range [tc0, tc0+ntc).  wsum / cell_idx are indexed by the absolute tc,
+// grid / counts by (tc - out_tc0) so that a chunk can land at the start of a workspace buffer.
+int grid_range(const float2 *vis, const float *uvw_m, const double *freqs_hz, double pixscale_rad, int T, int C,
+               int P, int B, int n_pix, int weighting, int tc0, int ntc, int out_tc0, float2 *grid, float *wsum,
+               int32_t *cell_idx, uint32_t *counts, cudaStream_t st);
+bool grid_needs_global_counts(int B, int n_pix, int weighting);
+int fft2d_range(float2 *grid, int n_pix, int batch, const float *scale, int scale_div, int scale_img_base,
+                float *image, float *image_imag, cudaStream_t st);
+
+}  // namespace blink

@@ -1,0 +1,227 @@
+// Cooperative register-resident inverse FFT building blocks (sm_100a).
+//
+// A group of TG = N/8 threads transforms NV vectors of N complex64 values at once.  Thread `tid`
+// of the group holds element n = tid + e*TG in register slot e (e = 0..7) before AND after the
+// transform (Stockham auto-sort, decimation in time, radices 8/4 chosen by plan_radix()).  Between
+// stages the values cross threads through a shared-memory exchange array addressed by an
+// Exchange policy; inside a stage everything is register arithmetic.
+//
+// Sign +, unnormalised: X[j] = sum_n x[n] exp(+2 pi i j n / N)   (eq. 5, reading R5).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace blink {
+
+constexpr int kE = 8;                                   // elements per thread per vector
+__host__ __device__ constexpr int kTwiddleNConst() { return 4096; }   // length of the W table
+
+__host__ __device__ constexpr int ilog2(int n) { return n <= 1 ? 0 : 1 + ilog2(n >> 1); }
+// number of radix-4 stages: log2 N = 3 a + 2 b with b in {0,1,2}
+__host__ __device__ constexpr int plan_n4(int n) { return (ilog2(n) % 3 == 0) ? 0 : (ilog2(n) % 3 == 2 ? 1 : 2); }
+__host__ __device__ constexpr int plan_n8(int n) { return (ilog2(n) - 2 * plan_n4(n)) / 3; }
+__host__ __device__ constexpr int plan_stages(int n) { return plan_n8(n) + plan_n4(n); }
+__host__ __device__ constexpr int plan_radix(int n, int s) { return s < plan_n8(n) ? 8 : 4; }
+
+__device__ __forceinline__ float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
+__device__ __forceinline__ float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
+__device__ __forceinline__ float2 cmul(float2 a, float2 w)
+{
+    return make_float2(fmaf(a.x, w.x, -a.y * w.y), fmaf(a.x, w.y, a.y * w.x));
+}
+__device__ __forceinline__ float2 mul_i(float2 a) { return make_float2(-a.y, a.x); }        // * (+i)
+
+// In-register inverse DFTs of length 2, 4, 8 (natural order in and out).
+__device__ __forceinline__ void dft2(float2 &a, float2 &b)
+{
+    float2 t = a;
+    a = cadd(t, b);
+    b = csub(t, b);
+}
+__device__ __forceinline__ void dft4(float2 &x0, float2 &x1, float2 &x2, float2 &x3)
+{
+    float2 t0 = cadd(x0, x2), t1 = csub(x0, x2), t2 = cadd(x1, x3), t3 = mul_i(csub(x1, x3));
+    x0 = cadd(t0, t2);
+    x1 = cadd(t1, t3);
+    x2 = csub(t0, t2);
+    x3 = csub(t1, t3);
+}
+__device__ __forceinline__ void dft8(float2 (&x)[8])
+{
+    // even / odd halves, then combine with w8^k = exp(+2 pi i k / 8)
+    dft4(x[0], x[2], x[4], x[6]);
+    dft4(x[1], x[3], x[5], x[7]);
+    const float r = 0.70710678118654752440f;
+    float2 o0 = x[1];
+    float2 o1 = make_float2((x[3].x - x[3].y) * r, (x[3].x + x[3].y) * r);        // * (1+i)/sqrt2
+    float2 o2 = mul_i(x[5]);
+    float2 o3 = make_float2((-x[7].x - x[7].y) * r, (x[7].x - x[7].y) * r);       // * (-1+i)/sqrt2
+    float2 e0 = x[0], e1 = x[2], e2 = x[4], e3 = x[6];
+    x[0] = cadd(e0, o0);  x[4] = csub(e0, o0);
+    x[1] = cadd(e1, o1);  x[5] = csub(e1, o1);
+    x[2] = cadd(e2, o2);  x[6] = csub(e2, o2);
+    x[3] = cadd(e3, o3);  x[7] = csub(e3, o3);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Exchange policies: where position w (0..N-1) of the group's vector(s) lives in shared memory.
+// ---------------------------------------------------------------------------------------------
+// One vector, float2 elements, one padding element every 8 (conflict-free for the stride-8 stores
+// of the first stage and the unit-stride loads).
+struct ExchangePadded1 {
+    float2 *base;
+    __device__ __forceinline__ static int slots(int n) { return n + (n >> 3); }
+    __device__ __forceinline__ void put(int w, const float2 (&v)[1]) const { base[w + (w >> 3)] = v[0]; }
+    __device__ __forceinline__ void get(int w, float2 (&v)[1]) const { v[0] = base[w + (w >> 3)]; }
+};
+
+// Two vectors (a column pair), float4 elements living INSIDE a TMA-written tile whose rows are
+// ROWB bytes wide and swizzled by the hardware (CU_TENSOR_MAP_SWIZZLE_{32,64,128}B for ROWB =
+// 32/64/128).  Position w is kept in tile row rho(w), 16-byte chunk `pair`; rho permutes the rows
+// so that the 8 lanes of a quarter warp always touch 8 different bank groups.
+template <int ROWB>
+struct ExchangeTilePair {
+    unsigned char *tile;            // 1024-byte aligned shared memory
+    int pair;                       // which 16-byte chunk of the row (= column pair)
+    __device__ __forceinline__ static int rho(int w) { return w ^ (((w >> 3) ^ (w >> 6)) & 7); }
+    __device__ __forceinline__ static uint32_t swz(uint32_t off)
+    {
+        constexpr uint32_t mask = ROWB == 128 ? 7u : (ROWB == 64 ? 3u : (ROWB == 32 ? 1u : 0u));
+        return off ^ (((off >> 7) & mask) << 4);
+    }
+    __device__ __forceinline__ float4 *at_row(int row) const
+    {
+        return reinterpret_cast<float4 *>(tile + swz((uint32_t)row * ROWB + (uint32_t)pair * 16u));
+    }
+    __device__ __forceinline__ void put(int w, const float2 (&v)[2]) const
+    {
+        *at_row(rho(w)) = make_float4(v[0].x, v[0].y, v[1].x, v[1].y);
+    }
+    __device__ __forceinline__ void get(int w, float2 (&v)[2]) const
+    {
+        float4 t = *at_row(rho(w));
+        v[0] = make_float2(t.x, t.y);
+        v[1] = make_float2(t.z, t.w);
+    }
+};
+
+// Two vectors, float4 elements in a private dense array (8 elements per 128-byte line), same rho.
+struct ExchangeDense2 {
+    float4 *base;
+    __device__ __forceinline__ static int rho(int w) { return w ^ (((w >> 3) ^ (w >> 6)) & 7); }
+    __device__ __forceinline__ void put(int w, const float2 (&v)[2]) const
+    {
+        base[rho(w)] = make_float4(v[0].x, v[0].y, v[1].x, v[1].y);
+    }
+    __device__ __forceinline__ void get(int w, float2 (&v)[2]) const
+    {
+        float4 t = base[rho(w)];
+        v[0] = make_float2(t.x, t.y);
+        v[1] = make_float2(t.z, t.w);
+    }
+};
+
+// ---------------------------------------------------------------------------------------------
+// One stage: twiddle (skipped when P == 1), radix-R butterflies in registers.
+//   v[nv][e] holds x[tid + e*TG].  Butterfly q (q = 0..8/R-1) is i = tid + q*TG and uses slots
+//   e = q + r*(8/R), r = 0..R-1.  Twiddle of input r: exp(+2 pi i r k / (P R)), k = i mod P, read
+//   from the W_4096 table `tw` (tw[m] = exp(+2 pi i m / 4096)).
+// ---------------------------------------------------------------------------------------------
+template <int N, int NV, int R, int P>
+__device__ __forceinline__ void stage_compute(float2 (&v)[NV][kE], int tid, const float2 *__restrict__ tw)
+{
+    constexpr int TG = N / kE;
+    constexpr int NB = kE / R;                         // butterflies per thread
+#pragma unroll
+    for (int q = 0; q < NB; ++q) {
+        const int i = tid + q * TG;
+        if constexpr (P > 1) {
+            const int k = i & (P - 1);
+            constexpr int step = kTwiddleNConst() / (P * R);
+#pragma unroll
+            for (int r = 1; r < R; ++r) {
+                const float2 w = __ldg(tw + r * k * step);
+#pragma unroll
+                for (int nv = 0; nv < NV; ++nv) v[nv][q + r * NB] = cmul(v[nv][q + r * NB], w);
+            }
+        }
+#pragma unroll
+        for (int nv = 0; nv < NV; ++nv) {
+            if constexpr (R == 8) {
+                float2 x[8];
+#pragma unroll
+                for (int r = 0; r < 8; ++r) x[r] = v[nv][q + r * NB];
+                dft8(x);
+#pragma unroll
+                for (int r = 0; r < 8; ++r) v[nv][q + r * NB] = x[r];
+            } else {
+                dft4(v[nv][q], v[nv][q + NB], v[nv][q + 2 * NB], v[nv][q + 3 * NB]);
+            }
+        }
+    }
+}
+
+// scatter the stage outputs to their Stockham positions: y[j + r*P], j = (i - k)*R + k
+template <int N, int NV, int R, int P, class X>
+__device__ __forceinline__ void stage_put(const float2 (&v)[NV][kE], int tid, const X &xch)
+{
+    constexpr int TG = N / kE;
+    constexpr int NB = kE / R;
+#pragma unroll
+    for (int q = 0; q < NB; ++q) {
+        const int i = tid + q * TG;
+        const int k = i & (P - 1);
+        const int j = (i - k) * R + k;
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            float2 t[NV];
+#pragma unroll
+            for (int nv = 0; nv < NV; ++nv) t[nv] = v[nv][q + r * NB];
+            xch.put(j + r * P, t);
+        }
+    }
+}
+
+template <int N, int NV, class X>
+__device__ __forceinline__ void stage_get(float2 (&v)[NV][kE], int tid, const X &xch)
+{
+    constexpr int TG = N / kE;
+#pragma unroll
+    for (int e = 0; e < kE; ++e) {
+        float2 t[NV];
+        xch.get(tid + e * TG, t);
+#pragma unroll
+        for (int nv = 0; nv < NV; ++nv) v[nv][e] = t[nv];
+    }
+}
+
+template <int N, int NV, int S, int P, class X, class Sync>
+struct FftStages {
+    __device__ __forceinline__ static void run(float2 (&v)[NV][kE], int tid, const X &xch,
+                                               const float2 *__restrict__ tw, Sync sync)
+    {
+        constexpr int R = plan_radix(N, S);
+        stage_compute<N, NV, R, P>(v, tid, tw);
+        if constexpr (S + 1 < plan_stages(N)) {
+            sync();                                      // everyone has finished reading the array
+            stage_put<N, NV, R, P, X>(v, tid, xch);
+            sync();                                      // all writes visible
+            stage_get<N, NV, X>(v, tid, xch);
+            FftStages<N, NV, S + 1, P * R, X, Sync>::run(v, tid, xch, tw, sync);
+        }
+        // last stage: output j + r*P with P = N/R is again slot layout tid + e*TG -- nothing to move
+    }
+};
+
+// Full transform.  `sync` must synchronise (at least) all threads of the group and must be called
+// by every thread the same number of times (use __syncthreads() when groups share a CTA).
+// NOTE: the first sync() also orders the caller's last reads of the exchange array (e.g. the
+// initial load out of a TMA tile that doubles as the exchange array) before the first put.
+template <int N, int NV, class X, class Sync>
+__device__ __forceinline__ void fft_inverse(float2 (&v)[NV][kE], int tid, const X &xch,
+                                            const float2 *__restrict__ tw, Sync sync)
+{
+    FftStages<N, NV, 0, 1, X, Sync>::run(v, tid, xch, tw, sync);
+}
+
+}  // namespace blink

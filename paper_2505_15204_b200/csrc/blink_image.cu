@@ -1,0 +1,200 @@
+// blink_image: steps a0-a5, visibilities in -> dirty images out, and its host-buffer twin.
+// Path selection (BLINK_OPT_IMAGE_PATH): fused kernel (blink_fused.cu) when the size is supported,
+// else the unfused chain grid -> row pass -> column pass over chunks of (t,c) that fit the workspace.
+#include <algorithm>
+
+#include "blink_common.cuh"
+
+namespace blink {
+
+// fused path (blink_fused.cu)
+bool fused_supported(int P, int B, int n_pix, int weighting);
+size_t fused_workspace_bytes(int n_pix, int ctas);
+int fused_default_ctas();
+int fused_image(const float2 *vis, const float *uvw_m, const double *freqs_hz, double pixscale_rad, int T, int C,
+                int P, int B, int n_pix, int weighting, int tc0, int ntc, float *image, float *wsum,
+                int32_t *cell_idx, void *workspace, size_t workspace_bytes, cudaStream_t st);
+int counts_only(const float *uvw_m, const double *freqs_hz, double pixscale_rad, int T, int C, int B, int n_pix,
+                int tc0, int ntc, uint32_t *counts, cudaStream_t st);
+
+static size_t unfused_bytes_per_tc(int P, int B, int n_pix, int weighting, bool have_counts)
+{
+    const size_t n2 = (size_t)n_pix * n_pix;
+    size_t b = (size_t)P * n2 * sizeof(float2);
+    if (!have_counts && grid_needs_global_counts(B, n_pix, weighting)) b += n2 * sizeof(uint32_t);
+    return b;
+}
+
+static bool use_fused(int P, int B, int n_pix, int weighting)
+{
+    const int path = option(BLINK_OPT_IMAGE_PATH);
+    if (path == 1) return false;
+    return fused_supported(P, B, n_pix, weighting);
+}
+
+static int image_device(const float2 *vis, const float *uvw_m, const double *freqs_hz, int T, int C, int P, int B,
+                        int n_pix, double pixscale_rad, int weighting, int tc0, int ntc, float *image, float *wsum,
+                        int32_t *cell_idx, uint32_t *counts, void *workspace, size_t workspace_bytes, cudaStream_t st)
+{
+    // image / wsum / cell_idx / counts are indexed by ABSOLUTE tc; the range [tc0, tc0+ntc) is processed
+    const size_t n2 = (size_t)n_pix * n_pix;
+    if (use_fused(P, B, n_pix, weighting)) {
+        int rc = fused_image(vis, uvw_m, freqs_hz, pixscale_rad, T, C, P, B, n_pix, weighting, tc0, ntc, image, wsum,
+                             cell_idx, workspace, workspace_bytes, st);
+        if (rc != BLINK_OK) return rc;
+        if (counts) return counts_only(uvw_m, freqs_hz, pixscale_rad, T, C, B, n_pix, tc0, ntc, counts, st);
+        return BLINK_OK;
+    }
+    const size_t per_tc = unfused_bytes_per_tc(P, B, n_pix, weighting, counts != nullptr);
+    if (!workspace || workspace_bytes < per_tc || !aligned16(workspace)) return BLINK_ERR_WORKSPACE;
+    const int chunk = (int)std::min<size_t>((size_t)ntc, workspace_bytes / per_tc);
+    float2 *wgrid = static_cast<float2 *>(workspace);
+    const bool ws_counts = per_tc > (size_t)P * n2 * sizeof(float2);
+    uint32_t *wcounts = ws_counts ? reinterpret_cast<uint32_t *>(wgrid + (size_t)chunk * P * n2) : nullptr;
+    for (int s = tc0; s < tc0 + ntc; s += chunk) {
+        const int m = std::min(chunk, tc0 + ntc - s);
+        // counts: caller's array (absolute index) or the workspace copy (chunk-relative)
+        uint32_t *cptr = counts ? counts + (size_t)s * n2 : wcounts;
+        int rc = grid_range(vis, uvw_m, freqs_hz, pixscale_rad, T, C, P, B, n_pix, weighting, s, m, s, wgrid, wsum,
+                            cell_idx, cptr, st);
+        if (rc != BLINK_OK) return rc;
+        rc = fft2d_range(wgrid, n_pix, m * P, wsum, P, s * P, image + (size_t)s * P * n2, nullptr, st);
+        if (rc != BLINK_OK) return rc;
+    }
+    return BLINK_OK;
+}
+
+}  // namespace blink
+
+using namespace blink;
+
+static int check_common(const void *vis, const void *uvw_m, const double *freqs_hz, int T, int C, int P, int B, int n_pix,
+                        double pixscale_rad, int weighting)
+{
+    if (!vis || !uvw_m || !freqs_hz) return BLINK_ERR_INVALID_ARG;
+    if (T < 1 || C < 1 || P < 1 || B < 1 || !(pixscale_rad > 0.0)) return BLINK_ERR_INVALID_ARG;
+    if (weighting != BLINK_W_NATURAL && weighting != BLINK_W_UNIFORM) return BLINK_ERR_INVALID_ARG;
+    if (!is_pow2(n_pix) || n_pix < 32 || n_pix > 4096 || B > kMaxBaselines) return BLINK_ERR_UNSUPPORTED;
+    if ((long long)T * C * P > 0x3fffffffLL) return BLINK_ERR_UNSUPPORTED;
+    return BLINK_OK;
+}
+
+extern "C" int blink_workspace_bytes(int op, int T, int C, int P, int B, int n_pix, int weighting, size_t *bytes,
+                                     size_t *min_bytes)
+{
+    if (!bytes) return BLINK_ERR_INVALID_ARG;
+    if (!is_pow2(n_pix) || n_pix < 32 || n_pix > 4096) return BLINK_ERR_UNSUPPORTED;
+    if (T < 1 || C < 1 || P < 1 || B < 0) return BLINK_ERR_INVALID_ARG;
+    const size_t n2 = (size_t)n_pix * n_pix;
+    size_t rec = 0, mn = 0;
+    switch (op) {
+        case BLINK_OP_GRID:
+            rec = mn = grid_needs_global_counts(B, n_pix, weighting) ? (size_t)T * C * n2 * sizeof(uint32_t) : 0;
+            break;
+        case BLINK_OP_FFT2D:
+            rec = mn = 0;
+            break;
+        case BLINK_OP_IMAGE:
+        case BLINK_OP_IMAGE_HOST: {
+            if (use_fused(P, B, n_pix, weighting)) {
+                int ctas = option(BLINK_OPT_FUSED_CTAS);
+                if (ctas <= 0) ctas = fused_default_ctas();
+                rec = fused_workspace_bytes(n_pix, ctas);
+                mn = fused_workspace_bytes(n_pix, 1);
+            } else {
+                const size_t per_tc = unfused_bytes_per_tc(P, B, n_pix, weighting, false);
+                mn = per_tc;
+                rec = per_tc * std::min<size_t>((size_t)T * C, 256);
+            }
+            if (op == BLINK_OP_IMAGE_HOST) {
+                // device staging: uvw for all timesteps, wsum, and two slots of one timestep of vis + images
+                size_t stage = align_up((size_t)T * B * 3 * sizeof(float), 256) + align_up((size_t)T * C * sizeof(float), 256) +
+                               2 * (align_up((size_t)C * P * B * sizeof(float2), 256) + align_up((size_t)C * P * n2 * sizeof(float), 256));
+                rec = 2 * align_up(rec, 256) + stage;             // one compute workspace per pipeline slot
+                mn = 2 * align_up(mn, 256) + stage;
+            }
+            break;
+        }
+        default:
+            return BLINK_ERR_INVALID_ARG;
+    }
+    *bytes = rec;
+    if (min_bytes) *min_bytes = mn;
+    return BLINK_OK;
+}
+
+extern "C" int blink_image(const blink_c64 *vis, const float *uvw_m, const double *freqs_hz, int T, int C, int P, int B,
+                           int n_pix, double pixscale_rad, int weighting, float *image, float *wsum, int32_t *cell_idx,
+                           uint32_t *counts, void *workspace, size_t workspace_bytes, void *stream)
+{
+    int rc = check_common(vis, uvw_m, freqs_hz, T, C, P, B, n_pix, pixscale_rad, weighting);
+    if (rc != BLINK_OK) return rc;
+    if (!image || !wsum) return BLINK_ERR_INVALID_ARG;
+    if (!aligned16(vis) || !aligned16(image) || (counts && !aligned16(counts))) return BLINK_ERR_INVALID_ARG;
+    rc = ensure_device();
+    if (rc != BLINK_OK) return rc;
+    return image_device(reinterpret_cast<const float2 *>(vis), uvw_m, freqs_hz, T, C, P, B, n_pix, pixscale_rad, weighting,
+                        0, T * C, image, wsum, cell_idx, counts, workspace, workspace_bytes,
+                        static_cast<cudaStream_t>(stream));
+}
+
+extern "C" int blink_image_host(const blink_c64 *vis_host, const float *uvw_m_host, const double *freqs_hz, int T, int C,
+                                int P, int B, int n_pix, double pixscale_rad, int weighting, float *image_host,
+                                float *wsum_host, void *workspace, size_t workspace_bytes)
+{
+    int rc = check_common(vis_host, uvw_m_host, freqs_hz, T, C, P, B, n_pix, pixscale_rad, weighting);
+    if (rc != BLINK_OK) return rc;
+    if (!image_host || !wsum_host || !workspace || !aligned16(workspace)) return BLINK_ERR_INVALID_ARG;
+    rc = ensure_device();
+    if (rc != BLINK_OK) return rc;
+    size_t need = 0, need_min = 0;
+    rc = blink_workspace_bytes(BLINK_OP_IMAGE_HOST, T, C, P, B, n_pix, weighting, &need, &need_min);
+    if (rc != BLINK_OK) return rc;
+    if (workspace_bytes < need_min) return BLINK_ERR_WORKSPACE;
+
+    const size_t n2 = (size_t)n_pix * n_pix;
+    const size_t uvw_b = align_up((size_t)T * B * 3 * sizeof(float), 256);
+    const size_t wsum_b = align_up((size_t)T * C * sizeof(float), 256);
+    const size_t vis_b = align_up((size_t)C * P * B * sizeof(float2), 256);
+    const size_t img_b = align_up((size_t)C * P * n2 * sizeof(float), 256);
+    const size_t stage = uvw_b + wsum_b + 2 * (vis_b + img_b);
+    unsigned char *w = static_cast<unsigned char *>(workspace);
+    float *d_uvw = reinterpret_cast<float *>(w);
+    float *d_wsum = reinterpret_cast<float *>(w + uvw_b);
+    unsigned char *slots = w + uvw_b + wsum_b;
+    unsigned char *compute_ws = w + stage;
+    const size_t compute_bytes = (workspace_bytes - stage) / 2 / 256 * 256;       // one half per slot
+
+    // two pipelines (slots): H2D vis(t) -> image(t) -> D2H images(t), each on its own stream
+    static cudaStream_t streams[2] = {nullptr, nullptr};
+    for (int k = 0; k < 2; ++k)
+        if (!streams[k]) BLINK_CUDA_TRY(cudaStreamCreateWithFlags(&streams[k], cudaStreamNonBlocking));
+    cudaEvent_t uvw_ready;
+    BLINK_CUDA_TRY(cudaEventCreateWithFlags(&uvw_ready, cudaEventDisableTiming));
+    BLINK_CUDA_TRY(cudaMemcpyAsync(d_uvw, uvw_m_host, (size_t)T * B * 3 * sizeof(float), cudaMemcpyHostToDevice, streams[0]));
+    BLINK_CUDA_TRY(cudaEventRecord(uvw_ready, streams[0]));
+    BLINK_CUDA_TRY(cudaStreamWaitEvent(streams[1], uvw_ready, 0));
+    int result = BLINK_OK;
+    for (int t = 0; t < T && result == BLINK_OK; ++t) {
+        const int k = t & 1;
+        cudaStream_t st = streams[k];
+        float2 *d_vis = reinterpret_cast<float2 *>(slots + (size_t)k * (vis_b + img_b));
+        float *d_img = reinterpret_cast<float *>(slots + (size_t)k * (vis_b + img_b) + vis_b);
+        const size_t vis_elems = (size_t)C * P * B;
+        BLINK_CUDA_TRY(cudaMemcpyAsync(d_vis, reinterpret_cast<const float2 *>(vis_host) + (size_t)t * vis_elems,
+                                       vis_elems * sizeof(float2), cudaMemcpyHostToDevice, st));
+        // one timestep as a T=1 problem: uvw of timestep t, outputs of timestep t
+        result = image_device(d_vis, d_uvw + (size_t)t * B * 3, freqs_hz, 1, C, P, B, n_pix, pixscale_rad, weighting, 0, C,
+                              d_img, d_wsum + (size_t)t * C, nullptr, nullptr, compute_ws + (size_t)k * compute_bytes,
+                              compute_bytes, st);
+        if (result != BLINK_OK) break;
+        BLINK_CUDA_TRY(cudaMemcpyAsync(image_host + (size_t)t * C * P * n2, d_img, (size_t)C * P * n2 * sizeof(float),
+                                       cudaMemcpyDeviceToHost, st));
+    }
+    BLINK_CUDA_TRY(cudaStreamSynchronize(streams[0]));
+    BLINK_CUDA_TRY(cudaStreamSynchronize(streams[1]));
+    if (result == BLINK_OK)
+        BLINK_CUDA_TRY(cudaMemcpy(wsum_host, d_wsum, (size_t)T * C * sizeof(float), cudaMemcpyDeviceToHost));
+    cudaEventDestroy(uvw_ready);
+    return result;
+}

@@ -1,0 +1,66 @@
+"""The C-ABI library builds, loads without a GPU and exports every symbol include/blinkimg.h declares;
+calls that need a device fail loudly (no CPU fallback)."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def so_path():
+    from paper_2505_15204_b200 import build
+    return build.build()
+
+
+def _declared_functions():
+    text = open(os.path.join(ROOT, "include", "blinkimg.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(blink_[a-z0-9_]+)\s*\(", text)))
+
+
+def test_header_symbols_exported(so_path):
+    names = _declared_functions()
+    assert {"blink_grid", "blink_fft2d_inverse", "blink_image", "blink_image_host", "blink_workspace_bytes"} <= set(names)
+    L = ctypes.CDLL(so_path)
+    for n in names:
+        assert hasattr(L, n), n
+    from paper_2505_15204_b200 import binding
+    assert sorted(binding.EXPORTS) == names
+
+
+def test_host_only_calls(so_path):
+    from paper_2505_15204_b200 import binding as bk
+    L = bk.lib()
+    assert L.blink_strerror(0).decode() == "ok" and L.blink_strerror(-2).decode() == "unsupported size"
+    bk.set_option(bk.OPT_GRID_CHUNK_B, 123)
+    v = ctypes.c_int(0)
+    assert L.blink_get_option(bk.OPT_GRID_CHUNK_B, ctypes.byref(v)) == 0 and v.value == 123
+    bk.set_option(bk.OPT_GRID_CHUNK_B, 0)
+    assert L.blink_set_option(99, 1) == -1
+    # workspace query is pure host arithmetic
+    rec, mn = bk.blink_workspace_bytes(bk.OP_FFT2D, 10, 1, 1, 0, 512, 0)
+    assert rec == 0 and mn == 0
+    bk.set_option(bk.OPT_IMAGE_PATH, 1)
+    rec, mn = bk.blink_workspace_bytes(bk.OP_IMAGE, 50, 768, 1, 8128, 512, 0)
+    bk.set_option(bk.OPT_IMAGE_PATH, 0)
+    assert mn == 512 * 512 * 8 and rec == 256 * mn
+    with pytest.raises(bk.BlinkError):
+        bk.blink_workspace_bytes(bk.OP_IMAGE, 1, 1, 1, 10, 100, 0)        # not a power of two
+
+
+def test_no_cpu_fallback_without_device(so_path):
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a device is present")
+    from paper_2505_15204_b200 import binding as bk
+    L = bk.lib()
+    buf = np.zeros(64, dtype=np.float32)
+    p = buf.ctypes.data_as(ctypes.c_void_p)
+    fr = np.array([150e6]).ctypes.data_as(ctypes.c_void_p)
+    rc = L.blink_image(p, p, fr, 1, 1, 1, 4, 32, 0.01, 0, p, p, None, None, p, 64, None)
+    assert rc == -4                                                      # BLINK_ERR_CUDA, and says why
+    assert L.blink_last_cuda_error().decode() != ""

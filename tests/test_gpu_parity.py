@@ -1,0 +1,245 @@
+"""GPU parity: libblinkimg (through the C ABI binding) against the CPU oracle, element by element.
+
+Bars (BASELINE.json north_star): per image max|I_gpu - I_oracle| <= 1e-4 * max|I_oracle|;
+cell_idx, counts, wsum bit-exact.  All inputs come from paper_2505_15204_b200.workloads (seeded).
+"""
+import numpy as np
+import pytest
+import torch
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-4
+
+
+@pytest.fixture(scope="module")
+def bk():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2505_15204_b200 import binding
+    binding.lib()                     # raises if the .so is missing: no fallback
+    yield binding
+    for k in (binding.OPT_IMAGE_PATH, binding.OPT_FUSED_CTAS, binding.OPT_GRID_CHUNK_B):
+        binding.set_option(k, 0)
+
+
+def _img_err(gpu, ref):
+    return float(np.max(np.abs(gpu.astype(np.float64) - ref)) / max(np.max(np.abs(ref)), 1e-300))
+
+
+def _check_images(bk, w, res, oracle_mod, ids=None):
+    vis, uvw = w.vis.cpu().numpy(), w.uvw_m.cpu().numpy()
+    n_img = w.T * w.C * w.P
+    ids = np.arange(n_img) if ids is None else np.asarray(ids)
+    ref, wref = oracle_mod.image_batch(vis, uvw, w.freqs_hz, w.n_pix, w.pixscale_rad, w.weighting, ids, nthreads=8)
+    img = res["image"][torch.as_tensor(ids, device=res["image"].device)].cpu().numpy()
+    wsum = res["wsum"].cpu().numpy()
+    worst = 0.0
+    for k, i in enumerate(ids):
+        assert wsum[i // w.P] == np.float32(wref[k]), (i, wsum[i // w.P], wref[k])
+        if wref[k] == 0:
+            assert np.all(img[k] == 0)
+            continue
+        worst = max(worst, _img_err(img[k], ref[k]))
+    assert worst <= TOL, worst
+    return worst
+
+
+# --------------------------------------------------------------------------- blink_fft2d_inverse
+@pytest.mark.parametrize("n,batch", [(32, 5), (64, 3), (128, 3), (256, 2), (512, 3), (1024, 2), (2048, 1), (4096, 1)])
+def test_fft2d_inverse_vs_oracle(bk, oracle_mod, n, batch):
+    rng = np.random.default_rng(100 + n)
+    g = (rng.normal(size=(batch, n, n)) + 1j * rng.normal(size=(batch, n, n))).astype(np.complex64)
+    # a few isolated bright cells so that sign / orientation / shift errors cannot hide in noise
+    g[0, n // 2 + 3, n // 2 - 5] += 50 * n
+    g[-1, 1, n - 2] += (30 - 40j) * n
+    scale = torch.tensor(rng.uniform(0.5, 2.0, batch).astype(np.float32), device="cuda")
+    r = bk.blink_fft2d_inverse(torch.tensor(g, device="cuda"), scale=scale, scale_stride_div=1, want_imag=True)
+    torch.cuda.synchronize()
+    re, im = r["image"].cpu().numpy(), r["imag"].cpu().numpy()
+    sc = scale.cpu().numpy().astype(np.float64)
+    for b in range(batch):
+        ref = oracle_mod.ifft2_radix2(g[b].astype(np.complex128)) / sc[b]
+        peak = np.max(np.abs(ref))
+        assert np.max(np.abs(re[b] - ref.real)) <= TOL * peak
+        assert np.max(np.abs(im[b] - ref.imag)) <= TOL * peak
+
+
+def test_fft2d_scale_semantics(bk, oracle_mod):
+    n, batch = 64, 6
+    rng = np.random.default_rng(1)
+    g = (rng.normal(size=(batch, n, n)) + 1j * rng.normal(size=(batch, n, n))).astype(np.complex64)
+    scale = torch.tensor([2.0, 0.0, 4.0], device="cuda")          # images per entry = 2; a zero entry -> zero image
+    r = bk.blink_fft2d_inverse(torch.tensor(g, device="cuda"), scale=scale, scale_stride_div=2)
+    img = r["image"].cpu().numpy()
+    for b, s in enumerate([2.0, 2.0, 0.0, 0.0, 4.0, 4.0]):
+        ref = oracle_mod.ifft2_radix2(g[b].astype(np.complex128)).real
+        if s == 0:
+            assert np.all(img[b] == 0)
+        else:
+            assert np.max(np.abs(img[b] - ref / s)) <= TOL * np.max(np.abs(ref / s))
+    r = bk.blink_fft2d_inverse(torch.tensor(g, device="cuda"))     # unscaled
+    ref = oracle_mod.ifft2_radix2(g[3].astype(np.complex128)).real
+    assert np.max(np.abs(r["image"][3].cpu().numpy() - ref)) <= TOL * np.max(np.abs(ref))
+
+
+# --------------------------------------------------------------------------- blink_grid
+def _check_grid(bk, oracle_mod, w):
+    from paper_2505_15204_b200 import workloads  # noqa: F401
+    r = bk.blink_grid(w.vis, w.uvw_m, w.freqs_hz, w.n_pix, w.pixscale_rad, w.weighting, want_cell_idx=True,
+                      want_counts=True)
+    torch.cuda.synchronize()
+    vis, uvw = w.vis.cpu().numpy(), w.uvw_m.cpu().numpy()
+    ci = r["cell_idx"].cpu().numpy()
+    assert np.array_equal(ci, oracle_mod.cells(uvw, w.freqs_hz, w.n_pix, w.pixscale_rad))       # bit-exact, every (t,c,b)
+    grid = r["grid"].cpu().numpy()
+    cnt = r["counts"].cpu().numpy().astype(np.uint32)
+    wsum = r["wsum"].cpu().numpy()
+    for t in range(w.T):
+        for c in range(w.C):
+            for p in range(w.P):
+                g, cn, W, _ = oracle_mod.grid_one(vis[t, c, p], uvw[t], w.freqs_hz[c], w.n_pix, w.pixscale_rad, w.weighting)
+                i = (t * w.C + c) * w.P + p
+                assert np.array_equal(cnt[t * w.C + c], cn)
+                assert wsum[t * w.C + c] == np.float32(W)
+                peak = max(np.max(np.abs(g)), 1e-30)
+                assert np.max(np.abs(grid[i] - g)) <= 1e-5 * peak
+
+
+@pytest.mark.parametrize("n,weighting", [(32, 0), (64, 1), (256, 0), (512, 1)])
+def test_grid_vs_oracle(bk, oracle_mod, n, weighting):
+    from paper_2505_15204_b200 import workloads
+    w = workloads.make_random(T=2, C=3, P=2, B=1500, n_pix=n, weighting=weighting, seed=n + weighting, device="cuda", fill=1.1)
+    _check_grid(bk, oracle_mod, w)
+
+
+@pytest.mark.parametrize("weighting", [0, 1])
+def test_grid_spill_path(bk, oracle_mod, weighting):
+    # chunks of 400 baselines: chunks after the first are added with global atomics
+    from paper_2505_15204_b200 import workloads
+    w = workloads.make_random(T=1, C=2, P=2, B=1500, n_pix=128, weighting=weighting, seed=77, device="cuda", fill=0.5)
+    bk.set_option(bk.OPT_GRID_CHUNK_B, 400)
+    try:
+        _check_grid(bk, oracle_mod, w)
+    finally:
+        bk.set_option(bk.OPT_GRID_CHUNK_B, 0)
+
+
+def test_grid_collisions_single_cell(bk, oracle_mod):
+    # every baseline in the same cell: worst-case shared-memory atomic contention, exact counts
+    from paper_2505_15204_b200 import workloads
+    w = workloads.make_random(T=1, C=1, P=1, B=3000, n_pix=64, weighting=1, seed=3, device="cuda")
+    w.uvw_m[:] = 0.0
+    w.uvw_m[0, :, 0] = 4.2
+    w.uvw_m[0, :, 1] = -7.7
+    _check_grid(bk, oracle_mod, w)
+
+
+# --------------------------------------------------------------------------- blink_image
+@pytest.mark.parametrize("path", [0, 1])
+def test_image_config1_full(bk, oracle_mod, path):
+    from paper_2505_15204_b200 import workloads
+    w = workloads.make_config(1, device="cuda")
+    bk.set_option(bk.OPT_IMAGE_PATH, path)
+    try:
+        res = bk.blink_image(w.vis, w.uvw_m, w.freqs_hz, w.n_pix, w.pixscale_rad, w.weighting, want_cell_idx=True,
+                             want_counts=True)
+        torch.cuda.synchronize()
+    finally:
+        bk.set_option(bk.OPT_IMAGE_PATH, 0)
+    _check_images(bk, w, res, oracle_mod)
+    uvw = w.uvw_m.cpu().numpy()
+    assert np.array_equal(res["cell_idx"].cpu().numpy(), oracle_mod.cells(uvw, w.freqs_hz, w.n_pix, w.pixscale_rad))
+    r1 = oracle_mod.image_one(w.vis[0, 0, 0].cpu().numpy(), uvw[0], w.freqs_hz[0], w.n_pix, w.pixscale_rad, 0)
+    assert np.array_equal(res["counts"][0].cpu().numpy().astype(np.uint32), r1["cnt"])
+    # the brightest source of the synthetic sky is where the image peaks (sanity on orientation end to end)
+    img = res["image"][0].cpu().numpy()
+    s = w.sources
+    k = int(np.argmax(s["flux"]))
+    h = w.n_pix // 2
+    yx = np.unravel_index(np.argmax(img), img.shape)
+    assert abs(yx[1] - (h + s["l"][k] / w.pixscale_rad)) <= 1.5 and abs(yx[0] - (h + s["m"][k] / w.pixscale_rad)) <= 1.5
+
+
+@pytest.mark.parametrize("cfg,T,C", [(2, 1, 3), (3, 2, 3), (4, 1, 2), (5, 1, 2)])
+@pytest.mark.parametrize("path", [0, 1])
+def test_image_reduced_configs(bk, oracle_mod, cfg, T, C, path):
+    from paper_2505_15204_b200 import workloads
+    w = workloads.make_config(cfg, device="cuda", T=T, C=C)
+    bk.set_option(bk.OPT_IMAGE_PATH, path)
+    try:
+        res = bk.blink_image(w.vis, w.uvw_m, w.freqs_hz, w.n_pix, w.pixscale_rad, w.weighting, want_cell_idx=True)
+        torch.cuda.synchronize()
+    finally:
+        bk.set_option(bk.OPT_IMAGE_PATH, 0)
+    n_img = w.T * w.C * w.P
+    ids = np.arange(n_img) if w.n_pix <= 1024 else np.array([0, n_img - 1, n_img // 2])
+    _check_images(bk, w, res, oracle_mod, ids)
+    assert np.array_equal(res["cell_idx"].cpu().numpy(),
+                          oracle_mod.cells(w.uvw_m.cpu().numpy(), w.freqs_hz, w.n_pix, w.pixscale_rad))
+
+
+@pytest.mark.parametrize("weighting", [0, 1])
+@pytest.mark.parametrize("path", [0, 1])
+def test_image_random_ragged(bk, oracle_mod, weighting, path):
+    # odd sizes everywhere: B not a multiple of anything, P = 3, off-grid samples, tiny workspace (forces chunking)
+    from paper_2505_15204_b200 import workloads
+    w = workloads.make_random(T=3, C=5, P=3, B=1237, n_pix=128, weighting=weighting, seed=5, device="cuda", fill=1.2)
+    rec, mn = bk.blink_workspace_bytes(bk.OP_IMAGE, w.T, w.C, w.P, w.B, w.n_pix, weighting)
+    ws = torch.empty(max(mn * 2, 16), dtype=torch.uint8, device="cuda")
+    bk.set_option(bk.OPT_IMAGE_PATH, path)
+    try:
+        res = bk.blink_image(w.vis, w.uvw_m, w.freqs_hz, w.n_pix, w.pixscale_rad, weighting, workspace=ws)
+        torch.cuda.synchronize()
+    finally:
+        bk.set_option(bk.OPT_IMAGE_PATH, 0)
+    _check_images(bk, w, res, oracle_mod)
+
+
+def test_image_degenerate_inputs(bk, oracle_mod):
+    from paper_2505_15204_b200 import workloads
+    # everything off the grid -> W = 0, zero images, cell_idx = -1
+    w = workloads.make_random(T=1, C=2, P=1, B=64, n_pix=64, weighting=0, seed=1, device="cuda")
+    w.uvw_m[:] = 1e7
+    res = bk.blink_image(w.vis, w.uvw_m, w.freqs_hz, w.n_pix, w.pixscale_rad, 0, want_cell_idx=True)
+    torch.cuda.synchronize()
+    assert torch.all(res["image"] == 0) and torch.all(res["wsum"] == 0) and torch.all(res["cell_idx"] == -1)
+    # a single baseline: closed form 2|V| cos(...) / W with W = 2
+    w = workloads.make_random(T=1, C=1, P=1, B=1, n_pix=64, weighting=0, seed=2, device="cuda", fill=0.5)
+    res = bk.blink_image(w.vis, w.uvw_m, w.freqs_hz, w.n_pix, w.pixscale_rad, 0)
+    _check_images(bk, w, res, oracle_mod)
+    # NaN uvw is dropped, the rest still imaged
+    w = workloads.make_random(T=1, C=1, P=1, B=50, n_pix=64, weighting=1, seed=4, device="cuda", fill=0.5)
+    w.uvw_m[0, 7, 0] = float("nan")
+    res = bk.blink_image(w.vis, w.uvw_m, w.freqs_hz, w.n_pix, w.pixscale_rad, 1, want_cell_idx=True)
+    assert int(res["cell_idx"][0, 0, 7]) == -1
+    _check_images(bk, w, res, oracle_mod)
+
+
+def test_unit_source_peak_is_one(bk):
+    # north_star check 1 on the GPU path itself: all V = 1 -> centre pixel 1.0 and it is the maximum
+    from paper_2505_15204_b200 import workloads
+    w = workloads.make_config(1, device="cuda")
+    w.vis[:] = 1.0
+    for wt in (0, 1):
+        res = bk.blink_image(w.vis, w.uvw_m, w.freqs_hz, w.n_pix, w.pixscale_rad, wt)
+        img = res["image"][0].cpu().numpy()
+        h = w.n_pix // 2
+        assert abs(img[h, h] - 1.0) < 1e-5 and img.max() <= img[h, h] + 1e-6
+
+
+def test_error_codes(bk):
+    import ctypes
+    L = bk.lib()
+    x = torch.zeros(64, device="cuda")
+    fr = np.array([150e6])
+    p = lambda t: ctypes.c_void_p(t.data_ptr())
+    f = fr.ctypes.data_as(ctypes.c_void_p)
+    # n_pix not a power of two / too small / too large
+    for n in (48, 16, 8192):
+        assert L.blink_image(p(x), p(x), f, 1, 1, 1, 4, n, 0.01, 0, p(x), p(x), None, None, p(x), 64, None) == -2
+    assert L.blink_image(None, p(x), f, 1, 1, 1, 4, 32, 0.01, 0, p(x), p(x), None, None, p(x), 64, None) == -1
+    assert L.blink_image(p(x), p(x), f, 1, 1, 1, 4, 32, -1.0, 0, p(x), p(x), None, None, p(x), 64, None) == -1
+    assert L.blink_image(p(x), p(x), f, 1, 1, 1, 4, 32, 0.01, 7, p(x), p(x), None, None, p(x), 64, None) == -1
+    assert L.blink_fft2d_inverse(p(x), 100, 1, None, 1, p(x), None, None, 0, None) == -2
+    assert L.blink_strerror(-3).decode() == "workspace too small"
