@@ -1,0 +1,318 @@
+#!/usr/bin/env python
+"""bench.py -- headline benchmark of libblinkimg on B200.
+
+One "step" = one pass of the whole hot path (steps a0..a5 of SURVEY.md section 8(a)) over one batch of
+synthetic visibilities: blink_image() on BASELINE.json config 3 (50 timesteps x 768 channels -> 38400 dirty
+images of 512 x 512, 8128 baselines) -- the configuration the metric is quoted on.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 3] [--impl reference]
+
+Prints ONE JSON line.  value = dirty images/s (whole job), device-resident inputs; e2e = the same through
+blink_image_host() with pinned HOST buffers (H2D of visibilities and D2H of every image inside the timed
+region); roofline = algorithmic bytes (M36 = 36 N^2 + 8 B per image + 12 T B) / kernel time /
+measured HBM peak; cpu_baseline = the CPU oracle, as it stands, on a bounded sample.
+Multi-GPU (torchrun): every rank images its own independent batch ("replicas / independent shards",
+PAPER.md L150, L322: each second of observation is independent) -- weak scaling, no collective on the data path.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+import torch
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_2505_15204_b200 import workloads  # noqa: E402
+
+FALLBACK_HBM_GBS = 6650.0          # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
+
+
+def model_bytes(T, C, P, B, N):
+    """Algorithmic bytes of one step: per image vis read (8B) + grid written (8N^2) + row pass
+    read+write (16N^2) + column pass read (8N^2) + image written (4N^2); uvw read once per timestep."""
+    n_img = T * C * P
+    return {"M36": n_img * (36 * N * N + 8 * B) + 12 * T * B,
+            "M20": n_img * (20 * N * N + 8 * B) + 12 * T * B,
+            "M4": n_img * (4 * N * N + 8 * B) + 12 * T * B}
+
+
+def hbm_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def cpu_oracle_leg(w_small, target_s: float = 15.0):
+    """Times the CPU oracle (oracle/, as it stands) on a bounded sample of the SAME workload shape."""
+    import oracle
+    cores = os.cpu_count() or 1
+    vis, uvw = w_small.vis.cpu().numpy(), w_small.uvw_m.cpu().numpy()
+    n_avail = w_small.T * w_small.C * w_small.P
+    ids = np.arange(min(n_avail, 2 * cores))
+    t0 = time.perf_counter()
+    oracle.image_batch(vis, uvw, w_small.freqs_hz, w_small.n_pix, w_small.pixscale_rad, w_small.weighting, ids, nthreads=cores)
+    dt = time.perf_counter() - t0
+    per = dt / len(ids)
+    n = int(max(len(ids), min(n_avail, target_s / max(per, 1e-6))))
+    n = max(cores, (n // cores) * cores)
+    ids = np.arange(min(n, n_avail))
+    t0 = time.perf_counter()
+    oracle.image_batch(vis, uvw, w_small.freqs_hz, w_small.n_pix, w_small.pixscale_rad, w_small.weighting, ids, nthreads=cores)
+    dt = time.perf_counter() - t0
+    return {"value": len(ids) / dt, "unit": "images/s", "cores": cores, "kind": "oracle",
+            "sample": f"{len(ids)} images ({w_small.n_pix}x{w_small.n_pix}, {w_small.B} baselines) of the same workload, "
+                      f"{dt:.1f} s wall, one image per task on {cores} threads"}
+
+
+def sample_workload(cfg: int, n_images: int):
+    """A slice of config `cfg` on the CPU with ~n_images images (first timesteps, channels spread over the band)."""
+    shp = workloads.config_shape(cfg)
+    C = max(1, min(shp["C"], n_images // max(1, shp["P"])))
+    T = max(1, min(shp["T"], -(-n_images // (C * shp["P"]))))
+    return workloads.make_config(cfg, device="cpu", T=T, C=C)
+
+
+def run_reference(args, rank: int):
+    """--impl reference: the oracle itself on the host cores (bounded sample per step)."""
+    if rank != 0:
+        return
+    shp = workloads.config_shape(args.config)
+    cores = os.cpu_count() or 1
+    per_step = max(cores, 4 * cores)
+    w = sample_workload(args.config, per_step)
+    import oracle
+    vis, uvw = w.vis.numpy(), w.uvw_m.numpy()
+    ids = np.arange(min(per_step, w.T * w.C * w.P))
+    run = lambda: oracle.image_batch(vis, uvw, w.freqs_hz, w.n_pix, w.pixscale_rad, w.weighting, ids, nthreads=cores)
+    for _ in range(args.warmup):
+        run()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        run()
+    dt = (time.perf_counter() - t0) / args.steps
+    val = len(ids) / dt
+    sample = f"{len(ids)} images per step of config {args.config} ({w.n_pix}x{w.n_pix}, {w.B} baselines), {cores} threads"
+    print(json.dumps({
+        "impl": "reference", "metric": "dirty_images_per_s", "value": val, "unit": "images/s", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"config{args.config}: bounded sample of {shp['T']}x{shp['C']}x{shp['P']} images "
+                               f"{shp['n_pix']}x{shp['n_pix']}, B={shp['B']}", "sample": sample},
+        "cpu_baseline": {"value": val, "unit": "images/s", "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": "images/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=3)
+    ap.add_argument("--impl", default="blink")
+    ap.add_argument("--path", type=int, default=0, help="BLINK_OPT_IMAGE_PATH: 0 auto, 1 unfused, 2 fused")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--T", type=int, default=None, help="reduce timesteps (debug only; invalidates the headline)")
+    args = ap.parse_args()
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank)
+        return
+    if args.warmup < 3:
+        args.warmup = 3
+
+    import torch.distributed as dist
+    from paper_2505_15204_b200 import binding as bk
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    bk.lib()
+    bk.set_option(bk.OPT_IMAGE_PATH, args.path)
+
+    # independent batch per rank ("each second of observation can be processed independently")
+    w = workloads.make_config(args.config, device=dev, T=args.T, seed=None if rank == 0 else 1000 + args.config + 100 * rank)
+    T, C, P, B, N = w.T, w.C, w.P, w.B, w.n_pix
+    n_img = T * C * P
+    image = torch.empty((n_img, N, N), dtype=torch.float32, device=dev)
+    wsum = torch.empty(T * C, dtype=torch.float32, device=dev)
+    rec, mn = bk.blink_workspace_bytes(bk.OP_IMAGE, T, C, P, B, N, w.weighting)
+    ws = torch.empty(max(rec, 16), dtype=torch.uint8, device=dev)
+
+    def step():
+        bk.blink_image(w.vis, w.uvw_m, w.freqs_hz, N, w.pixscale_rad, w.weighting, image=image, workspace=ws, wsum=wsum)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    launches0 = bk.kernel_launches()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+    barrier()
+    ev[0].record()
+    for k in range(args.steps):
+        step()
+        ev[k + 1].record()
+    barrier()
+    launches = bk.kernel_launches() - launches0
+    clocks = sampler.stop() if rank == 0 else None
+    total_ms = ev[0].elapsed_time(ev[-1])
+    per_step = [ev[k].elapsed_time(ev[k + 1]) for k in range(args.steps)]
+    tmax = torch.tensor([total_ms], device=dev)
+    if world > 1:
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+    total_ms = float(tmax.item())
+    ms_per_step = total_ms / args.steps
+    value = world * n_img / (ms_per_step * 1e-3)
+
+    # ---- end to end through the host-buffer entry point (rank-local, then max over ranks) -----------------
+    e2e = None
+    if not args.no_e2e:
+        try:
+            vis_h = torch.empty(w.vis.shape, dtype=torch.complex64, pin_memory=True)
+            vis_h.copy_(w.vis)
+            uvw_h = torch.empty(w.uvw_m.shape, dtype=torch.float32, pin_memory=True)
+            uvw_h.copy_(w.uvw_m)
+            img_h = torch.empty((n_img, N, N), dtype=torch.float32, pin_memory=True)
+            wsum_h = torch.empty(T * C, dtype=torch.float32, pin_memory=True)
+            rec_h, _ = bk.blink_workspace_bytes(bk.OP_IMAGE_HOST, T, C, P, B, N, w.weighting)
+            del image
+            torch.cuda.empty_cache()
+            ws_h = torch.empty(rec_h, dtype=torch.uint8, device=dev)
+            e_steps = max(1, min(args.steps, 3))
+            bk.blink_image_host(vis_h, uvw_h, w.freqs_hz, N, w.pixscale_rad, w.weighting, img_h, wsum_h, ws_h)  # warm-up
+            barrier()
+            t0 = time.perf_counter()
+            for _ in range(e_steps):
+                bk.blink_image_host(vis_h, uvw_h, w.freqs_hz, N, w.pixscale_rad, w.weighting, img_h, wsum_h, ws_h)
+            barrier()
+            dt = torch.tensor([(time.perf_counter() - t0) / e_steps], device=dev)
+            if world > 1:
+                dist.all_reduce(dt, op=dist.ReduceOp.MAX)
+            e2e = {"value": world * n_img / float(dt.item()), "unit": "images/s",
+                   "h2d_bytes_per_step": int(vis_h.numel() * 8 + uvw_h.numel() * 4),
+                   "d2h_bytes_per_step": int(img_h.numel() * 4 + wsum_h.numel() * 4),
+                   "steps": e_steps, "ms_per_step": float(dt.item()) * 1e3,
+                   "api": "blink_image_host (pinned host buffers, per-timestep H2D/compute/D2H pipeline)"}
+            del img_h, vis_h, ws_h
+        except Exception as ex:  # report, never hide
+            e2e = {"value": None, "unit": "images/s", "error": str(ex)[:200]}
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    mb = model_bytes(T, C, P, B, N)
+    peak, peak_src = hbm_peak()
+    kern_ms = float(np.mean(per_step))
+    achieved = mb["M36"] / (kern_ms * 1e-3) / 1e9
+    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "traffic": None, "peak_source": peak_src,
+                "kernel": "blink_image step (all kernels of the step, CUDA events on the launch stream)",
+                "algorithmic_bytes_per_step": mb["M36"], "model": "M36 = n_img*(36 N^2 + 8 B) + 12 T B",
+                "frac_M20": mb["M20"] / (kern_ms * 1e-3) / 1e9 / peak, "frac_M4": mb["M4"] / (kern_ms * 1e-3) / 1e9 / peak,
+                "kernel_ms": kern_ms}
+    prof = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(prof):
+        try:
+            tj = json.load(open(prof))
+            key = f"config{args.config}_path{args.path}"
+            if key in tj:
+                roofline["traffic"] = tj[key]["dram_bytes_per_step"]
+                roofline["traffic_source"] = tj[key].get("source")
+        except Exception:
+            pass
+    cpu = None
+    if not args.no_cpu:
+        cores = os.cpu_count() or 1
+        cpu = cpu_oracle_leg(sample_workload(args.config, 64 * cores))
+    out = {
+        "metric": "dirty_images_per_s", "value": value, "unit": "images/s", "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": f"config{args.config}: {T} timesteps x {C} channels x {P} pol = {n_img} images of {N}x{N}, "
+                               f"{B} baselines, {'natural' if w.weighting == 0 else 'uniform'} weighting",
+                   "per_gpu_images": n_img, "l2": "inputs (vis %.2f GB) and outputs (%.1f GB) larger than L2; no flush" %
+                   (w.vis.numel() * 8 / 1e9, n_img * N * N * 4 / 1e9),
+                   "image_path": args.path, "parallelism": f"independent batches x{world}"},
+        "gvis_per_s": value * B / 1e9,
+        "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu,
+        "ms_per_step_each": per_step,
+    }
+    print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()
