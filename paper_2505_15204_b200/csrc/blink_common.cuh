@@ -49,6 +49,35 @@ constexpr int kMaxBaselines = (1 << 18) - 1;
 constexpr int kTwiddleN = 4096;
 const float2 *twiddle_table();          // device pointer (after ensure_device())
 
+// per-channel scales travel as a kernel parameter (<= 1024 channels per launch)
+struct ScaleBlock { float s[1024]; };
+
+#ifdef __CUDACC__
+// step a1 (R2, R4): nearest cell of one baseline, bit-exact twin of the oracle's fp32 recipe
+__device__ __forceinline__ bool cell_coords(float u_m, float v_m, float s, int h, int &iu, int &iv)
+{
+    const float x = __fmul_rn(u_m, s);            // one IEEE fp32 multiply, never contracted
+    const float y = __fmul_rn(v_m, s);
+    const float xr = rintf(x), yr = rintf(y);     // round to nearest, ties to even
+    const float lim = (float)(h - 1);
+    if (!(fabsf(xr) <= lim && fabsf(yr) <= lim)) return false;      // NaN fails
+    iu = (int)xr;
+    iv = (int)yr;
+    return true;
+}
+__device__ __forceinline__ int cell_of(float u_m, float v_m, float s, int n, int h)
+{
+    int iu, iv;
+    if (!cell_coords(u_m, v_m, s, h, iu, iv)) return -1;
+    return (iv + h) * n + (iu + h);
+}
+__device__ __forceinline__ int mirror_of(int cell, int n)
+{
+    const int r = cell / n, q = cell - r * n;
+    return (n - r) * n + (n - q);                 // (h - iv)*N + (h - iu)
+}
+#endif
+
 // --- internal entry points used across translation units ---------------------------------------
 // gridder over the flattened (t,c) range [tc0, tc0+ntc).  wsum / cell_idx are indexed by the absolute tc,
 // grid / counts by (tc - out_tc0) so that a chunk can land at the start of a workspace buffer.

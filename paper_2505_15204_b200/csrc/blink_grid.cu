@@ -11,24 +11,6 @@ namespace blink {
 
 constexpr int kGridThreads = 512;
 constexpr int kTileCellsMax = 8192;               // 64 KB of complex64 per band tile
-constexpr int kItemBLocalBits = 18;
-
-struct ScaleBlock { float s[1024]; };
-
-__device__ __forceinline__ int cell_of(float u_m, float v_m, float s, int n, int h)
-{
-    const float x = __fmul_rn(u_m, s);            // one IEEE fp32 multiply, never contracted
-    const float y = __fmul_rn(v_m, s);
-    const float xr = rintf(x), yr = rintf(y);     // round to nearest, ties to even
-    const float lim = (float)(h - 1);
-    if (!(fabsf(xr) <= lim && fabsf(yr) <= lim)) return -1;      // NaN fails
-    return ((int)yr + h) * n + ((int)xr + h);
-}
-__device__ __forceinline__ int mirror_of(int cell, int n)
-{
-    const int r = cell / n, q = cell - r * n;
-    return (n - r) * n + (n - q);                 // (h - iv)*N + (h - iu)
-}
 
 struct GridArgs {
     const float2 *vis; const float *uvw_m;
