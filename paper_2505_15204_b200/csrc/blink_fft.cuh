@@ -122,27 +122,63 @@ struct ExchangeDense2 {
 };
 
 // ---------------------------------------------------------------------------------------------
+// Per-thread twiddle registers.  Which twiddles a thread needs depends only on (tid, stage, butterfly),
+// never on the data, so they are read ONCE per kernel from the W_4096 table (built in double on the
+// host) and kept in registers: per stage > 0 and butterfly q the powers w^1, w^2 (and w^4 for radix 8)
+// of w = exp(+2 pi i k / (P R)); the remaining powers are products of those (<= 2 extra roundings).
+// ---------------------------------------------------------------------------------------------
+template <int N>
+struct Twiddles {
+    static constexpr int S = plan_stages(N);
+    float2 w[S > 1 ? S - 1 : 1][2][3];                  // [stage-1][butterfly q][w1, w2, w4]
+
+    template <int ST, int P>
+    __device__ __forceinline__ void init_stage(int tid, const float2 *__restrict__ tw)
+    {
+        if constexpr (ST < S) {
+            constexpr int R = plan_radix(N, ST);
+            constexpr int TG = N / kE;
+            constexpr int NB = kE / R;
+            if constexpr (ST > 0) {
+                constexpr int step = kTwiddleNConst() / (P * R);
+#pragma unroll
+                for (int q = 0; q < NB; ++q) {
+                    const int k = (tid + q * TG) & (P - 1);
+                    w[ST - 1][q][0] = __ldg(tw + k * step);
+                    w[ST - 1][q][1] = __ldg(tw + 2 * k * step);
+                    if constexpr (R == 8) w[ST - 1][q][2] = __ldg(tw + 4 * k * step);
+                }
+            }
+            init_stage<ST + 1, P * R>(tid, tw);
+        }
+    }
+    __device__ __forceinline__ void init(int tid, const float2 *__restrict__ tw) { init_stage<0, 1>(tid, tw); }
+};
+
 // One stage: twiddle (skipped when P == 1), radix-R butterflies in registers.
 //   v[nv][e] holds x[tid + e*TG].  Butterfly q (q = 0..8/R-1) is i = tid + q*TG and uses slots
-//   e = q + r*(8/R), r = 0..R-1.  Twiddle of input r: exp(+2 pi i r k / (P R)), k = i mod P, read
-//   from the W_4096 table `tw` (tw[m] = exp(+2 pi i m / 4096)).
-// ---------------------------------------------------------------------------------------------
-template <int N, int NV, int R, int P>
-__device__ __forceinline__ void stage_compute(float2 (&v)[NV][kE], int tid, const float2 *__restrict__ tw)
+//   e = q + r*(8/R), r = 0..R-1.  Twiddle of input r: w^r, w = exp(+2 pi i k / (P R)), k = i mod P.
+template <int N, int NV, int R, int P, int ST>
+__device__ __forceinline__ void stage_compute(float2 (&v)[NV][kE], const Twiddles<N> &twr)
 {
-    constexpr int TG = N / kE;
     constexpr int NB = kE / R;                         // butterflies per thread
 #pragma unroll
     for (int q = 0; q < NB; ++q) {
-        const int i = tid + q * TG;
         if constexpr (P > 1) {
-            const int k = i & (P - 1);
-            constexpr int step = kTwiddleNConst() / (P * R);
+            float2 wp[R];
+            wp[1] = twr.w[ST - 1][q][0];
+            wp[2] = twr.w[ST - 1][q][1];
+            wp[3] = cmul(wp[1], wp[2]);
+            if constexpr (R == 8) {
+                wp[4] = twr.w[ST - 1][q][2];
+                wp[5] = cmul(wp[1], wp[4]);
+                wp[6] = cmul(wp[2], wp[4]);
+                wp[7] = cmul(wp[3], wp[4]);
+            }
 #pragma unroll
             for (int r = 1; r < R; ++r) {
-                const float2 w = __ldg(tw + r * k * step);
 #pragma unroll
-                for (int nv = 0; nv < NV; ++nv) v[nv][q + r * NB] = cmul(v[nv][q + r * NB], w);
+                for (int nv = 0; nv < NV; ++nv) v[nv][q + r * NB] = cmul(v[nv][q + r * NB], wp[r]);
             }
         }
 #pragma unroll
@@ -197,17 +233,17 @@ __device__ __forceinline__ void stage_get(float2 (&v)[NV][kE], int tid, const X 
 
 template <int N, int NV, int S, int P, class X, class Sync>
 struct FftStages {
-    __device__ __forceinline__ static void run(float2 (&v)[NV][kE], int tid, const X &xch,
-                                               const float2 *__restrict__ tw, Sync sync)
+    __device__ __forceinline__ static void run(float2 (&v)[NV][kE], int tid, const X &xch, const Twiddles<N> &twr,
+                                               Sync sync)
     {
         constexpr int R = plan_radix(N, S);
-        stage_compute<N, NV, R, P>(v, tid, tw);
+        stage_compute<N, NV, R, P, S>(v, twr);
         if constexpr (S + 1 < plan_stages(N)) {
             sync();                                      // everyone has finished reading the array
             stage_put<N, NV, R, P, X>(v, tid, xch);
             sync();                                      // all writes visible
             stage_get<N, NV, X>(v, tid, xch);
-            FftStages<N, NV, S + 1, P * R, X, Sync>::run(v, tid, xch, tw, sync);
+            FftStages<N, NV, S + 1, P * R, X, Sync>::run(v, tid, xch, twr, sync);
         }
         // last stage: output j + r*P with P = N/R is again slot layout tid + e*TG -- nothing to move
     }
@@ -218,10 +254,10 @@ struct FftStages {
 // NOTE: the first sync() also orders the caller's last reads of the exchange array (e.g. the
 // initial load out of a TMA tile that doubles as the exchange array) before the first put.
 template <int N, int NV, class X, class Sync>
-__device__ __forceinline__ void fft_inverse(float2 (&v)[NV][kE], int tid, const X &xch,
-                                            const float2 *__restrict__ tw, Sync sync)
+__device__ __forceinline__ void fft_inverse(float2 (&v)[NV][kE], int tid, const X &xch, const Twiddles<N> &twr,
+                                            Sync sync)
 {
-    FftStages<N, NV, 0, 1, X, Sync>::run(v, tid, xch, tw, sync);
+    FftStages<N, NV, 0, 1, X, Sync>::run(v, tid, xch, twr, sync);
 }
 
 }  // namespace blink

@@ -33,6 +33,8 @@ fft_rows_kernel(float2 *__restrict__ grid, long long n_rows, const float2 *__res
     const int tid = threadIdx.x % Cfg::TG;
     ExchangePadded1 xch{xbuf + (size_t)g * Cfg::SLOTS};
     auto sync = [] { __syncthreads(); };
+    Twiddles<N> twr;
+    twr.init(tid, tw);
     for (long long base = (long long)blockIdx.x * Cfg::G; base < n_rows; base += (long long)gridDim.x * Cfg::G) {
         const long long row = base + g;
         const bool valid = row < n_rows;
@@ -41,7 +43,7 @@ fft_rows_kernel(float2 *__restrict__ grid, long long n_rows, const float2 *__res
 #pragma unroll
         for (int e = 0; e < kE; ++e)                                   // transform index n = tid + e*TG lives in column n ^ h
             v[0][e] = valid ? p[tid + (e ^ (kE / 2)) * Cfg::TG] : make_float2(0.f, 0.f);
-        fft_inverse<N, 1>(v, tid, xch, tw, sync);
+        fft_inverse<N, 1>(v, tid, xch, twr, sync);
         if (valid) {
 #pragma unroll
             for (int e = 0; e < kE; ++e) p[tid + e * Cfg::TG] = v[0][e];
@@ -80,8 +82,9 @@ fft_cols_kernel(const __grid_constant__ CUtensorMap tmap, const float *__restric
 {
     using Cfg = ColCfg<N>;
     constexpr int h = N / 2;
-    extern __shared__ unsigned char smem_raw[];
-    unsigned char *tile = reinterpret_cast<unsigned char *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+    extern __shared__ __align__(1024) unsigned char smem_raw[];
+    // keep the pointer in the shared window (pointer arithmetic on the array, no integer round trip)
+    unsigned char *tile = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
     uint64_t *bar = reinterpret_cast<uint64_t *>(tile + Cfg::TILE_BYTES);
 
     const int col0 = blockIdx.x * Cfg::KC;                             // first (natural-order) column of the tile
@@ -112,7 +115,9 @@ fft_cols_kernel(const __grid_constant__ CUtensorMap tmap, const float *__restric
         v[1][e] = make_float2(t.z, t.w);
     }
     auto sync = [] { __syncthreads(); };
-    fft_inverse<N, 2>(v, tid, xch, tw, sync);
+    Twiddles<N> twr;
+    twr.init(tid, tw);
+    fft_inverse<N, 2>(v, tid, xch, twr, sync);
 
     // epilogue: scale, real part, fftshift (y = ky ^ h, x = kx ^ h), transposed through shared memory
     float s = 1.0f;

@@ -9,7 +9,7 @@ namespace blink {
 
 // fused path (blink_fused.cu)
 bool fused_supported(int P, int B, int n_pix, int weighting);
-size_t fused_workspace_bytes(int n_pix, int ctas);
+size_t fused_workspace_bytes(int T, int B, int n_pix, int ctas);
 int fused_default_ctas();
 int fused_image(const float2 *vis, const float *uvw_m, const double *freqs_hz, double pixscale_rad, int T, int C,
                 int P, int B, int n_pix, int weighting, int tc0, int ntc, float *image, float *wsum,
@@ -99,8 +99,8 @@ extern "C" int blink_workspace_bytes(int op, int T, int C, int P, int B, int n_p
             if (use_fused(P, B, n_pix, weighting)) {
                 int ctas = option(BLINK_OPT_FUSED_CTAS);
                 if (ctas <= 0) ctas = fused_default_ctas();
-                rec = fused_workspace_bytes(n_pix, ctas);
-                mn = fused_workspace_bytes(n_pix, 1);
+                rec = fused_workspace_bytes(T, B, n_pix, ctas);
+                mn = fused_workspace_bytes(T, B, n_pix, 1);
             } else {
                 const size_t per_tc = unfused_bytes_per_tc(P, B, n_pix, weighting, false);
                 mn = per_tc;
