@@ -66,13 +66,18 @@ __device__ __forceinline__ void dft8(float2 (&x)[8])
 // ---------------------------------------------------------------------------------------------
 // Exchange policies: where position w (0..N-1) of the group's vector(s) lives in shared memory.
 // ---------------------------------------------------------------------------------------------
-// One vector, float2 elements, one padding element every 8 (conflict-free for the stride-8 stores
-// of the first stage and the unit-stride loads).
+// XOR swizzle for arrays of 8-byte elements (16 per 128-byte bank row; a 64-bit access is served per
+// half warp).  Position w lives in slot xsw(w): bits 4..6 of w are folded into bits 0..2 and bit 6 also
+// into bit 3, so the 16 lanes of a half warp hit 16 different bank pairs for the unit-stride loads AND for
+// the stride-8 / stride-64 Stockham stores (padding w + w/8 cost a second wavefront on every load:
+// profiles/r1_fused.md capture b).  No padding: an N-element vector takes N slots.
+__device__ __forceinline__ int xsw(int w) { return w ^ ((w >> 4) & 7) ^ (((w >> 6) & 1) << 3); }
+
+// One vector, float2 elements.
 struct ExchangePadded1 {
     float2 *base;
-    __device__ __forceinline__ static int slots(int n) { return n + (n >> 3); }
-    __device__ __forceinline__ void put(int w, const float2 (&v)[1]) const { base[w + (w >> 3)] = v[0]; }
-    __device__ __forceinline__ void get(int w, float2 (&v)[1]) const { v[0] = base[w + (w >> 3)]; }
+    __device__ __forceinline__ void put(int w, const float2 (&v)[1]) const { base[xsw(w)] = v[0]; }
+    __device__ __forceinline__ void get(int w, float2 (&v)[1]) const { v[0] = base[xsw(w)]; }
 };
 
 // Two vectors (a column pair), float4 elements living INSIDE a TMA-written tile whose rows are

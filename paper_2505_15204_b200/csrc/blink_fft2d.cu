@@ -18,7 +18,7 @@ struct RowCfg {
     static constexpr int TG = N / kE;                                  // threads per row
     static constexpr int THREADS = TG > 256 ? TG : 256;
     static constexpr int G = THREADS / TG;                             // rows in flight per CTA
-    static constexpr int SLOTS = N + (N >> 3);
+    static constexpr int SLOTS = N;
     static constexpr size_t SMEM = (size_t)G * SLOTS * sizeof(float2);
 };
 

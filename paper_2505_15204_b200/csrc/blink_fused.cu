@@ -30,7 +30,7 @@ struct FusedCfg {
     static constexpr int G = kFusedThreads / TG;               // groups per CTA
     static constexpr int KU = 2 * G;                           // u-columns per pass-1 tile (2 per group)
     static constexpr int NT = H / KU;                          // pass-1 tiles in the half plane
-    static constexpr int SLOTS = N + (N >> 3);                 // padded column length
+    static constexpr int SLOTS = N;                            // column length (XOR-swizzled, no padding)
     static constexpr int KY = (8192 / N) < 16 ? (8192 / N) : 16;   // ky rows per pass-2 stage
     static constexpr int ROWB = KY * 8;                        // stage row bytes (= TMA swizzle span)
     static constexpr int PAIRS = KY / 2;
@@ -57,13 +57,13 @@ struct ExchangePadded2 {
     float2 *c0, *c1;
     __device__ __forceinline__ void put(int w, const float2 (&v)[2]) const
     {
-        const int o = w + (w >> 3);
+        const int o = xsw(w);
         c0[o] = v[0];
         c1[o] = v[1];
     }
     __device__ __forceinline__ void get(int w, float2 (&v)[2]) const
     {
-        const int o = w + (w >> 3);
+        const int o = xsw(w);
         v[0] = c0[o];
         v[1] = c1[o];
     }
@@ -178,7 +178,12 @@ fused_image_kernel(const FusedArgs a, const __grid_constant__ ScaleBlock sc, con
     const int tid = threadIdx.x % TG;
     const int lane = threadIdx.x & 31;
     float2 *scratch = a.scratch + (size_t)blockIdx.x * H * N;
-    auto sync = [] { __syncthreads(); };
+    // barrier over ONE transform group (its columns / exchange buffer are private to it)
+    auto sync = [g] {
+        if constexpr (TG == 32) __syncwarp();
+        else if constexpr (Cfg::G <= 15) asm volatile("bar.sync %0, %1;" ::"r"(g + 1), "r"(TG) : "memory");
+        else __syncthreads();
+    };
     const float lim = (float)(H - 1);
 
     if (threadIdx.x == 0) {
@@ -273,8 +278,8 @@ fused_image_kernel(const FusedArgs a, const __grid_constant__ ScaleBlock sc, con
                                 if (bb >> 31) vv.y = -vv.y;
                                 v[m] = vv;
                                 const int ul = iu - tl * KU, row = iv + H;
-                                o[m] = ul * SLOTS + row + (row >> 3);
-                                if (iu == 0) { const int row2 = H - iv; o2[m] = row2 + (row2 >> 3); }
+                                o[m] = ul * SLOTS + xsw(row);
+                                if (iu == 0) { const int row2 = H - iv; o2[m] = xsw(row2); }
                                 ++my_in;
                             }
                         }
@@ -335,8 +340,8 @@ fused_image_kernel(const FusedArgs a, const __grid_constant__ ScaleBlock sc, con
 #pragma unroll
                     for (int e = 0; e < kE; ++e) {                              // transform index n lives in centred row n ^ H
                         const int r = tid + (e ^ (kE / 2)) * TG;
-                        v[0][e] = c0[r + (r >> 3)];
-                        v[1][e] = c1[r + (r >> 3)];
+                        v[0][e] = c0[xsw(r)];
+                        v[1][e] = c1[xsw(r)];
                     }
                     fft_inverse<N, 2>(v, tid, xch, twr, sync);
                     float2 *d0 = scratch + (size_t)(tl * KU + 2 * g) * N, *d1 = d0 + N;
@@ -398,18 +403,15 @@ fused_image_kernel(const FusedArgs a, const __grid_constant__ ScaleBlock sc, con
                         if (u < ulim && u < H) q = *st.at_row(u);
                         z[0][e] = make_float2(q.x + q.w, q.z - q.y);
                     }
-                } else {
-#pragma unroll
-                    for (int e = 0; e < kE; ++e) z[0][e] = make_float2(0.f, 0.f);
                 }
                 __syncthreads();                                                // everyone has read this stage buffer
                 if (threadIdx.x == 0 && it + 2 < Cfg::NIT) {
                     fence_proxy_async();
                     issue(it + 2);
                 }
-                ExchangePadded1 xch{xbuf + (size_t)g * SLOTS};
-                fft_inverse<N, 1>(z, tid, xch, twr, sync);
                 if (g < Cfg::PAIRS) {
+                    ExchangePadded1 xch{xbuf + (size_t)g * SLOTS};
+                    fft_inverse<N, 1>(z, tid, xch, twr, sync);
                     const int ky = it * Cfg::KY + 2 * g;
                     float *r0 = img + (size_t)(ky ^ H) * N, *r1 = img + (size_t)((ky + 1) ^ H) * N;
 #pragma unroll
