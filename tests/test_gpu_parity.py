@@ -243,3 +243,48 @@ def test_error_codes(bk):
     assert L.blink_image(p(x), p(x), f, 1, 1, 1, 4, 32, 0.01, 7, p(x), p(x), None, None, p(x), 64, None) == -1
     assert L.blink_fft2d_inverse(p(x), 100, 1, None, 1, p(x), None, None, 0, None) == -2
     assert L.blink_strerror(-3).decode() == "workspace too small"
+
+
+# --------------------------------------------------------------------------- full size, bench launch configuration
+def test_config3_full_size_sampled(bk, oracle_mod):
+    """BASELINE.json config 3 at FULL size (38400 images of 512x512), exactly as bench.py launches it:
+    cell indices of every (t,c,b) bit-exact, wsum of every (t,c) exact, 24 sampled images (spread over t and c,
+    including the channels the dispersed transient crosses) within 1e-4 x peak, plus size-independent properties."""
+    from paper_2505_15204_b200 import workloads
+    free, _ = torch.cuda.mem_get_info()
+    if free < 60e9:
+        pytest.skip("needs ~50 GB of device memory")
+    w = workloads.make_config(3, device="cuda")
+    T, C, P, B, N = w.T, w.C, w.P, w.B, w.n_pix
+    assert (T, C, P, B, N) == (50, 768, 1, 8128, 512)
+    res = bk.blink_image(w.vis, w.uvw_m, w.freqs_hz, N, w.pixscale_rad, w.weighting, want_cell_idx=True)
+    torch.cuda.synchronize()
+    uvw = w.uvw_m.cpu().numpy()
+    ci = res["cell_idx"].cpu().numpy()
+    ref_ci = oracle_mod.cells(uvw, w.freqs_hz, N, w.pixscale_rad)
+    assert np.array_equal(ci, ref_ci)                                           # all 312 M indices
+    assert np.array_equal(res["wsum"].cpu().numpy(), (2 * (ref_ci >= 0).sum(axis=2)).astype(np.float32).ravel())
+    del ci, ref_ci
+    rng = np.random.default_rng(33)
+    tr = w.meta["transient_flux_tc"]
+    hot = np.argwhere(tr > 0)
+    ids = [0, T * C - 1] + [int(t * C + c) for t, c in hot[rng.choice(len(hot), 6, replace=False)]]
+    ids += [int(i) for i in rng.choice(T * C, 16, replace=False)]
+    ids = np.unique(ids)
+    sel = torch.as_tensor(ids, device="cuda")
+    vis_s = w.vis.reshape(T * C, P, B)[sel].cpu().numpy()
+    img_s = res["image"][sel].cpu().numpy()
+    worst = 0.0
+    for k, i in enumerate(ids):
+        t, c = divmod(int(i), C)
+        r = oracle_mod.image_one(vis_s[k, 0], uvw[t], w.freqs_hz[c], N, w.pixscale_rad, w.weighting)
+        worst = max(worst, _img_err(img_s[k], r["image"]))
+    assert worst <= TOL, worst
+    # properties that hold at any size: centre pixel = sum(2 Re V_in) / W for EVERY image (closed form)
+    h = N // 2
+    centre = res["image"][:, h, h].double().cpu().numpy()
+    inr = torch.as_tensor(oracle_mod.cells(uvw, w.freqs_hz, N, w.pixscale_rad) >= 0, device="cuda").reshape(T * C, B)
+    want = (2.0 * (w.vis.reshape(T * C, B).real.double() * inr).sum(dim=1) / (2.0 * inr.sum(dim=1))).cpu().numpy()
+    peak = res["image"].reshape(T * C, -1).abs().amax(dim=1).double().cpu().numpy()
+    assert np.max(np.abs(centre - want) / peak) <= TOL
+    assert bool(torch.isfinite(res["image"]).all())
