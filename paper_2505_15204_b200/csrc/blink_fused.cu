@@ -3,16 +3,18 @@
 // What makes this possible:
 //   * the gridded plane is Hermitian, G[-v][-u] = conj(G[v][u]) (every sample is gridded with its conjugate,
 //     reading R1), so only the half plane u >= 0 is gridded: N x N/2 cells (column u = N/2 is always empty, R4);
-//   * pass 1 transforms that half plane along v, one u-column at a time, in shared memory, and leaves
-//     H[u][ky] (N/2 x N complex64) in a per-CTA scratch in global memory (L2-resident at N = 512);
+//   * pass 1 grids and transforms that half plane along v, one u-column PAIR per transform group, in shared
+//     memory, and leaves H[u][ky] (N/2 x N complex64) in a per-CTA scratch in global memory (L2-resident);
 //   * pass 2 turns row pairs (ky, ky+1) into TWO real image rows with ONE N-point complex transform:
 //     Z[n] = S1[n] + i S2[n] (n < N/2), Z[N-n] = conj(S1[n]) + i conj(S2[n]);  Re z = row ky, Im z = row ky+1.
-//     Its input tiles [KY ky][N/2 u] are TRANSPOSED reads of the scratch, staged by TMA (128B-swizzled),
-//     double-buffered behind an mbarrier pipeline; the fftshift (index XOR N/2), the 1/W normalisation and the
+//     Its input tiles [KY ky][N/2 u] are TRANSPOSED reads of the scratch, staged by TMA (128B-swizzled) through a
+//     3-stage full/empty mbarrier pipeline; the fftshift (index XOR N/2), the 1/W normalisation and the
 //     real-part extraction are part of the store.
-// One persistent CTA per SM walks over (t,c) work items; per item it computes the cell indices once (bit-exact
-// twin of the oracle), bins the samples by u-tile with a counting sort in shared memory, and reuses the bins
-// for all P polarisations.  PAPER.md L190-194 (gridding, batched inverse 2D FFT, shift); L150 (fp32).
+// One persistent CTA per SM walks over (t,c) work items.  Inside a pass the transform groups (N/8 threads each)
+// run DECOUPLED: a group grids its own two columns with shared-memory atomics (the samples of a column are one
+// contiguous range of the per-timestep |u|-sorted baseline list), transforms them and moves on; only three
+// CTA-wide barriers per image remain.  The next image's visibility row is prefetched with a bulk async copy
+// while pass 2 runs.  PAPER.md L190-194 (gridding, batched inverse 2D FFT, shift); L150 (fp32).
 #include <algorithm>
 
 #include "blink_common.cuh"
@@ -26,21 +28,20 @@ constexpr int kFusedThreads = 512;
 template <int N>
 struct FusedCfg {
     static constexpr int H = N / 2;
-    static constexpr int TG = N / kE;                          // threads per transform
+    static constexpr int TG = N / kE;                          // threads per transform group
     static constexpr int G = kFusedThreads / TG;               // groups per CTA
-    static constexpr int KU = 2 * G;                           // u-columns per pass-1 tile (2 per group)
-    static constexpr int NT = H / KU;                          // pass-1 tiles in the half plane
-    static constexpr int SLOTS = N;                            // column length (XOR-swizzled, no padding)
-    static constexpr int KY = (8192 / N) < 16 ? (8192 / N) : 16;   // ky rows per pass-2 stage
-    static constexpr int ROWB = KY * 8;                        // stage row bytes (= TMA swizzle span)
-    static constexpr int PAIRS = KY / 2;
+    static constexpr int KY = (8192 / N) < 16 ? (8192 / N) : 16;   // ky rows per pass-2 sub-tile
+    static constexpr int ROWB = KY * 8;                        // sub-tile row bytes (= TMA swizzle span)
+    static constexpr int PPS = KY / 2;                         // row pairs per sub-tile
+    static constexpr int NSUB = G / PPS;                       // sub-tiles per stage: every group gets a pair
+    static constexpr int KYS = KY * NSUB;                      // ky rows per stage
+    static constexpr int NIT = N / KYS;                        // pass-2 stages per image
     static constexpr int BOX_ROWS = H < 256 ? H : 256;
-    static constexpr int NBOX = H / BOX_ROWS;
-    static constexpr int STAGE_BYTES = H * ROWB;
-    static constexpr int NIT = N / KY;                         // pass-2 stages per image
-    static constexpr int LOG_TILE = 13;                        // KU * N == 8192 cells per tile
-    static_assert(KU * N == 8192, "tile is 8192 cells");
-    static_assert(PAIRS <= G, "one pair per group per stage");
+    static constexpr int SUB_BYTES = H * ROWB;
+    static constexpr int STAGE_BYTES = NSUB * SUB_BYTES;       // 32 KB for every N
+    static constexpr int COL_BYTES = G * 2 * N * 8;            // pass-1 column pairs of all groups (64 KB)
+    static_assert(NSUB >= 1 && NSUB * PPS == G, "one row pair per group per stage");
+    static_assert(SUB_BYTES % 1024 == 0, "swizzled sub-tiles stay 1024-byte aligned");
 };
 
 struct FusedArgs {
@@ -69,26 +70,34 @@ struct ExchangePadded2 {
     }
 };
 
+// shared memory: vis row [B] float2 | column offsets [H+2] | pad to 1024 |
+//                union(pass 1: column pairs (+ counts), pass 2: NS stages + exchange arrays) | mbarriers
 template <int N>
-__host__ __device__ constexpr size_t fused_region_bytes(bool uniform)
+__host__ __device__ constexpr size_t fused_region_bytes(bool uniform, int ns)
 {
     using Cfg = FusedCfg<N>;
-    const size_t p1 = (size_t)Cfg::KU * Cfg::SLOTS * (uniform ? 12 : 8);
-    const size_t p2 = 2 * (size_t)Cfg::STAGE_BYTES + (size_t)Cfg::G * Cfg::SLOTS * 8;
+    const size_t p1 = (size_t)Cfg::COL_BYTES + (uniform ? (size_t)Cfg::COL_BYTES / 2 : 0);
+    const size_t p2 = (size_t)ns * Cfg::STAGE_BYTES + (size_t)Cfg::G * N * 8;
     return p1 > p2 ? p1 : p2;
 }
-// shared memory: vis row [B] float2 | tile offsets [NT+1] | owner ids [KU*SLOTS] u16 | pad to 1024 |
-//                union(pass-1 tile (+counts), pass-2 stages + exchange) | mbarriers
 template <int N>
 __host__ __device__ constexpr size_t fused_front_bytes(int B)
 {
-    using Cfg = FusedCfg<N>;
-    return (size_t)B * 8 + (size_t)(Cfg::NT + 1) * 4 + (size_t)Cfg::KU * Cfg::SLOTS * 2;
+    return (((size_t)B * 8 + 15) & ~(size_t)15) + (size_t)(FusedCfg<N>::H + 2) * 4;
 }
 template <int N>
-static size_t fused_smem_bytes(int B, bool uniform)
+static size_t fused_smem_bytes(int B, bool uniform, int ns)
 {
-    return align_up(fused_front_bytes<N>(B), 1024) + fused_region_bytes<N>(uniform) + 1024 + 64;
+    return align_up(fused_front_bytes<N>(B), 1024) + fused_region_bytes<N>(uniform, ns) + 1024 + 128;
+}
+constexpr size_t kSmemLimit = 227 * 1024;
+// pipeline depth that fits next to the visibility row: 3 stages, else 2, else 0 (not supported)
+template <int N>
+static int fused_stages(int B, bool uniform)
+{
+    if (fused_smem_bytes<N>(B, uniform, 3) <= kSmemLimit) return 3;
+    if (fused_smem_bytes<N>(B, uniform, 2) <= kSmemLimit) return 2;
+    return 0;
 }
 
 // ------------------------------------------------------------------------------------------ presort
@@ -149,210 +158,199 @@ presort_kernel(const float *__restrict__ uvw_m, int B, int np2, float *__restric
 }
 
 // ------------------------------------------------------------------------------------------ fused kernel
-template <int N>
+template <int N, int NS>
 __global__ void __launch_bounds__(kFusedThreads, 1)
 fused_image_kernel(const FusedArgs a, const __grid_constant__ ScaleBlock sc, const __grid_constant__ CUtensorMap tmap)
 {
     using Cfg = FusedCfg<N>;
-    constexpr int H = Cfg::H, TG = Cfg::TG, KU = Cfg::KU, NT = Cfg::NT, SLOTS = Cfg::SLOTS;
-    constexpr int IT = 2;                                      // samples per thread per accumulation round
+    constexpr int H = Cfg::H, TG = Cfg::TG, G = Cfg::G;
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     const bool uniform = a.weighting == BLINK_W_UNIFORM;
     const int B = a.B;
-
-    // ---- shared memory carve-up (pointer arithmetic on the array keeps every access in the shared window) ----
-    float2 *visrow = reinterpret_cast<float2 *>(smem_raw);                     // [B]
-    uint32_t *toff = reinterpret_cast<uint32_t *>(smem_raw + (size_t)B * 8);   // [NT+1]
-    unsigned short *own = reinterpret_cast<unsigned short *>(smem_raw + (size_t)B * 8 + (size_t)(NT + 1) * 4);
-    const uint32_t front = (uint32_t)fused_front_bytes<N>(B);
-    const uint32_t base_addr = smem_u32(smem_raw);
-    unsigned char *region = smem_raw + (((base_addr + front + 1023u) & ~1023u) - base_addr);
-    float2 *tile = reinterpret_cast<float2 *>(region);                         // pass 1: [KU][SLOTS]
-    uint32_t *cnt = reinterpret_cast<uint32_t *>(region + (size_t)KU * SLOTS * 8);   // pass 1 (uniform)
-    unsigned char *stage = region;                                             // pass 2: [2][STAGE_BYTES]
-    float2 *xbuf = reinterpret_cast<float2 *>(region + 2 * (size_t)Cfg::STAGE_BYTES);   // pass 2: [G][SLOTS]
-    uint64_t *bars = reinterpret_cast<uint64_t *>(region + fused_region_bytes<N>(uniform));   // full[2]
-    __shared__ int s_nin, s_occ;
-
     const int g = threadIdx.x / TG;
     const int tid = threadIdx.x % TG;
     const int lane = threadIdx.x & 31;
+
+    // ---- shared memory carve-up (pointer arithmetic on the array keeps every access in the shared window) ----
+    float2 *visrow = reinterpret_cast<float2 *>(smem_raw);                                        // [B]
+    uint32_t *coff = reinterpret_cast<uint32_t *>(smem_raw + (((size_t)B * 8 + 15) & ~(size_t)15));   // [H+2]
+    const uint32_t front = (uint32_t)fused_front_bytes<N>(B);
+    const uint32_t base_addr = smem_u32(smem_raw);
+    unsigned char *region = smem_raw + (((base_addr + front + 1023u) & ~1023u) - base_addr);
+    // pass 1: this group's column pair (XOR-swizzled slots) and, for uniform weighting, its cell counts
+    float2 *c0 = reinterpret_cast<float2 *>(region) + (size_t)g * 2 * N, *c1 = c0 + N;
+    uint32_t *n0 = reinterpret_cast<uint32_t *>(region + Cfg::COL_BYTES) + (size_t)g * 2 * N, *n1 = n0 + N;
+    // pass 2: NS stages of transposed scratch tiles, then one exchange array per group
+    unsigned char *stage = region;
+    float2 *xbuf = reinterpret_cast<float2 *>(region + (size_t)NS * Cfg::STAGE_BYTES) + (size_t)g * N;
+    uint64_t *full = reinterpret_cast<uint64_t *>(region + fused_region_bytes<N>(uniform, NS));   // [NS]
+    uint64_t *empty = full + NS;                                                                  // [NS]
+    uint64_t *visbar = empty + NS;
+    __shared__ int s_nin, s_occ, s_ncol;
+
     float2 *scratch = a.scratch + (size_t)blockIdx.x * H * N;
-    // barrier over ONE transform group (its columns / exchange buffer are private to it)
-    auto sync = [g] {
+    // barrier over ONE transform group (its columns / exchange array are private to it)
+    auto gsync = [g] {
         if constexpr (TG == 32) __syncwarp();
-        else if constexpr (Cfg::G <= 15) asm volatile("bar.sync %0, %1;" ::"r"(g + 1), "r"(TG) : "memory");
+        else if constexpr (G <= 15 && G > 1) asm volatile("bar.sync %0, %1;" ::"r"(g + 1), "r"(TG) : "memory");
         else __syncthreads();
     };
     const float lim = (float)(H - 1);
 
     if (threadIdx.x == 0) {
-        mbar_init(&bars[0], 1);
-        mbar_init(&bars[1], 1);
+        for (int k = 0; k < NS; ++k) {
+            mbar_init(&full[k], 1);
+            mbar_init(&empty[k], kFusedThreads);
+        }
+        mbar_init(visbar, 1);
         fence_mbar_init();
         tma_prefetch_desc(&tmap);
     }
-    uint32_t uses0 = 0, uses1 = 0;                                             // completed phases per barrier
+    // pipeline bookkeeping, identical in every thread: stage and use count of the next tile to consume
+    uint32_t cs = 0, ck = 0;
+    // producer (thread 0 only): stage and use count of the next tile to request
+    uint32_t fs = 0, fk = 0;
+    uint32_t vph = 0;
     Twiddles<N> twr;
     twr.init(tid, a.tw);
+    // visibility rows arrive by bulk async copy when every row start is 16-byte aligned (B even)
+    const bool bulk = (B & 1) == 0;
+    const int tc_end = a.tc0 + a.ntc;
     __syncthreads();
+    if (bulk && threadIdx.x == 0 && a.tc0 + (int)blockIdx.x < tc_end) {
+        mbar_expect_tx(visbar, (uint32_t)B * 8u);
+        bulk_load_1d(visrow, a.vis + (size_t)(a.tc0 + blockIdx.x) * a.P * B, (uint32_t)B * 8u, visbar);
+    }
 
-    for (int tc = a.tc0 + blockIdx.x; tc < a.tc0 + a.ntc; tc += gridDim.x) {
+    for (int tc = a.tc0 + blockIdx.x; tc < tc_end; tc += gridDim.x) {
         const int t = tc / a.C, c = tc - t * a.C;
         const float s = sc.s[c - a.c_base];
         const float *su = a.su + (size_t)t * B;
         const float *sv = a.sv + (size_t)t * B;
         const uint32_t *sb = a.sb + (size_t)t * B;
-
-        // u-tile of sorted sample j for this channel (NT = beyond the grid)
-        auto tile_of = [&](int j) -> int {
-            const float xr = rintf(__fmul_rn(__ldg(su + j), s));
-            return (xr <= lim) ? (int)xr / KU : NT;
+        // column of sorted sample value x = |u_m| for this channel (H = beyond the grid, NaN included)
+        auto col_of = [&](float x) -> int {
+            const float xr = rintf(__fmul_rn(x, s));
+            return (xr <= lim) ? (int)xr : H;
         };
-        // ---- tile boundaries: toff[tl] = first sorted sample whose tile is >= tl -------------------------
-        for (int i = threadIdx.x; i <= NT; i += kFusedThreads) toff[i] = (uint32_t)B;
-        if (threadIdx.x == 0) { s_nin = 0; s_occ = 0; }
-        __syncthreads();
-        for (int j = threadIdx.x; j < B; j += kFusedThreads) {
-            const int tj = tile_of(j);
-            const int tp = j > 0 ? tile_of(j - 1) : -1;
-            for (int tl = tp + 1; tl <= tj; ++tl) toff[tl] = (uint32_t)j;
-        }
-        // ---- optional output: cell index of every baseline, in baseline order (a1) -----------------------
-        if (a.cell_idx) {
-            const float *uvw = a.uvw_m + (size_t)t * B * 3;
-            for (int b = threadIdx.x; b < B; b += kFusedThreads)
-                a.cell_idx[(size_t)tc * B + b] = cell_of(uvw[3 * b], uvw[3 * b + 1], s, N, H);
-        }
-        __syncthreads();
-        const int j_end = (int)toff[NT];                                        // samples [0, j_end) have |iu| <= H-1
-        const int n_tiles = j_end > 0 ? tile_of(j_end - 1) + 1 : 0;
-        const int ulim = n_tiles * KU;                                          // scratch rows written by pass 1
-        const int n_box = (ulim + Cfg::BOX_ROWS - 1) / Cfg::BOX_ROWS;
+        int n_cp = 0, ulim = 0, n_box = 0;
         float wsum_val = 0.f;
 
         for (int p = 0; p < a.P; ++p) {
             const size_t img_idx = (size_t)tc * a.P + p;
             float *img = a.image + img_idx * N * N;
-            // ---- stage this image's visibility row in shared memory (coalesced, 16-byte loads when aligned) ----
-            __syncthreads();                                                    // previous readers of visrow are done
-            {
+            __syncthreads();                                    // (C) every group has finished the previous pass 2
+            {                                                   // the region was last used by pass 2: clear the columns
+                const int n16 = (Cfg::COL_BYTES + (uniform ? Cfg::COL_BYTES / 2 : 0)) / 16;
+                for (int i = threadIdx.x; i < n16; i += kFusedThreads)
+                    reinterpret_cast<float4 *>(region)[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+            }
+            if (p == 0) {
+                if (threadIdx.x == 0) { s_nin = 0; s_occ = 0; }
+                // ---- column offsets: coff[u] = first sorted sample whose column is >= u, u = 0..H+1 -------
+                // (sample j = B is a sentinel of column H+1, so every entry is written exactly once)
+                for (int j0 = threadIdx.x; j0 <= B; j0 += 4 * kFusedThreads) {
+                    float xs[4], xp[4];
+#pragma unroll
+                    for (int m = 0; m < 4; ++m) {
+                        const int j = j0 + m * kFusedThreads;
+                        xs[m] = j < B ? __ldg(su + j) : 0.f;
+                        xp[m] = (j > 0 && j <= B) ? __ldg(su + j - 1) : 0.f;
+                    }
+#pragma unroll
+                    for (int m = 0; m < 4; ++m) {
+                        const int j = j0 + m * kFusedThreads;
+                        if (j <= B) {
+                            const int cj = j < B ? col_of(xs[m]) : H + 1;
+                            const int cq = j > 0 ? col_of(xp[m]) : -1;
+                            for (int u = cq + 1; u <= cj; ++u) coff[u] = (uint32_t)j;
+                            if (cj >= H && cq < H) s_ncol = cq + 1;        // occupied columns are [0, cq]
+                        }
+                    }
+                }
+                // ---- optional output: cell index of every baseline, in baseline order (a1) ---------------
+                if (a.cell_idx) {
+                    const float *uvw = a.uvw_m + (size_t)t * B * 3;
+                    for (int b = threadIdx.x; b < B; b += kFusedThreads)
+                        a.cell_idx[(size_t)tc * B + b] = cell_of(uvw[3 * b], uvw[3 * b + 1], s, N, H);
+                }
+            }
+            if (!bulk) {                                        // odd B: rows are only 8-byte aligned
                 const float2 *vrow = a.vis + img_idx * B;
-                if (((img_idx * (size_t)B) & 1) == 0) {
-                    const float4 *src = reinterpret_cast<const float4 *>(vrow);
-                    float4 *dst = reinterpret_cast<float4 *>(visrow);
-                    for (int i = threadIdx.x; i < B / 2; i += kFusedThreads) dst[i] = __ldcs(src + i);
-                    if ((B & 1) && threadIdx.x == 0) visrow[B - 1] = vrow[B - 1];
-                } else {
-                    for (int i = threadIdx.x; i < B; i += kFusedThreads) visrow[i] = vrow[i];
+                for (int i = threadIdx.x; i < B; i += kFusedThreads) visrow[i] = vrow[i];
+            }
+            __syncthreads();                                    // (A)
+            if (p == 0) {
+                n_cp = (s_ncol + 1) / 2;                        // column pairs that hold samples
+                ulim = 2 * n_cp;                                // scratch rows written by pass 1
+                n_box = (ulim + Cfg::BOX_ROWS - 1) / Cfg::BOX_ROWS;
+            }
+            if (bulk) { mbar_wait(visbar, vph); vph ^= 1u; }
+
+            // ================= pass 1: each group grids and transforms column pairs (2cp, 2cp+1) ==========
+            int my_in = 0, my_occ = 0;
+            for (int cp = g; cp < n_cp; cp += G) {
+                const int u0 = 2 * cp;
+                const int k0 = (int)coff[u0], k1 = (int)coff[u0 + 1], k2 = (int)coff[u0 + 2];
+                gsync();                                        // the columns are zero again (own-slot clearing below)
+                for (int j = k0 + tid; j < k2; j += TG) {
+                    const float yr = rintf(__fmul_rn(__ldg(sv + j), s));
+                    if (fabsf(yr) <= lim) {                     // NaN fails; |iu| <= H-1 by construction
+                        const int iv = (int)yr;
+                        const uint32_t bb = __ldg(sb + j);
+                        float2 vv = visrow[bb & 0x7fffffffu];
+                        if (bb >> 31) vv.y = -vv.y;
+                        const bool second = j >= k1;
+                        float2 *col = second ? c1 : c0;
+                        const int o = xsw(iv + H);
+                        atomicAdd(&col[o].x, vv.x);
+                        atomicAdd(&col[o].y, vv.y);
+                        if (uniform) atomicAdd(second ? &n1[o] : &n0[o], 1u);
+                        if (u0 == 0 && !second) {               // iu == 0: the conjugate lies in column 0 too
+                            const int o2 = xsw(H - iv);
+                            atomicAdd(&c0[o2].x, vv.x);
+                            atomicAdd(&c0[o2].y, -vv.y);
+                            if (uniform) atomicAdd(&n0[o2], 1u);
+                        }
+                        ++my_in;
+                    }
+                }
+                gsync();
+                float2 v[2][kE];
+#pragma unroll
+                for (int e = 0; e < kE; ++e) {                  // transform index n lives in centred row n ^ H
+                    const int o = xsw(tid + (e ^ (kE / 2)) * TG);
+                    v[0][e] = c0[o];
+                    v[1][e] = c1[o];
+                    if (uniform) {                              // a3: divide by the cell count
+                        const uint32_t q0 = n0[o], q1 = n1[o];
+                        if (q0) {
+                            n0[o] = 0u;
+                            v[0][e].x = __fdiv_rn(v[0][e].x, (float)q0);
+                            v[0][e].y = __fdiv_rn(v[0][e].y, (float)q0);
+                            my_occ += (u0 == 0) ? 1 : 2;        // the mirror image of a u > 0 cell is occupied too
+                        }
+                        if (q1) {
+                            n1[o] = 0u;
+                            v[1][e].x = __fdiv_rn(v[1][e].x, (float)q1);
+                            v[1][e].y = __fdiv_rn(v[1][e].y, (float)q1);
+                            my_occ += 2;
+                        }
+                    }
+                }
+                ExchangePadded2 xch{c0, c1};
+                fft_inverse<N, 2>(v, tid, xch, twr, gsync);
+                float2 *d0 = scratch + (size_t)u0 * N, *d1 = d0 + N;
+#pragma unroll
+                for (int e = 0; e < kE; ++e) {
+                    const int o = xsw(tid + e * TG);            // the slots this thread read last: clear them
+                    c0[o] = make_float2(0.f, 0.f);
+                    c1[o] = make_float2(0.f, 0.f);
+                    d0[tid + e * TG] = v[0][e];
+                    d1[tid + e * TG] = v[1][e];
                 }
             }
-            int my_occ = 0, my_in = 0;
-            // ================= pass 1: grid a u-tile in shared memory, transform its columns along v =====
-            for (int tl = 0; tl < n_tiles; ++tl) {
-                __syncthreads();                                                // previous users of the region are done
-                for (int i = threadIdx.x; i < KU * SLOTS / 2; i += kFusedThreads)
-                    reinterpret_cast<float4 *>(tile)[i] = make_float4(0.f, 0.f, 0.f, 0.f);
-                if (uniform)
-                    for (int i = threadIdx.x; i < KU * SLOTS / 4; i += kFusedThreads)
-                        reinterpret_cast<uint4 *>(cnt)[i] = make_uint4(0u, 0u, 0u, 0u);
-                const int k0 = (int)toff[tl], k1 = (int)toff[tl + 1];
-                // accumulate in rounds of IT * 512 samples.  Shared-memory float atomics are CAS loops (~2 cycles per
-                // lane), and cells rarely collide, so: (1) every sample writes its id into the owner array, (2) the
-                // sample whose id survived adds with plain loads/stores, (3) only the losers (and the rare second
-                // half of an iu == 0 sample) use atomics.
-                for (int r0 = k0; r0 < k1; r0 += IT * kFusedThreads) {
-                    int o[IT], o2[IT];
-                    float2 v[IT];
-#pragma unroll
-                    for (int m = 0; m < IT; ++m) {
-                        o[m] = -1; o2[m] = -1;
-                        const int j = r0 + m * kFusedThreads + threadIdx.x;
-                        if (j < k1) {
-                            const float xr = rintf(__fmul_rn(__ldg(su + j), s));
-                            const float yr = rintf(__fmul_rn(__ldg(sv + j), s));
-                            if (fabsf(yr) <= lim) {                              // NaN fails; |iu| <= H-1 by construction
-                                const int iu = (int)xr, iv = (int)yr;
-                                const uint32_t bb = __ldg(sb + j);
-                                float2 vv = visrow[bb & 0x7fffffffu];
-                                if (bb >> 31) vv.y = -vv.y;
-                                v[m] = vv;
-                                const int ul = iu - tl * KU, row = iv + H;
-                                o[m] = ul * SLOTS + xsw(row);
-                                if (iu == 0) { const int row2 = H - iv; o2[m] = xsw(row2); }
-                                ++my_in;
-                            }
-                        }
-                    }
-                    __syncthreads();                                            // tile zeroed / previous round complete
-#pragma unroll
-                    for (int m = 0; m < IT; ++m)
-                        if (o[m] >= 0) own[o[m]] = (unsigned short)(m * kFusedThreads + threadIdx.x);
-                    __syncthreads();
-                    bool lose[IT];
-#pragma unroll
-                    for (int m = 0; m < IT; ++m) {
-                        lose[m] = false;
-                        if (o[m] >= 0) {
-                            if (own[o[m]] == (unsigned short)(m * kFusedThreads + threadIdx.x)) {
-                                float2 q = tile[o[m]];
-                                q.x += v[m].x; q.y += v[m].y;
-                                tile[o[m]] = q;
-                                if (uniform) cnt[o[m]] += 1u;
-                            } else {
-                                lose[m] = true;
-                            }
-                        }
-                    }
-                    __syncthreads();
-#pragma unroll
-                    for (int m = 0; m < IT; ++m) {
-                        if (lose[m]) {
-                            atomicAdd(&tile[o[m]].x, v[m].x);
-                            atomicAdd(&tile[o[m]].y, v[m].y);
-                            if (uniform) atomicAdd(&cnt[o[m]], 1u);
-                        }
-                        if (o2[m] >= 0) {                                       // iu == 0: the conjugate lies in column 0 too
-                            atomicAdd(&tile[o2[m]].x, v[m].x);
-                            atomicAdd(&tile[o2[m]].y, -v[m].y);
-                            if (uniform) atomicAdd(&cnt[o2[m]], 1u);
-                        }
-                    }
-                }
-                __syncthreads();
-                if (uniform) {                                                  // a3: divide by the cell count
-                    for (int i = threadIdx.x; i < KU * SLOTS; i += kFusedThreads) {
-                        const uint32_t cc = cnt[i];
-                        if (cc) {
-                            float2 q = tile[i];
-                            q.x = __fdiv_rn(q.x, (float)cc); q.y = __fdiv_rn(q.y, (float)cc);
-                            tile[i] = q;
-                            // occupied cells of the FULL plane: the mirror image of a u > 0 cell is occupied too
-                            my_occ += (tl == 0 && i < SLOTS) ? 1 : 2;
-                        }
-                    }
-                    __syncthreads();
-                }
-                {
-                    float2 *c0 = tile + (size_t)(2 * g) * SLOTS, *c1 = c0 + SLOTS;
-                    ExchangePadded2 xch{c0, c1};
-                    float2 v[2][kE];
-#pragma unroll
-                    for (int e = 0; e < kE; ++e) {                              // transform index n lives in centred row n ^ H
-                        const int r = tid + (e ^ (kE / 2)) * TG;
-                        v[0][e] = c0[xsw(r)];
-                        v[1][e] = c1[xsw(r)];
-                    }
-                    fft_inverse<N, 2>(v, tid, xch, twr, sync);
-                    float2 *d0 = scratch + (size_t)(tl * KU + 2 * g) * N, *d1 = d0 + N;
-#pragma unroll
-                    for (int e = 0; e < kE; ++e) {
-                        d0[tid + e * TG] = v[0][e];
-                        d1[tid + e * TG] = v[1][e];
-                    }
-                }
-            }
-            if (p == 0) {                                                       // weight sum (a3), shared by the P planes
+            if (p == 0) {                                       // weight sum (a3), shared by the P planes
 #pragma unroll
                 for (int d = 16; d > 0; d >>= 1) {
                     my_occ += __shfl_xor_sync(0xffffffffu, my_occ, d);
@@ -363,9 +361,17 @@ fused_image_kernel(const FusedArgs a, const __grid_constant__ ScaleBlock sc, con
             // scratch stores (generic proxy) must be visible to the TMA loads (async proxy) below
             __threadfence();
             asm volatile("fence.proxy.async;" ::: "memory");
-            __syncthreads();
+            __syncthreads();                                    // (B)
+            if (bulk && threadIdx.x == 0) {                     // prefetch the next image's visibility row
+                size_t nxt = img_idx + 1;
+                if (p + 1 == a.P) nxt = (tc + (int)gridDim.x < tc_end) ? (size_t)(tc + gridDim.x) * a.P : (size_t)-1;
+                if (nxt != (size_t)-1) {
+                    mbar_expect_tx(visbar, (uint32_t)B * 8u);
+                    bulk_load_1d(visrow, a.vis + nxt * B, (uint32_t)B * 8u, visbar);
+                }
+            }
             if (p == 0) wsum_val = uniform ? (float)s_occ : (float)(2 * s_nin);
-            if (wsum_val == 0.f) {                                              // W = 0: zero image (uniform over the CTA)
+            if (wsum_val == 0.f) {                              // W = 0: zero image (uniform over the CTA)
                 for (int i = threadIdx.x; i < N * N / 4; i += kFusedThreads)
                     reinterpret_cast<float4 *>(img)[i] = make_float4(0.f, 0.f, 0.f, 0.f);
                 continue;
@@ -373,58 +379,66 @@ fused_image_kernel(const FusedArgs a, const __grid_constant__ ScaleBlock sc, con
             const float inv_w = 1.0f / wsum_val;
 
             // ================= pass 2: row pairs -> two real image rows per transform ===================
-            auto issue = [&](int it) {                                          // thread 0 only
-                uint64_t *bar = &bars[it & 1];
-                unsigned char *dst = stage + (size_t)(it & 1) * Cfg::STAGE_BYTES;
-                mbar_expect_tx(bar, (uint32_t)(n_box * Cfg::BOX_ROWS * Cfg::ROWB));
-                for (int bx = 0; bx < n_box; ++bx)
-                    tma_load_3d(dst + (size_t)bx * Cfg::BOX_ROWS * Cfg::ROWB, &tmap, bar, 2 * it * Cfg::KY,
-                                bx * Cfg::BOX_ROWS, (int)blockIdx.x);
+            // full/empty pipeline over NS stage buffers.  Thread 0 is the producer: it requests tile `fill_it`
+            // as soon as every thread has released the buffer's previous contents, polling while it waits.
+            int fill_it = 0;
+            auto try_fill = [&]() {                             // thread 0 only
+                while (fill_it < Cfg::NIT) {
+                    if (fk > 0 && !mbar_test(&empty[fs], (fk & 1u) ^ 1u)) break;
+                    fence_proxy_async();
+                    uint64_t *bar = &full[fs];
+                    unsigned char *dst = stage + (size_t)fs * Cfg::STAGE_BYTES;
+                    mbar_expect_tx(bar, (uint32_t)(Cfg::NSUB * n_box * Cfg::BOX_ROWS * Cfg::ROWB));
+                    for (int sb_ = 0; sb_ < Cfg::NSUB; ++sb_)
+                        for (int bx = 0; bx < n_box; ++bx)
+                            tma_load_3d(dst + (size_t)sb_ * Cfg::SUB_BYTES + (size_t)bx * Cfg::BOX_ROWS * Cfg::ROWB, &tmap,
+                                        bar, 2 * (fill_it * Cfg::KYS + sb_ * Cfg::KY), bx * Cfg::BOX_ROWS, (int)blockIdx.x);
+                    ++fill_it;
+                    if (++fs == (uint32_t)NS) { fs = 0; ++fk; }
+                }
             };
-            if (threadIdx.x == 0) { issue(0); issue(1); }
+            if (threadIdx.x == 0) try_fill();
+            const int sub = g / Cfg::PPS, pair = g % Cfg::PPS;
             for (int it = 0; it < Cfg::NIT; ++it) {
-                const int sbuf = it & 1;
-                mbar_wait(&bars[sbuf], (sbuf ? uses1 : uses0) & 1u);
-                if (sbuf) ++uses1; else ++uses0;
+                if (threadIdx.x == 0) {
+                    while (!mbar_test(&full[cs], ck & 1u)) try_fill();
+                } else {
+                    mbar_wait(&full[cs], ck & 1u);
+                }
                 float2 z[1][kE];
-                if (g < Cfg::PAIRS) {
-                    ExchangeTilePair<Cfg::ROWB> st{stage + (size_t)sbuf * Cfg::STAGE_BYTES, g};
+                {
+                    ExchangeTilePair<Cfg::ROWB> st{stage + (size_t)cs * Cfg::STAGE_BYTES + (size_t)sub * Cfg::SUB_BYTES, pair};
 #pragma unroll
-                    for (int e = 0; e < kE / 2; ++e) {                          // n = u < H: S1 + i S2
+                    for (int e = 0; e < kE / 2; ++e) {          // n = u < H: S1 + i S2
                         const int u = tid + e * TG;
                         float4 q = make_float4(0.f, 0.f, 0.f, 0.f);
                         if (u < ulim) q = *st.at_row(u);
                         z[0][e] = make_float2(q.x - q.w, q.y + q.z);
                     }
 #pragma unroll
-                    for (int e = kE / 2; e < kE; ++e) {                         // n > H: conj(S1[N-n]) + i conj(S2[N-n])
-                        const int u = N - (tid + e * TG);                       // in [1, H]; u == H is the empty Nyquist column
+                    for (int e = kE / 2; e < kE; ++e) {         // n > H: conj(S1[N-n]) + i conj(S2[N-n])
+                        const int u = N - (tid + e * TG);       // in [1, H]; u == H is the empty Nyquist column
                         float4 q = make_float4(0.f, 0.f, 0.f, 0.f);
                         if (u < ulim && u < H) q = *st.at_row(u);
                         z[0][e] = make_float2(q.x + q.w, q.z - q.y);
                     }
                 }
-                __syncthreads();                                                // everyone has read this stage buffer
-                if (threadIdx.x == 0 && it + 2 < Cfg::NIT) {
-                    fence_proxy_async();
-                    issue(it + 2);
-                }
-                if (g < Cfg::PAIRS) {
-                    ExchangePadded1 xch{xbuf + (size_t)g * SLOTS};
-                    fft_inverse<N, 1>(z, tid, xch, twr, sync);
-                    const int ky = it * Cfg::KY + 2 * g;
-                    float *r0 = img + (size_t)(ky ^ H) * N, *r1 = img + (size_t)((ky + 1) ^ H) * N;
+                mbar_arrive(&empty[cs]);                        // this thread is done with the stage buffer
+                if (++cs == (uint32_t)NS) { cs = 0; ++ck; }
+                if (threadIdx.x == 0) try_fill();
+                ExchangePadded1 xch{xbuf};
+                fft_inverse<N, 1>(z, tid, xch, twr, gsync);
+                const int ky = it * Cfg::KYS + sub * Cfg::KY + 2 * pair;
+                float *r0 = img + (size_t)(ky ^ H) * N, *r1 = img + (size_t)((ky + 1) ^ H) * N;
 #pragma unroll
-                    for (int e = 0; e < kE; ++e) {
-                        const int x = (tid + e * TG) ^ H;
-                        __stcs(r0 + x, z[0][e].x * inv_w);
-                        __stcs(r1 + x, z[0][e].y * inv_w);
-                    }
+                for (int e = 0; e < kE; ++e) {
+                    const int x = (tid + e * TG) ^ H;
+                    __stcs(r0 + x, z[0][e].x * inv_w);
+                    __stcs(r1 + x, z[0][e].y * inv_w);
                 }
             }
         }
         if (threadIdx.x == 0) a.wsum[tc] = wsum_val;
-        __syncthreads();
     }
 }
 
@@ -450,16 +464,14 @@ bool fused_supported(int P, int B, int n_pix, int weighting)
     (void)P;
     if (B > kSortMaxB) return false;
     const bool uni = weighting == BLINK_W_UNIFORM;
-    size_t need;
     switch (n_pix) {
-        case 256: need = fused_smem_bytes<256>(B, uni); break;
-        case 512: need = fused_smem_bytes<512>(B, uni); break;
-        case 1024: need = fused_smem_bytes<1024>(B, uni); break;
-        case 2048: need = fused_smem_bytes<2048>(B, uni); break;
-        case 4096: need = fused_smem_bytes<4096>(B, uni); break;
+        case 256: return fused_stages<256>(B, uni) > 0;
+        case 512: return fused_stages<512>(B, uni) > 0;
+        case 1024: return fused_stages<1024>(B, uni) > 0;
+        case 2048: return fused_stages<2048>(B, uni) > 0;
+        case 4096: return fused_stages<4096>(B, uni) > 0;
         default: return false;
     }
-    return need <= 227 * 1024;
 }
 
 static size_t sort_bytes(int T, int B) { return align_up((size_t)T * B * 4, 256) * 3; }
@@ -516,8 +528,14 @@ static int launch_fused(const FusedArgs &base, const double *freqs_hz, double pi
         presort_kernel<<<base.T, kSortThreads, ssm, st>>>(base.uvw_m, base.B, np2, su, sv, sb);
         BLINK_LAUNCH_CHECK("presort_kernel");
     }
-    const size_t smem = fused_smem_bytes<N>(base.B, base.weighting == BLINK_W_UNIFORM);
-    BLINK_CUDA_TRY(cudaFuncSetAttribute(fused_image_kernel<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    const bool uni = base.weighting == BLINK_W_UNIFORM;
+    const int ns = fused_stages<N>(base.B, uni);
+    if (ns == 0) return BLINK_ERR_UNSUPPORTED;
+    const size_t smem = fused_smem_bytes<N>(base.B, uni, ns);
+    if (ns == 3)
+        BLINK_CUDA_TRY(cudaFuncSetAttribute(fused_image_kernel<N, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    else
+        BLINK_CUDA_TRY(cudaFuncSetAttribute(fused_image_kernel<N, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     CUtensorMap tmap;
     // scratch viewed as float32 [ctas][H rows (u)][2N (ky re/im)]; boxes of [BOX_ROWS u][KY ky]
     int rc = encode_tensor_map_3d_f32(&tmap, scratch, 2ull * N, (uint64_t)Cfg::H, (uint64_t)ctas, (uint64_t)N * 8,
@@ -532,7 +550,8 @@ static int launch_fused(const FusedArgs &base, const double *freqs_hz, double pi
                                   a.su = su; a.sv = sv; a.sb = sb;
                                   a.tw = twiddle_table();
                                   const int grid = ntc < ctas ? ntc : ctas;
-                                  fused_image_kernel<N><<<grid, kFusedThreads, smem, st>>>(a, sc, tmap);
+                                  if (ns == 3) fused_image_kernel<N, 3><<<grid, kFusedThreads, smem, st>>>(a, sc, tmap);
+                                  else fused_image_kernel<N, 2><<<grid, kFusedThreads, smem, st>>>(a, sc, tmap);
                                   BLINK_LAUNCH_CHECK("fused_image_kernel");
                                   return (int)BLINK_OK;
                               });
