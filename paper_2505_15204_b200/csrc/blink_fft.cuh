@@ -278,19 +278,24 @@ __device__ __forceinline__ void stage_get(float2 (&v)[NV][kE], int tid, const X 
     }
 }
 
-template <int N, int NV, int S, int P, class X, class Sync>
+struct NoHook {
+    __device__ __forceinline__ void operator()() const {}
+};
+
+template <int N, int NV, int S, int P, class X, class Sync, class Hook>
 struct FftStages {
     __device__ __forceinline__ static void run(float2 (&v)[NV][kE], int tid, const X &xch, const Twiddles<N> &twr,
-                                               Sync sync)
+                                               Sync sync, Hook hook)
     {
         constexpr int R = plan_radix(N, S);
         stage_compute<N, NV, R, P, S>(v, twr);
         if constexpr (S + 1 < plan_stages(N)) {
             sync();                                      // everyone has finished reading the array
+            if constexpr (S == 0) hook();                // every thread of the group has consumed its inputs
             stage_put<N, NV, R, P, X>(v, tid, xch);
             sync();                                      // all writes visible
             stage_get<N, NV, X>(v, tid, xch);
-            FftStages<N, NV, S + 1, P * R, X, Sync>::run(v, tid, xch, twr, sync);
+            FftStages<N, NV, S + 1, P * R, X, Sync, Hook>::run(v, tid, xch, twr, sync, hook);
         }
         // last stage: output j + r*P with P = N/R is again slot layout tid + e*TG -- nothing to move
     }
@@ -299,12 +304,13 @@ struct FftStages {
 // Full transform.  `sync` must synchronise (at least) all threads of the group and must be called
 // by every thread the same number of times (use __syncthreads() when groups share a CTA).
 // NOTE: the first sync() also orders the caller's last reads of the exchange array (e.g. the
-// initial load out of a TMA tile that doubles as the exchange array) before the first put.
-template <int N, int NV, class X, class Sync>
+// initial load out of a TMA tile that doubles as the exchange array) before the first put; `hook`
+// runs right after it (in every thread), when all inputs of the group's vectors are in registers.
+template <int N, int NV, class X, class Sync, class Hook = NoHook>
 __device__ __forceinline__ void fft_inverse(float2 (&v)[NV][kE], int tid, const X &xch, const Twiddles<N> &twr,
-                                            Sync sync)
+                                            Sync sync, Hook hook = Hook())
 {
-    FftStages<N, NV, 0, 1, X, Sync>::run(v, tid, xch, twr, sync);
+    FftStages<N, NV, 0, 1, X, Sync, Hook>::run(v, tid, xch, twr, sync, hook);
 }
 
 }  // namespace blink

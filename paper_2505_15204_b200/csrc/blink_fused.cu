@@ -50,7 +50,7 @@ struct FusedArgs {
     int tc0, ntc, c_base;
     float *image; float *wsum; int32_t *cell_idx;              // indexed by absolute tc / image
     float2 *scratch;                                           // [gridDim.x][H][N]
-    const float *su; const float *sv; const uint32_t *sb;      // per timestep: baselines sorted by |u| (presort_kernel)
+    const float *su; const uint2 *svb;                         // per timestep: baselines sorted by |u| (presort_kernel)
     const float2 *tw;
 };
 
@@ -76,7 +76,8 @@ template <int N>
 __host__ __device__ constexpr size_t fused_region_bytes(bool uniform, int ns)
 {
     using Cfg = FusedCfg<N>;
-    const size_t p1 = (size_t)Cfg::COL_BYTES + (uniform ? (size_t)Cfg::COL_BYTES / 2 : 0);
+    (void)uniform;                                             // columns | counts | staged samples (2 rounds x 8 bytes per thread)
+    const size_t p1 = (size_t)Cfg::COL_BYTES + (size_t)Cfg::COL_BYTES / 2 + (size_t)kFusedThreads * 16;
     const size_t p2 = (size_t)ns * Cfg::STAGE_BYTES + (size_t)Cfg::G * N * 8;
     return p1 > p2 ? p1 : p2;
 }
@@ -105,14 +106,13 @@ static int fused_stages(int B, bool uniform)
 // For every channel the u-tile of a sample, rint(|u_m| * s_c) / KU, is then non-decreasing along the sorted
 // order (fp32 multiply by s_c > 0 and rint are monotone), so a tile's samples are ONE contiguous range and no
 // per-image binning is needed.  The sample is stored folded into the half plane u >= 0:
-//   su = |u_m|, sv = (u_m < 0 ? -v_m : v_m), sb = b | (u_m < 0) << 31   (bit 31: use conj(V) at (-u,-v)).
+//   su = |u_m|, svb = { bits of sv = (u_m < 0 ? -v_m : v_m), b | (u_m < 0) << 31 }   (bit 31: use conj(V) at (-u,-v)).
 // rint(-x) = -rint(x) and (-a) * s = -(a * s) exactly, so the folded cell is exactly the mirror cell (R1, R2).
 constexpr int kSortThreads = 1024;
 constexpr int kSortMaxB = 16384;
 
 __global__ void __launch_bounds__(kSortThreads)
-presort_kernel(const float *__restrict__ uvw_m, int B, int np2, float *__restrict__ su, float *__restrict__ sv,
-               uint32_t *__restrict__ sb)
+presort_kernel(const float *__restrict__ uvw_m, int B, int np2, float *__restrict__ su, uint2 *__restrict__ svb)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     float *key = reinterpret_cast<float *>(smem_raw);
@@ -152,8 +152,7 @@ presort_kernel(const float *__restrict__ uvw_m, int B, int np2, float *__restric
         const float u = uvw[3 * b], v = uvw[3 * b + 1];
         const bool neg = u < 0.0f;
         su[(size_t)t * B + i] = fabsf(u);
-        sv[(size_t)t * B + i] = neg ? -v : v;
-        sb[(size_t)t * B + i] = b | (neg ? 0x80000000u : 0u);
+        svb[(size_t)t * B + i] = make_uint2(__float_as_uint(neg ? -v : v), b | (neg ? 0x80000000u : 0u));
     }
 }
 
@@ -180,13 +179,15 @@ fused_image_kernel(const FusedArgs a, const __grid_constant__ ScaleBlock sc, con
     // pass 1: this group's column pair (XOR-swizzled slots) and, for uniform weighting, its cell counts
     float2 *c0 = reinterpret_cast<float2 *>(region) + (size_t)g * 2 * N, *c1 = c0 + N;
     uint32_t *n0 = reinterpret_cast<uint32_t *>(region + Cfg::COL_BYTES) + (size_t)g * 2 * N, *n1 = n0 + N;
+    constexpr int kPre = 2;                                    // sample rounds staged ahead per unit
+    uint2 *pre = reinterpret_cast<uint2 *>(region + Cfg::COL_BYTES + Cfg::COL_BYTES / 2) + (size_t)g * kPre * TG;
     // pass 2: NS stages of transposed scratch tiles, then one exchange array per group
     unsigned char *stage = region;
     float2 *xbuf = reinterpret_cast<float2 *>(region + (size_t)NS * Cfg::STAGE_BYTES) + (size_t)g * N;
     uint64_t *full = reinterpret_cast<uint64_t *>(region + fused_region_bytes<N>(uniform, NS));   // [NS]
-    uint64_t *empty = full + NS;                                                                  // [NS]
-    uint64_t *visbar = empty + NS;
+    uint64_t *visbar = full + NS;
     __shared__ int s_nin, s_occ, s_ncol;
+    __shared__ unsigned s_done[4];                             // per stage buffer: groups that have released it (running count)
 
     float2 *scratch = a.scratch + (size_t)blockIdx.x * H * N;
     // barrier over ONE transform group (its columns / exchange array are private to it)
@@ -200,7 +201,7 @@ fused_image_kernel(const FusedArgs a, const __grid_constant__ ScaleBlock sc, con
     if (threadIdx.x == 0) {
         for (int k = 0; k < NS; ++k) {
             mbar_init(&full[k], 1);
-            mbar_init(&empty[k], kFusedThreads);
+            s_done[k] = 0u;
         }
         mbar_init(visbar, 1);
         fence_mbar_init();
@@ -208,8 +209,6 @@ fused_image_kernel(const FusedArgs a, const __grid_constant__ ScaleBlock sc, con
     }
     // pipeline bookkeeping, identical in every thread: stage and use count of the next tile to consume
     uint32_t cs = 0, ck = 0;
-    // producer (thread 0 only): stage and use count of the next tile to request
-    uint32_t fs = 0, fk = 0;
     uint32_t vph = 0;
     Twiddles<N> twr;
     twr.init(tid, a.tw);
@@ -226,8 +225,7 @@ fused_image_kernel(const FusedArgs a, const __grid_constant__ ScaleBlock sc, con
         const int t = tc / a.C, c = tc - t * a.C;
         const float s = sc.s[c - a.c_base];
         const float *su = a.su + (size_t)t * B;
-        const float *sv = a.sv + (size_t)t * B;
-        const uint32_t *sb = a.sb + (size_t)t * B;
+        const uint2 *svb = a.svb + (size_t)t * B;
         // column of sorted sample value x = |u_m| for this channel (H = beyond the grid, NaN included)
         auto col_of = [&](float x) -> int {
             const float xr = rintf(__fmul_rn(x, s));
@@ -289,32 +287,52 @@ fused_image_kernel(const FusedArgs a, const __grid_constant__ ScaleBlock sc, con
 
             // ================= pass 1: each group grids and transforms column pairs (2cp, 2cp+1) ==========
             int my_in = 0, my_occ = 0;
+            // one sample of this group's column pair: accumulate V (or conj V) into its cell with shared atomics
+            auto grid_one = [&](uint2 sq, bool second, bool col0) {
+                const float yr = rintf(__fmul_rn(__uint_as_float(sq.x), s));
+                if (fabsf(yr) <= lim) {                         // NaN fails; |iu| <= H-1 by construction
+                    const int iv = (int)yr;
+                    float2 vv = visrow[sq.y & 0x7fffffffu];
+                    if (sq.y >> 31) vv.y = -vv.y;
+                    float2 *col = second ? c1 : c0;
+                    const int o = xsw(iv + H);
+                    atomicAdd(&col[o].x, vv.x);
+                    atomicAdd(&col[o].y, vv.y);
+                    if (uniform) atomicAdd(second ? &n1[o] : &n0[o], 1u);
+                    if (col0) {                                 // iu == 0: the conjugate lies in column 0 too
+                        const int o2 = xsw(H - iv);
+                        atomicAdd(&c0[o2].x, vv.x);
+                        atomicAdd(&c0[o2].y, -vv.y);
+                        if (uniform) atomicAdd(&n0[o2], 1u);
+                    }
+                    ++my_in;
+                }
+            };
+            // the first kPre*TG samples of a unit are staged one unit ahead with cp.async (each thread copies
+            // exactly the entries it will consume, so no barrier is needed on the staging array)
+            auto prefetch = [&](int cp_) {
+                if (cp_ < n_cp) {
+                    const int q0 = (int)coff[2 * cp_], q2 = (int)coff[2 * cp_ + 2];
+#pragma unroll
+                    for (int m = 0; m < kPre; ++m) {
+                        const int j = q0 + tid + m * TG;
+                        if (j < q2) cp_async_8(&pre[m * TG + tid], svb + j);
+                    }
+                }
+            };
+            prefetch(g);
             for (int cp = g; cp < n_cp; cp += G) {
                 const int u0 = 2 * cp;
                 const int k0 = (int)coff[u0], k1 = (int)coff[u0 + 1], k2 = (int)coff[u0 + 2];
+                cp_async_wait_all();
                 gsync();                                        // the columns are zero again (own-slot clearing below)
-                for (int j = k0 + tid; j < k2; j += TG) {
-                    const float yr = rintf(__fmul_rn(__ldg(sv + j), s));
-                    if (fabsf(yr) <= lim) {                     // NaN fails; |iu| <= H-1 by construction
-                        const int iv = (int)yr;
-                        const uint32_t bb = __ldg(sb + j);
-                        float2 vv = visrow[bb & 0x7fffffffu];
-                        if (bb >> 31) vv.y = -vv.y;
-                        const bool second = j >= k1;
-                        float2 *col = second ? c1 : c0;
-                        const int o = xsw(iv + H);
-                        atomicAdd(&col[o].x, vv.x);
-                        atomicAdd(&col[o].y, vv.y);
-                        if (uniform) atomicAdd(second ? &n1[o] : &n0[o], 1u);
-                        if (u0 == 0 && !second) {               // iu == 0: the conjugate lies in column 0 too
-                            const int o2 = xsw(H - iv);
-                            atomicAdd(&c0[o2].x, vv.x);
-                            atomicAdd(&c0[o2].y, -vv.y);
-                            if (uniform) atomicAdd(&n0[o2], 1u);
-                        }
-                        ++my_in;
-                    }
+#pragma unroll
+                for (int m = 0; m < kPre; ++m) {
+                    const int j = k0 + tid + m * TG;
+                    if (j < k2) grid_one(pre[m * TG + tid], j >= k1, u0 == 0 && j < k1);
                 }
+                for (int j = k0 + tid + kPre * TG; j < k2; j += TG) grid_one(__ldg(svb + j), j >= k1, u0 == 0 && j < k1);
+                prefetch(cp + G);                               // lands while this unit is transformed
                 gsync();
                 float2 v[2][kE];
 #pragma unroll
@@ -379,32 +397,25 @@ fused_image_kernel(const FusedArgs a, const __grid_constant__ ScaleBlock sc, con
             const float inv_w = 1.0f / wsum_val;
 
             // ================= pass 2: row pairs -> two real image rows per transform ===================
-            // full/empty pipeline over NS stage buffers.  Thread 0 is the producer: it requests tile `fill_it`
-            // as soon as every thread has released the buffer's previous contents, polling while it waits.
-            int fill_it = 0;
-            auto try_fill = [&]() {                             // thread 0 only
-                while (fill_it < Cfg::NIT) {
-                    if (fk > 0 && !mbar_test(&empty[fs], (fk & 1u) ^ 1u)) break;
-                    fence_proxy_async();
-                    uint64_t *bar = &full[fs];
-                    unsigned char *dst = stage + (size_t)fs * Cfg::STAGE_BYTES;
-                    mbar_expect_tx(bar, (uint32_t)(Cfg::NSUB * n_box * Cfg::BOX_ROWS * Cfg::ROWB));
-                    for (int sb_ = 0; sb_ < Cfg::NSUB; ++sb_)
-                        for (int bx = 0; bx < n_box; ++bx)
-                            tma_load_3d(dst + (size_t)sb_ * Cfg::SUB_BYTES + (size_t)bx * Cfg::BOX_ROWS * Cfg::ROWB, &tmap,
-                                        bar, 2 * (fill_it * Cfg::KYS + sb_ * Cfg::KY), bx * Cfg::BOX_ROWS, (int)blockIdx.x);
-                    ++fill_it;
-                    if (++fs == (uint32_t)NS) { fs = 0; ++fk; }
-                }
+            // NS stage buffers behind `full` mbarriers.  A buffer is re-requested by whichever group is the LAST to
+            // have pulled its inputs out of it (a shared counter bumped by each group's leader right after the
+            // group's first barrier inside the transform), so refills start the moment the buffer is free.
+            auto request = [&](int it, uint32_t st_) {
+                fence_proxy_async();
+                uint64_t *bar = &full[st_];
+                unsigned char *dst = stage + (size_t)st_ * Cfg::STAGE_BYTES;
+                mbar_expect_tx(bar, (uint32_t)(Cfg::NSUB * n_box * Cfg::BOX_ROWS * Cfg::ROWB));
+                for (int sb_ = 0; sb_ < Cfg::NSUB; ++sb_)
+                    for (int bx = 0; bx < n_box; ++bx)
+                        tma_load_3d(dst + (size_t)sb_ * Cfg::SUB_BYTES + (size_t)bx * Cfg::BOX_ROWS * Cfg::ROWB, &tmap, bar,
+                                    2 * (it * Cfg::KYS + sb_ * Cfg::KY), bx * Cfg::BOX_ROWS, (int)blockIdx.x);
             };
-            if (threadIdx.x == 0) try_fill();
+            if (threadIdx.x == 0)
+                for (int it = 0; it < NS && it < Cfg::NIT; ++it) request(it, (cs + (uint32_t)it) % (uint32_t)NS);
             const int sub = g / Cfg::PPS, pair = g % Cfg::PPS;
             for (int it = 0; it < Cfg::NIT; ++it) {
-                if (threadIdx.x == 0) {
-                    while (!mbar_test(&full[cs], ck & 1u)) try_fill();
-                } else {
-                    mbar_wait(&full[cs], ck & 1u);
-                }
+                mbar_wait(&full[cs], ck & 1u);
+                const uint32_t st_used = cs;
                 float2 z[1][kE];
                 {
                     ExchangeTilePair<Cfg::ROWB> st{stage + (size_t)cs * Cfg::STAGE_BYTES + (size_t)sub * Cfg::SUB_BYTES, pair};
@@ -423,11 +434,17 @@ fused_image_kernel(const FusedArgs a, const __grid_constant__ ScaleBlock sc, con
                         z[0][e] = make_float2(q.x + q.w, q.z - q.y);
                     }
                 }
-                mbar_arrive(&empty[cs]);                        // this thread is done with the stage buffer
                 if (++cs == (uint32_t)NS) { cs = 0; ++ck; }
-                if (threadIdx.x == 0) try_fill();
+                auto release = [&] {                            // runs after the group's first barrier: inputs are in registers
+                    if (tid == 0) {
+                        __threadfence_block();                  // the group's reads (ordered by its barrier) before the count
+                        const unsigned old = atomicAdd(&s_done[st_used], 1u);
+                        __threadfence_block();
+                        if (old % (unsigned)G == (unsigned)(G - 1) && it + NS < Cfg::NIT) request(it + NS, st_used);
+                    }
+                };
                 ExchangePadded1 xch{xbuf};
-                fft_inverse<N, 1>(z, tid, xch, twr, gsync);
+                fft_inverse<N, 1>(z, tid, xch, twr, gsync, release);
                 const int ky = it * Cfg::KYS + sub * Cfg::KY + 2 * pair;
                 float *r0 = img + (size_t)(ky ^ H) * N, *r1 = img + (size_t)((ky + 1) ^ H) * N;
 #pragma unroll
@@ -514,18 +531,17 @@ static int launch_fused(const FusedArgs &base, const double *freqs_hz, double pi
     int ctas = option(BLINK_OPT_FUSED_CTAS);
     if (ctas <= 0) ctas = fused_default_ctas();
     ctas = (int)std::min<size_t>((size_t)ctas, (workspace_bytes - sortb) / per_cta);
-    // workspace: su | sv | sb (baselines of every timestep sorted by |u|) | per-CTA scratch
+    // workspace: su | svb (baselines of every timestep sorted by |u|) | per-CTA scratch
     unsigned char *wsp = static_cast<unsigned char *>(workspace);
     float *su = reinterpret_cast<float *>(wsp);
-    float *sv = reinterpret_cast<float *>(wsp + sortb / 3);
-    uint32_t *sb = reinterpret_cast<uint32_t *>(wsp + 2 * (sortb / 3));
+    uint2 *svb = reinterpret_cast<uint2 *>(wsp + sortb / 3);
     void *scratch = wsp + sortb;
     {
         int np2 = 1;
         while (np2 < base.B) np2 <<= 1;
         const size_t ssm = (size_t)np2 * 8;
         BLINK_CUDA_TRY(cudaFuncSetAttribute(presort_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ssm));
-        presort_kernel<<<base.T, kSortThreads, ssm, st>>>(base.uvw_m, base.B, np2, su, sv, sb);
+        presort_kernel<<<base.T, kSortThreads, ssm, st>>>(base.uvw_m, base.B, np2, su, svb);
         BLINK_LAUNCH_CHECK("presort_kernel");
     }
     const bool uni = base.weighting == BLINK_W_UNIFORM;
@@ -547,7 +563,7 @@ static int launch_fused(const FusedArgs &base, const double *freqs_hz, double pi
                                   FusedArgs a = base;
                                   a.tc0 = tc0; a.ntc = ntc; a.c_base = c_base;
                                   a.scratch = static_cast<float2 *>(scratch);
-                                  a.su = su; a.sv = sv; a.sb = sb;
+                                  a.su = su; a.svb = svb;
                                   a.tw = twiddle_table();
                                   const int grid = ntc < ctas ? ntc : ctas;
                                   if (ns == 3) fused_image_kernel<N, 3><<<grid, kFusedThreads, smem, st>>>(a, sc, tmap);

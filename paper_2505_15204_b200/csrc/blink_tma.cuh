@@ -64,6 +64,12 @@ __device__ __forceinline__ void bulk_load_1d(void *smem_dst, const void *gsrc, u
         ::"r"(smem_u32(smem_dst)), "l"(gsrc), "r"(bytes), "r"(smem_u32(bar))
         : "memory");
 }
+// 8-byte cp.async (LDGSTS) global -> shared and its completion wait (per-thread groups)
+__device__ __forceinline__ void cp_async_8(void *smem_dst, const void *gsrc)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(smem_u32(smem_dst)), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 // 3D tiled tensor load global -> shared, completion counted on `bar`
 __device__ __forceinline__ void tma_load_3d(void *smem_dst, const CUtensorMap *map, uint64_t *bar, int c0, int c1, int c2)
 {
