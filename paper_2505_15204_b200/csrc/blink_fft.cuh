@@ -174,18 +174,18 @@ struct ExchangeDense2 {
 // host) and kept in registers: per stage > 0 and butterfly q the powers w^1, w^2 (and w^4 for radix 8)
 // of w = exp(+2 pi i k / (P R)); the remaining powers are products of those (<= 2 extra roundings).
 // ---------------------------------------------------------------------------------------------
-template <int N>
+template <int N, int E = kE>
 struct Twiddles {
     static constexpr int S = plan_stages(N);
-    float2 w[S > 1 ? S - 1 : 1][2][3];                  // [stage-1][butterfly q][w1, w2, w4]
+    float2 w[S > 1 ? S - 1 : 1][E / 4][3];              // [stage-1][butterfly q][w1, w2, w4]
 
     template <int ST, int P>
     __device__ __forceinline__ void init_stage(int tid, const float2 *__restrict__ tw)
     {
         if constexpr (ST < S) {
             constexpr int R = plan_radix(N, ST);
-            constexpr int TG = N / kE;
-            constexpr int NB = kE / R;
+            constexpr int TG = N / E;
+            constexpr int NB = E / R;
             if constexpr (ST > 0) {
                 constexpr int step = kTwiddleNConst() / (P * R);
 #pragma unroll
@@ -205,10 +205,10 @@ struct Twiddles {
 // One stage: twiddle (skipped when P == 1), radix-R butterflies in registers.
 //   v[nv][e] holds x[tid + e*TG].  Butterfly q (q = 0..8/R-1) is i = tid + q*TG and uses slots
 //   e = q + r*(8/R), r = 0..R-1.  Twiddle of input r: w^r, w = exp(+2 pi i k / (P R)), k = i mod P.
-template <int N, int NV, int R, int P, int ST>
-__device__ __forceinline__ void stage_compute(float2 (&v)[NV][kE], const Twiddles<N> &twr)
+template <int N, int NV, int R, int P, int ST, int E>
+__device__ __forceinline__ void stage_compute(float2 (&v)[NV][E], const Twiddles<N, E> &twr)
 {
-    constexpr int NB = kE / R;                         // butterflies per thread
+    constexpr int NB = E / R;                         // butterflies per thread
 #pragma unroll
     for (int q = 0; q < NB; ++q) {
         if constexpr (P > 1) {
@@ -245,11 +245,11 @@ __device__ __forceinline__ void stage_compute(float2 (&v)[NV][kE], const Twiddle
 }
 
 // scatter the stage outputs to their Stockham positions: y[j + r*P], j = (i - k)*R + k
-template <int N, int NV, int R, int P, class X>
-__device__ __forceinline__ void stage_put(const float2 (&v)[NV][kE], int tid, const X &xch)
+template <int N, int NV, int R, int P, class X, int E>
+__device__ __forceinline__ void stage_put(const float2 (&v)[NV][E], int tid, const X &xch)
 {
-    constexpr int TG = N / kE;
-    constexpr int NB = kE / R;
+    constexpr int TG = N / E;
+    constexpr int NB = E / R;
 #pragma unroll
     for (int q = 0; q < NB; ++q) {
         const int i = tid + q * TG;
@@ -265,12 +265,12 @@ __device__ __forceinline__ void stage_put(const float2 (&v)[NV][kE], int tid, co
     }
 }
 
-template <int N, int NV, class X>
-__device__ __forceinline__ void stage_get(float2 (&v)[NV][kE], int tid, const X &xch)
+template <int N, int NV, class X, int E>
+__device__ __forceinline__ void stage_get(float2 (&v)[NV][E], int tid, const X &xch)
 {
-    constexpr int TG = N / kE;
+    constexpr int TG = N / E;
 #pragma unroll
-    for (int e = 0; e < kE; ++e) {
+    for (int e = 0; e < E; ++e) {
         float2 t[NV];
         xch.get(tid + e * TG, t);
 #pragma unroll
@@ -278,24 +278,26 @@ __device__ __forceinline__ void stage_get(float2 (&v)[NV][kE], int tid, const X 
     }
 }
 
+// Optional hook: called by every thread right after the k-th group barrier of a transform (k = 0, 1, ...).
 struct NoHook {
-    __device__ __forceinline__ void operator()() const {}
+    __device__ __forceinline__ void operator()(int) const {}
 };
 
-template <int N, int NV, int S, int P, class X, class Sync, class Hook>
+template <int N, int NV, int E, int S, int P, class X, class Sync, class Hook>
 struct FftStages {
-    __device__ __forceinline__ static void run(float2 (&v)[NV][kE], int tid, const X &xch, const Twiddles<N> &twr,
+    __device__ __forceinline__ static void run(float2 (&v)[NV][E], int tid, const X &xch, const Twiddles<N, E> &twr,
                                                Sync sync, Hook hook)
     {
         constexpr int R = plan_radix(N, S);
-        stage_compute<N, NV, R, P, S>(v, twr);
+        stage_compute<N, NV, R, P, S, E>(v, twr);
         if constexpr (S + 1 < plan_stages(N)) {
             sync();                                      // everyone has finished reading the array
-            if constexpr (S == 0) hook();                // every thread of the group has consumed its inputs
-            stage_put<N, NV, R, P, X>(v, tid, xch);
+            hook(2 * S);
+            stage_put<N, NV, R, P, X, E>(v, tid, xch);
             sync();                                      // all writes visible
-            stage_get<N, NV, X>(v, tid, xch);
-            FftStages<N, NV, S + 1, P * R, X, Sync, Hook>::run(v, tid, xch, twr, sync, hook);
+            hook(2 * S + 1);
+            stage_get<N, NV, X, E>(v, tid, xch);
+            FftStages<N, NV, E, S + 1, P * R, X, Sync, Hook>::run(v, tid, xch, twr, sync, hook);
         }
         // last stage: output j + r*P with P = N/R is again slot layout tid + e*TG -- nothing to move
     }
@@ -304,13 +306,13 @@ struct FftStages {
 // Full transform.  `sync` must synchronise (at least) all threads of the group and must be called
 // by every thread the same number of times (use __syncthreads() when groups share a CTA).
 // NOTE: the first sync() also orders the caller's last reads of the exchange array (e.g. the
-// initial load out of a TMA tile that doubles as the exchange array) before the first put; `hook`
-// runs right after it (in every thread), when all inputs of the group's vectors are in registers.
-template <int N, int NV, class X, class Sync, class Hook = NoHook>
-__device__ __forceinline__ void fft_inverse(float2 (&v)[NV][kE], int tid, const X &xch, const Twiddles<N> &twr,
+// initial load out of a TMA tile that doubles as the exchange array) before the first put; `hook(k)`
+// runs in every thread right after the k-th sync (callers use it to overlap their own loads with the transform).
+template <int N, int NV, int E, class X, class Sync, class Hook = NoHook>
+__device__ __forceinline__ void fft_inverse(float2 (&v)[NV][E], int tid, const X &xch, const Twiddles<N, E> &twr,
                                             Sync sync, Hook hook = Hook())
 {
-    FftStages<N, NV, 0, 1, X, Sync, Hook>::run(v, tid, xch, twr, sync, hook);
+    FftStages<N, NV, E, 0, 1, X, Sync, Hook>::run(v, tid, xch, twr, sync, hook);
 }
 
 }  // namespace blink

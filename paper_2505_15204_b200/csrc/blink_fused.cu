@@ -435,8 +435,8 @@ fused_image_kernel(const FusedArgs a, const __grid_constant__ ScaleBlock sc, con
                     }
                 }
                 if (++cs == (uint32_t)NS) { cs = 0; ++ck; }
-                auto release = [&] {                            // runs after the group's first barrier: inputs are in registers
-                    if (tid == 0) {
+                auto release = [&](int k) {                     // k == 0: right after the group's first barrier, inputs are in registers
+                    if (k == 0 && tid == 0) {
                         __threadfence_block();                  // the group's reads (ordered by its barrier) before the count
                         const unsigned old = atomicAdd(&s_done[st_used], 1u);
                         __threadfence_block();
