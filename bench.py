@@ -282,14 +282,15 @@ def main():
                 "algorithmic_bytes_per_step": mb["M36"], "model": "M36 = n_img*(36 N^2 + 8 B) + 12 T B",
                 "frac_M20": mb["M20"] / (kern_ms * 1e-3) / 1e9 / peak, "frac_M4": mb["M4"] / (kern_ms * 1e-3) / 1e9 / peak,
                 "kernel_ms": kern_ms}
-    prof = os.path.join(ROOT, "profiles", "traffic.json")
+    prof = os.path.join(ROOT, "profiles", "traffic.csv")      # DRAM bytes per step from the committed ncu capture
     if os.path.exists(prof):
         try:
-            tj = json.load(open(prof))
+            import csv
             key = f"config{args.config}_path{args.path}"
-            if key in tj:
-                roofline["traffic"] = tj[key]["dram_bytes_per_step"]
-                roofline["traffic_source"] = tj[key].get("source")
+            for row in csv.DictReader(open(prof)):
+                if row["key"] == key and args.T is None:
+                    roofline["traffic"] = int(row["dram_bytes_per_step"])
+                    roofline["traffic_source"] = row["source"]
         except Exception:
             pass
     cpu = None
