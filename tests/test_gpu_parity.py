@@ -196,6 +196,77 @@ def test_image_random_ragged(bk, oracle_mod, weighting, path):
     _check_images(bk, w, res, oracle_mod)
 
 
+@pytest.mark.parametrize("weighting", [0, 1])
+@pytest.mark.parametrize("B", [1237, 2048])
+def test_fused_ragged(bk, oracle_mod, weighting, B):
+    # the fused kernel itself (forced): odd B (rows only 8-byte aligned: no bulk-copy prefetch) and even B,
+    # P = 3 planes per (t,c), samples off the grid, 3 persistent CTAs for 6 (t,c) items, minimum workspace
+    from paper_2505_15204_b200 import workloads
+    w = workloads.make_random(T=2, C=3, P=3, B=B, n_pix=256, weighting=weighting, seed=11 + B, device="cuda", fill=1.15)
+    w.uvw_m[1, 5, 0] = float("nan")
+    rec, mn = bk.blink_workspace_bytes(bk.OP_IMAGE, w.T, w.C, w.P, w.B, w.n_pix, weighting)
+    bk.set_option(bk.OPT_IMAGE_PATH, 2)
+    bk.set_option(bk.OPT_FUSED_CTAS, 3)
+    try:
+        res = bk.blink_image(w.vis, w.uvw_m, w.freqs_hz, w.n_pix, w.pixscale_rad, weighting, want_cell_idx=True,
+                             want_counts=True)
+        torch.cuda.synchronize()
+        _check_images(bk, w, res, oracle_mod)
+        ws = torch.empty(mn, dtype=torch.uint8, device="cuda")              # room for one CTA's scratch only
+        res1 = bk.blink_image(w.vis, w.uvw_m, w.freqs_hz, w.n_pix, w.pixscale_rad, weighting, workspace=ws)
+        torch.cuda.synchronize()
+        _check_images(bk, w, res1, oracle_mod)
+    finally:
+        bk.set_option(bk.OPT_IMAGE_PATH, 0)
+        bk.set_option(bk.OPT_FUSED_CTAS, 0)
+    uvw = w.uvw_m.cpu().numpy()
+    assert np.array_equal(res["cell_idx"].cpu().numpy(), oracle_mod.cells(uvw, w.freqs_hz, w.n_pix, w.pixscale_rad))
+    cnt = res["counts"].cpu().numpy().astype(np.uint32)
+    for t in range(w.T):
+        for c in range(w.C):
+            r1 = oracle_mod.image_one(w.vis[t, c, 0].cpu().numpy(), uvw[t], w.freqs_hz[c], w.n_pix, w.pixscale_rad, weighting)
+            assert np.array_equal(cnt[t * w.C + c], r1["cnt"])
+
+
+@pytest.mark.parametrize("weighting,B", [(0, 13000), (1, 13001)])
+def test_fused_two_stage_pipeline(bk, oracle_mod, weighting, B):
+    # a visibility row this long leaves room for only two pass-2 stage buffers (the NS = 2 instantiation)
+    from paper_2505_15204_b200 import workloads
+    w = workloads.make_random(T=1, C=2, P=1, B=B, n_pix=256, weighting=weighting, seed=21, device="cuda", fill=0.8)
+    bk.set_option(bk.OPT_IMAGE_PATH, 2)
+    try:
+        res = bk.blink_image(w.vis, w.uvw_m, w.freqs_hz, w.n_pix, w.pixscale_rad, weighting)
+        torch.cuda.synchronize()
+    finally:
+        bk.set_option(bk.OPT_IMAGE_PATH, 0)
+    _check_images(bk, w, res, oracle_mod)
+
+
+@pytest.mark.parametrize("weighting", [0, 1])
+def test_fused_collisions_and_axis_column(bk, oracle_mod, weighting):
+    # worst cases of the shared-memory gridder: 1000 samples in ONE cell, 500 on the u = 0 column (their
+    # conjugates land in the same column, rows mirrored), 200 exactly at DC (sample and conjugate share the cell),
+    # the rest spread out
+    from paper_2505_15204_b200 import workloads
+    w = workloads.make_random(T=1, C=2, P=2, B=3000, n_pix=256, weighting=weighting, seed=31, device="cuda", fill=0.9)
+    cell_m = 299792458.0 / 150e6                                    # one uv cell in metres at the first channel
+    w.uvw_m[0, :1000, 0] = 17.2 * cell_m
+    w.uvw_m[0, :1000, 1] = -40.3 * cell_m
+    w.uvw_m[0, 1000:1500, 0] = 0.0
+    w.uvw_m[0, 1500:1700, 0] = 0.0
+    w.uvw_m[0, 1500:1700, 1] = 0.0
+    w.uvw_m[0, 1700:1800, 0] = -0.2 * cell_m                        # rounds to iu = -0 -> folded onto the u = 0 column
+    bk.set_option(bk.OPT_IMAGE_PATH, 2)
+    try:
+        res = bk.blink_image(w.vis, w.uvw_m, w.freqs_hz, w.n_pix, w.pixscale_rad, weighting, want_cell_idx=True)
+        torch.cuda.synchronize()
+    finally:
+        bk.set_option(bk.OPT_IMAGE_PATH, 0)
+    _check_images(bk, w, res, oracle_mod)
+    assert np.array_equal(res["cell_idx"].cpu().numpy(),
+                          oracle_mod.cells(w.uvw_m.cpu().numpy(), w.freqs_hz, w.n_pix, w.pixscale_rad))
+
+
 def test_image_degenerate_inputs(bk, oracle_mod):
     from paper_2505_15204_b200 import workloads
     # everything off the grid -> W = 0, zero images, cell_idx = -1
