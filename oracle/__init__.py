@@ -54,6 +54,8 @@ def lib():
         L.oracle_image_one.argtypes = [vp, vp, c_d, c_i, c_i, c_d, c_i, vp, vp, vp, vp, vp]
         L.oracle_image_batch.restype = c_i
         L.oracle_image_batch.argtypes = [vp, vp, vp, c_i, c_i, c_i, c_i, c_i, c_d, c_i, vp, c_i, vp, vp, c_i]
+        L.oracle_image_avg.restype = c_i
+        L.oracle_image_avg.argtypes = [vp, vp, vp, c_i, c_i, c_i, c_i, c_i, c_d, c_i, c_i, vp]
         _lib = L
     return _lib
 
@@ -159,3 +161,17 @@ def image_batch(vis, uvw_m, freqs_hz, n_pix: int, pixscale_rad: float, weighting
     if rc != 0:
         raise RuntimeError("oracle_image_batch failed")
     return images, wsum
+
+
+def image_avg(vis, uvw_m, freqs_hz, n_pix: int, pixscale_rad: float, weighting: int, avg_time: bool = False):
+    """Mean of the dirty images over channels (-> [T][P][N][N]) or over timesteps and channels (-> [P][N][N])."""
+    v = _c64(vis)
+    uvw = np.ascontiguousarray(uvw_m, dtype=np.float32)
+    fr = np.ascontiguousarray(freqs_hz, dtype=np.float64)
+    T, C, P, B = v.shape
+    out = np.empty(((P,) if avg_time else (T, P)) + (n_pix, n_pix), dtype=np.float64)
+    rc = lib().oracle_image_avg(_p(v), _p(uvw), _p(fr), T, C, P, B, int(n_pix), float(pixscale_rad),
+                                int(weighting), int(bool(avg_time)), _p(out))
+    if rc != 0:
+        raise RuntimeError("oracle_image_avg failed")
+    return out

@@ -23,6 +23,9 @@
  *   oracle_sparse_image           : == radix-2 image on a full-size image
  *   oracle_image_one              : unit source at phase centre -> 1.0 at [h][h]; on-grid offset
  *                                   source peaks at its pixel with value 1.0; |Im| < 1e-6 peak
+ *   oracle_image_avg              : unit sources -> 1.0 at the centre of the mean; == one numpy.fft transform
+ *                                   of the 1/W-weighted sum of independently re-gridded channels; centre-pixel
+ *                                   closed form with an empty channel counted in the mean
  * Nothing here is "parity unpinned".
  *
  * Build: gcc -O2 -ffp-contract=off -fPIC -shared -pthread -o liboracle.so blink_oracle.c -lm
@@ -330,5 +333,39 @@ int oracle_image_batch(const float *vis, const float *uvw_m, const double *freqs
         if (pthread_create(&th[k], NULL, batch_worker, &jobs[k]) != 0) return -1;
     }
     for (int k = 0; k < nthreads; ++k) pthread_join(th[k], NULL);
+    return 0;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * Averaged images ("Images belonging to the same time bin are averaged together";
+ * L251 "averaged in time over the entire processed time frame and frequency over the 30.72 MHz
+ * bandwidth"; reading R14): the plain definition -- image every (t, c, p) with
+ * oracle_image_one, then take the arithmetic mean over c (avg_time == 0: out [T][P][N][N]) or over
+ * (t, c) (avg_time != 0: out [P][N][N]).  Images with W == 0 are zero and still count in the mean.
+ * Pins (tests/test_oracle_pins.py): mean of unit-source images has 1.0 at the centre; linearity
+ * (equals the transform of the W-weighted sum of the grids, evaluated independently with numpy);
+ * centre pixel closed form mean_c(sum 2 Re V / W_c).
+ * ---------------------------------------------------------------------------------------- */
+int oracle_image_avg(const float *vis, const float *uvw_m, const double *freqs_hz,
+                     int T, int C, int P, int B, int n_pix, double pixscale_rad, int weighting,
+                     int avg_time, double *out)
+{
+    const size_t n2 = (size_t)n_pix * n_pix;
+    const size_t n_out = avg_time ? (size_t)P : (size_t)T * P;
+    double *img = (double *)malloc(sizeof(double) * n2);
+    if (!img) return -1;
+    for (size_t k = 0; k < n_out * n2; ++k) out[k] = 0.0;
+    for (int t = 0; t < T; ++t)
+        for (int c = 0; c < C; ++c)
+            for (int p = 0; p < P; ++p) {
+                const float *v = vis + 2 * ((((size_t)t * C + c) * P + p) * (size_t)B);
+                oracle_image_one(v, uvw_m + (size_t)t * B * 3, freqs_hz[c], B, n_pix, pixscale_rad,
+                                 weighting, img, NULL, NULL, NULL, NULL);
+                double *dst = out + (avg_time ? (size_t)p : (size_t)t * P + p) * n2;
+                for (size_t k = 0; k < n2; ++k) dst[k] += img[k];
+            }
+    const double inv = 1.0 / (avg_time ? (double)T * C : (double)C);
+    for (size_t k = 0; k < n_out * n2; ++k) out[k] *= inv;
+    free(img);
     return 0;
 }

@@ -353,3 +353,74 @@ def test_table7_byte_accounting():
     # PAPER.md L365-370 Table 7: float32 images, complex64 visibilities
     assert abs(38400 * 1200 ** 2 * 4 / 2 ** 30 - 206) < 0.5                      # "206 GB" images
     assert abs(38400 * 8256 * 4 * 8 / 2 ** 30 - 9.5) < 0.1                       # "9.5 GB" visibilities
+
+
+# ---------------------------------------------------------------------------------------------
+# averaged images (reading R14)
+# ---------------------------------------------------------------------------------------------
+def _avg_inputs(seed, T=2, C=4, P=2, B=60, N=32, ones=False):
+    rng = np.random.default_rng(seed)
+    fr = 150e6 + 1.5e6 * np.arange(C)                       # wide spacing: the channels grid to different cells
+    half_m = 0.8 * (N / 2) / (fr[-1] / 299792458.0)
+    uvw = rng.uniform(-half_m, half_m, (T, B, 3)).astype(np.float32)
+    vis = np.ones((T, C, P, B), np.complex64) if ones else \
+        (rng.normal(size=(T, C, P, B)) + 1j * rng.normal(size=(T, C, P, B))).astype(np.complex64)
+    return vis, uvw, fr, N, 1.0 / N
+
+
+@pytest.mark.parametrize("weighting", [0, 1])
+@pytest.mark.parametrize("avg_time", [False, True])
+def test_avg_unit_source_centre_is_one(oracle_mod, weighting, avg_time):
+    # every single image has exactly 1.0 at the phase centre when all V = 1, so their mean has too
+    vis, uvw, fr, N, pix = _avg_inputs(3, ones=True)
+    a = oracle_mod.image_avg(vis, uvw, fr, N, pix, weighting, avg_time)
+    assert np.allclose(a[..., N // 2, N // 2], 1.0, atol=1e-12)
+    assert np.all(a <= a[..., N // 2, N // 2][..., None, None] + 1e-12)
+
+
+@pytest.mark.parametrize("weighting", [0, 1])
+@pytest.mark.parametrize("avg_time", [False, True])
+def test_avg_linearity_numpy(oracle_mod, weighting, avg_time):
+    # independent evaluation: re-grid in numpy from the oracle's CELL INDICES only, sum the grids weighted by
+    # 1/W_c, transform ONCE with numpy.fft (library routine) -- the transform is linear, so this must be the mean
+    vis, uvw, fr, N, pix = _avg_inputs(5)
+    T, C, P, B = vis.shape
+    h = N // 2
+    ci = oracle_mod.cells(uvw, fr, N, pix)
+    acc = np.zeros(((1 if avg_time else T), P, N, N), np.complex128)
+    for t in range(T):
+        for c in range(C):
+            ok = ci[t, c] >= 0
+            r, q = ci[t, c][ok] // N, ci[t, c][ok] % N
+            cnt = np.zeros((N, N))
+            np.add.at(cnt, (r, q), 1)
+            np.add.at(cnt, (N - r, N - q), 1)
+            W = cnt.sum() if weighting == 0 else np.count_nonzero(cnt)
+            for p in range(P):
+                g = np.zeros((N, N), np.complex128)
+                np.add.at(g, (r, q), vis[t, c, p][ok].astype(np.complex128))
+                np.add.at(g, (N - r, N - q), np.conj(vis[t, c, p][ok].astype(np.complex128)))
+                if weighting == 1:
+                    g[cnt > 0] /= cnt[cnt > 0]
+                acc[0 if avg_time else t, p] += g / W
+    img = np.fft.fftshift(np.fft.ifft2(np.fft.ifftshift(acc, axes=(-2, -1))), axes=(-2, -1)).real * N * N
+    img /= (T * C) if avg_time else C
+    a = oracle_mod.image_avg(vis, uvw, fr, N, pix, weighting, avg_time)
+    want = img[0] if avg_time else img
+    assert np.max(np.abs(a - want)) <= 1e-10 * np.max(np.abs(want))
+
+
+def test_avg_centre_pixel_closed_form_and_zero_images_count(oracle_mod):
+    # centre pixel of one image = sum(2 Re V_in) / W; the mean divides by the NUMBER OF CHANNELS even when a
+    # channel has nothing on the grid (its image is zero)
+    vis, uvw, fr, N, pix = _avg_inputs(7, T=1, C=3, P=1)
+    fr = fr.copy()
+    fr[2] = 5e9                                              # this channel throws every sample off the grid
+    ci = oracle_mod.cells(uvw, fr, N, pix)
+    assert np.all(ci[0, 2] < 0)
+    a = oracle_mod.image_avg(vis, uvw, fr, N, pix, 0)
+    want = 0.0
+    for c in range(2):
+        ok = ci[0, c] >= 0
+        want += (2.0 * vis[0, c, 0][ok].real.astype(np.float64).sum()) / (2.0 * ok.sum())
+    assert abs(a[0, 0, N // 2, N // 2] - want / 3.0) <= 1e-12 * max(1.0, abs(want))
