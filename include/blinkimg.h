@@ -40,7 +40,7 @@ extern "C" {
 typedef struct blink_c64 { float re, im; } blink_c64;       /* == float2 == complex64 */
 
 enum { BLINK_W_NATURAL = 0, BLINK_W_UNIFORM = 1 };
-enum { BLINK_OP_GRID = 0, BLINK_OP_FFT2D = 1, BLINK_OP_IMAGE = 2, BLINK_OP_IMAGE_HOST = 3 };
+enum { BLINK_OP_GRID = 0, BLINK_OP_FFT2D = 1, BLINK_OP_IMAGE = 2, BLINK_OP_IMAGE_HOST = 3, BLINK_OP_IMAGE_AVG = 4 };
 enum {
     BLINK_OK = 0,
     BLINK_ERR_INVALID_ARG = -1,   /* NULL / misaligned pointer, non-positive size, bad enum          */
@@ -129,6 +129,24 @@ int blink_image_host(const blink_c64 *vis_host, const float *uvw_m_host, const d
                      int T, int C, int P, int B, int n_pix, double pixscale_rad, int weighting,
                      float *image_host, float *wsum_host,
                      void *workspace, size_t workspace_bytes);
+
+/*
+ * Dirty images averaged over fine channels, or over fine channels and timesteps ("Images
+ * belonging to the same time bin are averaged together"; L251 "averaged in time ... and frequency over the
+ * 30.72 MHz bandwidth"; reading R14):
+ *   avg_time == 0:  image_avg[t*P + p] = (1/C)     sum_c     image[(t*C + c)*P + p]        out [T*P][N][N]
+ *   avg_time != 0:  image_avg[p]       = (1/(T*C)) sum_{t,c} image[(t*C + c)*P + p]        out [P][N][N]
+ * with image[] exactly what blink_image produces (each image normalised by its own W; a (t,c) with W = 0
+ * contributes a zero image and still counts in the mean).  The individual images are never formed: by linearity
+ * the samples are scattered, pre-multiplied by 1/(n W_tc) (uniform: also by 1/count of their cell), into one
+ * combined uv grid per output image with global vector atomics, and only those grids are transformed.
+ * Inputs as blink_grid; wsum out [T*C] as blink_image.  `workspace` >= blink_workspace_bytes(BLINK_OP_IMAGE_AVG)
+ * (minimum via *min_bytes): the combined grids and, for uniform weighting, per-CTA count planes.
+ */
+int blink_image_avg(const blink_c64 *vis, const float *uvw_m, const double *freqs_hz,
+                    int T, int C, int P, int B, int n_pix, double pixscale_rad, int weighting,
+                    int avg_time, float *image_avg, float *wsum,
+                    void *workspace, size_t workspace_bytes, void *stream);
 
 #ifdef __cplusplus
 }

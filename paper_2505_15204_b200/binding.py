@@ -17,12 +17,12 @@ _SO = os.path.join(_HERE, "libblinkimg.so")
 _lib = None
 
 W_NATURAL, W_UNIFORM = 0, 1
-OP_GRID, OP_FFT2D, OP_IMAGE, OP_IMAGE_HOST = 0, 1, 2, 3
+OP_GRID, OP_FFT2D, OP_IMAGE, OP_IMAGE_HOST, OP_IMAGE_AVG = 0, 1, 2, 3, 4
 OPT_IMAGE_PATH, OPT_FUSED_CTAS, OPT_GRID_CHUNK_B = 0, 1, 2
 
 EXPORTS = ["blink_strerror", "blink_last_cuda_error", "blink_set_option", "blink_get_option",
            "blink_kernel_launches", "blink_workspace_bytes", "blink_grid", "blink_fft2d_inverse",
-           "blink_image", "blink_image_host"]
+           "blink_image", "blink_image_host", "blink_image_avg"]
 
 
 class BlinkError(RuntimeError):
@@ -62,6 +62,8 @@ def lib():
         L.blink_image.argtypes = [vp, vp, vp, i, i, i, i, i, d, i, vp, vp, vp, vp, vp, sz, vp]
         L.blink_image_host.restype = i
         L.blink_image_host.argtypes = [vp, vp, vp, i, i, i, i, i, d, i, vp, vp, vp, sz]
+        L.blink_image_avg.restype = i
+        L.blink_image_avg.argtypes = [vp, vp, vp, i, i, i, i, i, d, i, i, vp, vp, vp, sz, vp]
         _lib = L
     return _lib
 
@@ -169,6 +171,29 @@ def blink_image(vis: torch.Tensor, uvw_m: torch.Tensor, freqs_hz, n_pix: int, pi
                            _ptr(workspace), workspace.numel(), _stream(dev))
     _check(rc, "blink_image")
     return dict(image=image, wsum=wsum, cell_idx=cell_idx, counts=counts)
+
+
+def blink_image_avg(vis: torch.Tensor, uvw_m: torch.Tensor, freqs_hz, n_pix: int, pixscale_rad: float, weighting: int = 0,
+                    avg_time: bool = False, image_avg: Optional[torch.Tensor] = None,
+                    workspace: Optional[torch.Tensor] = None, wsum: Optional[torch.Tensor] = None):
+    """Mean of the dirty images over channels (-> [T*P][N][N]) or over timesteps and channels (-> [P][N][N])."""
+    _dev(vis, torch.complex64, "vis"); _dev(uvw_m, torch.float32, "uvw_m")
+    T, C, P, B = vis.shape
+    fr = _freqs(freqs_hz)
+    dev = vis.device
+    n_out = P if avg_time else T * P
+    if image_avg is None:
+        image_avg = torch.empty((n_out, n_pix, n_pix), dtype=torch.float32, device=dev)
+    if wsum is None:
+        wsum = torch.empty(T * C, dtype=torch.float32, device=dev)
+    if workspace is None:
+        rec, _ = blink_workspace_bytes(OP_IMAGE_AVG, T, C, P, B, n_pix, weighting)
+        workspace = torch.empty(max(rec, 16), dtype=torch.uint8, device=dev)
+    rc = lib().blink_image_avg(_ptr(vis), _ptr(uvw_m), fr.ctypes.data_as(ctypes.c_void_p), T, C, P, B, n_pix,
+                               float(pixscale_rad), int(weighting), int(bool(avg_time)), _ptr(image_avg), _ptr(wsum),
+                               _ptr(workspace), workspace.numel(), _stream(dev))
+    _check(rc, "blink_image_avg")
+    return dict(image_avg=image_avg, wsum=wsum)
 
 
 def blink_image_host(vis_host: torch.Tensor, uvw_host: torch.Tensor, freqs_hz, n_pix: int, pixscale_rad: float,

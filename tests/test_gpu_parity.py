@@ -359,3 +359,77 @@ def test_config3_full_size_sampled(bk, oracle_mod):
     peak = res["image"].reshape(T * C, -1).abs().amax(dim=1).double().cpu().numpy()
     assert np.max(np.abs(centre - want) / peak) <= TOL
     assert bool(torch.isfinite(res["image"]).all())
+
+
+# --------------------------------------------------------------------------- blink_image_avg
+def _check_avg(bk, oracle_mod, w, avg_time, workspace=None):
+    res = bk.blink_image_avg(w.vis, w.uvw_m, w.freqs_hz, w.n_pix, w.pixscale_rad, w.weighting, avg_time=avg_time,
+                             workspace=workspace)
+    torch.cuda.synchronize()
+    vis, uvw = w.vis.cpu().numpy(), w.uvw_m.cpu().numpy()
+    ref = oracle_mod.image_avg(vis, uvw, w.freqs_hz, w.n_pix, w.pixscale_rad, w.weighting, avg_time)
+    ref = ref.reshape(-1, w.n_pix, w.n_pix)
+    got = res["image_avg"].cpu().numpy()
+    assert got.shape == ref.shape
+    for k in range(ref.shape[0]):
+        assert _img_err(got[k], ref[k]) <= TOL, (k, _img_err(got[k], ref[k]))
+    # wsum is the per-(t,c) weight sum of blink_image, bit-exact
+    ci = oracle_mod.cells(uvw, w.freqs_hz, w.n_pix, w.pixscale_rad)
+    wsum = res["wsum"].cpu().numpy().reshape(w.T, w.C)
+    for t in range(w.T):
+        for c in range(w.C):
+            ok = ci[t, c] >= 0
+            if w.weighting == 0:
+                want = 2 * int(ok.sum())
+            else:
+                cells = ci[t, c][ok]
+                mir = (w.n_pix - cells // w.n_pix) * w.n_pix + (w.n_pix - cells % w.n_pix)
+                want = len(np.unique(np.concatenate([cells, mir])))
+            assert wsum[t, c] == np.float32(want)
+    return res
+
+
+@pytest.mark.parametrize("weighting", [0, 1])
+@pytest.mark.parametrize("avg_time", [False, True])
+def test_image_avg_random(bk, oracle_mod, weighting, avg_time):
+    from paper_2505_15204_b200 import workloads
+    w = workloads.make_random(T=3, C=5, P=2, B=1237, n_pix=128, weighting=weighting, seed=41, device="cuda", fill=1.1)
+    w.uvw_m[1, 9, 1] = float("nan")
+    _check_avg(bk, oracle_mod, w, avg_time)
+    if weighting == 1:                                          # minimum workspace: a single count plane
+        _, mn = bk.blink_workspace_bytes(bk.OP_IMAGE_AVG, w.T, w.C, w.P, w.B, w.n_pix, weighting)
+        _check_avg(bk, oracle_mod, w, avg_time, workspace=torch.empty(mn, dtype=torch.uint8, device="cuda"))
+
+
+@pytest.mark.parametrize("cfg,T,C", [(3, 2, 6), (4, 1, 3)])
+def test_image_avg_reduced_configs(bk, oracle_mod, cfg, T, C):
+    from paper_2505_15204_b200 import workloads
+    w = workloads.make_config(cfg, device="cuda", T=T, C=C)
+    res = _check_avg(bk, oracle_mod, w, False)
+    # the averaged image IS the mean of blink_image's images (same library, different path)
+    full = bk.blink_image(w.vis, w.uvw_m, w.freqs_hz, w.n_pix, w.pixscale_rad, w.weighting)
+    mean = full["image"].reshape(w.T, w.C, w.P, w.n_pix, w.n_pix).double().mean(dim=1).reshape(-1, w.n_pix, w.n_pix)
+    got = res["image_avg"].double()
+    assert float((got - mean).abs().max() / mean.abs().max()) <= TOL
+
+
+def test_image_avg_degenerate(bk, oracle_mod):
+    from paper_2505_15204_b200 import workloads
+    # all V = 1: every image has 1.0 at the centre, so has the mean; one channel entirely off the grid halves it
+    w = workloads.make_random(T=1, C=2, P=1, B=500, n_pix=64, weighting=0, seed=43, device="cuda", fill=0.7)
+    w.vis[:] = 1.0
+    r = bk.blink_image_avg(w.vis, w.uvw_m, w.freqs_hz, w.n_pix, w.pixscale_rad, 0)
+    assert abs(float(r["image_avg"][0, 32, 32]) - 1.0) < 1e-5
+    w.freqs_hz = np.array([w.freqs_hz[0], 5e10])
+    r = bk.blink_image_avg(w.vis, w.uvw_m, w.freqs_hz, w.n_pix, w.pixscale_rad, 0)
+    assert abs(float(r["image_avg"][0, 32, 32]) - 0.5) < 1e-5 and float(r["wsum"][1]) == 0.0
+    # everything off the grid: zero image
+    w.uvw_m[:] = 1e7
+    r = bk.blink_image_avg(w.vis, w.uvw_m, w.freqs_hz, w.n_pix, w.pixscale_rad, 1, avg_time=True)
+    assert torch.all(r["image_avg"] == 0) and torch.all(r["wsum"] == 0)
+    # many samples in one cell (atomic contention, uniform count = 2 cells)
+    w = workloads.make_random(T=1, C=3, P=1, B=2000, n_pix=64, weighting=1, seed=44, device="cuda")
+    w.uvw_m[:] = 0.0
+    w.uvw_m[0, :, 0] = 4.2
+    w.uvw_m[0, :, 1] = -7.7
+    _check_avg(bk, oracle_mod, w, False)
