@@ -171,6 +171,7 @@ def main():
     ap.add_argument("--path", type=int, default=0, help="BLINK_OPT_IMAGE_PATH: 0 auto, 1 unfused, 2 fused")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--no-avg", action="store_true")
     ap.add_argument("--T", type=int, default=None, help="reduce timesteps (debug only; invalidates the headline)")
     args = ap.parse_args()
 
@@ -234,6 +235,40 @@ def main():
     ms_per_step = total_ms / args.steps
     value = world * n_img / (ms_per_step * 1e-3)
 
+    # ---- channel-averaged images (blink_image_avg), same inputs, device-resident -------
+    avg = None
+    if not args.no_avg:
+        try:
+            rec_a, _ = bk.blink_workspace_bytes(bk.OP_IMAGE_AVG, T, C, P, B, N, w.weighting)
+            ws_a = torch.empty(max(rec_a, 16), dtype=torch.uint8, device=dev)
+            img_a = torch.empty((T * P, N, N), dtype=torch.float32, device=dev)
+            run_a = lambda: bk.blink_image_avg(w.vis, w.uvw_m, w.freqs_hz, N, w.pixscale_rad, w.weighting, avg_time=False,
+                                               image_avg=img_a, workspace=ws_a, wsum=wsum)
+            for _ in range(args.warmup):
+                run_a()
+            barrier()
+            l0 = bk.kernel_launches()
+            ea = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+            ea[0].record()
+            for _ in range(args.steps):
+                run_a()
+            ea[1].record()
+            barrier()
+            ms_a = torch.tensor([ea[0].elapsed_time(ea[1]) / args.steps], device=dev)
+            if world > 1:
+                dist.all_reduce(ms_a, op=dist.ReduceOp.MAX)
+            ms_a = float(ms_a.item())
+            bytes_a = n_img * 8 * B + 12 * T * B + T * P * 4 * N * N
+            avg = {"api": "blink_image_avg (mean over the C channels of every timestep; PAPER.md L284)",
+                   "ms_per_step": ms_a, "images_in_per_s": world * n_img / (ms_a * 1e-3),
+                   "gvis_per_s": world * n_img * B / (ms_a * 1e-3) / 1e9, "images_out": T * P,
+                   "gpu_launches_per_step": (bk.kernel_launches() - l0) // args.steps,
+                   "algorithmic_bytes_per_step": bytes_a, "model": "n_img*8B + 12TB + T*P*4N^2 (vis + uvw read once, averaged images written)",
+                   "hbm_gbs": bytes_a / (ms_a * 1e-3) / 1e9}
+            del ws_a, img_a
+        except Exception as ex:  # report, never hide
+            avg = {"error": str(ex)[:200]}
+
     # ---- end to end through the host-buffer entry point (rank-local, then max over ranks) -----------------
     e2e = None
     if not args.no_e2e:
@@ -293,6 +328,8 @@ def main():
                     roofline["traffic_source"] = row["source"]
         except Exception:
             pass
+    if avg and "hbm_gbs" in avg:
+        avg["frac_of_hbm_peak"] = avg["hbm_gbs"] / peak
     cpu = None
     if not args.no_cpu:
         cores = os.cpu_count() or 1
@@ -307,7 +344,7 @@ def main():
                    (w.vis.numel() * 8 / 1e9, n_img * N * N * 4 / 1e9),
                    "image_path": args.path, "parallelism": f"independent batches x{world}"},
         "gvis_per_s": value * B / 1e9,
-        "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu,
+        "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu, "avg_mode": avg,
         "ms_per_step_each": per_step,
     }
     print(json.dumps(out))

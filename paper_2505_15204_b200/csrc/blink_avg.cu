@@ -101,14 +101,103 @@ avg_grid_kernel(const AvgArgs a, const __grid_constant__ ScaleBlock sc)
     }
 }
 
+// ---- natural weighting: run-length scatter --------------------------------------------------------------
+// W of every (t,c) first (cells only, no visibilities).  Same thread layout as the scatter below: one thread per
+// (baseline, timestep, chunk of channels) keeps (u, v) in registers and walks the channels; a warp's 32 baselines
+// are counted with one ballot per channel into shared counters, flushed with one global atomic per channel.
+constexpr int kAvgChunk = 128;
+__global__ void __launch_bounds__(kAvgThreads)
+avg_count_kernel(const AvgArgs a, const __grid_constant__ ScaleBlock sc, unsigned *__restrict__ n_in, int t_lo, int c_lo, int nc,
+                 int nchunk, int bblocks)
+{
+    __shared__ unsigned s_cnt[kAvgChunk];
+    const int bx = (int)(blockIdx.x % (unsigned)bblocks);
+    int y = (int)(blockIdx.x / (unsigned)bblocks);
+    const int k = y % nchunk;
+    const int t = t_lo + y / nchunk;
+    const int b = bx * kAvgThreads + threadIdx.x;
+    for (int i = threadIdx.x; i < kAvgChunk; i += kAvgThreads) s_cnt[i] = 0u;
+    __syncthreads();
+    const int n = a.n, h = n / 2;
+    float u = __int_as_float(0x7fc00000), v = u;                        // NaN: never on the grid
+    if (b < a.B) { u = a.uvw_m[((size_t)t * a.B + b) * 3]; v = a.uvw_m[((size_t)t * a.B + b) * 3 + 1]; }
+    const int c0 = c_lo + k * kAvgChunk, c1 = min(c0 + kAvgChunk, c_lo + nc);
+    for (int c = c0; c < c1; ++c) {
+        const unsigned m = __ballot_sync(0xffffffffu, cell_of(u, v, sc.s[c - a.c_base], n, h) >= 0);
+        if ((threadIdx.x & 31) == 0 && m) atomicAdd(&s_cnt[c - c0], (unsigned)__popc(m));
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < c1 - c0; i += kAvgThreads)
+        if (s_cnt[i]) atomicAdd(&n_in[(size_t)t * a.C + c0 + i], s_cnt[i]);
+}
+// wsum[tc] = 2 * samples placed, winv[tc] = 1 / (n W) or 0 (in place over the counters)
+__global__ void avg_winv_kernel(const AvgArgs a, float *__restrict__ winv)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= a.ntc) return;
+    const int tc = a.tc0 + i;
+    const unsigned n_in = reinterpret_cast<const unsigned *>(winv)[tc];
+    const float W = (float)(2u * n_in);
+    a.wsum[tc] = W;
+    winv[tc] = n_in > 0u ? a.inv_navg / W : 0.f;
+}
+
+// One thread per (baseline, timestep, polarisation, chunk of kAvgChunk channels).  Along the channel axis a
+// baseline's cell moves slowly (the scale changes by 2.6e-4 per 40 kHz channel), so the thread keeps the
+// weighted sum of the current cell in registers and only touches the grid when the cell changes: ~20-60x fewer
+// atomics than one per sample.  Visibility reads stay coalesced (baseline is the fastest axis of vis).
+__global__ void __launch_bounds__(kAvgThreads)
+avg_scatter_runs_kernel(const AvgArgs a, const __grid_constant__ ScaleBlock sc, const float *__restrict__ winv, int t_lo,
+                        int c_lo, int nc, int nchunk, int bblocks)
+{
+    const int bx = (int)(blockIdx.x % (unsigned)bblocks);
+    int y = (int)(blockIdx.x / (unsigned)bblocks);
+    const int k = y % nchunk; y /= nchunk;
+    const int p = y % a.P;
+    const int t = t_lo + y / a.P;
+    const int b = bx * kAvgThreads + threadIdx.x;
+    if (b >= a.B) return;
+    const int n = a.n, h = n / 2;
+    const size_t n2 = (size_t)n * n;
+    const float u = a.uvw_m[((size_t)t * a.B + b) * 3], v = a.uvw_m[((size_t)t * a.B + b) * 3 + 1];
+    float2 *g = a.grid + (size_t)(a.avg_time ? p : t * a.P + p) * n2;
+    const int c0 = c_lo + k * kAvgChunk, c1 = min(c0 + kAvgChunk, c_lo + nc);
+    int cur = -1;
+    float2 acc = make_float2(0.f, 0.f);
+    auto flush = [&] {
+        if (cur >= 0) {
+            atomicAdd(&g[cur], acc);
+            atomicAdd(&g[mirror_of(cur, n)], make_float2(acc.x, -acc.y));
+        }
+    };
+#pragma unroll 4
+    for (int c = c0; c < c1; ++c) {
+        const int cell = cell_of(u, v, sc.s[c - a.c_base], n, h);
+        if (cell != cur) {
+            flush();
+            cur = cell;
+            acc = make_float2(0.f, 0.f);
+        }
+        if (cell >= 0) {
+            const float w = __ldg(winv + (size_t)t * a.C + c);
+            const float2 x = __ldcs(a.vis + ((size_t)(t * a.C + c) * a.P + p) * a.B + b);
+            acc.x = fmaf(x.x, w, acc.x);
+            acc.y = fmaf(x.y, w, acc.y);
+        }
+    }
+    flush();
+}
+
 static size_t avg_grid_bytes(int T, int P, int n_pix, int avg_time)
 {
     return align_up((size_t)(avg_time ? 1 : T) * P * n_pix * n_pix * sizeof(float2), 256);
 }
 static int avg_max_planes() { return 2 * (sm_count() > 0 ? sm_count() : 148); }
-size_t avg_workspace_bytes(int T, int P, int n_pix, int weighting, bool minimum)
+// workspace: combined grids | natural: winv [T*C] float | uniform: count planes
+size_t avg_workspace_bytes(int T, int C, int P, int n_pix, int weighting, bool minimum)
 {
     size_t b = avg_grid_bytes(T, P, n_pix, 0);
+    if (weighting == BLINK_W_NATURAL) b += align_up((size_t)T * C * sizeof(float), 256);
     if (weighting == BLINK_W_UNIFORM) {
         const size_t plane = (size_t)n_pix * n_pix * sizeof(uint32_t);
         size_t planes = minimum ? 1 : (size_t)avg_max_planes();
@@ -139,8 +228,10 @@ extern "C" int blink_image_avg(const blink_c64 *vis, const float *uvw_m, const d
     const size_t n2 = (size_t)n_pix * n_pix;
     const size_t gbytes = avg_grid_bytes(T, P, n_pix, avg_time ? 1 : 0);
     const size_t plane = n2 * sizeof(uint32_t);
-    if (!workspace || (reinterpret_cast<uintptr_t>(workspace) & 255u) || workspace_bytes < gbytes + (uni ? plane : 0))
+    const size_t winv_bytes = align_up((size_t)T * C * sizeof(float), 256);
+    if (!workspace || (reinterpret_cast<uintptr_t>(workspace) & 255u) || workspace_bytes < gbytes + (uni ? plane : winv_bytes))
         return BLINK_ERR_WORKSPACE;
+    float *winv = reinterpret_cast<float *>(static_cast<unsigned char *>(workspace) + gbytes);   // natural only
     float2 *grid = static_cast<float2 *>(workspace);
     uint32_t *cnt = uni ? reinterpret_cast<uint32_t *>(static_cast<unsigned char *>(workspace) + gbytes) : nullptr;
     int ctas = 8 * (sm_count() > 0 ? sm_count() : 148);
@@ -163,9 +254,26 @@ extern "C" int blink_image_avg(const blink_c64 *vis, const float *uvw_m, const d
         a.tc0 = tc; a.ntc = end - tc; a.c_base = c_base;
         a.grid = grid; a.wsum = wsum; a.cnt = cnt;
         a.inv_navg = (float)(1.0 / (avg_time ? (double)T * C : (double)C));
-        const int gridx = a.ntc < ctas ? a.ntc : ctas;
-        avg_grid_kernel<<<gridx, kAvgThreads, 0, st>>>(a, sc);
-        BLINK_LAUNCH_CHECK("avg_grid_kernel");
+        if (uni) {
+            const int gridx = a.ntc < ctas ? a.ntc : ctas;
+            avg_grid_kernel<<<gridx, kAvgThreads, 0, st>>>(a, sc);
+            BLINK_LAUNCH_CHECK("avg_grid_kernel");
+        } else {
+            // this segment: all timesteps x all channels (C <= 1024) or one timestep x one block of channels
+            const int nt = (C <= 1024) ? T : 1, nc = (C <= 1024) ? C : a.ntc;
+            const int nchunk = (nc + kAvgChunk - 1) / kAvgChunk, bblocks = (B + kAvgThreads - 1) / kAvgThreads;
+            if ((long long)bblocks * nchunk * nt > 0x7fffffffLL) return BLINK_ERR_UNSUPPORTED;
+            BLINK_CUDA_TRY(cudaMemsetAsync(winv + tc, 0, (size_t)a.ntc * sizeof(float), st));
+            avg_count_kernel<<<(unsigned)(bblocks * nchunk * nt), kAvgThreads, 0, st>>>(a, sc, reinterpret_cast<unsigned *>(winv), t, c,
+                                                                                       nc, nchunk, bblocks);
+            BLINK_LAUNCH_CHECK("avg_count_kernel");
+            avg_winv_kernel<<<(a.ntc + 255) / 256, 256, 0, st>>>(a, winv);
+            BLINK_LAUNCH_CHECK("avg_winv_kernel");
+            const long long blocks = (long long)bblocks * nchunk * P * nt;
+            if (blocks > 0x7fffffffLL) return BLINK_ERR_UNSUPPORTED;
+            avg_scatter_runs_kernel<<<(unsigned)blocks, kAvgThreads, 0, st>>>(a, sc, winv, t, c, nc, nchunk, bblocks);
+            BLINK_LAUNCH_CHECK("avg_scatter_runs_kernel");
+        }
         tc = end;
     }
     // steps a4-a5 on the combined grids: already normalised, so no scale

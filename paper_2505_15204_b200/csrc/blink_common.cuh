@@ -53,17 +53,25 @@ const float2 *twiddle_table();          // device pointer (after ensure_device()
 struct ScaleBlock { float s[1024]; };
 
 #ifdef __CUDACC__
+// Round to nearest, ties to even, WITHOUT the quarter-rate conversion unit (FRND / F2I): adding and subtracting
+// 1.5 * 2^23 with two correctly rounded fp32 adds (never contracted into an fma) gives exactly rint(x) for
+// |x| < 2^22, and the integer sits in the mantissa of the intermediate sum.  For larger |x| (and inf / NaN) the
+// result keeps its huge magnitude (or stays NaN), so the range test that follows still rejects it; `i` is only
+// meaningful once that test has passed.  Measured: the averaging path was bound by 4 FRND/F2I per sample.
+__device__ __forceinline__ float rint_rne(float x, int &i)
+{
+    const float t = __fadd_rn(x, 12582912.0f);
+    i = __float_as_int(t) - 0x4B400000;
+    return __fadd_rn(t, -12582912.0f);
+}
 // step a1 (R2, R4): nearest cell of one baseline, bit-exact twin of the oracle's fp32 recipe
 __device__ __forceinline__ bool cell_coords(float u_m, float v_m, float s, int h, int &iu, int &iv)
 {
     const float x = __fmul_rn(u_m, s);            // one IEEE fp32 multiply, never contracted
     const float y = __fmul_rn(v_m, s);
-    const float xr = rintf(x), yr = rintf(y);     // round to nearest, ties to even
+    const float xr = rint_rne(x, iu), yr = rint_rne(y, iv);     // round to nearest, ties to even
     const float lim = (float)(h - 1);
-    if (!(fabsf(xr) <= lim && fabsf(yr) <= lim)) return false;      // NaN fails
-    iu = (int)xr;
-    iv = (int)yr;
-    return true;
+    return fabsf(xr) <= lim && fabsf(yr) <= lim;                // NaN fails
 }
 __device__ __forceinline__ int cell_of(float u_m, float v_m, float s, int n, int h)
 {

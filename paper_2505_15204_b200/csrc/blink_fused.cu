@@ -228,8 +228,9 @@ fused_image_kernel(const FusedArgs a, const __grid_constant__ ScaleBlock sc, con
         const uint2 *svb = a.svb + (size_t)t * B;
         // column of sorted sample value x = |u_m| for this channel (H = beyond the grid, NaN included)
         auto col_of = [&](float x) -> int {
-            const float xr = rintf(__fmul_rn(x, s));
-            return (xr <= lim) ? (int)xr : H;
+            int i;
+            const float xr = rint_rne(__fmul_rn(x, s), i);
+            return (xr <= lim) ? i : H;
         };
         int n_cp = 0, ulim = 0, n_box = 0;
         float wsum_val = 0.f;
@@ -289,9 +290,9 @@ fused_image_kernel(const FusedArgs a, const __grid_constant__ ScaleBlock sc, con
             int my_in = 0, my_occ = 0;
             // one sample of this group's column pair: accumulate V (or conj V) into its cell with shared atomics
             auto grid_one = [&](uint2 sq, bool second, bool col0) {
-                const float yr = rintf(__fmul_rn(__uint_as_float(sq.x), s));
+                int iv;
+                const float yr = rint_rne(__fmul_rn(__uint_as_float(sq.x), s), iv);
                 if (fabsf(yr) <= lim) {                         // NaN fails; |iu| <= H-1 by construction
-                    const int iv = (int)yr;
                     float2 vv = visrow[sq.y & 0x7fffffffu];
                     if (sq.y >> 31) vv.y = -vv.y;
                     float2 *col = second ? c1 : c0;
