@@ -119,16 +119,72 @@ avg_count_kernel(const AvgArgs a, const __grid_constant__ ScaleBlock sc, unsigne
     for (int i = threadIdx.x; i < kAvgChunk; i += kAvgThreads) s_cnt[i] = 0u;
     __syncthreads();
     const int n = a.n, h = n / 2;
-    float u = __int_as_float(0x7fc00000), v = u;                        // NaN: never on the grid
-    if (b < a.B) { u = a.uvw_m[((size_t)t * a.B + b) * 3]; v = a.uvw_m[((size_t)t * a.B + b) * 3 + 1]; }
+    // A sample is on the grid iff |rint(u s)| <= h-1 and |rint(v s)| <= h-1.  h-1 is odd, so the tie |x| = h-1/2
+    // rounds away to h: the test is |u s| < h - 1/2 on the fp32 products, and because fp32 multiplication by
+    // s > 0 is monotone it is ONE product: max(|u|, |v|) * s < h - 1/2 (NaN in either coordinate fails).
+    float m_uv = __int_as_float(0x7fc00000);                            // NaN: never on the grid
+    if (b < a.B) {
+        const float u = a.uvw_m[((size_t)t * a.B + b) * 3], v = a.uvw_m[((size_t)t * a.B + b) * 3 + 1];
+        m_uv = (u == u && v == v) ? fmaxf(fabsf(u), fabsf(v)) : m_uv;
+    }
+    (void)n;
+    const float edge = (float)h - 0.5f;
     const int c0 = c_lo + k * kAvgChunk, c1 = min(c0 + kAvgChunk, c_lo + nc);
     for (int c = c0; c < c1; ++c) {
-        const unsigned m = __ballot_sync(0xffffffffu, cell_of(u, v, sc.s[c - a.c_base], n, h) >= 0);
+        const unsigned m = __ballot_sync(0xffffffffu, __fmul_rn(m_uv, sc.s[c - a.c_base]) < edge);
         if ((threadIdx.x & 31) == 0 && m) atomicAdd(&s_cnt[c - c0], (unsigned)__popc(m));
     }
     __syncthreads();
     for (int i = threadIdx.x; i < c1 - c0; i += kAvgThreads)
         if (s_cnt[i]) atomicAdd(&n_in[(size_t)t * a.C + c0 + i], s_cnt[i]);
+}
+// Faster route to the same counts when a timestep's baselines fit in shared memory: the predicate
+// max(|u|,|v|) * s < h - 1/2 is monotone in max(|u|,|v|), so sort that key once per timestep (bitonic, keys only)
+// and the count of every channel is ONE binary search with the exact predicate.
+constexpr int kAvgSortMaxB = 16384;
+__global__ void __launch_bounds__(1024) avg_sortm_kernel(const float *__restrict__ uvw_m, int B, int np2, float *__restrict__ sorted_m)
+{
+    extern __shared__ float key[];
+    const float *uvw = uvw_m + (size_t)blockIdx.x * B * 3;
+    for (int i = threadIdx.x; i < np2; i += 1024) {
+        float k = __int_as_float(0x7f800000);                            // +inf: padding, NaN coordinates
+        if (i < B) {
+            const float u = uvw[3 * i], v = uvw[3 * i + 1];
+            if (u == u && v == v) k = fmaxf(fabsf(u), fabsf(v));
+        }
+        key[i] = k;
+    }
+    __syncthreads();
+    for (int k = 2; k <= np2; k <<= 1)
+        for (int j = k >> 1; j > 0; j >>= 1) {
+            for (int i = threadIdx.x; i < np2; i += 1024) {
+                const int x = i ^ j;
+                if (x > i) {
+                    const float p = key[i], q = key[x];
+                    if ((p > q) == ((i & k) == 0)) { key[i] = q; key[x] = p; }
+                }
+            }
+            __syncthreads();
+        }
+    for (int i = threadIdx.x; i < B; i += 1024) sorted_m[(size_t)blockIdx.x * B + i] = key[i];
+}
+__global__ void avg_wsearch_kernel(const AvgArgs a, const __grid_constant__ ScaleBlock sc, const float *__restrict__ sorted_m,
+                                   float *__restrict__ winv)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= a.ntc) return;
+    const int tc = a.tc0 + i;
+    const int t = tc / a.C, c = tc - t * a.C;
+    const float s = sc.s[c - a.c_base], edge = (float)(a.n / 2) - 0.5f;
+    const float *m = sorted_m + (size_t)t * a.B;
+    int lo = 0, hi = a.B;                                               // first index whose sample is off the grid
+    while (lo < hi) {
+        const int mid = (lo + hi) >> 1;
+        if (__fmul_rn(__ldg(m + mid), s) < edge) lo = mid + 1; else hi = mid;
+    }
+    const float W = (float)(2 * lo);
+    a.wsum[tc] = W;
+    winv[tc] = lo > 0 ? a.inv_navg / W : 0.f;
 }
 // wsum[tc] = 2 * samples placed, winv[tc] = 1 / (n W) or 0 (in place over the counters)
 __global__ void avg_winv_kernel(const AvgArgs a, float *__restrict__ winv)
@@ -170,15 +226,23 @@ avg_scatter_runs_kernel(const AvgArgs a, const __grid_constant__ ScaleBlock sc, 
             atomicAdd(&g[mirror_of(cur, n)], make_float2(acc.x, -acc.y));
         }
     };
+    // the cell is a function of the two "magic sums" u s + 1.5 2^23, v s + 1.5 2^23 (blink_common.cuh rint_rne):
+    // while their bits do not change nothing has to be recomputed
+    const float lim = (float)(h - 1);
+    int pu = 0x7fffffff, pv = 0x7fffffff;
 #pragma unroll 4
     for (int c = c0; c < c1; ++c) {
-        const int cell = cell_of(u, v, sc.s[c - a.c_base], n, h);
-        if (cell != cur) {
+        const float s = sc.s[c - a.c_base];
+        const float tu = __fadd_rn(__fmul_rn(u, s), 12582912.0f), tv = __fadd_rn(__fmul_rn(v, s), 12582912.0f);
+        const int bu = __float_as_int(tu), bv = __float_as_int(tv);
+        if (bu != pu || bv != pv) {
             flush();
-            cur = cell;
+            pu = bu; pv = bv;
+            const float xr = __fadd_rn(tu, -12582912.0f), yr = __fadd_rn(tv, -12582912.0f);
+            cur = (fabsf(xr) <= lim && fabsf(yr) <= lim) ? (bv - 0x4B400000 + h) * n + (bu - 0x4B400000 + h) : -1;
             acc = make_float2(0.f, 0.f);
         }
-        if (cell >= 0) {
+        if (cur >= 0) {
             const float w = __ldg(winv + (size_t)t * a.C + c);
             const float2 x = __ldcs(a.vis + ((size_t)(t * a.C + c) * a.P + p) * a.B + b);
             acc.x = fmaf(x.x, w, acc.x);
@@ -194,10 +258,10 @@ static size_t avg_grid_bytes(int T, int P, int n_pix, int avg_time)
 }
 static int avg_max_planes() { return 2 * (sm_count() > 0 ? sm_count() : 148); }
 // workspace: combined grids | natural: winv [T*C] float | uniform: count planes
-size_t avg_workspace_bytes(int T, int C, int P, int n_pix, int weighting, bool minimum)
+size_t avg_workspace_bytes(int T, int C, int P, int B, int n_pix, int weighting, bool minimum)
 {
     size_t b = avg_grid_bytes(T, P, n_pix, 0);
-    if (weighting == BLINK_W_NATURAL) b += align_up((size_t)T * C * sizeof(float), 256);
+    if (weighting == BLINK_W_NATURAL) b += align_up((size_t)T * C * sizeof(float), 256) + (minimum ? 0 : align_up((size_t)T * B * sizeof(float), 256));
     if (weighting == BLINK_W_UNIFORM) {
         const size_t plane = (size_t)n_pix * n_pix * sizeof(uint32_t);
         size_t planes = minimum ? 1 : (size_t)avg_max_planes();
@@ -232,6 +296,20 @@ extern "C" int blink_image_avg(const blink_c64 *vis, const float *uvw_m, const d
     if (!workspace || (reinterpret_cast<uintptr_t>(workspace) & 255u) || workspace_bytes < gbytes + (uni ? plane : winv_bytes))
         return BLINK_ERR_WORKSPACE;
     float *winv = reinterpret_cast<float *>(static_cast<unsigned char *>(workspace) + gbytes);   // natural only
+    // sorted max(|u|,|v|) per timestep, when it fits in shared memory and in the workspace (else: ballot counting)
+    float *sorted_m = nullptr;
+    const size_t sm_bytes = align_up((size_t)T * B * sizeof(float), 256);
+    // (the sort costs ~0.1 ms whatever the batch: only worth it for large batches)
+    const int wopt = option(BLINK_OPT_AVG_WSUM);
+    const bool want_sort = wopt == 1 || (wopt == 0 && (long long)T * C * B >= (32LL << 20));
+    if (!uni && want_sort && B <= kAvgSortMaxB && workspace_bytes >= gbytes + winv_bytes + sm_bytes) {
+        sorted_m = reinterpret_cast<float *>(static_cast<unsigned char *>(workspace) + gbytes + winv_bytes);
+        int np2 = 1;
+        while (np2 < B) np2 <<= 1;
+        BLINK_CUDA_TRY(cudaFuncSetAttribute(avg_sortm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, np2 * 4));
+        avg_sortm_kernel<<<T, 1024, (size_t)np2 * 4, st>>>(uvw_m, B, np2, sorted_m);
+        BLINK_LAUNCH_CHECK("avg_sortm_kernel");
+    }
     float2 *grid = static_cast<float2 *>(workspace);
     uint32_t *cnt = uni ? reinterpret_cast<uint32_t *>(static_cast<unsigned char *>(workspace) + gbytes) : nullptr;
     int ctas = 8 * (sm_count() > 0 ? sm_count() : 148);
@@ -263,12 +341,17 @@ extern "C" int blink_image_avg(const blink_c64 *vis, const float *uvw_m, const d
             const int nt = (C <= 1024) ? T : 1, nc = (C <= 1024) ? C : a.ntc;
             const int nchunk = (nc + kAvgChunk - 1) / kAvgChunk, bblocks = (B + kAvgThreads - 1) / kAvgThreads;
             if ((long long)bblocks * nchunk * nt > 0x7fffffffLL) return BLINK_ERR_UNSUPPORTED;
-            BLINK_CUDA_TRY(cudaMemsetAsync(winv + tc, 0, (size_t)a.ntc * sizeof(float), st));
-            avg_count_kernel<<<(unsigned)(bblocks * nchunk * nt), kAvgThreads, 0, st>>>(a, sc, reinterpret_cast<unsigned *>(winv), t, c,
-                                                                                       nc, nchunk, bblocks);
-            BLINK_LAUNCH_CHECK("avg_count_kernel");
-            avg_winv_kernel<<<(a.ntc + 255) / 256, 256, 0, st>>>(a, winv);
-            BLINK_LAUNCH_CHECK("avg_winv_kernel");
+            if (sorted_m) {
+                avg_wsearch_kernel<<<(a.ntc + 255) / 256, 256, 0, st>>>(a, sc, sorted_m, winv);
+                BLINK_LAUNCH_CHECK("avg_wsearch_kernel");
+            } else {
+                BLINK_CUDA_TRY(cudaMemsetAsync(winv + tc, 0, (size_t)a.ntc * sizeof(float), st));
+                avg_count_kernel<<<(unsigned)(bblocks * nchunk * nt), kAvgThreads, 0, st>>>(a, sc, reinterpret_cast<unsigned *>(winv), t,
+                                                                                           c, nc, nchunk, bblocks);
+                BLINK_LAUNCH_CHECK("avg_count_kernel");
+                avg_winv_kernel<<<(a.ntc + 255) / 256, 256, 0, st>>>(a, winv);
+                BLINK_LAUNCH_CHECK("avg_winv_kernel");
+            }
             const long long blocks = (long long)bblocks * nchunk * P * nt;
             if (blocks > 0x7fffffffLL) return BLINK_ERR_UNSUPPORTED;
             avg_scatter_runs_kernel<<<(unsigned)blocks, kAvgThreads, 0, st>>>(a, sc, winv, t, c, nc, nchunk, bblocks);

@@ -14,7 +14,7 @@ int fused_default_ctas();
 int fused_image(const float2 *vis, const float *uvw_m, const double *freqs_hz, double pixscale_rad, int T, int C,
                 int P, int B, int n_pix, int weighting, int tc0, int ntc, float *image, float *wsum,
                 int32_t *cell_idx, void *workspace, size_t workspace_bytes, cudaStream_t st);
-size_t avg_workspace_bytes(int T, int C, int P, int n_pix, int weighting, bool minimum);   // blink_avg.cu
+size_t avg_workspace_bytes(int T, int C, int P, int B, int n_pix, int weighting, bool minimum);   // blink_avg.cu
 int counts_only(const float *uvw_m, const double *freqs_hz, double pixscale_rad, int T, int C, int B, int n_pix,
                 int tc0, int ntc, uint32_t *counts, cudaStream_t st);
 
@@ -117,8 +117,8 @@ extern "C" int blink_workspace_bytes(int op, int T, int C, int P, int B, int n_p
             break;
         }
         case BLINK_OP_IMAGE_AVG:
-            rec = avg_workspace_bytes(T, C, P, n_pix, weighting, false);
-            mn = avg_workspace_bytes(T, C, P, n_pix, weighting, true);
+            rec = avg_workspace_bytes(T, C, P, B, n_pix, weighting, false);
+            mn = avg_workspace_bytes(T, C, P, B, n_pix, weighting, true);
             break;
         default:
             return BLINK_ERR_INVALID_ARG;

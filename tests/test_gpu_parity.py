@@ -19,7 +19,7 @@ def bk():
     from paper_2505_15204_b200 import binding
     binding.lib()                     # raises if the .so is missing: no fallback
     yield binding
-    for k in (binding.OPT_IMAGE_PATH, binding.OPT_FUSED_CTAS, binding.OPT_GRID_CHUNK_B):
+    for k in (binding.OPT_IMAGE_PATH, binding.OPT_FUSED_CTAS, binding.OPT_GRID_CHUNK_B, binding.OPT_AVG_WSUM):
         binding.set_option(k, 0)
 
 
@@ -395,10 +395,15 @@ def test_image_avg_random(bk, oracle_mod, weighting, avg_time):
     from paper_2505_15204_b200 import workloads
     w = workloads.make_random(T=3, C=5, P=2, B=1237, n_pix=128, weighting=weighting, seed=41, device="cuda", fill=1.1)
     w.uvw_m[1, 9, 1] = float("nan")
-    _check_avg(bk, oracle_mod, w, avg_time)
-    if weighting == 1:                                          # minimum workspace: a single count plane
-        _, mn = bk.blink_workspace_bytes(bk.OP_IMAGE_AVG, w.T, w.C, w.P, w.B, w.n_pix, weighting)
-        _check_avg(bk, oracle_mod, w, avg_time, workspace=torch.empty(mn, dtype=torch.uint8, device="cuda"))
+    for wopt in (1, 2):                                         # weight sums by sort + binary search / by ballot counting
+        bk.set_option(bk.OPT_AVG_WSUM, wopt)
+        try:
+            _check_avg(bk, oracle_mod, w, avg_time)
+        finally:
+            bk.set_option(bk.OPT_AVG_WSUM, 0)
+    # minimum workspace: a single count plane (uniform) / weight sums by ballot counting instead of sort + search (natural)
+    _, mn = bk.blink_workspace_bytes(bk.OP_IMAGE_AVG, w.T, w.C, w.P, w.B, w.n_pix, weighting)
+    _check_avg(bk, oracle_mod, w, avg_time, workspace=torch.empty(mn, dtype=torch.uint8, device="cuda"))
 
 
 @pytest.mark.parametrize("cfg,T,C", [(3, 2, 6), (4, 1, 3)])
@@ -433,3 +438,30 @@ def test_image_avg_degenerate(bk, oracle_mod):
     w.uvw_m[0, :, 0] = 4.2
     w.uvw_m[0, :, 1] = -7.7
     _check_avg(bk, oracle_mod, w, False)
+
+
+def test_image_avg_config3_full_size(bk, oracle_mod):
+    """BASELINE.json config 3 at full size through blink_image_avg (the launch configuration bench.py times):
+    weight sums of all 38400 (t,c) exact; timestep 0's averaged image against the oracle's mean of its 768 images;
+    every timestep against the mean of blink_image's own images."""
+    from paper_2505_15204_b200 import workloads
+    free, _ = torch.cuda.mem_get_info()
+    if free < 60e9:
+        pytest.skip("needs ~50 GB of device memory")
+    w = workloads.make_config(3, device="cuda")
+    T, C, P, B, N = w.T, w.C, w.P, w.B, w.n_pix
+    res = bk.blink_image_avg(w.vis, w.uvw_m, w.freqs_hz, N, w.pixscale_rad, w.weighting)
+    torch.cuda.synchronize()
+    uvw = w.uvw_m.cpu().numpy()
+    ci = oracle_mod.cells(uvw, w.freqs_hz, N, w.pixscale_rad)
+    assert np.array_equal(res["wsum"].cpu().numpy(), (2 * (ci >= 0).sum(axis=2)).astype(np.float32).ravel())
+    del ci
+    ref0 = oracle_mod.image_avg(w.vis[:1].cpu().numpy(), uvw[:1], w.freqs_hz, N, w.pixscale_rad, w.weighting)[0, 0]
+    assert _img_err(res["image_avg"][0].cpu().numpy(), ref0) <= TOL
+    full = bk.blink_image(w.vis, w.uvw_m, w.freqs_hz, N, w.pixscale_rad, w.weighting)
+    torch.cuda.synchronize()
+    worst = 0.0
+    for t in range(T):
+        mean = full["image"][t * C:(t + 1) * C].double().mean(dim=0)
+        worst = max(worst, float((res["image_avg"][t].double() - mean).abs().max() / mean.abs().max()))
+    assert worst <= TOL, worst
