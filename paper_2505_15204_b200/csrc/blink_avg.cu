@@ -226,20 +226,12 @@ avg_scatter_runs_kernel(const AvgArgs a, const __grid_constant__ ScaleBlock sc, 
             atomicAdd(&g[mirror_of(cur, n)], make_float2(acc.x, -acc.y));
         }
     };
-    // the cell is a function of the two "magic sums" u s + 1.5 2^23, v s + 1.5 2^23 (blink_common.cuh rint_rne):
-    // while their bits do not change nothing has to be recomputed
-    const float lim = (float)(h - 1);
-    int pu = 0x7fffffff, pv = 0x7fffffff;
 #pragma unroll 4
     for (int c = c0; c < c1; ++c) {
-        const float s = sc.s[c - a.c_base];
-        const float tu = __fadd_rn(__fmul_rn(u, s), 12582912.0f), tv = __fadd_rn(__fmul_rn(v, s), 12582912.0f);
-        const int bu = __float_as_int(tu), bv = __float_as_int(tv);
-        if (bu != pu || bv != pv) {
+        const int cell = cell_of(u, v, sc.s[c - a.c_base], n, h);
+        if (cell != cur) {
             flush();
-            pu = bu; pv = bv;
-            const float xr = __fadd_rn(tu, -12582912.0f), yr = __fadd_rn(tv, -12582912.0f);
-            cur = (fabsf(xr) <= lim && fabsf(yr) <= lim) ? (bv - 0x4B400000 + h) * n + (bu - 0x4B400000 + h) : -1;
+            cur = cell;
             acc = make_float2(0.f, 0.f);
         }
         if (cur >= 0) {
