@@ -419,19 +419,25 @@ fused_image_kernel(const FusedArgs a, const __grid_constant__ ScaleBlock sc, con
                 const uint32_t st_used = cs;
                 float2 z[1][kE];
                 {
-                    ExchangeTilePair<Cfg::ROWB> st{stage + (size_t)cs * Cfg::STAGE_BYTES + (size_t)sub * Cfg::SUB_BYTES, pair};
+                    // 16 bytes (S1[u], S2[u]) per u out of the swizzled sub-tile.  The swizzle only involves bits of
+                    // (u mod 8) and TG is a multiple of 8, so the address is one per-thread base plus a compile-time
+                    // multiple of TG rows -- for u = tid + e TG as well as for the mirrored u = N - (tid + e TG).
+                    using XT = ExchangeTilePair<Cfg::ROWB>;
+                    const unsigned char *tile = stage + (size_t)cs * Cfg::STAGE_BYTES + (size_t)sub * Cfg::SUB_BYTES;
+                    const unsigned char *lo = tile + XT::swz((uint32_t)tid * Cfg::ROWB + (uint32_t)pair * 16u);
+                    const unsigned char *hi = tile + XT::swz((uint32_t)(TG - tid) * Cfg::ROWB + (uint32_t)pair * 16u);
 #pragma unroll
                     for (int e = 0; e < kE / 2; ++e) {          // n = u < H: S1 + i S2
-                        const int u = tid + e * TG;
                         float4 q = make_float4(0.f, 0.f, 0.f, 0.f);
-                        if (u < ulim) q = *st.at_row(u);
+                        if (tid < ulim - e * TG) q = *reinterpret_cast<const float4 *>(lo + (size_t)e * TG * Cfg::ROWB);
                         z[0][e] = make_float2(q.x - q.w, q.y + q.z);
                     }
 #pragma unroll
                     for (int e = kE / 2; e < kE; ++e) {         // n > H: conj(S1[N-n]) + i conj(S2[N-n])
-                        const int u = N - (tid + e * TG);       // in [1, H]; u == H is the empty Nyquist column
+                        // u = N - (tid + e TG) = (TG - tid) + (kE - 1 - e) TG, in [1, H]; u == H is the empty Nyquist column
                         float4 q = make_float4(0.f, 0.f, 0.f, 0.f);
-                        if (u < ulim && u < H) q = *st.at_row(u);
+                        const bool ok = (TG - tid) < ulim - (kE - 1 - e) * TG && (e > kE / 2 || tid > 0);
+                        if (ok) q = *reinterpret_cast<const float4 *>(hi + (size_t)(kE - 1 - e) * TG * Cfg::ROWB);
                         z[0][e] = make_float2(q.x + q.w, q.z - q.y);
                     }
                 }
@@ -447,12 +453,11 @@ fused_image_kernel(const FusedArgs a, const __grid_constant__ ScaleBlock sc, con
                 ExchangePadded1 xch{xbuf};
                 fft_inverse<N, 1>(z, tid, xch, twr, gsync, release);
                 const int ky = it * Cfg::KYS + sub * Cfg::KY + 2 * pair;
-                float *r0 = img + (size_t)(ky ^ H) * N, *r1 = img + (size_t)((ky + 1) ^ H) * N;
+                float *r0 = img + (size_t)(ky ^ H) * N + tid, *r1 = img + (size_t)((ky + 1) ^ H) * N + tid;
 #pragma unroll
-                for (int e = 0; e < kE; ++e) {
-                    const int x = (tid + e * TG) ^ H;
-                    __stcs(r0 + x, z[0][e].x * inv_w);
-                    __stcs(r1 + x, z[0][e].y * inv_w);
+                for (int e = 0; e < kE; ++e) {                  // x = (tid + e TG) ^ H = tid + (e ^ kE/2) TG: fftshift
+                    __stcs(r0 + (e ^ (kE / 2)) * TG, z[0][e].x * inv_w);
+                    __stcs(r1 + (e ^ (kE / 2)) * TG, z[0][e].y * inv_w);
                 }
             }
         }
