@@ -115,11 +115,25 @@ __device__ __forceinline__ void dft8(float2 (&x)[8])
 // profiles/r1_fused.md capture b).  No padding: an N-element vector takes N slots.
 __device__ __forceinline__ int xsw(int w) { return w ^ ((w >> 4) & 7) ^ (((w >> 6) & 1) << 3); }
 
+// Slot of position w = tid + e*TG (tid < TG, TG a power of two >= 32) in factored form: the swizzle only touches
+// bits 0..3, which belong to tid, and the bits of e*TG it depends on are compile-time, so
+//   xsw(tid + e*TG) = e*TG + (xsw(tid) ^ me(e)),  me(e) = swizzle mask of (e*TG mod 128).
+// With e known at compile time the unit-stride reads of a transform become one or two per-thread bases plus
+// immediate offsets instead of four integer instructions per access.
+template <int TG>
+__device__ __forceinline__ int xsw_e(int xsw_tid, int e)
+{
+    const int lowe = (e * TG) & 127;
+    return e * TG + (xsw_tid ^ ((lowe >> 4) ^ ((lowe >> 6) << 3)));
+}
+
 // One vector, float2 elements.
 struct ExchangePadded1 {
     float2 *base;
     __device__ __forceinline__ void put(int w, const float2 (&v)[1]) const { base[xsw(w)] = v[0]; }
     __device__ __forceinline__ void get(int w, float2 (&v)[1]) const { v[0] = base[xsw(w)]; }
+    template <int TG>
+    __device__ __forceinline__ void get_e(int tid, int e, float2 (&v)[1]) const { v[0] = base[xsw_e<TG>(xsw(tid), e)]; }
 };
 
 // Two vectors (a column pair), float4 elements living INSIDE a TMA-written tile whose rows are
@@ -150,6 +164,8 @@ struct ExchangeTilePair {
         v[0] = make_float2(t.x, t.y);
         v[1] = make_float2(t.z, t.w);
     }
+    template <int TG>
+    __device__ __forceinline__ void get_e(int tid, int e, float2 (&v)[2]) const { get(tid + e * TG, v); }
 };
 
 // Two vectors, float4 elements in a private dense array (8 elements per 128-byte line), same rho.
@@ -166,6 +182,8 @@ struct ExchangeDense2 {
         v[0] = make_float2(t.x, t.y);
         v[1] = make_float2(t.z, t.w);
     }
+    template <int TG>
+    __device__ __forceinline__ void get_e(int tid, int e, float2 (&v)[2]) const { get(tid + e * TG, v); }
 };
 
 // ---------------------------------------------------------------------------------------------
@@ -272,7 +290,7 @@ __device__ __forceinline__ void stage_get(float2 (&v)[NV][E], int tid, const X &
 #pragma unroll
     for (int e = 0; e < E; ++e) {
         float2 t[NV];
-        xch.get(tid + e * TG, t);
+        xch.template get_e<TG>(tid, e, t);
 #pragma unroll
         for (int nv = 0; nv < NV; ++nv) v[nv][e] = t[nv];
     }

@@ -68,6 +68,13 @@ struct ExchangePadded2 {
         v[0] = c0[o];
         v[1] = c1[o];
     }
+    template <int TG>
+    __device__ __forceinline__ void get_e(int tid, int e, float2 (&v)[2]) const
+    {
+        const int o = xsw_e<TG>(xsw(tid), e);
+        v[0] = c0[o];
+        v[1] = c1[o];
+    }
 };
 
 // shared memory: vis row [B] float2 | column offsets [H+2] | pad to 1024 |
@@ -338,7 +345,7 @@ fused_image_kernel(const FusedArgs a, const __grid_constant__ ScaleBlock sc, con
                 float2 v[2][kE];
 #pragma unroll
                 for (int e = 0; e < kE; ++e) {                  // transform index n lives in centred row n ^ H
-                    const int o = xsw(tid + (e ^ (kE / 2)) * TG);
+                    const int o = xsw_e<TG>(xsw(tid), e ^ (kE / 2));
                     v[0][e] = c0[o];
                     v[1][e] = c1[o];
                     if (uniform) {                              // a3: divide by the cell count
@@ -362,7 +369,7 @@ fused_image_kernel(const FusedArgs a, const __grid_constant__ ScaleBlock sc, con
                 float2 *d0 = scratch + (size_t)u0 * N, *d1 = d0 + N;
 #pragma unroll
                 for (int e = 0; e < kE; ++e) {
-                    const int o = xsw(tid + e * TG);            // the slots this thread read last: clear them
+                    const int o = xsw_e<TG>(xsw(tid), e);       // the slots this thread read last: clear them
                     c0[o] = make_float2(0.f, 0.f);
                     c1[o] = make_float2(0.f, 0.f);
                     d0[tid + e * TG] = v[0][e];
