@@ -134,6 +134,8 @@ struct ExchangePadded1 {
     __device__ __forceinline__ void get(int w, float2 (&v)[1]) const { v[0] = base[xsw(w)]; }
     template <int TG>
     __device__ __forceinline__ void get_e(int tid, int e, float2 (&v)[1]) const { v[0] = base[xsw_e<TG>(xsw(tid), e)]; }
+    // position wt + wr with disjoint bit fields (wt per thread, wr compile-time): xsw is XOR-linear
+    __device__ __forceinline__ void put2(int wt, int wr, const float2 (&v)[1]) const { base[xsw(wt) ^ xsw(wr)] = v[0]; }
 };
 
 // Two vectors (a column pair), float4 elements living INSIDE a TMA-written tile whose rows are
@@ -166,6 +168,7 @@ struct ExchangeTilePair {
     }
     template <int TG>
     __device__ __forceinline__ void get_e(int tid, int e, float2 (&v)[2]) const { get(tid + e * TG, v); }
+    __device__ __forceinline__ void put2(int wt, int wr, const float2 (&v)[2]) const { put(wt + wr, v); }
 };
 
 // Two vectors, float4 elements in a private dense array (8 elements per 128-byte line), same rho.
@@ -184,6 +187,7 @@ struct ExchangeDense2 {
     }
     template <int TG>
     __device__ __forceinline__ void get_e(int tid, int e, float2 (&v)[2]) const { get(tid + e * TG, v); }
+    __device__ __forceinline__ void put2(int wt, int wr, const float2 (&v)[2]) const { put(wt + wr, v); }
 };
 
 // ---------------------------------------------------------------------------------------------
@@ -272,13 +276,13 @@ __device__ __forceinline__ void stage_put(const float2 (&v)[NV][E], int tid, con
     for (int q = 0; q < NB; ++q) {
         const int i = tid + q * TG;
         const int k = i & (P - 1);
-        const int j = (i - k) * R + k;
+        const int j = (i - k) * R + k;                  // bits of j and of r*P never overlap (k < P, (i-k)*R multiple of P*R)
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             float2 t[NV];
 #pragma unroll
             for (int nv = 0; nv < NV; ++nv) t[nv] = v[nv][q + r * NB];
-            xch.put(j + r * P, t);
+            xch.put2(j, r * P, t);
         }
     }
 }

@@ -68,6 +68,12 @@ struct ExchangePadded2 {
         v[0] = c0[o];
         v[1] = c1[o];
     }
+    __device__ __forceinline__ void put2(int wt, int wr, const float2 (&v)[2]) const
+    {
+        const int o = xsw(wt) ^ xsw(wr);
+        c0[o] = v[0];
+        c1[o] = v[1];
+    }
     template <int TG>
     __device__ __forceinline__ void get_e(int tid, int e, float2 (&v)[2]) const
     {
