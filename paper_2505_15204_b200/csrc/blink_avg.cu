@@ -274,7 +274,7 @@ extern "C" int blink_image_avg(const blink_c64 *vis, const float *uvw_m, const d
     if (!vis || !uvw_m || !freqs_hz || !image_avg || !wsum) return BLINK_ERR_INVALID_ARG;
     if (T < 1 || C < 1 || P < 1 || B < 1 || !(pixscale_rad > 0.0)) return BLINK_ERR_INVALID_ARG;
     if (weighting != BLINK_W_NATURAL && weighting != BLINK_W_UNIFORM) return BLINK_ERR_INVALID_ARG;
-    if (!is_pow2(n_pix) || n_pix < 32 || n_pix > 4096 || B > kMaxBaselines) return BLINK_ERR_UNSUPPORTED;
+    if (!is_pow2(n_pix) || n_pix < 32 || n_pix > kMaxPix || B > kMaxBaselines) return BLINK_ERR_UNSUPPORTED;
     if ((long long)T * C * P > 0x3fffffffLL) return BLINK_ERR_UNSUPPORTED;
     if (!aligned16(vis) || !aligned16(image_avg)) return BLINK_ERR_INVALID_ARG;
     int rc = ensure_device();

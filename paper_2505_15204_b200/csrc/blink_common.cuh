@@ -30,6 +30,7 @@ int  ensure_device();             // checks for an sm_100 device, uploads the tw
 int  sm_count();
 
 static inline bool is_pow2(int n) { return n > 0 && (n & (n - 1)) == 0; }
+constexpr int kMaxPix = 8192;           // largest image side (the fused kernel stops at 4096: blink_image falls back to the unfused chain)
 static inline bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 static inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
@@ -45,8 +46,8 @@ static inline float scale_for(double f_hz, int n_pix, double pixscale_rad)
 constexpr int kMaxChannels = 4096;      // per-channel scales are passed to kernels through a device array
 constexpr int kMaxBaselines = (1 << 18) - 1;
 
-// device twiddle table W[m] = exp(+2 pi i m / 4096), m in [0, 4096), built in double on the host
-constexpr int kTwiddleN = 4096;
+// device twiddle table W[m] = exp(+2 pi i m / 8192), m in [0, 8192), built in double on the host
+constexpr int kTwiddleN = 8192;
 const float2 *twiddle_table();          // device pointer (after ensure_device())
 
 // per-channel scales travel as a kernel parameter (<= 1024 channels per launch)

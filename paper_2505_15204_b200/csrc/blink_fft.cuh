@@ -14,7 +14,7 @@
 namespace blink {
 
 constexpr int kE = 8;                                   // elements per thread per vector
-__host__ __device__ constexpr int kTwiddleNConst() { return 4096; }   // length of the W table
+__host__ __device__ constexpr int kTwiddleNConst() { return 8192; }   // length of the W table
 
 __host__ __device__ constexpr int ilog2(int n) { return n <= 1 ? 0 : 1 + ilog2(n >> 1); }
 // number of radix-4 stages: log2 N = 3 a + 2 b with b in {0,1,2}
@@ -192,14 +192,32 @@ struct ExchangeDense2 {
 
 // ---------------------------------------------------------------------------------------------
 // Per-thread twiddle registers.  Which twiddles a thread needs depends only on (tid, stage, butterfly),
-// never on the data, so they are read ONCE per kernel from the W_4096 table (built in double on the
+// never on the data, so they are read ONCE per kernel from the W_8192 table (built in double on the
 // host) and kept in registers: per stage > 0 and butterfly q the powers w^1, w^2 (and w^4 for radix 8)
 // of w = exp(+2 pi i k / (P R)); the remaining powers are products of those (<= 2 extra roundings).
+// N = 8192 runs with N/8 = 1024 threads per transform (64 registers each): there the three base twiddles are
+// fetched from the (L1-resident) table at every use instead.
 // ---------------------------------------------------------------------------------------------
 template <int N, int E = kE>
 struct Twiddles {
     static constexpr int S = plan_stages(N);
-    float2 w[S > 1 ? S - 1 : 1][E / 4][3];              // [stage-1][butterfly q][w1, w2, w4]
+    static constexpr bool kInRegs = N <= 4096;
+    float2 w[kInRegs ? (S > 1 ? S - 1 : 1) : 1][kInRegs ? E / 4 : 1][3];   // [stage-1][butterfly q][w1, w2, w4]
+    const float2 *table;
+    int tid_;
+
+    // base twiddle `idx` (0, 1, 2 -> w^1, w^2, w^4) of butterfly q in stage ST (radix R, sub-transform length P)
+    template <int ST, int R, int P>
+    __device__ __forceinline__ float2 base(int q, int idx) const
+    {
+        if constexpr (kInRegs) {
+            return w[ST - 1][q][idx];
+        } else {
+            constexpr int step = kTwiddleNConst() / (P * R);
+            const int k = (tid_ + q * (N / E)) & (P - 1);
+            return __ldg(table + (k * step << idx));
+        }
+    }
 
     template <int ST, int P>
     __device__ __forceinline__ void init_stage(int tid, const float2 *__restrict__ tw)
@@ -221,7 +239,12 @@ struct Twiddles {
             init_stage<ST + 1, P * R>(tid, tw);
         }
     }
-    __device__ __forceinline__ void init(int tid, const float2 *__restrict__ tw) { init_stage<0, 1>(tid, tw); }
+    __device__ __forceinline__ void init(int tid, const float2 *__restrict__ tw)
+    {
+        table = tw;
+        tid_ = tid;
+        if constexpr (kInRegs) init_stage<0, 1>(tid, tw);
+    }
 };
 
 // One stage: twiddle (skipped when P == 1), radix-R butterflies in registers.
@@ -235,11 +258,11 @@ __device__ __forceinline__ void stage_compute(float2 (&v)[NV][E], const Twiddles
     for (int q = 0; q < NB; ++q) {
         if constexpr (P > 1) {
             float2 wp[R];
-            wp[1] = twr.w[ST - 1][q][0];
-            wp[2] = twr.w[ST - 1][q][1];
+            wp[1] = twr.template base<ST, R, P>(q, 0);
+            wp[2] = twr.template base<ST, R, P>(q, 1);
             wp[3] = cmul(wp[1], wp[2]);
             if constexpr (R == 8) {
-                wp[4] = twr.w[ST - 1][q][2];
+                wp[4] = twr.template base<ST, R, P>(q, 2);
                 wp[5] = cmul(wp[1], wp[4]);
                 wp[6] = cmul(wp[2], wp[4]);
                 wp[7] = cmul(wp[3], wp[4]);

@@ -199,6 +199,7 @@ int fft2d_range(float2 *grid, int n_pix, int batch, const float *scale, int scal
         case 1024: return launch_fft2d<1024>(grid, batch, scale, scale_div, img_base, image, image_imag, st);
         case 2048: return launch_fft2d<2048>(grid, batch, scale, scale_div, img_base, image, image_imag, st);
         case 4096: return launch_fft2d<4096>(grid, batch, scale, scale_div, img_base, image, image_imag, st);
+        case 8192: return launch_fft2d<8192>(grid, batch, scale, scale_div, img_base, image, image_imag, st);
         default: return BLINK_ERR_UNSUPPORTED;
     }
 }
@@ -213,7 +214,7 @@ extern "C" int blink_fft2d_inverse(blink_c64 *grid, int n_pix, int batch, const 
     using namespace blink;
     if (grid == nullptr || image == nullptr || batch < 0) return BLINK_ERR_INVALID_ARG;
     if (!aligned16(grid) || !aligned16(image) || (image_imag && !aligned16(image_imag))) return BLINK_ERR_INVALID_ARG;
-    if (!is_pow2(n_pix) || n_pix < 32 || n_pix > 4096) return BLINK_ERR_UNSUPPORTED;
+    if (!is_pow2(n_pix) || n_pix < 32 || n_pix > kMaxPix) return BLINK_ERR_UNSUPPORTED;
     if (scale != nullptr && scale_stride_div < 1) return BLINK_ERR_INVALID_ARG;
     if (scale == nullptr) scale_stride_div = 1;
     int rc = ensure_device();

@@ -251,7 +251,7 @@ extern "C" int blink_grid(const blink_c64 *vis, const float *uvw_m, const double
     if (T < 1 || C < 1 || P < 1 || B < 1 || !(pixscale_rad > 0.0)) return BLINK_ERR_INVALID_ARG;
     if (weighting != BLINK_W_NATURAL && weighting != BLINK_W_UNIFORM) return BLINK_ERR_INVALID_ARG;
     if (!aligned16(vis) || !aligned16(grid) || (counts && !aligned16(counts))) return BLINK_ERR_INVALID_ARG;
-    if (!is_pow2(n_pix) || n_pix < 32 || n_pix > 4096 || B > kMaxBaselines) return BLINK_ERR_UNSUPPORTED;
+    if (!is_pow2(n_pix) || n_pix < 32 || n_pix > kMaxPix || B > kMaxBaselines) return BLINK_ERR_UNSUPPORTED;
     if ((long long)T * C > 0x7fffffffLL / 2) return BLINK_ERR_UNSUPPORTED;
     int rc = ensure_device();
     if (rc != BLINK_OK) return rc;

@@ -75,7 +75,7 @@ static int check_common(const void *vis, const void *uvw_m, const double *freqs_
     if (!vis || !uvw_m || !freqs_hz) return BLINK_ERR_INVALID_ARG;
     if (T < 1 || C < 1 || P < 1 || B < 1 || !(pixscale_rad > 0.0)) return BLINK_ERR_INVALID_ARG;
     if (weighting != BLINK_W_NATURAL && weighting != BLINK_W_UNIFORM) return BLINK_ERR_INVALID_ARG;
-    if (!is_pow2(n_pix) || n_pix < 32 || n_pix > 4096 || B > kMaxBaselines) return BLINK_ERR_UNSUPPORTED;
+    if (!is_pow2(n_pix) || n_pix < 32 || n_pix > kMaxPix || B > kMaxBaselines) return BLINK_ERR_UNSUPPORTED;
     if ((long long)T * C * P > 0x3fffffffLL) return BLINK_ERR_UNSUPPORTED;
     return BLINK_OK;
 }
@@ -84,7 +84,7 @@ extern "C" int blink_workspace_bytes(int op, int T, int C, int P, int B, int n_p
                                      size_t *min_bytes)
 {
     if (!bytes) return BLINK_ERR_INVALID_ARG;
-    if (!is_pow2(n_pix) || n_pix < 32 || n_pix > 4096) return BLINK_ERR_UNSUPPORTED;
+    if (!is_pow2(n_pix) || n_pix < 32 || n_pix > kMaxPix) return BLINK_ERR_UNSUPPORTED;
     if (T < 1 || C < 1 || P < 1 || B < 0) return BLINK_ERR_INVALID_ARG;
     const size_t n2 = (size_t)n_pix * n_pix;
     size_t rec = 0, mn = 0;

@@ -46,7 +46,7 @@ def _check_images(bk, w, res, oracle_mod, ids=None):
 
 
 # --------------------------------------------------------------------------- blink_fft2d_inverse
-@pytest.mark.parametrize("n,batch", [(32, 5), (64, 3), (128, 3), (256, 2), (512, 3), (1024, 2), (2048, 1), (4096, 1)])
+@pytest.mark.parametrize("n,batch", [(32, 5), (64, 3), (128, 3), (256, 2), (512, 3), (1024, 2), (2048, 1), (4096, 1), (8192, 1)])
 def test_fft2d_inverse_vs_oracle(bk, oracle_mod, n, batch):
     rng = np.random.default_rng(100 + n)
     g = (rng.normal(size=(batch, n, n)) + 1j * rng.normal(size=(batch, n, n))).astype(np.complex64)
@@ -307,7 +307,7 @@ def test_error_codes(bk):
     p = lambda t: ctypes.c_void_p(t.data_ptr())
     f = fr.ctypes.data_as(ctypes.c_void_p)
     # n_pix not a power of two / too small / too large
-    for n in (48, 16, 8192):
+    for n in (48, 16, 16384):
         assert L.blink_image(p(x), p(x), f, 1, 1, 1, 4, n, 0.01, 0, p(x), p(x), None, None, p(x), 64, None) == -2
     assert L.blink_image(None, p(x), f, 1, 1, 1, 4, 32, 0.01, 0, p(x), p(x), None, None, p(x), 64, None) == -1
     assert L.blink_image(p(x), p(x), f, 1, 1, 1, 4, 32, -1.0, 0, p(x), p(x), None, None, p(x), 64, None) == -1
@@ -465,3 +465,16 @@ def test_image_avg_config3_full_size(bk, oracle_mod):
         mean = full["image"][t * C:(t + 1) * C].double().mean(dim=0)
         worst = max(worst, float((res["image_avg"][t].double() - mean).abs().max() / mean.abs().max()))
     assert worst <= TOL, worst
+
+
+def test_image_8192(bk, oracle_mod):
+    """The paper's long-exposure image side (8192 x 8192): blink_image through the unfused chain
+    (the fused kernel stops at 4096) and the channel / time average, both against the oracle."""
+    from paper_2505_15204_b200 import workloads
+    w = workloads.make_random(T=1, C=2, P=1, B=3000, n_pix=8192, weighting=0, seed=51, device="cuda", fill=0.6)
+    res = bk.blink_image(w.vis, w.uvw_m, w.freqs_hz, w.n_pix, w.pixscale_rad, w.weighting, want_cell_idx=True)
+    torch.cuda.synchronize()
+    _check_images(bk, w, res, oracle_mod, [1])
+    assert np.array_equal(res["cell_idx"].cpu().numpy(),
+                          oracle_mod.cells(w.uvw_m.cpu().numpy(), w.freqs_hz, w.n_pix, w.pixscale_rad))
+    _check_avg(bk, oracle_mod, w, True)
