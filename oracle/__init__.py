@@ -56,6 +56,8 @@ def lib():
         L.oracle_image_batch.argtypes = [vp, vp, vp, c_i, c_i, c_i, c_i, c_i, c_d, c_i, vp, c_i, vp, vp, c_i]
         L.oracle_image_avg.restype = c_i
         L.oracle_image_avg.argtypes = [vp, vp, vp, c_i, c_i, c_i, c_i, c_i, c_d, c_i, c_i, vp]
+        L.oracle_apply_gains.restype = None
+        L.oracle_apply_gains.argtypes = [vp, vp, vp, c_i, c_i, c_i, c_i, c_i, vp]
         _lib = L
     return _lib
 
@@ -174,4 +176,17 @@ def image_avg(vis, uvw_m, freqs_hz, n_pix: int, pixscale_rad: float, weighting: 
                                 int(weighting), int(bool(avg_time)), _p(out))
     if rc != 0:
         raise RuntimeError("oracle_image_avg failed")
+    return out
+
+
+def apply_gains(vis, gains, ant_pairs):
+    """vis [T][C][P][B] complex64, gains [C][P][A] complex64, ant_pairs [B][2] int32 -> corrected vis (complex64)."""
+    v = _c64(vis)
+    g = _c64(gains)
+    ap = np.ascontiguousarray(ant_pairs, dtype=np.int32)
+    T, C, P, B = v.shape
+    A = g.shape[2]
+    assert g.shape[:2] == (C, P) and ap.shape == (B, 2) and ap.min() >= 0 and ap.max() < A
+    out = np.empty_like(v)
+    lib().oracle_apply_gains(_p(v), _p(g), _p(ap), T, C, P, B, A, _p(out))
     return out

@@ -26,6 +26,8 @@
  *   oracle_image_avg              : unit sources -> 1.0 at the centre of the mean; == one numpy.fft transform
  *                                   of the 1/W-weighted sum of independently re-gridded channels; centre-pixel
  *                                   closed form with an empty channel counted in the mean
+ *   oracle_apply_gains            : identity for unit gains; pure phases rotate by phi_a1 - phi_a2; independent
+ *                                   numpy evaluation; undoing a simulated corruption restores the image
  * Nothing here is "parity unpinned".
  *
  * Build: gcc -O2 -ffp-contract=off -fPIC -shared -pthread -o liboracle.so blink_oracle.c -lm
@@ -368,4 +370,34 @@ int oracle_image_avg(const float *vis, const float *uvw_m, const double *freqs_h
     for (size_t k = 0; k < n_out * n2; ++k) out[k] *= inv;
     free(img);
     return 0;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * Calibration / cable / geometric corrections as per-antenna complex gains (PAPER.md L182-184:
+ * "precomputed calibration solutions are applied to visibilities, followed by geometric and cable
+ * length corrections ... Visibilities are one-to-one mapped to GPU threads"; reading R15):
+ *   V'[t][c][p][b] = g[c][p][a1(b)] * conj(g[c][p][a2(b)]) * V[t][c][p][b]
+ * evaluated in double, stored back as complex64 (the paper corrects its fp32 visibilities in place).
+ * A per-antenna phase exp(i phi_a) covers cable length and geometric delay (both are differences of
+ * per-antenna delays).  Pins (tests/test_oracle_pins.py): unit gains are the identity; pure phases
+ * rotate by phi_a1 - phi_a2 and keep |V|; an independent numpy evaluation; applying the gains that undo
+ * a simulated corruption restores the uncorrupted image.
+ * ---------------------------------------------------------------------------------------- */
+void oracle_apply_gains(const float *vis, const float *gains, const int32_t *ant_pairs,
+                        int T, int C, int P, int B, int A, float *vis_out)
+{
+    for (int t = 0; t < T; ++t)
+        for (int c = 0; c < C; ++c)
+            for (int p = 0; p < P; ++p) {
+                const float *g = gains + 2 * (((size_t)c * P + p) * (size_t)A);
+                const size_t row = (((size_t)t * C + c) * P + p) * (size_t)B;
+                for (int b = 0; b < B; ++b) {
+                    const int a1 = ant_pairs[2 * b], a2 = ant_pairs[2 * b + 1];
+                    const double g1r = g[2 * a1], g1i = g[2 * a1 + 1], g2r = g[2 * a2], g2i = g[2 * a2 + 1];
+                    const double fr = g1r * g2r + g1i * g2i, fi = g1i * g2r - g1r * g2i;      /* g1 * conj(g2) */
+                    const double vr = vis[2 * (row + b)], vi = vis[2 * (row + b) + 1];
+                    vis_out[2 * (row + b)] = (float)(fr * vr - fi * vi);
+                    vis_out[2 * (row + b) + 1] = (float)(fr * vi + fi * vr);
+                }
+            }
 }
