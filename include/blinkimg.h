@@ -149,6 +149,24 @@ int blink_image_avg(const blink_c64 *vis, const float *uvw_m, const double *freq
                     int avg_time, float *image_avg, float *wsum,
                     void *workspace, size_t workspace_bytes, void *stream);
 
+/*
+ * Visibility corrections as per-antenna complex gains ("precomputed calibration solutions are
+ * applied to visibilities, followed by geometric and cable length corrections"; reading R15):
+ *   V'[t][c][p][b] = g[c][p][a1(b)] * conj(g[c][p][a2(b)]) * V[t][c][p][b]
+ *   gains      in  [C][P][A] complex64 (a per-antenna phase carries the cable-length and geometric delays)
+ *   ant_pairs  in  [B][2] int32, (a1, a2) of every baseline, 0 <= a < A; 8-byte aligned
+ * blink_apply_gains corrects `vis` IN PLACE, one thread per visibility (the paper's own form).
+ * blink_image_cal is blink_image with the correction fused into the gridder's load: `vis` is not modified and
+ * never written.  It needs the fused kernel (256 <= n_pix <= 4096, B <= 16384), else BLINK_ERR_UNSUPPORTED --
+ * use blink_apply_gains followed by blink_image there.  Other arguments as blink_image.
+ */
+int blink_apply_gains(blink_c64 *vis, const blink_c64 *gains, const int32_t *ant_pairs,
+                      int T, int C, int P, int B, int A, void *stream);
+int blink_image_cal(const blink_c64 *vis, const float *uvw_m, const double *freqs_hz,
+                    const blink_c64 *gains, const int32_t *ant_pairs, int A,
+                    int T, int C, int P, int B, int n_pix, double pixscale_rad, int weighting,
+                    float *image, float *wsum, void *workspace, size_t workspace_bytes, void *stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -22,7 +22,7 @@ OPT_IMAGE_PATH, OPT_FUSED_CTAS, OPT_GRID_CHUNK_B, OPT_AVG_WSUM = 0, 1, 2, 3
 
 EXPORTS = ["blink_strerror", "blink_last_cuda_error", "blink_set_option", "blink_get_option",
            "blink_kernel_launches", "blink_workspace_bytes", "blink_grid", "blink_fft2d_inverse",
-           "blink_image", "blink_image_host", "blink_image_avg"]
+           "blink_image", "blink_image_host", "blink_image_avg", "blink_apply_gains", "blink_image_cal"]
 
 
 class BlinkError(RuntimeError):
@@ -64,6 +64,10 @@ def lib():
         L.blink_image_host.argtypes = [vp, vp, vp, i, i, i, i, i, d, i, vp, vp, vp, sz]
         L.blink_image_avg.restype = i
         L.blink_image_avg.argtypes = [vp, vp, vp, i, i, i, i, i, d, i, i, vp, vp, vp, sz, vp]
+        L.blink_apply_gains.restype = i
+        L.blink_apply_gains.argtypes = [vp, vp, vp, i, i, i, i, i, vp]
+        L.blink_image_cal.restype = i
+        L.blink_image_cal.argtypes = [vp, vp, vp, vp, vp, i, i, i, i, i, i, d, i, vp, vp, vp, sz, vp]
         _lib = L
     return _lib
 
@@ -194,6 +198,38 @@ def blink_image_avg(vis: torch.Tensor, uvw_m: torch.Tensor, freqs_hz, n_pix: int
                                _ptr(workspace), workspace.numel(), _stream(dev))
     _check(rc, "blink_image_avg")
     return dict(image_avg=image_avg, wsum=wsum)
+
+
+def blink_apply_gains(vis: torch.Tensor, gains: torch.Tensor, ant_pairs: torch.Tensor):
+    """In place: vis[t][c][p][b] *= gains[c][p][a1] * conj(gains[c][p][a2]); ant_pairs [B][2] int32 (CUDA)."""
+    _dev(vis, torch.complex64, "vis"); _dev(gains, torch.complex64, "gains"); _dev(ant_pairs, torch.int32, "ant_pairs")
+    T, C, P, B = vis.shape
+    rc = lib().blink_apply_gains(_ptr(vis), _ptr(gains), _ptr(ant_pairs), T, C, P, B, gains.shape[2], _stream(vis.device))
+    _check(rc, "blink_apply_gains")
+    return vis
+
+
+def blink_image_cal(vis: torch.Tensor, uvw_m: torch.Tensor, freqs_hz, gains: torch.Tensor, ant_pairs: torch.Tensor,
+                    n_pix: int, pixscale_rad: float, weighting: int = 0, image: Optional[torch.Tensor] = None,
+                    workspace: Optional[torch.Tensor] = None, wsum: Optional[torch.Tensor] = None):
+    """blink_image with per-antenna gain corrections fused into the gridder's load (vis is left untouched)."""
+    _dev(vis, torch.complex64, "vis"); _dev(uvw_m, torch.float32, "uvw_m")
+    _dev(gains, torch.complex64, "gains"); _dev(ant_pairs, torch.int32, "ant_pairs")
+    T, C, P, B = vis.shape
+    fr = _freqs(freqs_hz)
+    dev = vis.device
+    if image is None:
+        image = torch.empty((T * C * P, n_pix, n_pix), dtype=torch.float32, device=dev)
+    if wsum is None:
+        wsum = torch.empty(T * C, dtype=torch.float32, device=dev)
+    if workspace is None:
+        rec, _ = blink_workspace_bytes(OP_IMAGE, T, C, P, B, n_pix, weighting)
+        workspace = torch.empty(max(rec, 16), dtype=torch.uint8, device=dev)
+    rc = lib().blink_image_cal(_ptr(vis), _ptr(uvw_m), fr.ctypes.data_as(ctypes.c_void_p), _ptr(gains), _ptr(ant_pairs),
+                               gains.shape[2], T, C, P, B, n_pix, float(pixscale_rad), int(weighting), _ptr(image),
+                               _ptr(wsum), _ptr(workspace), workspace.numel(), _stream(dev))
+    _check(rc, "blink_image_cal")
+    return dict(image=image, wsum=wsum)
 
 
 def blink_image_host(vis_host: torch.Tensor, uvw_host: torch.Tensor, freqs_hz, n_pix: int, pixscale_rad: float,

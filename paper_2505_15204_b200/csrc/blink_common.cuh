@@ -50,6 +50,13 @@ constexpr int kMaxBaselines = (1 << 18) - 1;
 constexpr int kTwiddleN = 8192;
 const float2 *twiddle_table();          // device pointer (after ensure_device())
 
+// per-antenna gain corrections fused into the gridder's load (R15): V' = g[c][p][a1] conj(g[c][p][a2]) V
+struct GainRef {
+    const float2 *gains = nullptr;      // [C][P][A] complex64 (device) or NULL
+    const int2 *ant = nullptr;          // [B] antenna pair (a1, a2) of every baseline (device)
+    int A = 0;
+};
+
 // per-channel scales travel as a kernel parameter (<= 1024 channels per launch)
 struct ScaleBlock { float s[1024]; };
 

@@ -52,6 +52,7 @@ struct FusedArgs {
     float2 *scratch;                                           // [gridDim.x][H][N]
     const float *su; const uint2 *svb;                         // per timestep: baselines sorted by |u| (presort_kernel)
     const float2 *tw;
+    GainRef cal;                                               // optional per-antenna gains applied at the load
 };
 
 struct ExchangePadded2 {
@@ -307,6 +308,12 @@ fused_image_kernel(const FusedArgs a, const __grid_constant__ ScaleBlock sc, con
                 const float yr = rint_rne(__fmul_rn(__uint_as_float(sq.x), s), iv);
                 if (fabsf(yr) <= lim) {                         // NaN fails; |iu| <= H-1 by construction
                     float2 vv = visrow[sq.y & 0x7fffffffu];
+                    if (a.cal.gains) {                          // corrections fused into the load (R15)
+                        const int2 ap = __ldg(a.cal.ant + (sq.y & 0x7fffffffu));
+                        const float2 *gc = a.cal.gains + ((size_t)c * a.P + p) * a.cal.A;
+                        const float2 g1 = __ldg(gc + ap.x), g2 = __ldg(gc + ap.y);
+                        vv = cmul(vv, cmul(g1, make_float2(g2.x, -g2.y)));
+                    }
                     if (sq.y >> 31) vv.y = -vv.y;
                     float2 *col = second ? c1 : c0;
                     const int o = xsw(iv + H);
@@ -594,9 +601,10 @@ static int launch_fused(const FusedArgs &base, const double *freqs_hz, double pi
 
 int fused_image(const float2 *vis, const float *uvw_m, const double *freqs_hz, double pixscale_rad, int T, int C, int P,
                 int B, int n_pix, int weighting, int tc0, int ntc, float *image, float *wsum, int32_t *cell_idx,
-                void *workspace, size_t workspace_bytes, cudaStream_t st)
+                void *workspace, size_t workspace_bytes, cudaStream_t st, GainRef cal)
 {
     FusedArgs a{};
+    a.cal = cal;
     a.vis = vis; a.uvw_m = uvw_m; a.T = T; a.C = C; a.P = P; a.B = B; a.weighting = weighting;
     a.tc0 = tc0; a.ntc = ntc; a.image = image; a.wsum = wsum; a.cell_idx = cell_idx;
     switch (n_pix) {

@@ -13,7 +13,7 @@ size_t fused_workspace_bytes(int T, int B, int n_pix, int ctas);
 int fused_default_ctas();
 int fused_image(const float2 *vis, const float *uvw_m, const double *freqs_hz, double pixscale_rad, int T, int C,
                 int P, int B, int n_pix, int weighting, int tc0, int ntc, float *image, float *wsum,
-                int32_t *cell_idx, void *workspace, size_t workspace_bytes, cudaStream_t st);
+                int32_t *cell_idx, void *workspace, size_t workspace_bytes, cudaStream_t st, GainRef cal);
 size_t avg_workspace_bytes(int T, int C, int P, int B, int n_pix, int weighting, bool minimum);   // blink_avg.cu
 int counts_only(const float *uvw_m, const double *freqs_hz, double pixscale_rad, int T, int C, int B, int n_pix,
                 int tc0, int ntc, uint32_t *counts, cudaStream_t st);
@@ -35,13 +35,15 @@ static bool use_fused(int P, int B, int n_pix, int weighting)
 
 static int image_device(const float2 *vis, const float *uvw_m, const double *freqs_hz, int T, int C, int P, int B,
                         int n_pix, double pixscale_rad, int weighting, int tc0, int ntc, float *image, float *wsum,
-                        int32_t *cell_idx, uint32_t *counts, void *workspace, size_t workspace_bytes, cudaStream_t st)
+                        int32_t *cell_idx, uint32_t *counts, void *workspace, size_t workspace_bytes, cudaStream_t st,
+                        GainRef cal = GainRef())
 {
     // image / wsum / cell_idx / counts are indexed by ABSOLUTE tc; the range [tc0, tc0+ntc) is processed
     const size_t n2 = (size_t)n_pix * n_pix;
+    if (cal.gains && !use_fused(P, B, n_pix, weighting)) return BLINK_ERR_UNSUPPORTED;   // gains are fused into the fused kernel only
     if (use_fused(P, B, n_pix, weighting)) {
         int rc = fused_image(vis, uvw_m, freqs_hz, pixscale_rad, T, C, P, B, n_pix, weighting, tc0, ntc, image, wsum,
-                             cell_idx, workspace, workspace_bytes, st);
+                             cell_idx, workspace, workspace_bytes, st, cal);
         if (rc != BLINK_OK) return rc;
         if (counts) return counts_only(uvw_m, freqs_hz, pixscale_rad, T, C, B, n_pix, tc0, ntc, counts, st);
         return BLINK_OK;
@@ -63,6 +65,23 @@ static int image_device(const float2 *vis, const float *uvw_m, const double *fre
         if (rc != BLINK_OK) return rc;
     }
     return BLINK_OK;
+}
+
+// One thread per visibility, in place: the paper's own form of the corrections.
+__global__ void apply_gains_kernel(float2 *__restrict__ vis, const float2 *__restrict__ gains, const int2 *__restrict__ ant,
+                                   long long n_rows, int C, int P, int B, int A)
+{
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= B) return;
+    const int2 ap = ant[b];
+    for (long long row = blockIdx.y; row < n_rows; row += gridDim.y) {            // row = (t*C + c)*P + p
+        const int p = (int)(row % P), c = (int)((row / P) % C);
+        const float2 *gc = gains + ((size_t)c * P + p) * A;
+        const float2 g1 = __ldg(gc + ap.x), g2 = __ldg(gc + ap.y);
+        const float2 f = make_float2(g1.x * g2.x + g1.y * g2.y, g1.y * g2.x - g1.x * g2.y);   // g1 conj(g2)
+        const float2 v = vis[row * B + b];
+        vis[row * B + b] = make_float2(f.x * v.x - f.y * v.y, f.x * v.y + f.y * v.x);
+    }
 }
 
 }  // namespace blink
@@ -202,4 +221,49 @@ extern "C" int blink_image_host(const blink_c64 *vis_host, const float *uvw_m_ho
         BLINK_CUDA_TRY(cudaMemcpy(wsum_host, d_wsum, (size_t)T * C * sizeof(float), cudaMemcpyDeviceToHost));
     cudaEventDestroy(uvw_ready);
     return result;
+}
+
+
+static int check_gains(const void *gains, const void *ant_pairs, int A)
+{
+    if (!gains || !ant_pairs || A < 1) return BLINK_ERR_INVALID_ARG;
+    if ((reinterpret_cast<uintptr_t>(gains) & 7u) || (reinterpret_cast<uintptr_t>(ant_pairs) & 7u)) return BLINK_ERR_INVALID_ARG;
+    return BLINK_OK;
+}
+
+extern "C" int blink_apply_gains(blink_c64 *vis, const blink_c64 *gains, const int32_t *ant_pairs, int T, int C, int P, int B,
+                                 int A, void *stream)
+{
+    if (!vis || T < 1 || C < 1 || P < 1 || B < 1) return BLINK_ERR_INVALID_ARG;
+    int rc = check_gains(gains, ant_pairs, A);
+    if (rc != BLINK_OK) return rc;
+    rc = ensure_device();
+    if (rc != BLINK_OK) return rc;
+    const long long n_rows = (long long)T * C * P;
+    dim3 grid((B + 255) / 256, (unsigned)std::min<long long>(n_rows, 65535));
+    apply_gains_kernel<<<grid, 256, 0, static_cast<cudaStream_t>(stream)>>>(
+        reinterpret_cast<float2 *>(vis), reinterpret_cast<const float2 *>(gains), reinterpret_cast<const int2 *>(ant_pairs), n_rows,
+        C, P, B, A);
+    BLINK_LAUNCH_CHECK("apply_gains_kernel");
+    return BLINK_OK;
+}
+
+extern "C" int blink_image_cal(const blink_c64 *vis, const float *uvw_m, const double *freqs_hz, const blink_c64 *gains,
+                               const int32_t *ant_pairs, int A, int T, int C, int P, int B, int n_pix, double pixscale_rad,
+                               int weighting, float *image, float *wsum, void *workspace, size_t workspace_bytes, void *stream)
+{
+    int rc = check_common(vis, uvw_m, freqs_hz, T, C, P, B, n_pix, pixscale_rad, weighting);
+    if (rc != BLINK_OK) return rc;
+    if (!image || !wsum || !aligned16(vis) || !aligned16(image)) return BLINK_ERR_INVALID_ARG;
+    rc = check_gains(gains, ant_pairs, A);
+    if (rc != BLINK_OK) return rc;
+    rc = ensure_device();
+    if (rc != BLINK_OK) return rc;
+    GainRef cal;
+    cal.gains = reinterpret_cast<const float2 *>(gains);
+    cal.ant = reinterpret_cast<const int2 *>(ant_pairs);
+    cal.A = A;
+    return image_device(reinterpret_cast<const float2 *>(vis), uvw_m, freqs_hz, T, C, P, B, n_pix, pixscale_rad, weighting,
+                        0, T * C, image, wsum, nullptr, nullptr, workspace, workspace_bytes,
+                        static_cast<cudaStream_t>(stream), cal);
 }

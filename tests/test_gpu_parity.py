@@ -478,3 +478,58 @@ def test_image_8192(bk, oracle_mod):
     assert np.array_equal(res["cell_idx"].cpu().numpy(),
                           oracle_mod.cells(w.uvw_m.cpu().numpy(), w.freqs_hz, w.n_pix, w.pixscale_rad))
     _check_avg(bk, oracle_mod, w, True)
+
+
+# --------------------------------------------------------------------------- per-antenna gains
+def _gain_setup(w, n_ant, seed):
+    rng = np.random.default_rng(seed)
+    pairs = np.array([(i, j) for i in range(n_ant) for j in range(i)], dtype=np.int32)
+    assert len(pairs) >= w.B
+    pairs = pairs[rng.permutation(len(pairs))[:w.B]].copy()
+    gains = (rng.uniform(0.6, 1.4, (w.C, w.P, n_ant)) * np.exp(1j * rng.uniform(-np.pi, np.pi, (w.C, w.P, n_ant)))).astype(np.complex64)
+    return gains, pairs
+
+
+@pytest.mark.parametrize("weighting", [0, 1])
+def test_gains_fused_and_in_place(bk, oracle_mod, weighting):
+    from paper_2505_15204_b200 import workloads
+    w = workloads.make_random(T=2, C=3, P=2, B=1237, n_pix=256, weighting=weighting, seed=61, device="cuda", fill=1.05)
+    gains, pairs = _gain_setup(w, 64, 62)
+    vis_before = w.vis.clone()
+    g_d, p_d = torch.tensor(gains, device="cuda"), torch.tensor(pairs, device="cuda")
+    res = bk.blink_image_cal(w.vis, w.uvw_m, w.freqs_hz, g_d, p_d, w.n_pix, w.pixscale_rad, weighting)
+    torch.cuda.synchronize()
+    assert torch.equal(w.vis, vis_before)                                  # the fused path never writes the visibilities
+    # oracle: apply the gains (definition), then image
+    fixed = oracle_mod.apply_gains(w.vis.cpu().numpy(), gains, pairs)
+    w_fixed = workloads.Workload(**{**w.__dict__, "vis": torch.tensor(fixed)})
+    _check_images(bk, w_fixed, res, oracle_mod)
+    # the in-place kernel against the oracle's corrected visibilities, element by element
+    v2 = w.vis.clone()
+    bk.blink_apply_gains(v2, g_d, p_d)
+    torch.cuda.synchronize()
+    got = v2.cpu().numpy()
+    assert np.max(np.abs(got - fixed)) <= 2e-6 * np.max(np.abs(fixed))
+    # unit gains are the identity, bit for bit
+    v3 = w.vis.clone()
+    bk.blink_apply_gains(v3, torch.ones_like(g_d), p_d)
+    assert torch.equal(v3, w.vis)
+
+
+def test_gains_config3_reduced_and_unsupported(bk, oracle_mod):
+    from paper_2505_15204_b200 import workloads
+    w = workloads.make_config(3, device="cuda", T=2, C=4)
+    n_ant = 128
+    pairs = np.array([(i, j) for i in range(n_ant) for j in range(i)], dtype=np.int32)    # the generator's baseline order
+    rng = np.random.default_rng(63)
+    gains = (rng.uniform(0.8, 1.2, (w.C, w.P, n_ant)) * np.exp(1j * rng.uniform(-1, 1, (w.C, w.P, n_ant)))).astype(np.complex64)
+    g_d, p_d = torch.tensor(gains, device="cuda"), torch.tensor(pairs, device="cuda")
+    res = bk.blink_image_cal(w.vis, w.uvw_m, w.freqs_hz, g_d, p_d, w.n_pix, w.pixscale_rad, w.weighting)
+    fixed = oracle_mod.apply_gains(w.vis.cpu().numpy(), gains, pairs)
+    w_fixed = workloads.Workload(**{**w.__dict__, "vis": torch.tensor(fixed)})
+    _check_images(bk, w_fixed, res, oracle_mod)
+    # below the fused kernel's sizes the fused correction is refused (apply in place + blink_image instead)
+    ws = workloads.make_random(T=1, C=1, P=1, B=100, n_pix=64, weighting=0, seed=64, device="cuda")
+    with pytest.raises(bk.BlinkError):
+        bk.blink_image_cal(ws.vis, ws.uvw_m, ws.freqs_hz, torch.ones((1, 1, 128), dtype=torch.complex64, device="cuda"),
+                           p_d[:100].contiguous(), ws.n_pix, ws.pixscale_rad, 0)
