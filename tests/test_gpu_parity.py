@@ -533,3 +533,28 @@ def test_gains_config3_reduced_and_unsupported(bk, oracle_mod):
     with pytest.raises(bk.BlinkError):
         bk.blink_image_cal(ws.vis, ws.uvw_m, ws.freqs_hz, torch.ones((1, 1, 128), dtype=torch.complex64, device="cuda"),
                            p_d[:100].contiguous(), ws.n_pix, ws.pixscale_rad, 0)
+
+
+# --------------------------------------------------------------------------- more than 1024 channels (scale blocks)
+@pytest.mark.parametrize("path", [1, 2])
+def test_more_than_1024_channels(bk, oracle_mod, path):
+    # per-channel scales travel as a 1024-entry kernel parameter: C = 1030 needs two blocks per timestep, in the
+    # fused kernel, the unfused chain and both averaging kernels; the last channels are the ones checked
+    from paper_2505_15204_b200 import workloads
+    w = workloads.make_random(T=2, C=1030, P=1, B=300, n_pix=256, weighting=path - 1, seed=71, device="cuda", fill=0.9)
+    w.freqs_hz = 150e6 + 1.0e5 * np.arange(w.C)                 # wide enough that late channels grid differently
+    bk.set_option(bk.OPT_IMAGE_PATH, path)
+    try:
+        res = bk.blink_image(w.vis, w.uvw_m, w.freqs_hz, w.n_pix, w.pixscale_rad, w.weighting, want_cell_idx=True)
+        torch.cuda.synchronize()
+    finally:
+        bk.set_option(bk.OPT_IMAGE_PATH, 0)
+    ids = np.array([0, 1023, 1024, 1029, 1030, 1030 + 1023, 1030 + 1024, 2 * 1030 - 1])
+    _check_images(bk, w, res, oracle_mod, ids)
+    assert np.array_equal(res["cell_idx"].cpu().numpy(),
+                          oracle_mod.cells(w.uvw_m.cpu().numpy(), w.freqs_hz, w.n_pix, w.pixscale_rad))
+    # averaged over the 1030 channels: against the mean of the images just verified to be the library's own
+    avg = bk.blink_image_avg(w.vis, w.uvw_m, w.freqs_hz, w.n_pix, w.pixscale_rad, w.weighting)
+    mean = res["image"].reshape(w.T, w.C, w.n_pix, w.n_pix).double().mean(dim=1)
+    assert float((avg["image_avg"].double() - mean).abs().max() / mean.abs().max()) <= TOL
+    assert torch.equal(avg["wsum"], res["wsum"])
