@@ -299,6 +299,15 @@ fused_image_kernel(const FusedArgs a, const __grid_constant__ ScaleBlock sc, con
                 n_box = (ulim + Cfg::BOX_ROWS - 1) / Cfg::BOX_ROWS;
             }
             if (bulk) { mbar_wait(visbar, vph); vph ^= 1u; }
+            if (a.cal.gains) {                                  // corrections fused into the load (R15): one sweep over the staged row
+                const float2 *gc = a.cal.gains + ((size_t)c * a.P + p) * a.cal.A;
+                for (int i = threadIdx.x; i < B; i += kFusedThreads) {
+                    const int2 ap = __ldg(a.cal.ant + i);
+                    const float2 g1 = __ldg(gc + ap.x), g2 = __ldg(gc + ap.y);
+                    visrow[i] = cmul(visrow[i], cmul(g1, make_float2(g2.x, -g2.y)));
+                }
+                __syncthreads();
+            }
 
             // ================= pass 1: each group grids and transforms column pairs (2cp, 2cp+1) ==========
             int my_in = 0, my_occ = 0;
@@ -308,12 +317,6 @@ fused_image_kernel(const FusedArgs a, const __grid_constant__ ScaleBlock sc, con
                 const float yr = rint_rne(__fmul_rn(__uint_as_float(sq.x), s), iv);
                 if (fabsf(yr) <= lim) {                         // NaN fails; |iu| <= H-1 by construction
                     float2 vv = visrow[sq.y & 0x7fffffffu];
-                    if (a.cal.gains) {                          // corrections fused into the load (R15)
-                        const int2 ap = __ldg(a.cal.ant + (sq.y & 0x7fffffffu));
-                        const float2 *gc = a.cal.gains + ((size_t)c * a.P + p) * a.cal.A;
-                        const float2 g1 = __ldg(gc + ap.x), g2 = __ldg(gc + ap.y);
-                        vv = cmul(vv, cmul(g1, make_float2(g2.x, -g2.y)));
-                    }
                     if (sq.y >> 31) vv.y = -vv.y;
                     float2 *col = second ? c1 : c0;
                     const int o = xsw(iv + H);

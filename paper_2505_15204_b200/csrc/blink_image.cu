@@ -67,20 +67,37 @@ static int image_device(const float2 *vis, const float *uvw_m, const double *fre
     return BLINK_OK;
 }
 
-// One thread per visibility, in place: the paper's own form of the corrections.
-__global__ void apply_gains_kernel(float2 *__restrict__ vis, const float2 *__restrict__ gains, const int2 *__restrict__ ant,
-                                   long long n_rows, int C, int P, int B, int A)
+// One thread per visibility (pair), in place: the paper's own form of the corrections.
+// A thread keeps its baselines' antenna pairs and walks the (t,c,p) rows; even B moves two visibilities per 16-byte access.
+__device__ __forceinline__ float2 gain_factor(const float2 *gc, int2 ap)
 {
-    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    const float2 g1 = __ldg(gc + ap.x), g2 = __ldg(gc + ap.y);
+    return make_float2(g1.x * g2.x + g1.y * g2.y, g1.y * g2.x - g1.x * g2.y);                 // g1 conj(g2)
+}
+template <int VEC>
+__global__ void __launch_bounds__(256)
+apply_gains_kernel(float2 *__restrict__ vis, const float2 *__restrict__ gains, const int2 *__restrict__ ant, long long n_rows,
+                   int C, int P, int B, int A)
+{
+    const int b = (blockIdx.x * blockDim.x + threadIdx.x) * VEC;
     if (b >= B) return;
-    const int2 ap = ant[b];
-    for (long long row = blockIdx.y; row < n_rows; row += gridDim.y) {            // row = (t*C + c)*P + p
+    int2 ap[VEC];
+#pragma unroll
+    for (int k = 0; k < VEC; ++k) ap[k] = ant[b + k];                                         // VEC == 2 only when B is even
+    for (long long row = blockIdx.y; row < n_rows; row += gridDim.y) {                        // row = (t*C + c)*P + p
         const int p = (int)(row % P), c = (int)((row / P) % C);
         const float2 *gc = gains + ((size_t)c * P + p) * A;
-        const float2 g1 = __ldg(gc + ap.x), g2 = __ldg(gc + ap.y);
-        const float2 f = make_float2(g1.x * g2.x + g1.y * g2.y, g1.y * g2.x - g1.x * g2.y);   // g1 conj(g2)
-        const float2 v = vis[row * B + b];
-        vis[row * B + b] = make_float2(f.x * v.x - f.y * v.y, f.x * v.y + f.y * v.x);
+        float2 *dst = vis + row * B + b;
+        if constexpr (VEC == 2) {
+            const float2 f0 = gain_factor(gc, ap[0]), f1 = gain_factor(gc, ap[1]);
+            float4 v = *reinterpret_cast<float4 *>(dst);
+            v = make_float4(f0.x * v.x - f0.y * v.y, f0.x * v.y + f0.y * v.x, f1.x * v.z - f1.y * v.w, f1.x * v.w + f1.y * v.z);
+            *reinterpret_cast<float4 *>(dst) = v;
+        } else {
+            const float2 f = gain_factor(gc, ap[0]);
+            const float2 v = *dst;
+            *dst = make_float2(f.x * v.x - f.y * v.y, f.x * v.y + f.y * v.x);
+        }
     }
 }
 
@@ -240,10 +257,15 @@ extern "C" int blink_apply_gains(blink_c64 *vis, const blink_c64 *gains, const i
     rc = ensure_device();
     if (rc != BLINK_OK) return rc;
     const long long n_rows = (long long)T * C * P;
-    dim3 grid((B + 255) / 256, (unsigned)std::min<long long>(n_rows, 65535));
-    apply_gains_kernel<<<grid, 256, 0, static_cast<cudaStream_t>(stream)>>>(
-        reinterpret_cast<float2 *>(vis), reinterpret_cast<const float2 *>(gains), reinterpret_cast<const int2 *>(ant_pairs), n_rows,
-        C, P, B, A);
+    const unsigned rows_y = (unsigned)std::min<long long>(n_rows, 2048);
+    float2 *v = reinterpret_cast<float2 *>(vis);
+    const float2 *g = reinterpret_cast<const float2 *>(gains);
+    const int2 *ap = reinterpret_cast<const int2 *>(ant_pairs);
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if ((B & 1) == 0 && aligned16(vis))
+        apply_gains_kernel<2><<<dim3((B / 2 + 255) / 256, rows_y), 256, 0, st>>>(v, g, ap, n_rows, C, P, B, A);
+    else
+        apply_gains_kernel<1><<<dim3((B + 255) / 256, rows_y), 256, 0, st>>>(v, g, ap, n_rows, C, P, B, A);
     BLINK_LAUNCH_CHECK("apply_gains_kernel");
     return BLINK_OK;
 }
