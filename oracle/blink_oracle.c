@@ -19,7 +19,9 @@
  *                                   3-antenna hand case
  *   oracle_idft2_direct           : single-cell closed form cos(2 pi (ku x + kv y)/N + arg V)
  *   oracle_ifft2_radix2           : == oracle_idft2_direct on 32x32 (north_star check 4),
- *                                   == numpy.fft.ifft2 with shifts, Parseval, linearity
+ *                                   == numpy.fft.ifft2 with shifts, Parseval, linearity; sizes that are not a
+ *                                   power of two (direct 1D sums): == oracle_idft2_direct at 12 and 20,
+ *                                   == numpy.fft.ifft2 at 30, 48, 150, single-cell closed form at 1200
  *   oracle_sparse_image           : == radix-2 image on a full-size image
  *   oracle_image_one              : unit source at phase centre -> 1.0 at [h][h]; on-grid offset
  *                                   source peaks at its pixel with value 1.0; |Im| < 1e-6 peak
@@ -227,7 +229,38 @@ static void fft1d_radix2_inverse(double *re, double *im, int n)
     }
 }
 
-/* out[y][x] (complex, double pairs) = centred unnormalised inverse 2D DFT of grid[r][q] */
+/* Sizes that are not a power of two (the paper images at 1200 x 1200): the 1D transform is the
+ * plain sum X[j] = sum_k x[k] e^{+2 pi i j k / n}, O(n^2), with the n roots of unity tabulated once and indexed
+ * by (j k) mod n (exact periodicity, no large arguments).  Same sign and normalisation as the radix-2 routine. */
+static void dft1d_direct_inverse(double *re, double *im, int n)
+{
+    double *wr = (double *)malloc(sizeof(double) * n), *wi = (double *)malloc(sizeof(double) * n);
+    double *xr = (double *)malloc(sizeof(double) * n), *xi = (double *)malloc(sizeof(double) * n);
+    for (int m = 0; m < n; ++m) {
+        double a = 2.0 * ORACLE_PI * (double)m / (double)n;
+        wr[m] = cos(a); wi[m] = sin(a);
+        xr[m] = re[m]; xi[m] = im[m];
+    }
+    for (int j = 0; j < n; ++j) {
+        double sr = 0.0, si = 0.0;
+        int m = 0;                                        /* (j*k) mod n, advanced by j per term */
+        for (int k = 0; k < n; ++k) {
+            sr += xr[k] * wr[m] - xi[k] * wi[m];
+            si += xr[k] * wi[m] + xi[k] * wr[m];
+            m += j; if (m >= n) m -= n;
+        }
+        re[j] = sr; im[j] = si;
+    }
+    free(wr); free(wi); free(xr); free(xi);
+}
+static void fft1d_inverse_any(double *re, double *im, int n)
+{
+    if ((n & (n - 1)) == 0) fft1d_radix2_inverse(re, im, n);
+    else dft1d_direct_inverse(re, im, n);
+}
+
+/* out[y][x] (complex, double pairs) = centred unnormalised inverse 2D DFT of grid[r][q]
+ * (radix-2 rows and columns when n is a power of two, direct 1D sums otherwise) */
 void oracle_ifft2_radix2(const double *grid, int n, double *out)
 {
     const int h = n / 2;
@@ -240,7 +273,7 @@ void oracle_ifft2_radix2(const double *grid, int n, double *out)
             re[k] = grid[2 * ((size_t)r * n + q)];
             im[k] = grid[2 * ((size_t)r * n + q) + 1];
         }
-        fft1d_radix2_inverse(re, im, n);
+        fft1d_inverse_any(re, im, n);
         for (int j = 0; j < n; ++j) {
             int x = (j + h) % n;
             tmp[2 * ((size_t)r * n + x)] = re[j];
@@ -254,7 +287,7 @@ void oracle_ifft2_radix2(const double *grid, int n, double *out)
             re[k] = tmp[2 * ((size_t)r * n + x)];
             im[k] = tmp[2 * ((size_t)r * n + x) + 1];
         }
-        fft1d_radix2_inverse(re, im, n);
+        fft1d_inverse_any(re, im, n);
         for (int j = 0; j < n; ++j) {
             int y = (j + h) % n;
             out[2 * ((size_t)y * n + x)] = re[j];

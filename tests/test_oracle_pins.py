@@ -475,3 +475,43 @@ def test_gains_undo_corruption_restores_image(oracle_mod):
     c = oracle_mod.image_one(obs[0, 0, 0], uvw[0], f, N, 1.0 / N, 0)["image"]
     assert np.max(np.abs(a - b)) <= 1e-5 * np.max(np.abs(a))
     assert np.max(np.abs(a - c)) > 1e-2 * np.max(np.abs(a))                                   # the corruption was visible
+
+
+# ---------------------------------------------------------------------------------------------
+# image sides that are not a power of two (1200 x 1200)
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n", [12, 20])
+def test_non_pow2_transform_vs_bruteforce(oracle_mod, n):
+    rng = np.random.default_rng(300 + n)
+    g = rng.normal(size=(n, n)) + 1j * rng.normal(size=(n, n))
+    a, b = oracle_mod.ifft2_radix2(g), oracle_mod.idft2_direct(g)            # row-column 1D sums vs the O(N^4) definition
+    assert np.max(np.abs(a - b)) < 1e-11 * np.max(np.abs(b))
+
+
+@pytest.mark.parametrize("n", [30, 48, 150])
+def test_non_pow2_transform_vs_numpy_library(oracle_mod, n):
+    rng = np.random.default_rng(400 + n)
+    g = rng.normal(size=(n, n)) + 1j * rng.normal(size=(n, n))
+    a = oracle_mod.ifft2_radix2(g)
+    b = np.fft.fftshift(np.fft.ifft2(np.fft.ifftshift(g))) * (n * n)
+    assert np.max(np.abs(a - b)) < 1e-11 * np.max(np.abs(b))
+    assert abs((np.abs(a) ** 2).sum() / (n * n * (np.abs(g) ** 2).sum()) - 1) < 1e-12     # Parseval
+
+
+def test_non_pow2_single_cell_closed_form_and_unit_source(oracle_mod):
+    # the paper's own image side: one Hermitian pair of cells -> a cosine fringe with the stated sign, orientation, shift
+    n, ku, kv, V = 1200, 37, -211, 0.7 - 1.9j
+    h = n // 2
+    g = np.zeros((n, n), dtype=np.complex128)
+    g[kv + h, ku + h] = V
+    g[h - kv, h - ku] = np.conj(V)
+    out = oracle_mod.ifft2_radix2(g)
+    want = _closed_form_single_cell(n, ku, kv, V)
+    assert np.max(np.abs(out.real - want)) < 1e-9 and np.max(np.abs(out.imag)) < 1e-9
+    # whole image at a side of 240: all V = 1 -> exactly 1.0 at the phase centre, which is the maximum
+    rng = np.random.default_rng(5)
+    n = 240
+    uvw = rng.uniform(-60, 60, (200, 3)).astype(np.float32)
+    r = oracle_mod.image_one(np.ones(200, np.complex64), uvw, 150e6, n, 1.0 / n, 0)
+    assert abs(r["image"][n // 2, n // 2] - 1.0) < 1e-12 and r["image"].max() <= r["image"][n // 2, n // 2] + 1e-12
+    assert r["W"] == 2 * np.count_nonzero(r["cell_idx"] >= 0)
