@@ -44,7 +44,7 @@ enum { BLINK_OP_GRID = 0, BLINK_OP_FFT2D = 1, BLINK_OP_IMAGE = 2, BLINK_OP_IMAGE
 enum {
     BLINK_OK = 0,
     BLINK_ERR_INVALID_ARG = -1,   /* NULL / misaligned pointer, non-positive size, bad enum          */
-    BLINK_ERR_UNSUPPORTED = -2,   /* n_pix not a power of two in [32, 8192]; B too large (> 2^18-1)   */
+    BLINK_ERR_UNSUPPORTED = -2,   /* n_pix odd, outside [32, 8192] or with a prime factor > 5; B > 2^18-1 */
     BLINK_ERR_WORKSPACE   = -3,   /* workspace smaller than blink_workspace_bytes() reports           */
     BLINK_ERR_CUDA        = -4    /* a CUDA runtime/driver call failed: see blink_last_cuda_error()   */
 };

@@ -147,8 +147,10 @@ def blink_fft2d_inverse(grid: torch.Tensor, scale: Optional[torch.Tensor] = None
     imag = torch.empty((batch, n, n), dtype=torch.float32, device=dev) if want_imag else None
     if scale is not None:
         _dev(scale, torch.float32, "scale")
+    rec, _ = blink_workspace_bytes(OP_FFT2D, batch, 1, 1, 0, n, 0)         # non-zero only for sides that are not 2^k
+    ws = torch.empty(rec, dtype=torch.uint8, device=dev) if rec else None
     rc = lib().blink_fft2d_inverse(_ptr(grid), n, batch, _ptr(scale), int(scale_stride_div), _ptr(image), _ptr(imag),
-                                   None, 0, _stream(dev))
+                                   _ptr(ws), rec, _stream(dev))
     _check(rc, "blink_fft2d_inverse")
     return dict(image=image, imag=imag)
 

@@ -246,7 +246,8 @@ avg_scatter_runs_kernel(const AvgArgs a, const __grid_constant__ ScaleBlock sc, 
 
 static size_t avg_grid_bytes(int T, int P, int n_pix, int avg_time)
 {
-    return align_up((size_t)(avg_time ? 1 : T) * P * n_pix * n_pix * sizeof(float2), 256);
+    // the combined grids, then (sides that are not a power of two) the transform's twiddle table
+    return align_up((size_t)(avg_time ? 1 : T) * P * n_pix * n_pix * sizeof(float2), 256) + gfft_workspace_bytes(n_pix);
 }
 static int avg_max_planes() { return 2 * (sm_count() > 0 ? sm_count() : 148); }
 // workspace: combined grids | natural: winv [T*C] float | uniform: count planes
@@ -274,7 +275,7 @@ extern "C" int blink_image_avg(const blink_c64 *vis, const float *uvw_m, const d
     if (!vis || !uvw_m || !freqs_hz || !image_avg || !wsum) return BLINK_ERR_INVALID_ARG;
     if (T < 1 || C < 1 || P < 1 || B < 1 || !(pixscale_rad > 0.0)) return BLINK_ERR_INVALID_ARG;
     if (weighting != BLINK_W_NATURAL && weighting != BLINK_W_UNIFORM) return BLINK_ERR_INVALID_ARG;
-    if (!is_pow2(n_pix) || n_pix < 32 || n_pix > kMaxPix || B > kMaxBaselines) return BLINK_ERR_UNSUPPORTED;
+    if (!size_supported(n_pix) || B > kMaxBaselines) return BLINK_ERR_UNSUPPORTED;
     if ((long long)T * C * P > 0x3fffffffLL) return BLINK_ERR_UNSUPPORTED;
     if (!aligned16(vis) || !aligned16(image_avg)) return BLINK_ERR_INVALID_ARG;
     int rc = ensure_device();
@@ -352,5 +353,7 @@ extern "C" int blink_image_avg(const blink_c64 *vis, const float *uvw_m, const d
         tc = end;
     }
     // steps a4-a5 on the combined grids: already normalised, so no scale
-    return fft2d_range(grid, n_pix, n_out, nullptr, 1, 0, image_avg, nullptr, st);
+    float2 *tw_generic = is_pow2(n_pix) ? nullptr
+                                        : reinterpret_cast<float2 *>(static_cast<unsigned char *>(workspace) + gbytes - gfft_workspace_bytes(n_pix));
+    return fft2d_range(grid, n_pix, n_out, nullptr, 1, 0, image_avg, nullptr, st, tw_generic);
 }

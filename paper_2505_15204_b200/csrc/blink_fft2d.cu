@@ -187,9 +187,12 @@ static int launch_fft2d(float2 *grid, int batch, const float *scale, int scale_d
 }
 
 int fft2d_range(float2 *grid, int n_pix, int batch, const float *scale, int scale_div, int img_base, float *image,
-                float *image_imag, cudaStream_t st)
+                float *image_imag, cudaStream_t st, float2 *tw_generic)
 {
     if (batch == 0) return BLINK_OK;
+    if (!is_pow2(n_pix))
+        return size_supported(n_pix) ? gfft2d_range(grid, n_pix, batch, scale, scale_div, img_base, image, image_imag, tw_generic, st)
+                                     : (int)BLINK_ERR_UNSUPPORTED;
     switch (n_pix) {
         case 32: return launch_fft2d<32>(grid, batch, scale, scale_div, img_base, image, image_imag, st);
         case 64: return launch_fft2d<64>(grid, batch, scale, scale_div, img_base, image, image_imag, st);
@@ -210,15 +213,20 @@ extern "C" int blink_fft2d_inverse(blink_c64 *grid, int n_pix, int batch, const 
                                    float *image, float *image_imag, void *workspace, size_t workspace_bytes,
                                    void *stream)
 {
-    (void)workspace; (void)workspace_bytes;
     using namespace blink;
     if (grid == nullptr || image == nullptr || batch < 0) return BLINK_ERR_INVALID_ARG;
     if (!aligned16(grid) || !aligned16(image) || (image_imag && !aligned16(image_imag))) return BLINK_ERR_INVALID_ARG;
-    if (!is_pow2(n_pix) || n_pix < 32 || n_pix > kMaxPix) return BLINK_ERR_UNSUPPORTED;
+    if (!size_supported(n_pix)) return BLINK_ERR_UNSUPPORTED;
     if (scale != nullptr && scale_stride_div < 1) return BLINK_ERR_INVALID_ARG;
     if (scale == nullptr) scale_stride_div = 1;
     int rc = ensure_device();
     if (rc != BLINK_OK) return rc;
+    float2 *tw_generic = nullptr;                              // sides that are not a power of two: twiddle table in the workspace
+    if (!is_pow2(n_pix)) {
+        if (!workspace || (reinterpret_cast<uintptr_t>(workspace) & 15u) || workspace_bytes < gfft_workspace_bytes(n_pix))
+            return BLINK_ERR_WORKSPACE;
+        tw_generic = static_cast<float2 *>(workspace);
+    }
     return fft2d_range(reinterpret_cast<float2 *>(grid), n_pix, batch, scale, scale_stride_div, 0, image, image_imag,
-                       static_cast<cudaStream_t>(stream));
+                       static_cast<cudaStream_t>(stream), tw_generic);
 }

@@ -1,0 +1,209 @@
+// Centred inverse 2D transform for image sides that are NOT a power of two (N even, N = 2^a 3^b 5^c; the paper
+// images at 1200 x 1200).  Same definition as blink_fft2d.cu (sign +, unnormalised, fftshift,
+// 1/scale, real part; readings R5-R7), different machinery: a mixed-radix Stockham transform whose every stage
+// goes through shared memory (two ping-pong arrays), radices 4, 2, 3, 5, twiddles from an N-entry table
+// exp(+2 pi i m / N) that an init kernel writes (in double) into the caller's workspace.
+//   pass 1 (gfft_rows_kernel): rows, in place, input taken at the centred column (n + h) mod N, output in natural x;
+//   pass 2 (gfft_cols_kernel): KC columns per CTA, output row / column moved by h again, scaled, real part stored.
+// This is the fallback for the paper's own sizes, not a tuned path.
+#include <algorithm>
+
+#include "blink_common.cuh"
+#include "blink_fft.cuh"
+
+namespace blink {
+
+constexpr int kGThreads = 256;
+struct GPlan {
+    int n, nst;
+    int radix[16];
+};
+
+__global__ void gfft_twiddle_kernel(float2 *tw, int n)
+{
+    const int m = blockIdx.x * blockDim.x + threadIdx.x;
+    if (m >= n) return;
+    double s, c;
+    sincospi(2.0 * (double)m / (double)n, &s, &c);
+    tw[m] = make_float2((float)c, (float)s);
+}
+
+__device__ __forceinline__ void gdft3(float2 &x0, float2 &x1, float2 &x2)
+{
+    const float2 t = cadd(x1, x2), d = csub(x1, x2);
+    const float2 m = make_float2(x0.x - 0.5f * t.x, x0.y - 0.5f * t.y);
+    const float2 q = make_float2(0.86602540378443864676f * d.x, 0.86602540378443864676f * d.y);
+    x0 = cadd(x0, t);
+    x1 = make_float2(m.x - q.y, m.y + q.x);                    // m + i q
+    x2 = make_float2(m.x + q.y, m.y - q.x);                    // m - i q
+}
+__device__ __forceinline__ void gdft5(float2 &x0, float2 &x1, float2 &x2, float2 &x3, float2 &x4)
+{
+    const float c1 = 0.30901699437494742410f, c2 = -0.80901699437494742410f;      // cos(2 pi / 5), cos(4 pi / 5)
+    const float s1 = 0.95105651629515357212f, s2 = 0.58778525229247312917f;       // sin(2 pi / 5), sin(4 pi / 5)
+    const float2 a1 = cadd(x1, x4), a2 = cadd(x2, x3), b1 = csub(x1, x4), b2 = csub(x2, x3);
+    const float2 p1 = make_float2(x0.x + c1 * a1.x + c2 * a2.x, x0.y + c1 * a1.y + c2 * a2.y);
+    const float2 p2 = make_float2(x0.x + c2 * a1.x + c1 * a2.x, x0.y + c2 * a1.y + c1 * a2.y);
+    const float2 q1 = make_float2(s1 * b1.x + s2 * b2.x, s1 * b1.y + s2 * b2.y);
+    const float2 q2 = make_float2(s2 * b1.x - s1 * b2.x, s2 * b1.y - s1 * b2.y);
+    x0 = cadd(x0, cadd(a1, a2));
+    x1 = make_float2(p1.x - q1.y, p1.y + q1.x);                // p1 + i q1
+    x4 = make_float2(p1.x + q1.y, p1.y - q1.x);
+    x2 = make_float2(p2.x - q2.y, p2.y + q2.x);                // p2 + i q2
+    x3 = make_float2(p2.x + q2.y, p2.y - q2.x);
+}
+
+// One Stockham stage (radix R, sub-transform length P) of `nt` independent transforms of length n:
+// src[tr][i + r*(n/R)] -> dst[tr][(i - k)*R + k + r*P], k = i mod P, inputs r >= 1 twiddled by W_n^(r k n/(P R)).
+template <int R>
+__device__ __forceinline__ void gstage(const float2 *__restrict__ src, float2 *__restrict__ dst, int nt, int n, int P,
+                                       const float2 *__restrict__ tw)
+{
+    const int nb = n / R, step = n / (P * R);
+    for (int idx = threadIdx.x; idx < nt * nb; idx += kGThreads) {
+        const int tr = idx / nb, i = idx - tr * nb;
+        const int k = i % P;
+        const float2 *s = src + (size_t)tr * n + i;
+        float2 x[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) x[r] = s[r * nb];
+        if (P > 1) {
+#pragma unroll
+            for (int r = 1; r < R; ++r) x[r] = cmul(x[r], __ldg(tw + r * k * step));
+        }
+        if constexpr (R == 2) dft2(x[0], x[1]);
+        if constexpr (R == 3) gdft3(x[0], x[1], x[2]);
+        if constexpr (R == 4) dft4(x[0], x[1], x[2], x[3]);
+        if constexpr (R == 5) gdft5(x[0], x[1], x[2], x[3], x[4]);
+        float2 *d = dst + (size_t)tr * n + (i - k) * R + k;
+#pragma unroll
+        for (int r = 0; r < R; ++r) d[r * P] = x[r];
+    }
+}
+
+// all stages; returns the array that holds the result (natural order)
+__device__ __forceinline__ float2 *gfft_run(float2 *a, float2 *b, int nt, const GPlan &pl, const float2 *tw)
+{
+    int P = 1;
+    for (int s = 0; s < pl.nst; ++s) {
+        const int R = pl.radix[s];
+        if (R == 4) gstage<4>(a, b, nt, pl.n, P, tw);
+        else if (R == 2) gstage<2>(a, b, nt, pl.n, P, tw);
+        else if (R == 3) gstage<3>(a, b, nt, pl.n, P, tw);
+        else gstage<5>(a, b, nt, pl.n, P, tw);
+        __syncthreads();
+        float2 *t = a; a = b; b = t;
+        P *= R;
+    }
+    return a;
+}
+
+// ------------------------------------------------------------------------------------------ rows
+__global__ void __launch_bounds__(kGThreads)
+gfft_rows_kernel(float2 *__restrict__ grid, long long n_rows, const GPlan pl, const float2 *__restrict__ tw, int nr)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int n = pl.n, h = n / 2;
+    float2 *a = reinterpret_cast<float2 *>(smem_raw), *b = a + (size_t)nr * n;
+    for (long long base = (long long)blockIdx.x * nr; base < n_rows; base += (long long)gridDim.x * nr) {
+        const int cnt = (int)(n_rows - base < nr ? n_rows - base : nr);
+        for (int idx = threadIdx.x; idx < cnt * n; idx += kGThreads) {
+            const int tr = idx / n, j = idx - tr * n;
+            int q = j + h;                                     // transform index j lives in centred column (j + h) mod n
+            if (q >= n) q -= n;
+            a[(size_t)tr * n + j] = grid[(base + tr) * n + q];
+        }
+        __syncthreads();
+        const float2 *res = gfft_run(a, b, cnt, pl, tw);
+        for (int idx = threadIdx.x; idx < cnt * n; idx += kGThreads) {
+            const int tr = idx / n, j = idx - tr * n;
+            grid[(base + tr) * n + j] = res[(size_t)tr * n + j];                // natural (unshifted) x order
+        }
+        __syncthreads();
+    }
+}
+
+// ------------------------------------------------------------------------------------------ columns + epilogue
+__global__ void __launch_bounds__(kGThreads)
+gfft_cols_kernel(const float2 *__restrict__ grid, const GPlan pl, const float2 *__restrict__ tw, int kc, const float *__restrict__ scale,
+                 int scale_div, int img_base, float *__restrict__ image, float *__restrict__ image_imag)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int n = pl.n, h = n / 2;
+    float2 *a = reinterpret_cast<float2 *>(smem_raw), *b = a + (size_t)kc * n;
+    const int x0 = blockIdx.x * kc, img = blockIdx.y;
+    const size_t img_off = (size_t)img * n * n;
+    for (int idx = threadIdx.x; idx < n * kc; idx += kGThreads) {
+        const int j = idx / kc, c = idx - j * kc;              // c fastest: kc consecutive columns of one row
+        int r = j + h;                                         // transform index j lives in centred row (j + h) mod n
+        if (r >= n) r -= n;
+        a[(size_t)c * n + j] = grid[img_off + (size_t)r * n + x0 + c];
+    }
+    __syncthreads();
+    const float2 *res = gfft_run(a, b, kc, pl, tw);
+    float s = 1.0f;
+    if (scale != nullptr) {
+        const float w = scale[(img_base + img) / scale_div];
+        s = (w != 0.0f) ? 1.0f / w : 0.0f;
+    }
+    for (int idx = threadIdx.x; idx < n * kc; idx += kGThreads) {
+        const int j = idx / kc, c = idx - j * kc;
+        int y = j + h, x = x0 + c + h;                         // fftshift of both axes
+        if (y >= n) y -= n;
+        if (x >= n) x -= n;
+        const float2 v = res[(size_t)c * n + j];
+        image[img_off + (size_t)y * n + x] = v.x * s;
+        if (image_imag != nullptr) image_imag[img_off + (size_t)y * n + x] = v.y * s;
+    }
+}
+
+// ------------------------------------------------------------------------------------------ host
+bool size_supported(int n)
+{
+    if (n < 32 || n > kMaxPix || (n & 1)) return false;
+    while (n % 2 == 0) n /= 2;
+    while (n % 3 == 0) n /= 3;
+    while (n % 5 == 0) n /= 5;
+    return n == 1;
+}
+size_t gfft_workspace_bytes(int n) { return is_pow2(n) ? 0 : align_up((size_t)n * sizeof(float2), 256); }
+
+int gfft2d_range(float2 *grid, int n, int batch, const float *scale, int scale_div, int img_base, float *image,
+                 float *image_imag, float2 *tw, cudaStream_t st)
+{
+    if (batch == 0) return BLINK_OK;
+    if (!tw) return BLINK_ERR_WORKSPACE;
+    GPlan pl{};
+    pl.n = n;
+    int m = n;
+    while (m % 4 == 0) { pl.radix[pl.nst++] = 4; m /= 4; }
+    while (m % 2 == 0) { pl.radix[pl.nst++] = 2; m /= 2; }
+    while (m % 3 == 0) { pl.radix[pl.nst++] = 3; m /= 3; }
+    while (m % 5 == 0) { pl.radix[pl.nst++] = 5; m /= 5; }
+    if (m != 1) return BLINK_ERR_UNSUPPORTED;
+    gfft_twiddle_kernel<<<(n + 255) / 256, 256, 0, st>>>(tw, n);
+    BLINK_LAUNCH_CHECK("gfft_twiddle_kernel");
+    const size_t per = 2 * (size_t)n * sizeof(float2);          // ping + pong of one transform
+    const size_t budget = 200 * 1024;
+    int nr = (int)std::min<size_t>(4, budget / per);
+    int kc = 1;
+    for (int c = 8; c >= 1; c >>= 1)
+        if ((n / 2) % c == 0 && (size_t)c * per <= budget) { kc = c; break; }
+    if (nr < 1) return BLINK_ERR_UNSUPPORTED;
+    BLINK_CUDA_TRY(cudaFuncSetAttribute(gfft_rows_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(nr * per)));
+    BLINK_CUDA_TRY(cudaFuncSetAttribute(gfft_cols_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(kc * per)));
+    const long long n_rows = (long long)batch * n;
+    const long long want = (n_rows + nr - 1) / nr, cap = (long long)sm_count() * 8;
+    gfft_rows_kernel<<<(unsigned)(want < cap ? want : cap), kGThreads, nr * per, st>>>(grid, n_rows, pl, tw, nr);
+    BLINK_LAUNCH_CHECK("gfft_rows_kernel");
+    for (int b0 = 0; b0 < batch; b0 += 65535) {
+        const int nb = batch - b0 < 65535 ? batch - b0 : 65535;
+        gfft_cols_kernel<<<dim3(n / kc, nb), kGThreads, kc * per, st>>>(grid + (size_t)b0 * n * n, pl, tw, kc, scale, scale_div,
+                                                                       img_base + b0, image + (size_t)b0 * n * n,
+                                                                       image_imag ? image_imag + (size_t)b0 * n * n : nullptr);
+        BLINK_LAUNCH_CHECK("gfft_cols_kernel");
+    }
+    return BLINK_OK;
+}
+
+}  // namespace blink

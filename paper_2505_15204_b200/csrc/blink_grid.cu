@@ -113,8 +113,10 @@ grid_tiles_kernel(const GridArgs a, const __grid_constant__ ScaleBlock sc)
                 }
                 __syncthreads();
                 float2 *gdst = a.grid + ((size_t)otc * a.P + p) * n2 + (size_t)band * a.tile_cells;
+                // cells of this band that exist (n2 is a multiple of 4, so pairs / quads never straddle the end)
+                const int tile_n = (int)min((size_t)a.tile_cells, n2 - (size_t)band * a.tile_cells);
                 if (!multi) {
-                    for (int i = threadIdx.x * 2; i < a.tile_cells; i += kGridThreads * 2) {
+                    for (int i = threadIdx.x * 2; i < tile_n; i += kGridThreads * 2) {
                         float2 v0 = tile[i], v1 = tile[i + 1];
                         const uint32_t c0 = cnt[i], c1 = cnt[i + 1];
                         if (uniform) {
@@ -125,19 +127,19 @@ grid_tiles_kernel(const GridArgs a, const __grid_constant__ ScaleBlock sc)
                         __stcs(reinterpret_cast<float4 *>(gdst + i), make_float4(v0.x, v0.y, v1.x, v1.y));
                     }
                 } else if (ch == 0) {
-                    for (int i = threadIdx.x * 2; i < a.tile_cells; i += kGridThreads * 2)
+                    for (int i = threadIdx.x * 2; i < tile_n; i += kGridThreads * 2)
                         *reinterpret_cast<float4 *>(gdst + i) = make_float4(tile[i].x, tile[i].y, tile[i + 1].x, tile[i + 1].y);
                 } else {                                        // spill: add the touched cells with global atomics
-                    for (int i = threadIdx.x; i < a.tile_cells; i += kGridThreads)
+                    for (int i = threadIdx.x; i < tile_n; i += kGridThreads)
                         if (cnt[i]) { atomicAdd(&gdst[i].x, tile[i].x); atomicAdd(&gdst[i].y, tile[i].y); }
                 }
                 if (p == 0 && gcounts) {
                     uint32_t *cdst = gcounts + (size_t)band * a.tile_cells;
                     if (!multi || ch == 0) {
-                        for (int i = threadIdx.x * 4; i < a.tile_cells; i += kGridThreads * 4)
+                        for (int i = threadIdx.x * 4; i < tile_n; i += kGridThreads * 4)
                             *reinterpret_cast<uint4 *>(cdst + i) = *reinterpret_cast<const uint4 *>(cnt + i);
                     } else {
-                        for (int i = threadIdx.x; i < a.tile_cells; i += kGridThreads)
+                        for (int i = threadIdx.x; i < tile_n; i += kGridThreads)
                             if (cnt[i]) atomicAdd(&cdst[i], cnt[i]);
                     }
                 }
@@ -174,6 +176,13 @@ grid_tiles_kernel(const GridArgs a, const __grid_constant__ ScaleBlock sc)
     }
 }
 
+// band tile: a power of two number of cells (the band of a cell is a shift), at most 8192
+static int grid_tile_cells(size_t n2)
+{
+    int t = kTileCellsMax;
+    while ((size_t)t > n2) t >>= 1;
+    return t;
+}
 static size_t grid_smem_bytes(int tile_cells, int n_bands, int chunk_b)
 {
     return (size_t)tile_cells * 12 + (size_t)(2 * n_bands + 1) * 4 + (size_t)chunk_b * 8 + 16;
@@ -183,8 +192,8 @@ static size_t grid_smem_bytes(int tile_cells, int n_bands, int chunk_b)
 static int grid_chunk_capacity(int n_pix)
 {
     const size_t n2 = (size_t)n_pix * n_pix;
-    const int tile_cells = (int)(n2 < (size_t)kTileCellsMax ? n2 : kTileCellsMax);
-    const int n_bands = (int)(n2 / tile_cells);
+    const int tile_cells = grid_tile_cells(n2);
+    const int n_bands = (int)((n2 + tile_cells - 1) / tile_cells);
     const size_t fixed = grid_smem_bytes(tile_cells, n_bands, 0);
     const size_t avail = 227 * 1024 - 1024 - fixed;
     size_t cap = avail / 8;
@@ -209,8 +218,8 @@ int grid_range(const float2 *vis, const float *uvw_m, const double *freqs_hz, do
     GridArgs a;
     a.vis = vis; a.uvw_m = uvw_m; a.T = T; a.C = C; a.P = P; a.B = B; a.n = n_pix; a.weighting = weighting;
     a.out_tc0 = out_tc0; a.grid = grid; a.wsum = wsum; a.cell_idx = cell_idx; a.counts = counts;
-    a.tile_cells = (int)(n2 < (size_t)kTileCellsMax ? n2 : kTileCellsMax);
-    a.n_bands = (int)(n2 / a.tile_cells);
+    a.tile_cells = grid_tile_cells(n2);
+    a.n_bands = (int)((n2 + a.tile_cells - 1) / a.tile_cells);          // the last band may be partial (sides that are not a power of two)
     int chunk = option(BLINK_OPT_GRID_CHUNK_B);
     const int cap = grid_chunk_capacity(n_pix);
     if (chunk <= 0 || chunk > cap) chunk = cap;
@@ -251,7 +260,7 @@ extern "C" int blink_grid(const blink_c64 *vis, const float *uvw_m, const double
     if (T < 1 || C < 1 || P < 1 || B < 1 || !(pixscale_rad > 0.0)) return BLINK_ERR_INVALID_ARG;
     if (weighting != BLINK_W_NATURAL && weighting != BLINK_W_UNIFORM) return BLINK_ERR_INVALID_ARG;
     if (!aligned16(vis) || !aligned16(grid) || (counts && !aligned16(counts))) return BLINK_ERR_INVALID_ARG;
-    if (!is_pow2(n_pix) || n_pix < 32 || n_pix > kMaxPix || B > kMaxBaselines) return BLINK_ERR_UNSUPPORTED;
+    if (!size_supported(n_pix) || B > kMaxBaselines) return BLINK_ERR_UNSUPPORTED;
     if ((long long)T * C > 0x7fffffffLL / 2) return BLINK_ERR_UNSUPPORTED;
     int rc = ensure_device();
     if (rc != BLINK_OK) return rc;

@@ -49,7 +49,11 @@ static int image_device(const float2 *vis, const float *uvw_m, const double *fre
         return BLINK_OK;
     }
     const size_t per_tc = unfused_bytes_per_tc(P, B, n_pix, weighting, counts != nullptr);
-    if (!workspace || workspace_bytes < per_tc || !aligned16(workspace)) return BLINK_ERR_WORKSPACE;
+    const size_t twb = gfft_workspace_bytes(n_pix);            // sides that are not a power of two: twiddle table first
+    if (!workspace || workspace_bytes < twb + per_tc || !aligned16(workspace)) return BLINK_ERR_WORKSPACE;
+    float2 *tw_generic = twb ? static_cast<float2 *>(workspace) : nullptr;
+    workspace = static_cast<unsigned char *>(workspace) + twb;
+    workspace_bytes -= twb;
     const int chunk = (int)std::min<size_t>((size_t)ntc, workspace_bytes / per_tc);
     float2 *wgrid = static_cast<float2 *>(workspace);
     const bool ws_counts = per_tc > (size_t)P * n2 * sizeof(float2);
@@ -61,7 +65,7 @@ static int image_device(const float2 *vis, const float *uvw_m, const double *fre
         int rc = grid_range(vis, uvw_m, freqs_hz, pixscale_rad, T, C, P, B, n_pix, weighting, s, m, s, wgrid, wsum,
                             cell_idx, cptr, st);
         if (rc != BLINK_OK) return rc;
-        rc = fft2d_range(wgrid, n_pix, m * P, wsum, P, s * P, image + (size_t)s * P * n2, nullptr, st);
+        rc = fft2d_range(wgrid, n_pix, m * P, wsum, P, s * P, image + (size_t)s * P * n2, nullptr, st, tw_generic);
         if (rc != BLINK_OK) return rc;
     }
     return BLINK_OK;
@@ -111,7 +115,7 @@ static int check_common(const void *vis, const void *uvw_m, const double *freqs_
     if (!vis || !uvw_m || !freqs_hz) return BLINK_ERR_INVALID_ARG;
     if (T < 1 || C < 1 || P < 1 || B < 1 || !(pixscale_rad > 0.0)) return BLINK_ERR_INVALID_ARG;
     if (weighting != BLINK_W_NATURAL && weighting != BLINK_W_UNIFORM) return BLINK_ERR_INVALID_ARG;
-    if (!is_pow2(n_pix) || n_pix < 32 || n_pix > kMaxPix || B > kMaxBaselines) return BLINK_ERR_UNSUPPORTED;
+    if (!size_supported(n_pix) || B > kMaxBaselines) return BLINK_ERR_UNSUPPORTED;
     if ((long long)T * C * P > 0x3fffffffLL) return BLINK_ERR_UNSUPPORTED;
     return BLINK_OK;
 }
@@ -120,7 +124,7 @@ extern "C" int blink_workspace_bytes(int op, int T, int C, int P, int B, int n_p
                                      size_t *min_bytes)
 {
     if (!bytes) return BLINK_ERR_INVALID_ARG;
-    if (!is_pow2(n_pix) || n_pix < 32 || n_pix > kMaxPix) return BLINK_ERR_UNSUPPORTED;
+    if (!size_supported(n_pix)) return BLINK_ERR_UNSUPPORTED;
     if (T < 1 || C < 1 || P < 1 || B < 0) return BLINK_ERR_INVALID_ARG;
     const size_t n2 = (size_t)n_pix * n_pix;
     size_t rec = 0, mn = 0;
@@ -129,7 +133,7 @@ extern "C" int blink_workspace_bytes(int op, int T, int C, int P, int B, int n_p
             rec = mn = grid_needs_global_counts(B, n_pix, weighting) ? (size_t)T * C * n2 * sizeof(uint32_t) : 0;
             break;
         case BLINK_OP_FFT2D:
-            rec = mn = 0;
+            rec = mn = gfft_workspace_bytes(n_pix);
             break;
         case BLINK_OP_IMAGE:
         case BLINK_OP_IMAGE_HOST: {
@@ -140,8 +144,8 @@ extern "C" int blink_workspace_bytes(int op, int T, int C, int P, int B, int n_p
                 mn = fused_workspace_bytes(T, B, n_pix, 1);
             } else {
                 const size_t per_tc = unfused_bytes_per_tc(P, B, n_pix, weighting, false);
-                mn = per_tc;
-                rec = per_tc * std::min<size_t>((size_t)T * C, 256);
+                mn = gfft_workspace_bytes(n_pix) + per_tc;
+                rec = gfft_workspace_bytes(n_pix) + per_tc * std::min<size_t>((size_t)T * C, 256);
             }
             if (op == BLINK_OP_IMAGE_HOST) {
                 // device staging: uvw for all timesteps, wsum, and two slots of one timestep of vis + images

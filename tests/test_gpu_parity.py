@@ -307,12 +307,13 @@ def test_error_codes(bk):
     p = lambda t: ctypes.c_void_p(t.data_ptr())
     f = fr.ctypes.data_as(ctypes.c_void_p)
     # n_pix not a power of two / too small / too large
-    for n in (48, 16, 16384):
+    for n in (66, 45, 16, 16384):                               # prime factor 11, odd, too small, too large
         assert L.blink_image(p(x), p(x), f, 1, 1, 1, 4, n, 0.01, 0, p(x), p(x), None, None, p(x), 64, None) == -2
     assert L.blink_image(None, p(x), f, 1, 1, 1, 4, 32, 0.01, 0, p(x), p(x), None, None, p(x), 64, None) == -1
     assert L.blink_image(p(x), p(x), f, 1, 1, 1, 4, 32, -1.0, 0, p(x), p(x), None, None, p(x), 64, None) == -1
     assert L.blink_image(p(x), p(x), f, 1, 1, 1, 4, 32, 0.01, 7, p(x), p(x), None, None, p(x), 64, None) == -1
-    assert L.blink_fft2d_inverse(p(x), 100, 1, None, 1, p(x), None, None, 0, None) == -2
+    assert L.blink_fft2d_inverse(p(x), 98, 1, None, 1, p(x), None, None, 0, None) == -2        # 2 * 7^2
+    assert L.blink_fft2d_inverse(p(x), 100, 1, None, 1, p(x), None, None, 0, None) == -3       # needs its twiddle workspace
     assert L.blink_strerror(-3).decode() == "workspace too small"
 
 
@@ -558,3 +559,51 @@ def test_more_than_1024_channels(bk, oracle_mod, path):
     mean = res["image"].reshape(w.T, w.C, w.n_pix, w.n_pix).double().mean(dim=1)
     assert float((avg["image_avg"].double() - mean).abs().max() / mean.abs().max()) <= TOL
     assert torch.equal(avg["wsum"], res["wsum"])
+
+
+# --------------------------------------------------------------------------- sides that are not a power of two
+@pytest.mark.parametrize("n,batch", [(48, 3), (240, 2), (1200, 1)])
+def test_fft2d_non_pow2(bk, oracle_mod, n, batch):
+    rng = np.random.default_rng(500 + n)
+    g = (rng.normal(size=(batch, n, n)) + 1j * rng.normal(size=(batch, n, n))).astype(np.complex64)
+    g[0, n // 2 + 3, n // 2 - 5] += 50 * n
+    g[-1, 1, n - 2] += (30 - 40j) * n
+    scale = torch.tensor(rng.uniform(0.5, 2.0, batch).astype(np.float32), device="cuda")
+    r = bk.blink_fft2d_inverse(torch.tensor(g, device="cuda"), scale=scale, scale_stride_div=1, want_imag=True)
+    torch.cuda.synchronize()
+    re, im = r["image"].cpu().numpy(), r["imag"].cpu().numpy()
+    sc = scale.cpu().numpy().astype(np.float64)
+    for b in range(batch):
+        ref = oracle_mod.ifft2_radix2(g[b].astype(np.complex128)) / sc[b]
+        peak = np.max(np.abs(ref))
+        assert np.max(np.abs(re[b] - ref.real)) <= TOL * peak
+        assert np.max(np.abs(im[b] - ref.imag)) <= TOL * peak
+
+
+@pytest.mark.parametrize("n,weighting", [(48, 1), (240, 0), (1200, 1)])
+def test_grid_and_image_non_pow2(bk, oracle_mod, n, weighting):
+    from paper_2505_15204_b200 import workloads
+    w = workloads.make_random(T=1, C=2, P=2, B=1500, n_pix=n, weighting=weighting, seed=n + weighting, device="cuda", fill=1.1)
+    _check_grid(bk, oracle_mod, w)
+    res = bk.blink_image(w.vis, w.uvw_m, w.freqs_hz, w.n_pix, w.pixscale_rad, w.weighting, want_cell_idx=True)
+    torch.cuda.synchronize()
+    _check_images(bk, w, res, oracle_mod, [0, 3] if n == 1200 else None)
+    assert np.array_equal(res["cell_idx"].cpu().numpy(),
+                          oracle_mod.cells(w.uvw_m.cpu().numpy(), w.freqs_hz, w.n_pix, w.pixscale_rad))
+    if n <= 240:
+        _check_avg(bk, oracle_mod, w, False)
+        _check_avg(bk, oracle_mod, w, True)
+
+
+def test_image_1200_paper_size(bk, oracle_mod):
+    """The paper's high-time-resolution image side (1200 x 1200): config-3 visibilities imaged at 1200,
+    individually and channel-averaged, against the oracle."""
+    from paper_2505_15204_b200 import workloads
+    w = workloads.make_config(3, device="cuda", T=1, C=4)
+    w.n_pix, w.pixscale_rad = 1200, 0.6 / 1200
+    res = bk.blink_image(w.vis, w.uvw_m, w.freqs_hz, w.n_pix, w.pixscale_rad, w.weighting)
+    torch.cuda.synchronize()
+    _check_images(bk, w, res, oracle_mod, [0, 3])
+    avg = bk.blink_image_avg(w.vis, w.uvw_m, w.freqs_hz, w.n_pix, w.pixscale_rad, w.weighting)
+    mean = res["image"].double().mean(dim=0)
+    assert float((avg["image_avg"][0].double() - mean).abs().max() / mean.abs().max()) <= TOL
