@@ -13,7 +13,7 @@
 
 namespace blink {
 
-constexpr int kGThreads = 256;
+constexpr int kGRowThreads = 512, kGColThreads = 1024;
 struct GPlan {
     int n, nst;
     int radix[16];
@@ -53,17 +53,24 @@ __device__ __forceinline__ void gdft5(float2 &x0, float2 &x1, float2 &x2, float2
     x3 = make_float2(p2.x + q2.y, p2.y - q2.x);
 }
 
-// One Stockham stage (radix R, sub-transform length P) of `nt` independent transforms of length n:
-// src[tr][i + r*(n/R)] -> dst[tr][(i - k)*R + k + r*P], k = i mod P, inputs r >= 1 twiddled by W_n^(r k n/(P R)).
+// exact i / d for 0 <= i < 2^16 by a float reciprocal ((i + 1/2) / d is at least 1/(2d) away from an integer, far
+// more than the rounding error of the product)
+__device__ __forceinline__ int fdiv_small(int i, int d, float inv_d) { (void)d; return (int)(((float)i + 0.5f) * inv_d); }
+
+// One Stockham stage (radix R, sub-transform length P) of `nt` independent transforms of length n stored with
+// leading dimension ld: src[tr][i + r*(n/R)] -> dst[tr][(i - k)*R + k + r*P], k = i mod P, inputs r >= 1
+// twiddled by W_n^(r k n/(P R)).  Reads are unit-stride in i; writes are runs of P consecutive elements, which is
+// why the plan puts the odd radices first (P grows past a warp before the radix-4 stages: no bank conflicts there).
 template <int R>
-__device__ __forceinline__ void gstage(const float2 *__restrict__ src, float2 *__restrict__ dst, int nt, int n, int P,
+__device__ __forceinline__ void gstage(const float2 *__restrict__ src, float2 *__restrict__ dst, int nt, int n, int ld, int P,
                                        const float2 *__restrict__ tw)
 {
     const int nb = n / R, step = n / (P * R);
-    for (int idx = threadIdx.x; idx < nt * nb; idx += kGThreads) {
-        const int tr = idx / nb, i = idx - tr * nb;
-        const int k = i % P;
-        const float2 *s = src + (size_t)tr * n + i;
+    const float inv_nb = 1.0f / (float)nb, inv_p = 1.0f / (float)P;
+    for (int idx = threadIdx.x; idx < nt * nb; idx += blockDim.x) {
+        const int tr = fdiv_small(idx, nb, inv_nb), i = idx - tr * nb;
+        const int k = i - P * fdiv_small(i, P, inv_p);
+        const float2 *s = src + (size_t)tr * ld + i;
         float2 x[R];
 #pragma unroll
         for (int r = 0; r < R; ++r) x[r] = s[r * nb];
@@ -75,22 +82,22 @@ __device__ __forceinline__ void gstage(const float2 *__restrict__ src, float2 *_
         if constexpr (R == 3) gdft3(x[0], x[1], x[2]);
         if constexpr (R == 4) dft4(x[0], x[1], x[2], x[3]);
         if constexpr (R == 5) gdft5(x[0], x[1], x[2], x[3], x[4]);
-        float2 *d = dst + (size_t)tr * n + (i - k) * R + k;
+        float2 *d = dst + (size_t)tr * ld + (i - k) * R + k;
 #pragma unroll
         for (int r = 0; r < R; ++r) d[r * P] = x[r];
     }
 }
 
 // all stages; returns the array that holds the result (natural order)
-__device__ __forceinline__ float2 *gfft_run(float2 *a, float2 *b, int nt, const GPlan &pl, const float2 *tw)
+__device__ __forceinline__ float2 *gfft_run(float2 *a, float2 *b, int nt, int ld, const GPlan &pl, const float2 *tw)
 {
     int P = 1;
     for (int s = 0; s < pl.nst; ++s) {
         const int R = pl.radix[s];
-        if (R == 4) gstage<4>(a, b, nt, pl.n, P, tw);
-        else if (R == 2) gstage<2>(a, b, nt, pl.n, P, tw);
-        else if (R == 3) gstage<3>(a, b, nt, pl.n, P, tw);
-        else gstage<5>(a, b, nt, pl.n, P, tw);
+        if (R == 4) gstage<4>(a, b, nt, pl.n, ld, P, tw);
+        else if (R == 2) gstage<2>(a, b, nt, pl.n, ld, P, tw);
+        else if (R == 3) gstage<3>(a, b, nt, pl.n, ld, P, tw);
+        else gstage<5>(a, b, nt, pl.n, ld, P, tw);
         __syncthreads();
         float2 *t = a; a = b; b = t;
         P *= R;
@@ -99,7 +106,7 @@ __device__ __forceinline__ float2 *gfft_run(float2 *a, float2 *b, int nt, const 
 }
 
 // ------------------------------------------------------------------------------------------ rows
-__global__ void __launch_bounds__(kGThreads)
+__global__ void __launch_bounds__(kGRowThreads)
 gfft_rows_kernel(float2 *__restrict__ grid, long long n_rows, const GPlan pl, const float2 *__restrict__ tw, int nr)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -107,15 +114,15 @@ gfft_rows_kernel(float2 *__restrict__ grid, long long n_rows, const GPlan pl, co
     float2 *a = reinterpret_cast<float2 *>(smem_raw), *b = a + (size_t)nr * n;
     for (long long base = (long long)blockIdx.x * nr; base < n_rows; base += (long long)gridDim.x * nr) {
         const int cnt = (int)(n_rows - base < nr ? n_rows - base : nr);
-        for (int idx = threadIdx.x; idx < cnt * n; idx += kGThreads) {
+        for (int idx = threadIdx.x; idx < cnt * n; idx += kGRowThreads) {
             const int tr = idx / n, j = idx - tr * n;
             int q = j + h;                                     // transform index j lives in centred column (j + h) mod n
             if (q >= n) q -= n;
             a[(size_t)tr * n + j] = grid[(base + tr) * n + q];
         }
         __syncthreads();
-        const float2 *res = gfft_run(a, b, cnt, pl, tw);
-        for (int idx = threadIdx.x; idx < cnt * n; idx += kGThreads) {
+        const float2 *res = gfft_run(a, b, cnt, n, pl, tw);
+        for (int idx = threadIdx.x; idx < cnt * n; idx += kGRowThreads) {
             const int tr = idx / n, j = idx - tr * n;
             grid[(base + tr) * n + j] = res[(size_t)tr * n + j];                // natural (unshifted) x order
         }
@@ -124,34 +131,35 @@ gfft_rows_kernel(float2 *__restrict__ grid, long long n_rows, const GPlan pl, co
 }
 
 // ------------------------------------------------------------------------------------------ columns + epilogue
-__global__ void __launch_bounds__(kGThreads)
+__global__ void __launch_bounds__(kGColThreads)
 gfft_cols_kernel(const float2 *__restrict__ grid, const GPlan pl, const float2 *__restrict__ tw, int kc, const float *__restrict__ scale,
                  int scale_div, int img_base, float *__restrict__ image, float *__restrict__ image_imag)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int n = pl.n, h = n / 2;
-    float2 *a = reinterpret_cast<float2 *>(smem_raw), *b = a + (size_t)kc * n;
+    const int ld = n + 1;                                      // odd leading dimension: the kc columns of a row fall in different banks
+    float2 *a = reinterpret_cast<float2 *>(smem_raw), *b = a + (size_t)kc * ld;
     const int x0 = blockIdx.x * kc, img = blockIdx.y;
     const size_t img_off = (size_t)img * n * n;
-    for (int idx = threadIdx.x; idx < n * kc; idx += kGThreads) {
+    for (int idx = threadIdx.x; idx < n * kc; idx += kGColThreads) {
         const int j = idx / kc, c = idx - j * kc;              // c fastest: kc consecutive columns of one row
         int r = j + h;                                         // transform index j lives in centred row (j + h) mod n
         if (r >= n) r -= n;
-        a[(size_t)c * n + j] = grid[img_off + (size_t)r * n + x0 + c];
+        a[(size_t)c * ld + j] = grid[img_off + (size_t)r * n + x0 + c];
     }
     __syncthreads();
-    const float2 *res = gfft_run(a, b, kc, pl, tw);
+    const float2 *res = gfft_run(a, b, kc, ld, pl, tw);
     float s = 1.0f;
     if (scale != nullptr) {
         const float w = scale[(img_base + img) / scale_div];
         s = (w != 0.0f) ? 1.0f / w : 0.0f;
     }
-    for (int idx = threadIdx.x; idx < n * kc; idx += kGThreads) {
+    for (int idx = threadIdx.x; idx < n * kc; idx += kGColThreads) {
         const int j = idx / kc, c = idx - j * kc;
         int y = j + h, x = x0 + c + h;                         // fftshift of both axes
         if (y >= n) y -= n;
         if (x >= n) x -= n;
-        const float2 v = res[(size_t)c * n + j];
+        const float2 v = res[(size_t)c * ld + j];
         image[img_off + (size_t)y * n + x] = v.x * s;
         if (image_imag != nullptr) image_imag[img_off + (size_t)y * n + x] = v.y * s;
     }
@@ -176,14 +184,14 @@ int gfft2d_range(float2 *grid, int n, int batch, const float *scale, int scale_d
     GPlan pl{};
     pl.n = n;
     int m = n;
+    while (m % 5 == 0) { pl.radix[pl.nst++] = 5; m /= 5; }     // odd radices first (see gstage)
+    while (m % 3 == 0) { pl.radix[pl.nst++] = 3; m /= 3; }
     while (m % 4 == 0) { pl.radix[pl.nst++] = 4; m /= 4; }
     while (m % 2 == 0) { pl.radix[pl.nst++] = 2; m /= 2; }
-    while (m % 3 == 0) { pl.radix[pl.nst++] = 3; m /= 3; }
-    while (m % 5 == 0) { pl.radix[pl.nst++] = 5; m /= 5; }
     if (m != 1) return BLINK_ERR_UNSUPPORTED;
     gfft_twiddle_kernel<<<(n + 255) / 256, 256, 0, st>>>(tw, n);
     BLINK_LAUNCH_CHECK("gfft_twiddle_kernel");
-    const size_t per = 2 * (size_t)n * sizeof(float2);          // ping + pong of one transform
+    const size_t per = 2 * (size_t)(n + 1) * sizeof(float2);    // ping + pong of one transform (padded leading dimension)
     const size_t budget = 200 * 1024;
     int nr = (int)std::min<size_t>(4, budget / per);
     int kc = 1;
@@ -194,11 +202,11 @@ int gfft2d_range(float2 *grid, int n, int batch, const float *scale, int scale_d
     BLINK_CUDA_TRY(cudaFuncSetAttribute(gfft_cols_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(kc * per)));
     const long long n_rows = (long long)batch * n;
     const long long want = (n_rows + nr - 1) / nr, cap = (long long)sm_count() * 8;
-    gfft_rows_kernel<<<(unsigned)(want < cap ? want : cap), kGThreads, nr * per, st>>>(grid, n_rows, pl, tw, nr);
+    gfft_rows_kernel<<<(unsigned)(want < cap ? want : cap), kGRowThreads, nr * per, st>>>(grid, n_rows, pl, tw, nr);
     BLINK_LAUNCH_CHECK("gfft_rows_kernel");
     for (int b0 = 0; b0 < batch; b0 += 65535) {
         const int nb = batch - b0 < 65535 ? batch - b0 : 65535;
-        gfft_cols_kernel<<<dim3(n / kc, nb), kGThreads, kc * per, st>>>(grid + (size_t)b0 * n * n, pl, tw, kc, scale, scale_div,
+        gfft_cols_kernel<<<dim3(n / kc, nb), kGColThreads, kc * per, st>>>(grid + (size_t)b0 * n * n, pl, tw, kc, scale, scale_div,
                                                                        img_base + b0, image + (size_t)b0 * n * n,
                                                                        image_imag ? image_imag + (size_t)b0 * n * n : nullptr);
         BLINK_LAUNCH_CHECK("gfft_cols_kernel");
