@@ -14,7 +14,7 @@
  *   a5  inverse FFT along v (columns)   /  batched over all grids; sign +, unnormalised (R5)
  *       + fftshift (L194), * 1/W (R6), real part  ->  float32 dirty image (L150: fp32 throughout)
  *
- * Image index i = (t*C + c)*P + p, n_img = T*C*P.  N = n_pix, h = N/2.  All arrays are dense,
+ * Image index i = (t*C + c)*P + p, n_img = T*C*P.  N = n_pix (even, 32..8192, no prime factor above 5), h = N/2.  All arrays are dense,
  * row-major, last index fastest.  "centred" means the DC cell / phase-centre pixel is [h][h];
  * column index = u / l axis, row index = v / m axis (R7, R8).
  *
