@@ -103,6 +103,8 @@ int blink_grid(const blink_c64 *vis, const float *uvw_m, const double *freqs_hz,
  *   image_imag  out OPTIONAL [batch][N][N] float32: the imaginary part, same scaling (debug / tests)
  * Row pass in shared memory, then a column pass whose tiles are staged by TMA with the fftshift,
  * the 1/W normalisation and the real-part extraction fused into its store.
+ * Sides that are not a power of two run a mixed-radix transform instead and need `workspace` >=
+ * blink_workspace_bytes(BLINK_OP_FFT2D) (an N-entry twiddle table); powers of two need none.
  */
 int blink_fft2d_inverse(blink_c64 *grid, int n_pix, int batch,
                         const float *scale, int scale_stride_div,
