@@ -49,7 +49,12 @@ def test_host_only_calls(so_path):
     bk.set_option(bk.OPT_IMAGE_PATH, 0)
     assert mn == 512 * 512 * 8 and rec == 256 * mn
     with pytest.raises(bk.BlinkError):
-        bk.blink_workspace_bytes(bk.OP_IMAGE, 1, 1, 1, 10, 100, 0)        # not a power of two
+        bk.blink_workspace_bytes(bk.OP_IMAGE, 1, 1, 1, 10, 98, 0)         # 2 * 7^2: a prime factor above 5
+    with pytest.raises(bk.BlinkError):
+        bk.blink_workspace_bytes(bk.OP_IMAGE, 1, 1, 1, 10, 45, 0)         # odd
+    # sides that are not a power of two need an N-entry twiddle table for the mixed-radix transform
+    rec, mn = bk.blink_workspace_bytes(bk.OP_FFT2D, 1, 1, 1, 0, 1200, 0)
+    assert rec == mn == 1200 * 8 + (-1200 * 8) % 256
 
 
 def test_no_cpu_fallback_without_device(so_path):
