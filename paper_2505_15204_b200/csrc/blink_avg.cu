@@ -355,5 +355,5 @@ extern "C" int blink_image_avg(const blink_c64 *vis, const float *uvw_m, const d
     // steps a4-a5 on the combined grids: already normalised, so no scale
     float2 *tw_generic = is_pow2(n_pix) ? nullptr
                                         : reinterpret_cast<float2 *>(static_cast<unsigned char *>(workspace) + gbytes - gfft_workspace_bytes(n_pix));
-    return fft2d_range(grid, n_pix, n_out, nullptr, 1, 0, image_avg, nullptr, st, tw_generic);
+    return fft2d_range(grid, n_pix, n_out, nullptr, 1, 0, image_avg, nullptr, st, tw_generic, true);
 }

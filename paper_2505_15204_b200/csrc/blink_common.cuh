@@ -101,13 +101,14 @@ int grid_range(const float2 *vis, const float *uvw_m, const double *freqs_hz, do
                int P, int B, int n_pix, int weighting, int tc0, int ntc, int out_tc0, float2 *grid, float *wsum,
                int32_t *cell_idx, uint32_t *counts, cudaStream_t st);
 bool grid_needs_global_counts(int B, int n_pix, int weighting);
+// hermitian: the grids come from the library's own gridders (G[-v][-u] = conj G[v][u], row / column -N/2 empty)
 // tw_generic: device array of n_pix complex64 (gfft_workspace_bytes) for sides that are not a power of two, else unused
 int fft2d_range(float2 *grid, int n_pix, int batch, const float *scale, int scale_div, int scale_img_base,
-                float *image, float *image_imag, cudaStream_t st, float2 *tw_generic = nullptr);
+                float *image, float *image_imag, cudaStream_t st, float2 *tw_generic = nullptr, bool hermitian = false);
 // image sides: even, 32..kMaxPix, only prime factors 2, 3, 5 (powers of two run the tuned kernels)
 bool size_supported(int n_pix);
 size_t gfft_workspace_bytes(int n_pix);
 int gfft2d_range(float2 *grid, int n, int batch, const float *scale, int scale_div, int img_base, float *image,
-                 float *image_imag, float2 *tw, cudaStream_t st);
+                 float *image_imag, float2 *tw, cudaStream_t st, bool hermitian);
 
 }  // namespace blink

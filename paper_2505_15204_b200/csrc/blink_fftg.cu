@@ -107,8 +107,10 @@ __device__ __forceinline__ float2 *gfft_run(float2 *a, float2 *b, int nt, int ld
 
 // ------------------------------------------------------------------------------------------ rows
 __global__ void __launch_bounds__(kGRowThreads)
-gfft_rows_kernel(float2 *__restrict__ grid, long long n_rows, const GPlan pl, const float2 *__restrict__ tw, int nr)
+gfft_rows_kernel(float2 *__restrict__ grid, long long n_rows, const GPlan pl, const float2 *__restrict__ tw, int nr, int rows_per_img,
+                 int row_off)
 {
+    // logical row L -> image L / rows_per_img, row row_off + L % rows_per_img (Hermitian grids: only the rows v >= 0)
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int n = pl.n, h = n / 2;
     float2 *a = reinterpret_cast<float2 *>(smem_raw), *b = a + (size_t)nr * n;
@@ -118,13 +120,17 @@ gfft_rows_kernel(float2 *__restrict__ grid, long long n_rows, const GPlan pl, co
             const int tr = idx / n, j = idx - tr * n;
             int q = j + h;                                     // transform index j lives in centred column (j + h) mod n
             if (q >= n) q -= n;
-            a[(size_t)tr * n + j] = grid[(base + tr) * n + q];
+            const long long L = base + tr;
+            const long long grow = (L / rows_per_img) * n + row_off + (L % rows_per_img);
+            a[(size_t)tr * n + j] = grid[grow * n + q];
         }
         __syncthreads();
         const float2 *res = gfft_run(a, b, cnt, n, pl, tw);
         for (int idx = threadIdx.x; idx < cnt * n; idx += kGRowThreads) {
             const int tr = idx / n, j = idx - tr * n;
-            grid[(base + tr) * n + j] = res[(size_t)tr * n + j];                // natural (unshifted) x order
+            const long long L = base + tr;
+            const long long grow = (L / rows_per_img) * n + row_off + (L % rows_per_img);
+            grid[grow * n + j] = res[(size_t)tr * n + j];                       // natural (unshifted) x order
         }
         __syncthreads();
     }
@@ -165,6 +171,46 @@ gfft_cols_kernel(const float2 *__restrict__ grid, const GPlan pl, const float2 *
     }
 }
 
+// Hermitian grids (everything the library's own gridders produce: G[-v][-u] = conj G[v][u], row and column -N/2
+// empty): after the row pass R[-v][x] = conj R[v][x], so only the rows v >= 0 were transformed, and two columns
+// x1, x2 become ONE complex transform Z[v] = R[v][x1] + i R[v][x2], Z[-v] = conj R[v][x1] + i conj R[v][x2] whose
+// real part is image column x1 and imaginary part image column x2.  Half the reads, half the transforms.
+__global__ void __launch_bounds__(kGColThreads)
+gfft_cols_herm_kernel(const float2 *__restrict__ grid, const GPlan pl, const float2 *__restrict__ tw, int kc, const float *__restrict__ scale,
+                      int scale_div, int img_base, float *__restrict__ image)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int n = pl.n, h = n / 2, np = kc / 2;                // np column pairs = transforms per CTA
+    const int ld = n + 1;
+    float2 *a = reinterpret_cast<float2 *>(smem_raw), *b = a + (size_t)np * ld;
+    const int x0 = blockIdx.x * kc, img = blockIdx.y;
+    const size_t img_off = (size_t)img * n * n;
+    for (int idx = threadIdx.x; idx < h * np; idx += kGColThreads) {
+        const int v = idx / np, p = idx - v * np;              // p fastest: consecutive 16-byte column pairs of one row
+        const float4 q = *reinterpret_cast<const float4 *>(grid + img_off + (size_t)(h + v) * n + x0 + 2 * p);
+        a[(size_t)p * ld + v] = make_float2(q.x - q.w, q.y + q.z);                   // S1 + i S2
+        if (v > 0) a[(size_t)p * ld + n - v] = make_float2(q.x + q.w, q.z - q.y);    // conj S1 + i conj S2
+    }
+    for (int p = threadIdx.x; p < np; p += kGColThreads) a[(size_t)p * ld + h] = make_float2(0.f, 0.f);   // the empty row -N/2
+    __syncthreads();
+    const float2 *res = gfft_run(a, b, np, ld, pl, tw);
+    float s = 1.0f;
+    if (scale != nullptr) {
+        const float w = scale[(img_base + img) / scale_div];
+        s = (w != 0.0f) ? 1.0f / w : 0.0f;
+    }
+    for (int idx = threadIdx.x; idx < n * np; idx += kGColThreads) {
+        const int j = idx / np, p = idx - j * np;
+        int y = j + h, x = x0 + 2 * p + h, x1 = x0 + 2 * p + 1 + h;      // fftshift of both axes
+        if (y >= n) y -= n;
+        if (x >= n) x -= n;
+        if (x1 >= n) x1 -= n;
+        const float2 z = res[(size_t)p * ld + j];
+        image[img_off + (size_t)y * n + x] = z.x * s;
+        image[img_off + (size_t)y * n + x1] = z.y * s;
+    }
+}
+
 // ------------------------------------------------------------------------------------------ host
 bool size_supported(int n)
 {
@@ -177,8 +223,9 @@ bool size_supported(int n)
 size_t gfft_workspace_bytes(int n) { return is_pow2(n) ? 0 : align_up((size_t)n * sizeof(float2), 256); }
 
 int gfft2d_range(float2 *grid, int n, int batch, const float *scale, int scale_div, int img_base, float *image,
-                 float *image_imag, float2 *tw, cudaStream_t st)
+                 float *image_imag, float2 *tw, cudaStream_t st, bool hermitian)
 {
+    if (image_imag) hermitian = false;                          // the imaginary part is only defined for the general transform
     if (batch == 0) return BLINK_OK;
     if (!tw) return BLINK_ERR_WORKSPACE;
     GPlan pl{};
@@ -200,15 +247,28 @@ int gfft2d_range(float2 *grid, int n, int batch, const float *scale, int scale_d
     if (nr < 1) return BLINK_ERR_UNSUPPORTED;
     BLINK_CUDA_TRY(cudaFuncSetAttribute(gfft_rows_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(nr * per)));
     BLINK_CUDA_TRY(cudaFuncSetAttribute(gfft_cols_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(kc * per)));
-    const long long n_rows = (long long)batch * n;
+    const int rows_per_img = hermitian ? n / 2 : n, row_off = hermitian ? n / 2 : 0;
+    const long long n_rows = (long long)batch * rows_per_img;
     const long long want = (n_rows + nr - 1) / nr, cap = (long long)sm_count() * 8;
-    gfft_rows_kernel<<<(unsigned)(want < cap ? want : cap), kGRowThreads, nr * per, st>>>(grid, n_rows, pl, tw, nr);
+    gfft_rows_kernel<<<(unsigned)(want < cap ? want : cap), kGRowThreads, nr * per, st>>>(grid, n_rows, pl, tw, nr, rows_per_img, row_off);
     BLINK_LAUNCH_CHECK("gfft_rows_kernel");
+    // Hermitian: kc columns are kc/2 transforms; keep two CTAs per SM when the arrays allow it
+    int kch = 2;
+    for (int c = 16; c >= 2; c >>= 1)
+        if (n % c == 0 && (size_t)(c / 2) * per <= 100 * 1024) { kch = c; break; }
+    if (hermitian && (size_t)(kch / 2) * per > budget) hermitian = false;
+    if (hermitian)
+        BLINK_CUDA_TRY(cudaFuncSetAttribute(gfft_cols_herm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)((kch / 2) * per)));
     for (int b0 = 0; b0 < batch; b0 += 65535) {
         const int nb = batch - b0 < 65535 ? batch - b0 : 65535;
-        gfft_cols_kernel<<<dim3(n / kc, nb), kGColThreads, kc * per, st>>>(grid + (size_t)b0 * n * n, pl, tw, kc, scale, scale_div,
-                                                                       img_base + b0, image + (size_t)b0 * n * n,
-                                                                       image_imag ? image_imag + (size_t)b0 * n * n : nullptr);
+        if (hermitian)
+            gfft_cols_herm_kernel<<<dim3(n / kch, nb), kGColThreads, (kch / 2) * per, st>>>(grid + (size_t)b0 * n * n, pl, tw, kch, scale,
+                                                                                          scale_div, img_base + b0,
+                                                                                          image + (size_t)b0 * n * n);
+        else
+            gfft_cols_kernel<<<dim3(n / kc, nb), kGColThreads, kc * per, st>>>(grid + (size_t)b0 * n * n, pl, tw, kc, scale, scale_div,
+                                                                           img_base + b0, image + (size_t)b0 * n * n,
+                                                                           image_imag ? image_imag + (size_t)b0 * n * n : nullptr);
         BLINK_LAUNCH_CHECK("gfft_cols_kernel");
     }
     return BLINK_OK;

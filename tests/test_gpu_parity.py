@@ -580,7 +580,7 @@ def test_fft2d_non_pow2(bk, oracle_mod, n, batch):
         assert np.max(np.abs(im[b] - ref.imag)) <= TOL * peak
 
 
-@pytest.mark.parametrize("n,weighting", [(48, 1), (240, 0), (1200, 1)])
+@pytest.mark.parametrize("n,weighting", [(48, 1), (90, 0), (240, 0), (1200, 1)])
 def test_grid_and_image_non_pow2(bk, oracle_mod, n, weighting):
     from paper_2505_15204_b200 import workloads
     w = workloads.make_random(T=1, C=2, P=2, B=1500, n_pix=n, weighting=weighting, seed=n + weighting, device="cuda", fill=1.1)
