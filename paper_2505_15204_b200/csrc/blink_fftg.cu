@@ -13,7 +13,7 @@
 
 namespace blink {
 
-constexpr int kGRowThreads = 512, kGColThreads = 1024;
+constexpr int kGRowThreads = 512, kGColThreads = 512;
 struct GPlan {
     int n, nst;
     int radix[16];
@@ -76,7 +76,7 @@ __device__ __forceinline__ void gstage(const float2 *__restrict__ src, float2 *_
         for (int r = 0; r < R; ++r) x[r] = s[r * nb];
         if (P > 1) {
 #pragma unroll
-            for (int r = 1; r < R; ++r) x[r] = cmul(x[r], __ldg(tw + r * k * step));
+            for (int r = 1; r < R; ++r) x[r] = cmul(x[r], tw[r * k * step]);
         }
         if constexpr (R == 2) dft2(x[0], x[1]);
         if constexpr (R == 3) gdft3(x[0], x[1], x[2]);
@@ -114,6 +114,9 @@ gfft_rows_kernel(float2 *__restrict__ grid, long long n_rows, const GPlan pl, co
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int n = pl.n, h = n / 2;
     float2 *a = reinterpret_cast<float2 *>(smem_raw), *b = a + (size_t)nr * n;
+    float2 *stw = b + (size_t)nr * n;                          // the twiddle table, staged once per CTA
+    for (int m = threadIdx.x; m < n; m += kGRowThreads) stw[m] = tw[m];
+    __syncthreads();
     for (long long base = (long long)blockIdx.x * nr; base < n_rows; base += (long long)gridDim.x * nr) {
         const int cnt = (int)(n_rows - base < nr ? n_rows - base : nr);
         for (int idx = threadIdx.x; idx < cnt * n; idx += kGRowThreads) {
@@ -125,7 +128,7 @@ gfft_rows_kernel(float2 *__restrict__ grid, long long n_rows, const GPlan pl, co
             a[(size_t)tr * n + j] = grid[grow * n + q];
         }
         __syncthreads();
-        const float2 *res = gfft_run(a, b, cnt, n, pl, tw);
+        const float2 *res = gfft_run(a, b, cnt, n, pl, stw);
         for (int idx = threadIdx.x; idx < cnt * n; idx += kGRowThreads) {
             const int tr = idx / n, j = idx - tr * n;
             const long long L = base + tr;
@@ -145,6 +148,8 @@ gfft_cols_kernel(const float2 *__restrict__ grid, const GPlan pl, const float2 *
     const int n = pl.n, h = n / 2;
     const int ld = n + 1;                                      // odd leading dimension: the kc columns of a row fall in different banks
     float2 *a = reinterpret_cast<float2 *>(smem_raw), *b = a + (size_t)kc * ld;
+    float2 *stw = b + (size_t)kc * ld;
+    for (int m = threadIdx.x; m < n; m += kGColThreads) stw[m] = tw[m];
     const int x0 = blockIdx.x * kc, img = blockIdx.y;
     const size_t img_off = (size_t)img * n * n;
     for (int idx = threadIdx.x; idx < n * kc; idx += kGColThreads) {
@@ -154,7 +159,7 @@ gfft_cols_kernel(const float2 *__restrict__ grid, const GPlan pl, const float2 *
         a[(size_t)c * ld + j] = grid[img_off + (size_t)r * n + x0 + c];
     }
     __syncthreads();
-    const float2 *res = gfft_run(a, b, kc, ld, pl, tw);
+    const float2 *res = gfft_run(a, b, kc, ld, pl, stw);
     float s = 1.0f;
     if (scale != nullptr) {
         const float w = scale[(img_base + img) / scale_div];
@@ -183,6 +188,8 @@ gfft_cols_herm_kernel(const float2 *__restrict__ grid, const GPlan pl, const flo
     const int n = pl.n, h = n / 2, np = kc / 2;                // np column pairs = transforms per CTA
     const int ld = n + 1;
     float2 *a = reinterpret_cast<float2 *>(smem_raw), *b = a + (size_t)np * ld;
+    float2 *stw = b + (size_t)np * ld;
+    for (int m = threadIdx.x; m < n; m += kGColThreads) stw[m] = tw[m];
     const int x0 = blockIdx.x * kc, img = blockIdx.y;
     const size_t img_off = (size_t)img * n * n;
     for (int idx = threadIdx.x; idx < h * np; idx += kGColThreads) {
@@ -193,7 +200,7 @@ gfft_cols_herm_kernel(const float2 *__restrict__ grid, const GPlan pl, const flo
     }
     for (int p = threadIdx.x; p < np; p += kGColThreads) a[(size_t)p * ld + h] = make_float2(0.f, 0.f);   // the empty row -N/2
     __syncthreads();
-    const float2 *res = gfft_run(a, b, np, ld, pl, tw);
+    const float2 *res = gfft_run(a, b, np, ld, pl, stw);
     float s = 1.0f;
     if (scale != nullptr) {
         const float w = scale[(img_base + img) / scale_div];
@@ -239,34 +246,35 @@ int gfft2d_range(float2 *grid, int n, int batch, const float *scale, int scale_d
     gfft_twiddle_kernel<<<(n + 255) / 256, 256, 0, st>>>(tw, n);
     BLINK_LAUNCH_CHECK("gfft_twiddle_kernel");
     const size_t per = 2 * (size_t)(n + 1) * sizeof(float2);    // ping + pong of one transform (padded leading dimension)
-    const size_t budget = 200 * 1024;
+    const size_t twb = (size_t)n * sizeof(float2);              // + the twiddle table staged in shared memory
+    const size_t budget = 200 * 1024 - twb;
     int nr = (int)std::min<size_t>(4, budget / per);
     int kc = 1;
     for (int c = 8; c >= 1; c >>= 1)
         if ((n / 2) % c == 0 && (size_t)c * per <= budget) { kc = c; break; }
     if (nr < 1) return BLINK_ERR_UNSUPPORTED;
-    BLINK_CUDA_TRY(cudaFuncSetAttribute(gfft_rows_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(nr * per)));
-    BLINK_CUDA_TRY(cudaFuncSetAttribute(gfft_cols_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(kc * per)));
+    BLINK_CUDA_TRY(cudaFuncSetAttribute(gfft_rows_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(nr * per + twb)));
+    BLINK_CUDA_TRY(cudaFuncSetAttribute(gfft_cols_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(kc * per + twb)));
     const int rows_per_img = hermitian ? n / 2 : n, row_off = hermitian ? n / 2 : 0;
     const long long n_rows = (long long)batch * rows_per_img;
     const long long want = (n_rows + nr - 1) / nr, cap = (long long)sm_count() * 8;
-    gfft_rows_kernel<<<(unsigned)(want < cap ? want : cap), kGRowThreads, nr * per, st>>>(grid, n_rows, pl, tw, nr, rows_per_img, row_off);
+    gfft_rows_kernel<<<(unsigned)(want < cap ? want : cap), kGRowThreads, nr * per + twb, st>>>(grid, n_rows, pl, tw, nr, rows_per_img, row_off);
     BLINK_LAUNCH_CHECK("gfft_rows_kernel");
     // Hermitian: kc columns are kc/2 transforms; keep two CTAs per SM when the arrays allow it
     int kch = 2;
     for (int c = 16; c >= 2; c >>= 1)
-        if (n % c == 0 && (size_t)(c / 2) * per <= 100 * 1024) { kch = c; break; }
+        if (n % c == 0 && (size_t)(c / 2) * per + twb <= 100 * 1024) { kch = c; break; }
     if (hermitian && (size_t)(kch / 2) * per > budget) hermitian = false;
     if (hermitian)
-        BLINK_CUDA_TRY(cudaFuncSetAttribute(gfft_cols_herm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)((kch / 2) * per)));
+        BLINK_CUDA_TRY(cudaFuncSetAttribute(gfft_cols_herm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)((kch / 2) * per + twb)));
     for (int b0 = 0; b0 < batch; b0 += 65535) {
         const int nb = batch - b0 < 65535 ? batch - b0 : 65535;
         if (hermitian)
-            gfft_cols_herm_kernel<<<dim3(n / kch, nb), kGColThreads, (kch / 2) * per, st>>>(grid + (size_t)b0 * n * n, pl, tw, kch, scale,
+            gfft_cols_herm_kernel<<<dim3(n / kch, nb), kGColThreads, (kch / 2) * per + twb, st>>>(grid + (size_t)b0 * n * n, pl, tw, kch, scale,
                                                                                           scale_div, img_base + b0,
                                                                                           image + (size_t)b0 * n * n);
         else
-            gfft_cols_kernel<<<dim3(n / kc, nb), kGColThreads, kc * per, st>>>(grid + (size_t)b0 * n * n, pl, tw, kc, scale, scale_div,
+            gfft_cols_kernel<<<dim3(n / kc, nb), kGColThreads, kc * per + twb, st>>>(grid + (size_t)b0 * n * n, pl, tw, kc, scale, scale_div,
                                                                            img_base + b0, image + (size_t)b0 * n * n,
                                                                            image_imag ? image_imag + (size_t)b0 * n * n : nullptr);
         BLINK_LAUNCH_CHECK("gfft_cols_kernel");
