@@ -74,9 +74,15 @@ __device__ __forceinline__ void gstage(const float2 *__restrict__ src, float2 *_
         float2 x[R];
 #pragma unroll
         for (int r = 0; r < R; ++r) x[r] = s[r * nb];
-        if (P > 1) {
-#pragma unroll
-            for (int r = 1; r < R; ++r) x[r] = cmul(x[r], tw[r * k * step]);
+        if (P > 1) {                                           // one table read per butterfly; w^2.. are products (<= 2 extra roundings)
+            const float2 w1 = tw[k * step];
+            x[1] = cmul(x[1], w1);
+            if constexpr (R >= 3) {
+                const float2 w2 = cmul(w1, w1);
+                x[2] = cmul(x[2], w2);
+                if constexpr (R >= 4) x[3] = cmul(x[3], cmul(w1, w2));
+                if constexpr (R >= 5) x[4] = cmul(x[4], cmul(w2, w2));
+            }
         }
         if constexpr (R == 2) dft2(x[0], x[1]);
         if constexpr (R == 3) gdft3(x[0], x[1], x[2]);
