@@ -254,7 +254,7 @@ int gfft2d_range(float2 *grid, int n, int batch, const float *scale, int scale_d
     const size_t per = 2 * (size_t)(n + 1) * sizeof(float2);    // ping + pong of one transform (padded leading dimension)
     const size_t twb = (size_t)n * sizeof(float2);              // + the twiddle table staged in shared memory
     const size_t budget = 200 * 1024 - twb;
-    int nr = (int)std::min<size_t>(4, budget / per);
+    int nr = (int)std::min<size_t>(2, budget / per);
     int kc = 1;
     for (int c = 8; c >= 1; c >>= 1)
         if ((n / 2) % c == 0 && (size_t)c * per <= budget) { kc = c; break; }
