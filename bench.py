@@ -316,7 +316,10 @@ def main():
                 "kernel": "blink_image step (all kernels of the step, CUDA events on the launch stream)",
                 "algorithmic_bytes_per_step": mb["M36"], "model": "M36 = n_img*(36 N^2 + 8 B) + 12 T B",
                 "frac_M20": mb["M20"] / (kern_ms * 1e-3) / 1e9 / peak, "frac_M4": mb["M4"] / (kern_ms * 1e-3) / 1e9 / peak,
-                "kernel_ms": kern_ms}
+                "kernel_ms": kern_ms,
+                "note": "M36 is SURVEY 8(d)'s contract model (grid written, read and rewritten by two passes); the fused kernel never "
+                        "materialises the grid, so frac exceeds 1 by construction -- frac_M4 (compulsory: visibilities in, images out) "
+                        "and traffic (ncu DRAM bytes) are the honest companions"}
     prof = os.path.join(ROOT, "profiles", "traffic.csv")      # DRAM bytes per step from the committed ncu capture
     if os.path.exists(prof):
         try:
