@@ -24,6 +24,7 @@ struct AvgArgs {
     float *wsum;                  // [T*C]
     uint32_t *cnt;                // uniform weighting: [gridDim.x][n*n] count planes, all zero between items
     float inv_navg;               // 1 / (number of images per output)
+    float *wq;                    // uniform, fast route: [T*C][B] weight of every sample, 1 / (n W count) or 0 (else NULL)
 };
 
 // One persistent CTA per (t,c) item.  Sweep 1 finds the weight sum W of the item (natural: samples placed;
@@ -66,8 +67,14 @@ avg_grid_kernel(const AvgArgs a, const __grid_constant__ ScaleBlock sc)
         for (int k = 0; k < kAvgThreads / 32; ++k) { n_in += s_in[k]; n_first += s_first[k]; }
         const float W = uniform ? (float)n_first : (float)(2 * n_in);
         if (threadIdx.x == 0) a.wsum[tc] = W;
-        // ---- sweep 2: weighted scatter into the combined grids ---------------------------------------
-        if (W > 0.f) {
+        // ---- sweep 2 ------------------------------------------------------------------------------------
+        if (a.wq) {                                                     // fast route: only the per-sample weights; the
+            const float wbase = W > 0.f ? a.inv_navg / W : 0.f;         // run-length scatter kernel does the adding
+            for (int b = threadIdx.x; b < B; b += kAvgThreads) {
+                const int cell = cell_of(uvw[3 * b], uvw[3 * b + 1], s, n, h);
+                a.wq[(size_t)tc * B + b] = cell >= 0 ? wbase / (float)__ldcg(&cnt[cell]) : 0.f;
+            }
+        } else if (W > 0.f) {                                           // weighted scatter into the combined grids
             const float wbase = a.inv_navg / W;
             for (int b = threadIdx.x; b < B; b += kAvgThreads) {
                 const int cell = cell_of(uvw[3 * b], uvw[3 * b + 1], s, n, h);
@@ -203,7 +210,8 @@ __global__ void avg_winv_kernel(const AvgArgs a, float *__restrict__ winv)
 // weighted sum of the current cell in registers and only touches the grid when the cell changes: ~20-60x fewer
 // atomics than one per sample.  Visibility reads stay coalesced (baseline is the fastest axis of vis).
 __global__ void __launch_bounds__(kAvgThreads)
-avg_scatter_runs_kernel(const AvgArgs a, const __grid_constant__ ScaleBlock sc, const float *__restrict__ winv, int t_lo,
+avg_scatter_runs_kernel(const AvgArgs a, const __grid_constant__ ScaleBlock sc, const float *__restrict__ winv,
+                        const float *__restrict__ wq, int t_lo,
                         int c_lo, int nc, int nchunk, int bblocks)
 {
     const int bx = (int)(blockIdx.x % (unsigned)bblocks);
@@ -235,7 +243,7 @@ avg_scatter_runs_kernel(const AvgArgs a, const __grid_constant__ ScaleBlock sc, 
             acc = make_float2(0.f, 0.f);
         }
         if (cur >= 0) {
-            const float w = __ldg(winv + (size_t)t * a.C + c);
+            const float w = wq ? __ldcs(wq + ((size_t)t * a.C + c) * a.B + b) : __ldg(winv + (size_t)t * a.C + c);
             const float2 x = __ldcs(a.vis + ((size_t)(t * a.C + c) * a.P + p) * a.B + b);
             acc.x = fmaf(x.x, w, acc.x);
             acc.y = fmaf(x.y, w, acc.y);
@@ -260,6 +268,7 @@ size_t avg_workspace_bytes(int T, int C, int P, int B, int n_pix, int weighting,
         size_t planes = minimum ? 1 : (size_t)avg_max_planes();
         if (!minimum) planes = std::max<size_t>(1, std::min<size_t>(planes, ((size_t)2 << 30) / plane));
         b += planes * plane;
+        if (!minimum) b += align_up((size_t)T * C * B * sizeof(float), 256);   // per-sample weights: the run-length scatter route
     }
     return b;
 }
@@ -306,7 +315,18 @@ extern "C" int blink_image_avg(const blink_c64 *vis, const float *uvw_m, const d
     float2 *grid = static_cast<float2 *>(workspace);
     uint32_t *cnt = uni ? reinterpret_cast<uint32_t *>(static_cast<unsigned char *>(workspace) + gbytes) : nullptr;
     int ctas = 8 * (sm_count() > 0 ? sm_count() : 148);
-    if (uni) ctas = (int)std::min<size_t>((size_t)avg_max_planes(), (workspace_bytes - gbytes) / plane);
+    // uniform, fast route: per-sample weights [T*C][B] behind the count planes, when the workspace has room for them
+    float *wq = nullptr;
+    const size_t wq_bytes = align_up((size_t)T * C * B * sizeof(float), 256);
+    if (uni) {
+        size_t avail = workspace_bytes - gbytes;
+        if (avail >= plane + wq_bytes) {
+            ctas = (int)std::min<size_t>((size_t)avg_max_planes(), (avail - wq_bytes) / plane);
+            wq = reinterpret_cast<float *>(static_cast<unsigned char *>(workspace) + gbytes + (size_t)ctas * plane);
+        } else {
+            ctas = (int)std::min<size_t>((size_t)avg_max_planes(), avail / plane);
+        }
+    }
     BLINK_CUDA_TRY(cudaMemsetAsync(grid, 0, gbytes, st));
     if (uni) BLINK_CUDA_TRY(cudaMemsetAsync(cnt, 0, (size_t)ctas * plane, st));
     const int n_out = (avg_time ? 1 : T) * P;
@@ -325,10 +345,19 @@ extern "C" int blink_image_avg(const blink_c64 *vis, const float *uvw_m, const d
         a.tc0 = tc; a.ntc = end - tc; a.c_base = c_base;
         a.grid = grid; a.wsum = wsum; a.cnt = cnt;
         a.inv_navg = (float)(1.0 / (avg_time ? (double)T * C : (double)C));
+        a.wq = wq;
         if (uni) {
             const int gridx = a.ntc < ctas ? a.ntc : ctas;
             avg_grid_kernel<<<gridx, kAvgThreads, 0, st>>>(a, sc);
             BLINK_LAUNCH_CHECK("avg_grid_kernel");
+            if (wq) {
+                const int nt = (C <= 1024) ? T : 1, nc = (C <= 1024) ? C : a.ntc;
+                const int nchunk = (nc + kAvgChunk - 1) / kAvgChunk, bblocks = (B + kAvgThreads - 1) / kAvgThreads;
+                const long long blocks = (long long)bblocks * nchunk * P * nt;
+                if (blocks > 0x7fffffffLL) return BLINK_ERR_UNSUPPORTED;
+                avg_scatter_runs_kernel<<<(unsigned)blocks, kAvgThreads, 0, st>>>(a, sc, nullptr, wq, t, c, nc, nchunk, bblocks);
+                BLINK_LAUNCH_CHECK("avg_scatter_runs_kernel");
+            }
         } else {
             // this segment: all timesteps x all channels (C <= 1024) or one timestep x one block of channels
             const int nt = (C <= 1024) ? T : 1, nc = (C <= 1024) ? C : a.ntc;
@@ -347,7 +376,7 @@ extern "C" int blink_image_avg(const blink_c64 *vis, const float *uvw_m, const d
             }
             const long long blocks = (long long)bblocks * nchunk * P * nt;
             if (blocks > 0x7fffffffLL) return BLINK_ERR_UNSUPPORTED;
-            avg_scatter_runs_kernel<<<(unsigned)blocks, kAvgThreads, 0, st>>>(a, sc, winv, t, c, nc, nchunk, bblocks);
+            avg_scatter_runs_kernel<<<(unsigned)blocks, kAvgThreads, 0, st>>>(a, sc, winv, nullptr, t, c, nc, nchunk, bblocks);
             BLINK_LAUNCH_CHECK("avg_scatter_runs_kernel");
         }
         tc = end;
