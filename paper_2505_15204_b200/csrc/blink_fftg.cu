@@ -61,10 +61,42 @@ __device__ __forceinline__ int fdiv_small(int i, int d, float inv_d) { (void)d; 
 // leading dimension ld: src[tr][i + r*(n/R)] -> dst[tr][(i - k)*R + k + r*P], k = i mod P, inputs r >= 1
 // twiddled by W_n^(r k n/(P R)).  Reads are unit-stride in i; writes are runs of P consecutive elements, which is
 // why the plan puts the odd radices first (P grows past a warp before the radix-4 stages: no bank conflicts there).
-template <int R>
-__device__ __forceinline__ void gstage(const float2 *__restrict__ src, float2 *__restrict__ dst, int nt, int n, int ld, int P,
+// NN / PP: n and P when they are known at compile time (the paper's side 1200 has its own instantiation: every
+// division and remainder below becomes a multiply-shift and the stage loop is specialised), else 0 = run-time values.
+template <int R, int NN = 0, int PP = 0>
+__device__ __forceinline__ void gstage(const float2 *__restrict__ src, float2 *__restrict__ dst, int nt, int n_rt, int ld, int p_rt,
                                        const float2 *__restrict__ tw)
 {
+    const int n = NN ? NN : n_rt, P = PP ? PP : p_rt;
+    if constexpr (NN != 0 && PP != 0) {
+        constexpr int nb = NN / R, step = NN / (PP * R);
+        for (int idx = threadIdx.x; idx < nt * nb; idx += blockDim.x) {
+            const int tr = idx / nb, i = idx - tr * nb;
+            const int k = i % PP;
+            const float2 *s = src + (size_t)tr * ld + i;
+            float2 x[R];
+#pragma unroll
+            for (int r = 0; r < R; ++r) x[r] = s[r * nb];
+            if constexpr (PP > 1) {
+                const float2 w1 = tw[k * step];
+                x[1] = cmul(x[1], w1);
+                if constexpr (R >= 3) {
+                    const float2 w2 = cmul(w1, w1);
+                    x[2] = cmul(x[2], w2);
+                    if constexpr (R >= 4) x[3] = cmul(x[3], cmul(w1, w2));
+                    if constexpr (R >= 5) x[4] = cmul(x[4], cmul(w2, w2));
+                }
+            }
+            if constexpr (R == 2) dft2(x[0], x[1]);
+            if constexpr (R == 3) gdft3(x[0], x[1], x[2]);
+            if constexpr (R == 4) dft4(x[0], x[1], x[2], x[3]);
+            if constexpr (R == 5) gdft5(x[0], x[1], x[2], x[3], x[4]);
+            float2 *d = dst + (size_t)tr * ld + (i - k) * R + k;
+#pragma unroll
+            for (int r = 0; r < R; ++r) d[r * PP] = x[r];
+        }
+        return;
+    }
     const int nb = n / R, step = n / (P * R);
     const float inv_nb = 1.0f / (float)nb, inv_p = 1.0f / (float)P;
     for (int idx = threadIdx.x; idx < nt * nb; idx += blockDim.x) {
@@ -95,8 +127,17 @@ __device__ __forceinline__ void gstage(const float2 *__restrict__ src, float2 *_
 }
 
 // all stages; returns the array that holds the result (natural order)
+template <int NN>
 __device__ __forceinline__ float2 *gfft_run(float2 *a, float2 *b, int nt, int ld, const GPlan &pl, const float2 *tw)
 {
+    if constexpr (NN == 1200) {                                // 5 * 5 * 3 * 4 * 4, the plan gfft2d_range builds for 1200
+        gstage<5, 1200, 1>(a, b, nt, 1200, ld, 1, tw);   __syncthreads();
+        gstage<5, 1200, 5>(b, a, nt, 1200, ld, 5, tw);   __syncthreads();
+        gstage<3, 1200, 25>(a, b, nt, 1200, ld, 25, tw); __syncthreads();
+        gstage<4, 1200, 75>(b, a, nt, 1200, ld, 75, tw); __syncthreads();
+        gstage<4, 1200, 300>(a, b, nt, 1200, ld, 300, tw); __syncthreads();
+        return b;
+    }
     int P = 1;
     for (int s = 0; s < pl.nst; ++s) {
         const int R = pl.radix[s];
@@ -112,13 +153,14 @@ __device__ __forceinline__ float2 *gfft_run(float2 *a, float2 *b, int nt, int ld
 }
 
 // ------------------------------------------------------------------------------------------ rows
+template <int NN>
 __global__ void __launch_bounds__(kGRowThreads)
 gfft_rows_kernel(float2 *__restrict__ grid, long long n_rows, const GPlan pl, const float2 *__restrict__ tw, int nr, int rows_per_img,
                  int row_off)
 {
     // logical row L -> image L / rows_per_img, row row_off + L % rows_per_img (Hermitian grids: only the rows v >= 0)
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int n = pl.n, h = n / 2;
+    const int n = NN ? NN : pl.n, h = n / 2;
     float2 *a = reinterpret_cast<float2 *>(smem_raw), *b = a + (size_t)nr * n;
     float2 *stw = b + (size_t)nr * n;                          // the twiddle table, staged once per CTA
     for (int m = threadIdx.x; m < n; m += kGRowThreads) stw[m] = tw[m];
@@ -134,7 +176,7 @@ gfft_rows_kernel(float2 *__restrict__ grid, long long n_rows, const GPlan pl, co
             a[(size_t)tr * n + j] = grid[grow * n + q];
         }
         __syncthreads();
-        const float2 *res = gfft_run(a, b, cnt, n, pl, stw);
+        const float2 *res = gfft_run<NN>(a, b, cnt, n, pl, stw);
         for (int idx = threadIdx.x; idx < cnt * n; idx += kGRowThreads) {
             const int tr = idx / n, j = idx - tr * n;
             const long long L = base + tr;
@@ -146,12 +188,13 @@ gfft_rows_kernel(float2 *__restrict__ grid, long long n_rows, const GPlan pl, co
 }
 
 // ------------------------------------------------------------------------------------------ columns + epilogue
+template <int NN>
 __global__ void __launch_bounds__(kGColThreads)
 gfft_cols_kernel(const float2 *__restrict__ grid, const GPlan pl, const float2 *__restrict__ tw, int kc, const float *__restrict__ scale,
                  int scale_div, int img_base, float *__restrict__ image, float *__restrict__ image_imag)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int n = pl.n, h = n / 2;
+    const int n = NN ? NN : pl.n, h = n / 2;
     const int ld = n + 1;                                      // odd leading dimension: the kc columns of a row fall in different banks
     float2 *a = reinterpret_cast<float2 *>(smem_raw), *b = a + (size_t)kc * ld;
     float2 *stw = b + (size_t)kc * ld;
@@ -165,7 +208,7 @@ gfft_cols_kernel(const float2 *__restrict__ grid, const GPlan pl, const float2 *
         a[(size_t)c * ld + j] = grid[img_off + (size_t)r * n + x0 + c];
     }
     __syncthreads();
-    const float2 *res = gfft_run(a, b, kc, ld, pl, stw);
+    const float2 *res = gfft_run<NN>(a, b, kc, ld, pl, stw);
     float s = 1.0f;
     if (scale != nullptr) {
         const float w = scale[(img_base + img) / scale_div];
@@ -186,12 +229,13 @@ gfft_cols_kernel(const float2 *__restrict__ grid, const GPlan pl, const float2 *
 // empty): after the row pass R[-v][x] = conj R[v][x], so only the rows v >= 0 were transformed, and two columns
 // x1, x2 become ONE complex transform Z[v] = R[v][x1] + i R[v][x2], Z[-v] = conj R[v][x1] + i conj R[v][x2] whose
 // real part is image column x1 and imaginary part image column x2.  Half the reads, half the transforms.
+template <int NN>
 __global__ void __launch_bounds__(kGColThreads)
 gfft_cols_herm_kernel(const float2 *__restrict__ grid, const GPlan pl, const float2 *__restrict__ tw, int kc, const float *__restrict__ scale,
                       int scale_div, int img_base, float *__restrict__ image)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int n = pl.n, h = n / 2, np = kc / 2;                // np column pairs = transforms per CTA
+    const int n = NN ? NN : pl.n, h = n / 2, np = kc / 2;                // np column pairs = transforms per CTA
     const int ld = n + 1;
     float2 *a = reinterpret_cast<float2 *>(smem_raw), *b = a + (size_t)np * ld;
     float2 *stw = b + (size_t)np * ld;
@@ -206,7 +250,7 @@ gfft_cols_herm_kernel(const float2 *__restrict__ grid, const GPlan pl, const flo
     }
     for (int p = threadIdx.x; p < np; p += kGColThreads) a[(size_t)p * ld + h] = make_float2(0.f, 0.f);   // the empty row -N/2
     __syncthreads();
-    const float2 *res = gfft_run(a, b, np, ld, pl, stw);
+    const float2 *res = gfft_run<NN>(a, b, np, ld, pl, stw);
     float s = 1.0f;
     if (scale != nullptr) {
         const float w = scale[(img_base + img) / scale_div];
@@ -259,12 +303,16 @@ int gfft2d_range(float2 *grid, int n, int batch, const float *scale, int scale_d
     for (int c = 8; c >= 1; c >>= 1)
         if ((n / 2) % c == 0 && (size_t)c * per <= budget) { kc = c; break; }
     if (nr < 1) return BLINK_ERR_UNSUPPORTED;
-    BLINK_CUDA_TRY(cudaFuncSetAttribute(gfft_rows_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(nr * per + twb)));
-    BLINK_CUDA_TRY(cudaFuncSetAttribute(gfft_cols_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(kc * per + twb)));
+    // the paper's side has compile-time instantiations (same algorithm, constant index arithmetic)
+    auto rows_k = n == 1200 ? gfft_rows_kernel<1200> : gfft_rows_kernel<0>;
+    auto cols_k = n == 1200 ? gfft_cols_kernel<1200> : gfft_cols_kernel<0>;
+    auto herm_k = n == 1200 ? gfft_cols_herm_kernel<1200> : gfft_cols_herm_kernel<0>;
+    BLINK_CUDA_TRY(cudaFuncSetAttribute(rows_k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(nr * per + twb)));
+    BLINK_CUDA_TRY(cudaFuncSetAttribute(cols_k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(kc * per + twb)));
     const int rows_per_img = hermitian ? n / 2 : n, row_off = hermitian ? n / 2 : 0;
     const long long n_rows = (long long)batch * rows_per_img;
     const long long want = (n_rows + nr - 1) / nr, cap = (long long)sm_count() * 8;
-    gfft_rows_kernel<<<(unsigned)(want < cap ? want : cap), kGRowThreads, nr * per + twb, st>>>(grid, n_rows, pl, tw, nr, rows_per_img, row_off);
+    rows_k<<<(unsigned)(want < cap ? want : cap), kGRowThreads, nr * per + twb, st>>>(grid, n_rows, pl, tw, nr, rows_per_img, row_off);
     BLINK_LAUNCH_CHECK("gfft_rows_kernel");
     // Hermitian: kc columns are kc/2 transforms; keep two CTAs per SM when the arrays allow it
     int kch = 2;
@@ -272,15 +320,15 @@ int gfft2d_range(float2 *grid, int n, int batch, const float *scale, int scale_d
         if (n % c == 0 && (size_t)(c / 2) * per + twb <= 100 * 1024) { kch = c; break; }
     if (hermitian && (size_t)(kch / 2) * per > budget) hermitian = false;
     if (hermitian)
-        BLINK_CUDA_TRY(cudaFuncSetAttribute(gfft_cols_herm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)((kch / 2) * per + twb)));
+        BLINK_CUDA_TRY(cudaFuncSetAttribute(herm_k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)((kch / 2) * per + twb)));
     for (int b0 = 0; b0 < batch; b0 += 65535) {
         const int nb = batch - b0 < 65535 ? batch - b0 : 65535;
         if (hermitian)
-            gfft_cols_herm_kernel<<<dim3(n / kch, nb), kGColThreads, (kch / 2) * per + twb, st>>>(grid + (size_t)b0 * n * n, pl, tw, kch, scale,
+            herm_k<<<dim3(n / kch, nb), kGColThreads, (kch / 2) * per + twb, st>>>(grid + (size_t)b0 * n * n, pl, tw, kch, scale,
                                                                                           scale_div, img_base + b0,
                                                                                           image + (size_t)b0 * n * n);
         else
-            gfft_cols_kernel<<<dim3(n / kc, nb), kGColThreads, kc * per + twb, st>>>(grid + (size_t)b0 * n * n, pl, tw, kc, scale, scale_div,
+            cols_k<<<dim3(n / kc, nb), kGColThreads, kc * per + twb, st>>>(grid + (size_t)b0 * n * n, pl, tw, kc, scale, scale_div,
                                                                            img_base + b0, image + (size_t)b0 * n * n,
                                                                            image_imag ? image_imag + (size_t)b0 * n * n : nullptr);
         BLINK_LAUNCH_CHECK("gfft_cols_kernel");
