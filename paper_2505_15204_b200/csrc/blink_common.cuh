@@ -99,7 +99,7 @@ __device__ __forceinline__ int mirror_of(int cell, int n)
 // grid / counts by (tc - out_tc0) so that a chunk can land at the start of a workspace buffer.
 int grid_range(const float2 *vis, const float *uvw_m, const double *freqs_hz, double pixscale_rad, int T, int C,
                int P, int B, int n_pix, int weighting, int tc0, int ntc, int out_tc0, float2 *grid, float *wsum,
-               int32_t *cell_idx, uint32_t *counts, cudaStream_t st);
+               int32_t *cell_idx, uint32_t *counts, cudaStream_t st, bool half_only = false);
 bool grid_needs_global_counts(int B, int n_pix, int weighting);
 // hermitian: the grids come from the library's own gridders (G[-v][-u] = conj G[v][u], row / column -N/2 empty)
 // tw_generic: device array of n_pix complex64 (gfft_workspace_bytes) for sides that are not a power of two, else unused

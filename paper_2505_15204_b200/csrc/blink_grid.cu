@@ -18,6 +18,7 @@ struct GridArgs {
     int tc0, c_base, out_tc0;                     // first flattened (t,c) of this launch; channel of s[0]; tc of grid[0]
     float2 *grid; float *wsum; int32_t *cell_idx; uint32_t *counts;     // wsum/cell_idx by absolute tc, grid/counts by tc - out_tc0
     int chunk_b, n_chunks, tile_cells, n_bands;
+    int half_only;                                // the consumer only reads rows v >= 0 (Hermitian transform): skip the bands below
 };
 
 __global__ void __launch_bounds__(kGridThreads)
@@ -95,6 +96,7 @@ grid_tiles_kernel(const GridArgs a, const __grid_constant__ ScaleBlock sc)
         for (int band = 0; band < a.n_bands; ++band) {
             const uint32_t k0 = off[band], k1 = off[band + 1];
             if (multi && ch > 0 && k0 == k1) continue;         // nothing to spill for this band (uniform branch)
+            if (a.half_only && (size_t)(band + 1) * a.tile_cells <= (size_t)h * n) continue;   // rows v < 0 only: never read
             for (int p = 0; p < a.P; ++p) {
                 for (int i = threadIdx.x; i < a.tile_cells; i += kGridThreads) {
                     tile[i] = make_float2(0.f, 0.f);
@@ -123,7 +125,14 @@ grid_tiles_kernel(const GridArgs a, const __grid_constant__ ScaleBlock sc)
                             if (c0) { v0.x /= (float)c0; v0.y /= (float)c0; }
                             if (c1) { v1.x /= (float)c1; v1.y /= (float)c1; }
                         }
-                        if (p == 0) my_occ += (c0 != 0) + (c1 != 0);
+                        if (p == 0) {
+                            if (!a.half_only) {
+                                my_occ += (c0 != 0) + (c1 != 0);
+                            } else {                            // occupied cells of the full plane from the rows v >= 0:
+                                const size_t gi = (size_t)band * a.tile_cells + i;      // row v = 0 mirrors onto itself, rows v > 0 count twice
+                                if (gi >= (size_t)h * n) my_occ += ((c0 != 0) + (c1 != 0)) * (gi < (size_t)(h + 1) * n ? 1 : 2);
+                            }
+                        }
                         __stcs(reinterpret_cast<float4 *>(gdst + i), make_float4(v0.x, v0.y, v1.x, v1.y));
                     }
                 } else if (ch == 0) {
@@ -210,7 +219,7 @@ bool grid_needs_global_counts(int B, int n_pix, int weighting)
 
 int grid_range(const float2 *vis, const float *uvw_m, const double *freqs_hz, double pixscale_rad, int T, int C, int P,
                int B, int n_pix, int weighting, int tc0, int ntc, int out_tc0, float2 *grid, float *wsum,
-               int32_t *cell_idx, uint32_t *counts, cudaStream_t st)
+               int32_t *cell_idx, uint32_t *counts, cudaStream_t st, bool half_only)
 {
     (void)T;
     if (ntc <= 0) return BLINK_OK;
@@ -227,6 +236,7 @@ int grid_range(const float2 *vis, const float *uvw_m, const double *freqs_hz, do
     a.chunk_b = chunk;
     a.n_chunks = B > 0 ? (B + chunk - 1) / chunk : 1;
     if (a.n_chunks > 1 && weighting == BLINK_W_UNIFORM && counts == nullptr) return BLINK_ERR_WORKSPACE;
+    a.half_only = (half_only && a.n_chunks == 1 && counts == nullptr) ? 1 : 0;
     const size_t smem = grid_smem_bytes(a.tile_cells, a.n_bands, a.chunk_b);
     BLINK_CUDA_TRY(cudaFuncSetAttribute(grid_tiles_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     // sub-ranges that stay inside one timestep's block of <= 1024 channels (scales travel as a kernel parameter)

@@ -63,7 +63,7 @@ static int image_device(const float2 *vis, const float *uvw_m, const double *fre
         // counts: caller's array (absolute index) or the workspace copy (chunk-relative)
         uint32_t *cptr = counts ? counts + (size_t)s * n2 : wcounts;
         int rc = grid_range(vis, uvw_m, freqs_hz, pixscale_rad, T, C, P, B, n_pix, weighting, s, m, s, wgrid, wsum,
-                            cell_idx, cptr, st);
+                            cell_idx, cptr, st, /*half_only=*/!is_pow2(n_pix));
         if (rc != BLINK_OK) return rc;
         rc = fft2d_range(wgrid, n_pix, m * P, wsum, P, s * P, image + (size_t)s * P * n2, nullptr, st, tw_generic, true);
         if (rc != BLINK_OK) return rc;
