@@ -190,3 +190,103 @@ def apply_gains(vis, gains, ant_pairs):
     out = np.empty_like(v)
     lib().oracle_apply_gains(_p(v), _p(g), _p(ap), T, C, P, B, A, _p(out))
     return out
+
+
+# ---- convolutional gridding (reading R16) ----------------------------------
+def _conv_protos():
+    L = lib()
+    if getattr(L, "_conv_ready", False):
+        return L
+    c_f, c_d, c_i, vp = ctypes.c_float, ctypes.c_double, ctypes.c_int, ctypes.c_void_p
+    L.oracle_bessel_i0.restype = c_d
+    L.oracle_bessel_i0.argtypes = [c_d]
+    L.oracle_kb.restype = c_d
+    L.oracle_kb.argtypes = [c_d, c_i, c_d]
+    L.oracle_conv_taps.restype = None
+    L.oracle_conv_taps.argtypes = [c_d, c_i, c_d, vp]
+    L.oracle_conv_taper.restype = c_d
+    L.oracle_conv_taper.argtypes = [c_d, c_i, c_d]
+    L.oracle_cell_conv.restype = ctypes.c_int32
+    L.oracle_cell_conv.argtypes = [c_f, c_f, c_f, c_i, c_i, vp, vp]
+    L.oracle_grid_conv_one.restype = c_d
+    L.oracle_grid_conv_one.argtypes = [vp, vp, c_d, c_i, c_i, c_d, c_i, c_d, vp, vp]
+    L.oracle_image_conv_one.restype = c_d
+    L.oracle_image_conv_one.argtypes = [vp, vp, c_d, c_i, c_i, c_d, c_i, c_d, vp, vp, vp, vp]
+    L.oracle_image_conv_batch.restype = c_i
+    L.oracle_image_conv_batch.argtypes = [vp, vp, vp, c_i, c_i, c_i, c_i, c_i, c_d, c_i, c_d, vp, c_i, vp, vp, c_i]
+    L._conv_ready = True
+    return L
+
+
+def bessel_i0(x: float) -> float:
+    return float(_conv_protos().oracle_bessel_i0(float(x)))
+
+
+def kb(d: float, support: int, beta: float) -> float:
+    return float(_conv_protos().oracle_kb(float(d), int(support), float(beta)))
+
+
+def conv_taps(f: float, support: int, beta: float) -> np.ndarray:
+    w = np.empty(int(support), dtype=np.float64)
+    _conv_protos().oracle_conv_taps(float(f), int(support), float(beta), _p(w))
+    return w
+
+
+def conv_taper(n_pix: int, support: int, beta: float) -> np.ndarray:
+    """c((x - h)/N) for x = 0..N-1."""
+    L = _conv_protos()
+    h = n_pix // 2
+    return np.array([L.oracle_conv_taper((x - h) / n_pix, int(support), float(beta)) for x in range(n_pix)])
+
+
+def cell_conv(u_m, v_m, s, n_pix: int, support: int):
+    """-> (cell or -1, fx, fy)"""
+    fx, fy = ctypes.c_double(0.0), ctypes.c_double(0.0)
+    c = _conv_protos().oracle_cell_conv(float(np.float32(u_m)), float(np.float32(v_m)), float(np.float32(s)),
+                                        int(n_pix), int(support), ctypes.byref(fx), ctypes.byref(fy))
+    return int(c), fx.value, fy.value
+
+
+def grid_conv_one(vis_b, uvw_t, f_hz: float, n_pix: int, pixscale_rad: float, support: int, beta: float):
+    """-> (grid complex128 [N][N] centred, W, cell_idx int32 [B])"""
+    v = _c64(vis_b)
+    uvw = np.ascontiguousarray(uvw_t, dtype=np.float32)
+    B = v.shape[0]
+    grid = np.empty((n_pix, n_pix), dtype=np.complex128)
+    ci = np.empty(B, dtype=np.int32)
+    W = _conv_protos().oracle_grid_conv_one(_p(v), _p(uvw), float(f_hz), B, int(n_pix), float(pixscale_rad),
+                                            int(support), float(beta), _p(grid), _p(ci))
+    return grid, W, ci
+
+
+def image_conv_one(vis_b, uvw_t, f_hz: float, n_pix: int, pixscale_rad: float, support: int, beta: float,
+                   want_imag: bool = False):
+    v = _c64(vis_b)
+    uvw = np.ascontiguousarray(uvw_t, dtype=np.float32)
+    B = v.shape[0]
+    img = np.empty((n_pix, n_pix), dtype=np.float64)
+    im = np.empty((n_pix, n_pix), dtype=np.float64) if want_imag else None
+    grid = np.empty((n_pix, n_pix), dtype=np.complex128)
+    ci = np.empty(B, dtype=np.int32)
+    W = _conv_protos().oracle_image_conv_one(_p(v), _p(uvw), float(f_hz), B, int(n_pix), float(pixscale_rad),
+                                             int(support), float(beta), _p(img), _p(im), _p(grid), _p(ci))
+    return dict(image=img, imag=im, grid=grid, W=W, cell_idx=ci)
+
+
+def image_conv_batch(vis, uvw_m, freqs_hz, n_pix: int, pixscale_rad: float, support: int, beta: float,
+                     img_ids=None, nthreads: int = 1):
+    v = _c64(vis)
+    uvw = np.ascontiguousarray(uvw_m, dtype=np.float32)
+    fr = np.ascontiguousarray(freqs_hz, dtype=np.float64)
+    T, C, P, B = v.shape
+    if img_ids is None:
+        img_ids = np.arange(T * C * P)
+    ids = np.ascontiguousarray(img_ids, dtype=np.int64)
+    images = np.empty((len(ids), n_pix, n_pix), dtype=np.float64)
+    wsum = np.empty(len(ids), dtype=np.float64)
+    rc = _conv_protos().oracle_image_conv_batch(_p(v), _p(uvw), _p(fr), T, C, P, B, int(n_pix), float(pixscale_rad),
+                                                int(support), float(beta), _p(ids), len(ids), _p(images), _p(wsum),
+                                                int(nthreads))
+    if rc != 0:
+        raise RuntimeError("oracle_image_conv_batch failed")
+    return images, wsum

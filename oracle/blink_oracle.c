@@ -434,3 +434,193 @@ void oracle_apply_gains(const float *vis, const float *gains, const int32_t *ant
                 }
             }
 }
+
+/* ------------------------------------------------------------------------------------------
+ * Convolutional (anti-aliasing) gridding -- SURVEY 8(f) rank 2.  PAPER.md L192: "Visibilities are not
+ * convolved with any kernel at this stage, a feature to be introduced in the near future to alleviate the
+ * effects of source aliasing"; L351 "The implementation of a gridding kernel to minimise aliasing is in
+ * progress".  The paper defines no kernel, so DESIGN.md reading R16 fixes one (the separable Kaiser-Bessel
+ * window that WSClean, the paper's comparison imager, uses by default):
+ *
+ *   k(d)   = I0(beta sqrt(1 - (2 d / S)^2)) / I0(beta)   for |d| <= S/2, else 0      (S odd: 1, 3, 5, 7)
+ *   x      = u_m * s_c (ONE fp32 multiply, as in a1), iu0 = rint(x), fx = x - iu0 in [-1/2, 1/2]  (exact)
+ *   taps   j = -r..r (r = (S-1)/2) at column iu0 + j, distance d = j - fx from the sample,
+ *          weight wx_j = k(j - fx) / sum_i k(i - fx)       (normalised: the S taps of an axis sum to 1)
+ *   the same along v; cell (iv0 + i, iu0 + j) += wy_i wx_j V, mirror cell (-(iv0+i), -(iu0+j)) += wy_i wx_j conj(V)
+ *          (the Hermitian sample at (-x,-y) has offsets -fx, -fy and k is even: exactly the mirrored taps)
+ *   range  a sample is dropped (with its conjugate) when |iu0| or |iv0| > h - 1 - r, so that the whole
+ *          support stays inside |iu|, |iv| <= h - 1 (reading R4 extended)
+ *   W      natural weighting only: W = 2 B_in (every sample carries total weight 1)
+ *   image  I[y][x] = (1/W) Re IDFT(G)[y][x] / (c((y-h)/N) c((x-h)/N)),   the grid correction
+ *          c(xi) = int_{-S/2}^{S/2} k(d) cos(2 pi d xi) dd / int_{-S/2}^{S/2} k(d) dd      (c(0) = 1)
+ * S = 1 is nearest-cell gridding (the only tap has normalised weight 1): the S = 1 GRID equals
+ * oracle_grid_one's; the library itself offers S = 3, 5, 7.
+ * Pins (tests/test_oracle_pins.py): I0 series vs scipy.special.i0 / numpy.i0; taps sum to 1, are symmetric
+ * at fx = 0 and mirror under fx -> -fx; S = 1 grid == oracle_grid_one; sum(G) = sum 2 Re V; Hermitian;
+ * independent numpy re-gridding (np.add.at over an outer product); quadrature taper vs the closed form
+ * sinh(sqrt(beta^2 - (pi S xi)^2)) / sqrt(...) normalised; unit source -> exactly 1.0 at the centre;
+ * single off-grid baseline: the corrected image is closer to the exact (ungridded) cosine than nearest-cell
+ * gridding is, inside the central half of the field.
+ * ---------------------------------------------------------------------------------------- */
+static double bessel_i0_series(double x)
+{
+    /* I0(x) = sum_k ((x/2)^2)^k / (k!)^2 ; terms decay once k > x/2 ; |x| <= ~60 here */
+    const double q = 0.25 * x * x;
+    double term = 1.0, sum = 1.0;
+    for (int k = 1; k < 500; ++k) {
+        term *= q / ((double)k * (double)k);
+        sum += term;
+        if (term < 1e-17 * sum) break;
+    }
+    return sum;
+}
+double oracle_bessel_i0(double x) { return bessel_i0_series(x); }
+
+double oracle_kb(double d, int S, double beta)
+{
+    const double a = 2.0 * d / (double)S;
+    const double z = 1.0 - a * a;
+    if (z < 0.0) return (z > -1e-14) ? 1.0 / bessel_i0_series(beta) : 0.0;   /* |d| = S/2 up to rounding */
+    return bessel_i0_series(beta * sqrt(z)) / bessel_i0_series(beta);
+}
+
+/* w[0..S) : normalised tap weights of one axis for fractional offset f = x - rint(x) */
+void oracle_conv_taps(double f, int S, double beta, double *w)
+{
+    const int r = (S - 1) / 2;
+    double sum = 0.0;
+    for (int j = -r; j <= r; ++j) { w[j + r] = oracle_kb((double)j - f, S, beta); sum += w[j + r]; }
+    for (int j = 0; j < S; ++j) w[j] /= sum;
+}
+
+/* grid correction c(xi), xi = (pixel - h)/N in [-1/2, 1/2): composite Simpson over the support */
+double oracle_conv_taper(double xi, int S, double beta)
+{
+    const int M = 8192;                             /* even number of intervals */
+    const double lo = -0.5 * (double)S, hstep = (double)S / (double)M;
+    double num = 0.0, den = 0.0;
+    for (int m = 0; m <= M; ++m) {
+        const double d = lo + hstep * (double)m;
+        const double wq = (m == 0 || m == M) ? 1.0 : ((m & 1) ? 4.0 : 2.0);
+        const double kd = oracle_kb(d, S, beta);
+        num += wq * kd * cos(2.0 * ORACLE_PI * d * xi);
+        den += wq * kd;
+    }
+    return num / den;
+}
+
+/* nearest cell of the convolutional gridder: oracle_cell with the tighter range h-1-r; -1 when dropped.
+ * fx, fy (may be NULL) receive the exact offsets x - iu0, y - iv0. */
+int32_t oracle_cell_conv(float u_m, float v_m, float s, int n_pix, int S, double *fx, double *fy)
+{
+    const int h = n_pix / 2, r = (S - 1) / 2;
+    volatile float x = u_m * s;
+    volatile float y = v_m * s;
+    float xr = nearbyintf(x);
+    float yr = nearbyintf(y);
+    const float lim = (float)(h - 1 - r);
+    if (!(fabsf(xr) <= lim && fabsf(yr) <= lim)) return -1;
+    if (fx) *fx = (double)x - (double)xr;
+    if (fy) *fy = (double)y - (double)yr;
+    return (int32_t)(((int)yr + h) * n_pix + ((int)xr + h));
+}
+
+double oracle_grid_conv_one(const float *vis, const float *uvw_t, double f_hz, int B, int n_pix,
+                            double pixscale_rad, int S, double beta, double *grid, int32_t *cell_idx)
+{
+    const size_t n2 = (size_t)n_pix * n_pix;
+    const int h = n_pix / 2, r = (S - 1) / 2;
+    fesetround(FE_TONEAREST);
+    memset(grid, 0, n2 * 2 * sizeof(double));
+    float s = oracle_scale(f_hz, n_pix, pixscale_rad);
+    double W = 0.0, wx[16], wy[16];
+    for (int b = 0; b < B; ++b) {
+        double fx, fy;
+        int32_t cell = oracle_cell_conv(uvw_t[3 * b], uvw_t[3 * b + 1], s, n_pix, S, &fx, &fy);
+        if (cell_idx) cell_idx[b] = cell;
+        if (cell < 0) continue;
+        const int iv0 = cell / n_pix - h, iu0 = cell % n_pix - h;
+        oracle_conv_taps(fx, S, beta, wx);
+        oracle_conv_taps(fy, S, beta, wy);
+        const double re = (double)vis[2 * b], im = (double)vis[2 * b + 1];
+        for (int i = -r; i <= r; ++i)
+            for (int j = -r; j <= r; ++j) {
+                const double w = wy[i + r] * wx[j + r];
+                const size_t k = (size_t)(iv0 + i + h) * n_pix + (size_t)(iu0 + j + h);
+                const size_t km = (size_t)(h - (iv0 + i)) * n_pix + (size_t)(h - (iu0 + j));
+                grid[2 * k] += w * re;   grid[2 * k + 1] += w * im;
+                grid[2 * km] += w * re;  grid[2 * km + 1] -= w * im;
+            }
+        W += 2.0;
+    }
+    return W;
+}
+
+double oracle_image_conv_one(const float *vis, const float *uvw_t, double f_hz, int B, int n_pix,
+                             double pixscale_rad, int S, double beta, double *image, double *image_im,
+                             double *grid_out, int32_t *cell_idx)
+{
+    const size_t n2 = (size_t)n_pix * n_pix;
+    const int h = n_pix / 2;
+    double *grid = grid_out ? grid_out : (double *)malloc(sizeof(double) * 2 * n2);
+    double *cimg = (double *)malloc(sizeof(double) * 2 * n2);
+    double *c = (double *)malloc(sizeof(double) * n_pix);
+    double W = oracle_grid_conv_one(vis, uvw_t, f_hz, B, n_pix, pixscale_rad, S, beta, grid, cell_idx);
+    oracle_ifft2_radix2(grid, n_pix, cimg);
+    for (int x = 0; x < n_pix; ++x) c[x] = oracle_conv_taper((double)(x - h) / (double)n_pix, S, beta);
+    double inv = (W > 0.0) ? 1.0 / W : 0.0;
+    for (int y = 0; y < n_pix; ++y)
+        for (int x = 0; x < n_pix; ++x) {
+            const size_t p = (size_t)y * n_pix + x;
+            const double corr = inv / (c[y] * c[x]);
+            image[p] = cimg[2 * p] * corr;
+            if (image_im) image_im[p] = cimg[2 * p + 1] * corr;
+        }
+    free(cimg); free(c);
+    if (!grid_out) free(grid);
+    return W;
+}
+
+/* batch driver, as oracle_image_batch */
+typedef struct {
+    const float *vis, *uvw_m; const double *freqs_hz;
+    int T, C, P, B, n_pix, S; double pixscale_rad, beta;
+    const int64_t *img_ids; int n_ids; double *images; double *wsum;
+    int tid, nthreads;
+} conv_job_t;
+
+static void *conv_worker(void *arg)
+{
+    conv_job_t *j = (conv_job_t *)arg;
+    const size_t n2 = (size_t)j->n_pix * j->n_pix;
+    for (int k = j->tid; k < j->n_ids; k += j->nthreads) {
+        int64_t i = j->img_ids[k];
+        int p = (int)(i % j->P);
+        int c = (int)((i / j->P) % j->C);
+        int t = (int)(i / ((int64_t)j->P * j->C));
+        const float *v = j->vis + 2 * ((((size_t)t * j->C + c) * j->P + p) * (size_t)j->B);
+        const float *uvw = j->uvw_m + (size_t)t * j->B * 3;
+        j->wsum[k] = oracle_image_conv_one(v, uvw, j->freqs_hz[c], j->B, j->n_pix, j->pixscale_rad, j->S, j->beta,
+                                           j->images + (size_t)k * n2, NULL, NULL, NULL);
+    }
+    return NULL;
+}
+
+int oracle_image_conv_batch(const float *vis, const float *uvw_m, const double *freqs_hz,
+                            int T, int C, int P, int B, int n_pix, double pixscale_rad, int S, double beta,
+                            const int64_t *img_ids, int n_ids, double *images, double *wsum, int nthreads)
+{
+    if (nthreads < 1) nthreads = 1;
+    if (nthreads > 256) nthreads = 256;
+    if (S < 1 || S > 15 || !(S & 1)) return -2;
+    pthread_t th[256];
+    conv_job_t jobs[256];
+    for (int k = 0; k < nthreads; ++k) {
+        conv_job_t jb = { vis, uvw_m, freqs_hz, T, C, P, B, n_pix, S, pixscale_rad, beta,
+                          img_ids, n_ids, images, wsum, k, nthreads };
+        jobs[k] = jb;
+        if (pthread_create(&th[k], NULL, conv_worker, &jobs[k]) != 0) return -1;
+    }
+    for (int k = 0; k < nthreads; ++k) pthread_join(th[k], NULL);
+    return 0;
+}
