@@ -40,7 +40,8 @@ extern "C" {
 typedef struct blink_c64 { float re, im; } blink_c64;       /* == float2 == complex64 */
 
 enum { BLINK_W_NATURAL = 0, BLINK_W_UNIFORM = 1 };
-enum { BLINK_OP_GRID = 0, BLINK_OP_FFT2D = 1, BLINK_OP_IMAGE = 2, BLINK_OP_IMAGE_HOST = 3, BLINK_OP_IMAGE_AVG = 4 };
+enum { BLINK_OP_GRID = 0, BLINK_OP_FFT2D = 1, BLINK_OP_IMAGE = 2, BLINK_OP_IMAGE_HOST = 3, BLINK_OP_IMAGE_AVG = 4,
+       BLINK_OP_IMAGE_CONV = 5 };
 enum {
     BLINK_OK = 0,
     BLINK_ERR_INVALID_ARG = -1,   /* NULL / misaligned pointer, non-positive size, bad enum          */
@@ -168,6 +169,35 @@ int blink_image_cal(const blink_c64 *vis, const float *uvw_m, const double *freq
                     const blink_c64 *gains, const int32_t *ant_pairs, int A,
                     int T, int C, int P, int B, int n_pix, double pixscale_rad, int weighting,
                     float *image, float *wsum, void *workspace, size_t workspace_bytes, void *stream);
+
+/*
+ * blink_image with a convolutional (anti-aliasing) gridding kernel -- the step the paper names as its next one
+ * ("Visibilities are not convolved with any kernel at this stage, a feature to be introduced in the
+ * near future to alleviate the effects of source aliasing"; L351).  The paper defines no kernel; DESIGN.md reading
+ * R16 fixes the one used here:
+ *   k(d)   = I0(beta sqrt(1 - (2d/S)^2)) / I0(beta), |d| <= S/2   (Kaiser-Bessel window, S = support = 3, 5 or 7 cells)
+ *   x      = u_m * s_c (one fp32 multiply, as step a1), iu0 = rint(x), fx = x - iu0; the same along v
+ *   taps   cell (iv0+i, iu0+j), i,j = -r..r, r = (S-1)/2, += wy_i wx_j V with wx_j = k(j - fx) / sum_j' k(j' - fx)
+ *          (the S taps of an axis sum to 1), and the mirror cell += wy_i wx_j conj(V)
+ *   range  a sample (and its conjugate) is dropped when |iu0| or |iv0| > h-1-r: the whole support stays on the grid
+ *   W      natural weighting: 2 * (samples placed); uniform weighting is not offered with a kernel
+ *   image  = Re IDFT(G) / W / (c((y-h)/N) c((x-h)/N)), c(xi) = (sinh(q)/q) / (sinh(beta)/beta),
+ *            q = sqrt(beta^2 - (pi S xi)^2): the transform of the window, normalised to c(0) = 1 (grid correction)
+ *   support   3, 5 or 7, else BLINK_ERR_UNSUPPORTED
+ *   beta      <= 0 selects 2.34 * support; otherwise 1.7 * support <= beta <= 60 (the correction must stay positive
+ *             over the whole image), else BLINK_ERR_INVALID_ARG
+ *   cell_idx  out OPTIONAL [T][C][B]: the NEAREST cell (iv0+h)*N + (iu0+h) of every baseline, -1 if dropped
+ * Runs in the fused kernel only: n_pix a power of two in [256, 4096] and B <= 16384, else BLINK_ERR_UNSUPPORTED.
+ * `workspace` >= blink_workspace_bytes(BLINK_OP_IMAGE_CONV) minimum, 256-byte aligned.  Other arguments as blink_image.
+ * The tap weights are evaluated as degree-13 polynomials in the offset, fitted on the host at every call;
+ * blink_conv_taps_host (HOST pointers, no GPU needed) returns the weights exactly as the kernel evaluates them for
+ * one offset f in [-1/2, 1/2], plus the largest deviation of the fit from the window's definition (tests).
+ */
+int blink_image_conv(const blink_c64 *vis, const float *uvw_m, const double *freqs_hz,
+                     int T, int C, int P, int B, int n_pix, double pixscale_rad, int support, double beta,
+                     float *image, float *wsum, int32_t *cell_idx,
+                     void *workspace, size_t workspace_bytes, void *stream);
+int blink_conv_taps_host(double f, int support, double beta, float *w /* HOST [support] */, double *fit_error /* HOST, opt */);
 
 #ifdef __cplusplus
 }

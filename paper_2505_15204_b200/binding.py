@@ -17,12 +17,13 @@ _SO = os.path.join(_HERE, "libblinkimg.so")
 _lib = None
 
 W_NATURAL, W_UNIFORM = 0, 1
-OP_GRID, OP_FFT2D, OP_IMAGE, OP_IMAGE_HOST, OP_IMAGE_AVG = 0, 1, 2, 3, 4
+OP_GRID, OP_FFT2D, OP_IMAGE, OP_IMAGE_HOST, OP_IMAGE_AVG, OP_IMAGE_CONV = 0, 1, 2, 3, 4, 5
 OPT_IMAGE_PATH, OPT_FUSED_CTAS, OPT_GRID_CHUNK_B, OPT_AVG_WSUM = 0, 1, 2, 3
 
 EXPORTS = ["blink_strerror", "blink_last_cuda_error", "blink_set_option", "blink_get_option",
            "blink_kernel_launches", "blink_workspace_bytes", "blink_grid", "blink_fft2d_inverse",
-           "blink_image", "blink_image_host", "blink_image_avg", "blink_apply_gains", "blink_image_cal"]
+           "blink_image", "blink_image_host", "blink_image_avg", "blink_apply_gains", "blink_image_cal",
+           "blink_image_conv", "blink_conv_taps_host"]
 
 
 class BlinkError(RuntimeError):
@@ -68,6 +69,10 @@ def lib():
         L.blink_apply_gains.argtypes = [vp, vp, vp, i, i, i, i, i, vp]
         L.blink_image_cal.restype = i
         L.blink_image_cal.argtypes = [vp, vp, vp, vp, vp, i, i, i, i, i, i, d, i, vp, vp, vp, sz, vp]
+        L.blink_image_conv.restype = i
+        L.blink_image_conv.argtypes = [vp, vp, vp, i, i, i, i, i, d, i, d, vp, vp, vp, vp, sz, vp]
+        L.blink_conv_taps_host.restype = i
+        L.blink_conv_taps_host.argtypes = [d, i, d, vp, ctypes.POINTER(d)]
         _lib = L
     return _lib
 
@@ -232,6 +237,38 @@ def blink_image_cal(vis: torch.Tensor, uvw_m: torch.Tensor, freqs_hz, gains: tor
                                _ptr(wsum), _ptr(workspace), workspace.numel(), _stream(dev))
     _check(rc, "blink_image_cal")
     return dict(image=image, wsum=wsum)
+
+
+def blink_image_conv(vis: torch.Tensor, uvw_m: torch.Tensor, freqs_hz, n_pix: int, pixscale_rad: float, support: int,
+                     beta: float = 0.0, image: Optional[torch.Tensor] = None, workspace: Optional[torch.Tensor] = None,
+                     wsum: Optional[torch.Tensor] = None, want_cell_idx: bool = False):
+    """blink_image with the Kaiser-Bessel gridding kernel of odd support 3 / 5 / 7 (natural weighting, grid-corrected)."""
+    _dev(vis, torch.complex64, "vis"); _dev(uvw_m, torch.float32, "uvw_m")
+    T, C, P, B = vis.shape
+    fr = _freqs(freqs_hz)
+    dev = vis.device
+    if image is None:
+        image = torch.empty((T * C * P, n_pix, n_pix), dtype=torch.float32, device=dev)
+    if wsum is None:
+        wsum = torch.empty(T * C, dtype=torch.float32, device=dev)
+    cell_idx = torch.empty((T, C, B), dtype=torch.int32, device=dev) if want_cell_idx else None
+    if workspace is None:
+        rec, _ = blink_workspace_bytes(OP_IMAGE_CONV, T, C, P, B, n_pix, 0)
+        workspace = torch.empty(max(rec, 16), dtype=torch.uint8, device=dev)
+    rc = lib().blink_image_conv(_ptr(vis), _ptr(uvw_m), fr.ctypes.data_as(ctypes.c_void_p), T, C, P, B, n_pix,
+                                float(pixscale_rad), int(support), float(beta), _ptr(image), _ptr(wsum), _ptr(cell_idx),
+                                _ptr(workspace), workspace.numel(), _stream(dev))
+    _check(rc, "blink_image_conv")
+    return dict(image=image, wsum=wsum, cell_idx=cell_idx)
+
+
+def blink_conv_taps_host(f: float, support: int, beta: float = 0.0):
+    """-> (float32 [support] tap weights as the kernel evaluates them, largest deviation of the fit). No GPU needed."""
+    w = np.empty(int(support), dtype=np.float32)
+    err = ctypes.c_double(0.0)
+    rc = lib().blink_conv_taps_host(float(f), int(support), float(beta), w.ctypes.data_as(ctypes.c_void_p), ctypes.byref(err))
+    _check(rc, "blink_conv_taps_host")
+    return w, err.value
 
 
 def blink_image_host(vis_host: torch.Tensor, uvw_host: torch.Tensor, freqs_hz, n_pix: int, pixscale_rad: float,

@@ -73,18 +73,18 @@ __device__ __forceinline__ float rint_rne(float x, int &i)
     return __fadd_rn(t, -12582912.0f);
 }
 // step a1 (R2, R4): nearest cell of one baseline, bit-exact twin of the oracle's fp32 recipe
-__device__ __forceinline__ bool cell_coords(float u_m, float v_m, float s, int h, int &iu, int &iv)
+__device__ __forceinline__ bool cell_coords(float u_m, float v_m, float s, int h, int &iu, int &iv, int r = 0)
 {
     const float x = __fmul_rn(u_m, s);            // one IEEE fp32 multiply, never contracted
     const float y = __fmul_rn(v_m, s);
     const float xr = rint_rne(x, iu), yr = rint_rne(y, iv);     // round to nearest, ties to even
-    const float lim = (float)(h - 1);
+    const float lim = (float)(h - 1 - r);                       // r: support radius of the convolutional gridder (R16)
     return fabsf(xr) <= lim && fabsf(yr) <= lim;                // NaN fails
 }
-__device__ __forceinline__ int cell_of(float u_m, float v_m, float s, int n, int h)
+__device__ __forceinline__ int cell_of(float u_m, float v_m, float s, int n, int h, int r = 0)
 {
     int iu, iv;
-    if (!cell_coords(u_m, v_m, s, h, iu, iv)) return -1;
+    if (!cell_coords(u_m, v_m, s, h, iu, iv, r)) return -1;
     return (iv + h) * n + (iu + h);
 }
 __device__ __forceinline__ int mirror_of(int cell, int n)

@@ -69,3 +69,38 @@ def test_no_cpu_fallback_without_device(so_path):
     rc = L.blink_image(p, p, fr, 1, 1, 1, 4, 32, 0.01, 0, p, p, None, None, p, 64, None)
     assert rc == -4                                                      # BLINK_ERR_CUDA, and says why
     assert L.blink_last_cuda_error().decode() != ""
+
+
+def test_conv_taps_host_logic_against_oracle(so_path, oracle_mod):
+    # the polynomial form of the normalised Kaiser-Bessel taps (host fit + the kernel's fp32 Horner evaluation)
+    # against the oracle's direct evaluation of the definition (reading R16)
+    from paper_2505_15204_b200 import binding as bk
+    for S in (3, 5, 7):
+        for beta in (0.0, 1.8 * S, 3.0 * S):
+            b = beta if beta > 0 else 2.34 * S
+            worst = 0.0
+            for f in np.linspace(-0.5, 0.5, 41):
+                w, fit = bk.blink_conv_taps_host(f, S, beta)
+                assert fit < 2e-7
+                ref = oracle_mod.conv_taps(float(np.float32(f)), S, b)
+                worst = max(worst, float(np.max(np.abs(w.astype(np.float64) - ref))))
+                assert abs(float(w.astype(np.float64).sum()) - 1.0) < 1e-6
+            assert worst < 1e-6, (S, beta, worst)
+
+
+def test_conv_argument_checks(so_path):
+    from paper_2505_15204_b200 import binding as bk
+    L = bk.lib()
+    w = np.zeros(8, np.float32)
+    wp = w.ctypes.data_as(ctypes.c_void_p)
+    assert L.blink_conv_taps_host(0.1, 4, 0.0, wp, None) == -2            # even support
+    assert L.blink_conv_taps_host(0.1, 9, 0.0, wp, None) == -2
+    assert L.blink_conv_taps_host(0.1, 5, 5.0, wp, None) == -1            # beta below 1.7 S: the correction has a null
+    assert L.blink_conv_taps_host(0.7, 5, 0.0, wp, None) == -1            # offset outside [-1/2, 1/2]
+    rec, mn = bk.blink_workspace_bytes(bk.OP_IMAGE_CONV, 50, 768, 1, 8128, 512, 0)
+    rec0, mn0 = bk.blink_workspace_bytes(bk.OP_IMAGE, 50, 768, 1, 8128, 512, 0)
+    assert rec == rec0 + 2048 and mn == mn0 + 2048                        # + the 512-entry correction table
+    with pytest.raises(bk.BlinkError):
+        bk.blink_workspace_bytes(bk.OP_IMAGE_CONV, 1, 1, 1, 100, 1200, 0)  # fused kernel only: powers of two
+    with pytest.raises(bk.BlinkError):
+        bk.blink_workspace_bytes(bk.OP_IMAGE_CONV, 1, 1, 1, 100, 128, 0)

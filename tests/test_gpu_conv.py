@@ -1,0 +1,208 @@
+"""GPU parity of blink_image_conv (convolutional gridding, reading R16) against the
+CPU oracle, through the C ABI.
+
+Bars: wsum and the nearest-cell index of every baseline bit-exact.  Images: north_star's rule (max abs error
+<= 1e-4 x peak) applies to what the transform produces, i.e. BEFORE the grid correction 1 / (c(y) c(x)) -- the
+correction is an exact per-pixel factor that grows towards the image edge (up to ~3000x in the corners for
+S = 7) and scales the fp32 rounding error of that pixel with it.  So the test compares
+    max |I_gpu - I_oracle| c(y) c(x)  <=  1e-4 * max |I_oracle| c(y) c(x)
+and, in the central half of the field (where the correction is below ~4), the plain rule as well.
+"""
+import numpy as np
+import pytest
+import torch
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-4
+
+
+@pytest.fixture(scope="module")
+def bk():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2505_15204_b200 import binding
+    binding.lib()
+    yield binding
+    binding.set_option(binding.OPT_FUSED_CTAS, 0)
+
+
+def _beta(S):
+    return 2.34 * S
+
+
+def _check_conv(w, res, oracle_mod, S, beta=0.0, ids=None, check_cells=True):
+    vis, uvw = w.vis.cpu().numpy(), w.uvw_m.cpu().numpy()
+    b = beta if beta > 0 else _beta(S)
+    n, h = w.n_pix, w.n_pix // 2
+    n_img = w.T * w.C * w.P
+    ids = np.arange(n_img) if ids is None else np.asarray(ids)
+    ref, wref = oracle_mod.image_conv_batch(vis, uvw, w.freqs_hz, n, w.pixscale_rad, S, b, ids, nthreads=8)
+    img = res["image"][torch.as_tensor(ids, device=res["image"].device)].cpu().numpy().astype(np.float64)
+    wsum = res["wsum"].cpu().numpy()
+    c = oracle_mod.conv_taper(n, S, b)
+    cc = np.outer(c, c)
+    q = slice(h - n // 4, h + n // 4)
+    worst = worst_c = 0.0
+    for k, i in enumerate(ids):
+        assert wsum[i // w.P] == np.float32(wref[k]), (i, wsum[i // w.P], wref[k])
+        if wref[k] == 0:
+            assert np.all(img[k] == 0)
+            continue
+        worst = max(worst, float(np.max(np.abs(img[k] - ref[k]) * cc) / np.max(np.abs(ref[k]) * cc)))
+        worst_c = max(worst_c, float(np.max(np.abs(img[k] - ref[k])[q, q]) / np.max(np.abs(ref[k][q, q]))))
+    assert worst <= TOL and worst_c <= TOL, (worst, worst_c)
+    if check_cells and res.get("cell_idx") is not None:
+        ci = res["cell_idx"].cpu().numpy()
+        for t in range(w.T):
+            for cch in range(w.C):
+                want = oracle_mod.grid_conv_one(vis[t, cch, 0], uvw[t], w.freqs_hz[cch], n, w.pixscale_rad, S, b)[2]
+                assert np.array_equal(ci[t, cch], want)
+    return worst
+
+
+@pytest.mark.parametrize("S", [3, 5, 7])
+@pytest.mark.parametrize("B", [1237, 2048])
+def test_conv_random_ragged(bk, oracle_mod, S, B):
+    # odd / even B (plain loads vs bulk-copy prefetch), P = 3, samples off the (tighter) range, NaN, 3 CTAs for 6 items
+    from paper_2505_15204_b200 import workloads
+    w = workloads.make_random(T=2, C=3, P=3, B=B, n_pix=256, weighting=0, seed=100 + B + S, device="cuda", fill=1.1)
+    w.uvw_m[1, 5, 0] = float("nan")
+    w.uvw_m[0, 9, 1] = float("nan")
+    bk.set_option(bk.OPT_FUSED_CTAS, 3)
+    try:
+        res = bk.blink_image_conv(w.vis, w.uvw_m, w.freqs_hz, w.n_pix, w.pixscale_rad, S, want_cell_idx=True)
+        torch.cuda.synchronize()
+        _check_conv(w, res, oracle_mod, S)
+        _, mn = bk.blink_workspace_bytes(bk.OP_IMAGE_CONV, w.T, w.C, w.P, w.B, w.n_pix, 0)
+        ws = torch.empty(mn, dtype=torch.uint8, device="cuda")              # one CTA's scratch only
+        res1 = bk.blink_image_conv(w.vis, w.uvw_m, w.freqs_hz, w.n_pix, w.pixscale_rad, S, workspace=ws)
+        torch.cuda.synchronize()
+        _check_conv(w, res1, oracle_mod, S)
+    finally:
+        bk.set_option(bk.OPT_FUSED_CTAS, 0)
+
+
+@pytest.mark.parametrize("S", [3, 5, 7])
+def test_conv_axis_columns_and_collisions(bk, oracle_mod, S):
+    # the folded half plane: supports that straddle u = 0 (their taps at u < 0 come back as the conjugate's taps),
+    # samples on the u = 0 column and at DC, many samples in one cell, supports that touch the range limit exactly
+    from paper_2505_15204_b200 import workloads
+    n = 256
+    w = workloads.make_random(T=1, C=2, P=2, B=3000, n_pix=n, weighting=0, seed=131, device="cuda", fill=0.9)
+    cell_m = 299792458.0 / 150e6
+    r = S // 2
+    w.uvw_m[0, :600, 0] = 17.2 * cell_m
+    w.uvw_m[0, :600, 1] = -40.3 * cell_m
+    w.uvw_m[0, 600:800, 0] = 0.0
+    w.uvw_m[0, 800:900, 0] = 0.0
+    w.uvw_m[0, 800:900, 1] = 0.0
+    for k, x in enumerate([-0.2, 0.3, -0.6, 0.7, 1.4, -1.5, 2.5, -2.6, 3.2, -3.49, 0.5, -0.5]):
+        w.uvw_m[0, 900 + 50 * k:950 + 50 * k, 0] = x * cell_m
+    lim = n // 2 - 1 - r
+    w.uvw_m[0, 1500:1520, 0] = lim * cell_m * 0.99999              # nearest column exactly at the limit (first channel)
+    w.uvw_m[0, 1520:1540, 1] = -lim * cell_m * 0.99999
+    w.uvw_m[0, 1540:1560, 0] = (lim + 0.6) * cell_m                # one cell beyond: dropped
+    res = bk.blink_image_conv(w.vis, w.uvw_m, w.freqs_hz, n, w.pixscale_rad, S, want_cell_idx=True)
+    torch.cuda.synchronize()
+    _check_conv(w, res, oracle_mod, S)
+
+
+@pytest.mark.parametrize("cfg,T,C,S", [(1, 1, 1, 5), (2, 1, 3, 7), (3, 2, 3, 3), (3, 2, 2, 7)])
+def test_conv_reduced_configs(bk, oracle_mod, cfg, T, C, S):
+    from paper_2505_15204_b200 import workloads
+    w = workloads.make_config(cfg, device="cuda", T=T, C=C)
+    res = bk.blink_image_conv(w.vis, w.uvw_m, w.freqs_hz, w.n_pix, w.pixscale_rad, S, want_cell_idx=True)
+    torch.cuda.synchronize()
+    _check_conv(w, res, oracle_mod, S)
+
+
+@pytest.mark.parametrize("n,S", [(2048, 3), (4096, 5)])
+def test_conv_large_sides(bk, oracle_mod, n, S):
+    from paper_2505_15204_b200 import workloads
+    w = workloads.make_random(T=1, C=2, P=1, B=4000, n_pix=n, weighting=0, seed=7 + n, device="cuda", fill=1.02)
+    res = bk.blink_image_conv(w.vis, w.uvw_m, w.freqs_hz, n, w.pixscale_rad, S, want_cell_idx=True)
+    torch.cuda.synchronize()
+    _check_conv(w, res, oracle_mod, S, ids=[1])
+
+
+def test_conv_two_stage_pipeline_and_beta(bk, oracle_mod):
+    # B = 13000 leaves room for two pass-2 stage buffers only (NS = 2); a caller-chosen beta
+    from paper_2505_15204_b200 import workloads
+    w = workloads.make_random(T=1, C=2, P=1, B=13000, n_pix=256, weighting=0, seed=221, device="cuda", fill=0.8)
+    res = bk.blink_image_conv(w.vis, w.uvw_m, w.freqs_hz, w.n_pix, w.pixscale_rad, 5, beta=9.5)
+    torch.cuda.synchronize()
+    _check_conv(w, res, oracle_mod, 5, beta=9.5)
+
+
+def test_conv_degenerate_and_unit_source(bk, oracle_mod):
+    from paper_2505_15204_b200 import workloads
+    w = workloads.make_random(T=1, C=2, P=1, B=64, n_pix=256, weighting=0, seed=1, device="cuda")
+    w.uvw_m[:] = 1e7                                                # everything off the grid
+    res = bk.blink_image_conv(w.vis, w.uvw_m, w.freqs_hz, w.n_pix, w.pixscale_rad, 3, want_cell_idx=True)
+    torch.cuda.synchronize()
+    assert torch.all(res["image"] == 0) and torch.all(res["wsum"] == 0) and torch.all(res["cell_idx"] == -1)
+    w = workloads.make_random(T=1, C=1, P=1, B=1, n_pix=256, weighting=0, seed=2, device="cuda", fill=0.5)
+    res = bk.blink_image_conv(w.vis, w.uvw_m, w.freqs_hz, w.n_pix, w.pixscale_rad, 7)
+    _check_conv(w, res, oracle_mod, 7)                              # a single baseline
+    w = workloads.make_config(1, device="cuda")                     # all V = 1 -> centre pixel 1.0 (normalised taps, c(0) = 1)
+    w.vis[:] = 1.0
+    h = w.n_pix // 2
+    for S in (3, 5, 7):
+        img = bk.blink_image_conv(w.vis, w.uvw_m, w.freqs_hz, w.n_pix, w.pixscale_rad, S)["image"][0].cpu().numpy()
+        assert abs(img[h, h] - 1.0) < 1e-5
+
+
+def test_conv_error_codes(bk):
+    import ctypes
+    L = bk.lib()
+    x = torch.zeros(1 << 20, device="cuda")
+    fr = np.array([150e6])
+    p = lambda t: ctypes.c_void_p(t.data_ptr())
+    f = fr.ctypes.data_as(ctypes.c_void_p)
+    call = lambda n, S, beta, ws=4 << 20: L.blink_image_conv(p(x), p(x), f, 1, 1, 1, 4, n, 0.01, S, beta, p(x), p(x), None,
+                                                              p(x), ws, None)
+    assert call(256, 4, 0.0) == -2 and call(256, 9, 0.0) == -2 and call(256, 1, 0.0) == -2
+    assert call(128, 3, 0.0) == -2 and call(1200, 3, 0.0) == -2     # fused kernel only
+    assert call(256, 5, 6.0) == -1                                  # beta below 1.7 S
+    assert call(256, 5, 0.0, ws=1024) == -3
+
+
+def test_conv_config3_full_size_sampled(bk, oracle_mod):
+    """BASELINE.json config 3 at full size in the launch configuration bench.py --conv times (S = 5): wsum of every
+    (t,c) exact, sampled images within tolerance, centre-pixel closed form for every image."""
+    from paper_2505_15204_b200 import workloads
+    free, _ = torch.cuda.mem_get_info()
+    if free < 60e9:
+        pytest.skip("needs ~50 GB of device memory")
+    w = workloads.make_config(3, device="cuda")
+    T, C, P, B, N = w.T, w.C, w.P, w.B, w.n_pix
+    S, r, h = 5, 2, N // 2
+    res = bk.blink_image_conv(w.vis, w.uvw_m, w.freqs_hz, N, w.pixscale_rad, S)
+    torch.cuda.synchronize()
+    uvw = w.uvw_m.cpu().numpy()
+    ci = oracle_mod.cells(uvw, w.freqs_hz, N, w.pixscale_rad)       # nearest cells (a1); conv range is tighter by r
+    iv, iu = ci // N - h, ci % N - h
+    inr = (ci >= 0) & (np.abs(iu) <= h - 1 - r) & (np.abs(iv) <= h - 1 - r)
+    assert np.array_equal(res["wsum"].cpu().numpy(), (2 * inr.sum(axis=2)).astype(np.float32).ravel())
+    rng = np.random.default_rng(35)
+    ids = np.unique([0, T * C - 1] + [int(i) for i in rng.choice(T * C, 8, replace=False)])
+    sel = torch.as_tensor(ids, device="cuda")
+    c = oracle_mod.conv_taper(N, S, _beta(S))
+    cc = np.outer(c, c)
+    img_s = res["image"][sel].cpu().numpy().astype(np.float64)
+    vis_s = w.vis.reshape(T * C, B)[sel].cpu().numpy()
+    worst = 0.0
+    for k, i in enumerate(ids):
+        t, cch = divmod(int(i), C)
+        ref = oracle_mod.image_conv_one(vis_s[k], uvw[t], w.freqs_hz[cch], N, w.pixscale_rad, S, _beta(S))["image"]
+        worst = max(worst, float(np.max(np.abs(img_s[k] - ref) * cc) / np.max(np.abs(ref) * cc)))
+    assert worst <= TOL, worst
+    # closed form for EVERY image: taps sum to 1 and c(0) = 1, so the centre pixel is sum(2 Re V_in) / W
+    centre = res["image"][:, h, h].double().cpu().numpy()
+    inr_t = torch.as_tensor(inr, device="cuda").reshape(T * C, B)
+    want = (2.0 * (w.vis.reshape(T * C, B).real.double() * inr_t).sum(dim=1) / (2.0 * inr_t.sum(dim=1))).cpu().numpy()
+    q = slice(h - N // 4, h + N // 4)
+    peak = res["image"][:, q, q].reshape(T * C, -1).abs().amax(dim=1).double().cpu().numpy()
+    assert np.max(np.abs(centre - want) / peak) <= TOL
+    assert bool(torch.isfinite(res["image"]).all())
