@@ -199,7 +199,7 @@ extern "C" int blink_image_conv(const blink_c64 *vis, const float *uvw_m, const 
     FusedArgs a{};
     a.vis = reinterpret_cast<const float2 *>(vis); a.uvw_m = uvw_m; a.T = T; a.C = C; a.P = P; a.B = B;
     a.weighting = BLINK_W_NATURAL; a.tc0 = 0; a.ntc = T * C; a.image = image; a.wsum = wsum; a.cell_idx = cell_idx;
-    a.inv_taper = inv_c;
+    poly.inv_taper = inv_c;                          // [N] 1 / c((x - h)/N), read by the image store
     const int R = (support - 1) / 2;
     switch (n_pix) {
         case 256: return launch_conv<256>(a, R, freqs_hz, pixscale_rad, workspace, workspace_bytes, st, &poly, extra);

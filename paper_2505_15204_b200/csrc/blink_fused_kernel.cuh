@@ -39,7 +39,6 @@ struct FusedArgs {
     const float *su; const uint2 *svb;                         // per timestep: baselines sorted by |u| (presort_kernel)
     const float2 *tw;
     GainRef cal;                                               // optional per-antenna gains applied at the load
-    const float *inv_taper;                                    // convolutional gridding: [N] 1 / c((x - h)/N), else NULL
 };
 
 // Convolutional gridding (reading R16): the NORMALISED tap weight of tap j = -R..R of one axis,
@@ -48,7 +47,7 @@ struct FusedArgs {
 // host in double (Chebyshev interpolation, conv_fit_taps in blink_fused_conv.cu) and travel as a kernel parameter.
 constexpr int kConvTerms = 14;
 constexpr int kConvMaxSupport = 7;
-struct ConvPoly { float c[kConvMaxSupport][kConvTerms]; };     // c[j + R][k] multiplies f^k
+struct ConvPoly { float c[kConvMaxSupport][kConvTerms]; const float *inv_taper; };     // c[j + R][k] multiplies f^k
 
 struct ExchangePadded2 {
     float2 *c0, *c1;
@@ -282,6 +281,7 @@ fused_image_kernel(const FusedArgs a, const __grid_constant__ ScaleBlock sc, con
             // columns iu0-R..iu0+R; the taps at columns <= 0 are ALSO the conjugate sample's taps mirrored into u >= 0
             // (k is even, so the Hermitian sample at (-x,-y) has exactly the mirrored weights).
             auto conv_one = [&](int j, int u0) {
+                if constexpr (R == 0) return;
                 int iu0, iv0;
                 const float x = __fmul_rn(__ldg(su + j), s);
                 const float xr = rint_rne(x, iu0);              // in range by construction of the sample range
@@ -301,6 +301,17 @@ fused_image_kernel(const FusedArgs a, const __grid_constant__ ScaleBlock sc, con
                     for (int k = kConvTerms - 2; k >= 0; --k) w = fmaf(w, fy, cpoly.c[i][k]);
                     wy[i] = w;
                 }
+                // S taps of one column.  (Measured: fp32 atomicAdd on shared memory is a load + CAS spin loop per scalar on
+                // sm_100, yet an optimistic batch of 64-bit CAS on the (re, im) pairs -- S loads, S CAS in flight, retry only
+                // on interference -- was 1.4x (S = 5) to 2.1x (S = 7) SLOWER than the plain per-scalar adds below.)
+                auto add_taps = [&](float2 *col, int row0, int dir, float ar, float ai) {
+#pragma unroll
+                    for (int i = 0; i < S; ++i) {
+                        const int o = xsw(row0 + dir * i);
+                        atomicAdd(&col[o].x, wy[i] * ar);
+                        atomicAdd(&col[o].y, wy[i] * ai);
+                    }
+                };
                 auto wx_of = [&](int jj) {                      // tap jj - R of the u axis (dynamic index: LDC)
                     float w = cpoly.c[jj][kConvTerms - 1];
 #pragma unroll
@@ -314,25 +325,13 @@ fused_image_kernel(const FusedArgs a, const __grid_constant__ ScaleBlock sc, con
                     const int jd = u - iu0;                     // direct tap that lands in column u
                     if (jd >= -R && jd <= R) {
                         const float wx = wx_of(jd + R);
-                        const float ar = wx * vv.x, ai = wx * vv.y;
-#pragma unroll
-                        for (int i = 0; i < S; ++i) {
-                            const int o = xsw(iv0 + i - R + H);
-                            atomicAdd(&col[o].x, wy[i] * ar);
-                            atomicAdd(&col[o].y, wy[i] * ai);
-                        }
+                        add_taps(col, iv0 - R + H, 1, wx * vv.x, wx * vv.y);
                         if (jd == 0) ++my_in;                   // the sample's own column: counted once
                     }
                     const int jm = -u - iu0;                    // tap at column -u, mirrored: conj(V) at row -(iv0 + i)
                     if (jm >= -R) {
                         const float wx = wx_of(jm + R);
-                        const float ar = wx * vv.x, ai = -wx * vv.y;
-#pragma unroll
-                        for (int i = 0; i < S; ++i) {
-                            const int o = xsw(H - (iv0 + i - R));
-                            atomicAdd(&col[o].x, wy[i] * ar);
-                            atomicAdd(&col[o].y, wy[i] * ai);
-                        }
+                        add_taps(col, H - (iv0 - R), -1, wx * vv.x, -wx * vv.y);
                     }
                 }
             };
@@ -497,10 +496,10 @@ fused_image_kernel(const FusedArgs a, const __grid_constant__ ScaleBlock sc, con
                         __stcs(r1 + (e ^ (kE / 2)) * TG, z[0][e].y * inv_w);
                     }
                 } else {                                        // grid correction 1 / (c(y) c(x)) rides on the same store
-                    const float t0 = inv_w * __ldg(a.inv_taper + (ky ^ H)), t1 = inv_w * __ldg(a.inv_taper + ((ky + 1) ^ H));
+                    const float t0 = inv_w * __ldg(cpoly.inv_taper + (ky ^ H)), t1 = inv_w * __ldg(cpoly.inv_taper + ((ky + 1) ^ H));
 #pragma unroll
                     for (int e = 0; e < kE; ++e) {
-                        const float tx = __ldg(a.inv_taper + tid + (e ^ (kE / 2)) * TG);
+                        const float tx = __ldg(cpoly.inv_taper + tid + (e ^ (kE / 2)) * TG);
                         __stcs(r0 + (e ^ (kE / 2)) * TG, z[0][e].x * (t0 * tx));
                         __stcs(r1 + (e ^ (kE / 2)) * TG, z[0][e].y * (t1 * tx));
                     }
