@@ -173,6 +173,8 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-avg", action="store_true")
+    ap.add_argument("--no-conv", action="store_true")
+    ap.add_argument("--conv-support", type=int, default=5, help="support of the gridding kernel timed in conv_mode (3, 5, 7)")
     ap.add_argument("--T", type=int, default=None, help="reduce timesteps (debug only; invalidates the headline)")
     args = ap.parse_args()
 
@@ -276,6 +278,37 @@ def main():
         except Exception as ex:  # report, never hide
             avg = {"error": str(ex)[:200]}
 
+    # ---- convolutional gridding (blink_image_conv), same inputs and outputs -------------------
+    conv = None
+    if not args.no_conv and w.weighting == 0:
+        try:
+            S = args.conv_support
+            rec_c, _ = bk.blink_workspace_bytes(bk.OP_IMAGE_CONV, T, C, P, B, N, 0)
+            ws_c = torch.empty(max(rec_c, 16), dtype=torch.uint8, device=dev)
+            run_c = lambda: bk.blink_image_conv(w.vis, w.uvw_m, w.freqs_hz, N, w.pixscale_rad, S, image=image,
+                                                workspace=ws_c, wsum=wsum)
+            for _ in range(args.warmup):
+                run_c()
+            barrier()
+            ec = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+            ec[0].record()
+            for _ in range(args.steps):
+                run_c()
+            ec[1].record()
+            barrier()
+            ms_c = torch.tensor([ec[0].elapsed_time(ec[1]) / args.steps], device=dev)
+            if world > 1:
+                dist.all_reduce(ms_c, op=dist.ReduceOp.MAX)
+            ms_c = float(ms_c.item())
+            conv = {"api": f"blink_image_conv (Kaiser-Bessel, support {S}, beta {2.34 * S:.2f}; PAPER.md L192, L351; DESIGN.md R16)",
+                    "support": S, "ms_per_step": ms_c, "images_per_s": world * n_img / (ms_c * 1e-3),
+                    "gvis_per_s": world * n_img * B / (ms_c * 1e-3) / 1e9,
+                    "g_tap_cells_per_s": world * n_img * B * S * S * 2 / (ms_c * 1e-3) / 1e9,
+                    "frac_M4": (n_img * (4 * N * N + 8 * B) + 12 * T * B) / (ms_c * 1e-3) / 1e9 / hbm_peak()[0]}
+            del ws_c
+        except Exception as ex:  # report, never hide
+            conv = {"error": str(ex)[:200]}
+
     # ---- end to end through the host-buffer entry point (rank-local, then max over ranks) -----------------
     e2e = None
     if not args.no_e2e:
@@ -354,7 +387,7 @@ def main():
                    (w.vis.numel() * 8 / 1e9, n_img * N * N * 4 / 1e9),
                    "image_path": args.path, "parallelism": f"independent batches x{world}"},
         "gvis_per_s": value * B / 1e9,
-        "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu, "avg_mode": avg,
+        "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu, "avg_mode": avg, "conv_mode": conv,
         "ms_per_step_each": per_step,
     }
     print(json.dumps(out))
