@@ -290,3 +290,20 @@ def image_conv_batch(vis, uvw_m, freqs_hz, n_pix: int, pixscale_rad: float, supp
     if rc != 0:
         raise RuntimeError("oracle_image_conv_batch failed")
     return images, wsum
+
+
+# ---- CMAC correlator (reading R17) -------------------------------------------
+def correlate(volt, n_t: int, n_avg: int) -> np.ndarray:
+    """volt [F][A][Ns][2] int8 -> vis [T][C][A(A+1)/2] complex64 (lower triangle, autos included)."""
+    v = np.ascontiguousarray(volt, dtype=np.int8)
+    F, A, Ns, two = v.shape
+    assert two == 2
+    L = lib()
+    L.oracle_correlate.restype = ctypes.c_int
+    L.oracle_correlate.argtypes = [ctypes.c_void_p] + [ctypes.c_int] * 5 + [ctypes.c_void_p]
+    T, C = Ns // n_t, F // n_avg
+    out = np.empty((T, C, A * (A + 1) // 2), dtype=np.complex64)
+    rc = L.oracle_correlate(_p(v), F, A, Ns, int(n_t), int(n_avg), _p(out))
+    if rc != 0:
+        raise ValueError("oracle_correlate: Ns must be a multiple of n_t and F of n_avg")
+    return out

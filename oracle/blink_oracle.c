@@ -624,3 +624,51 @@ int oracle_image_conv_batch(const float *vis, const float *uvw_m, const double *
     for (int k = 0; k < nthreads; ++k) pthread_join(th[k], NULL);
     return 0;
 }
+
+/* ------------------------------------------------------------------------------------------
+ * CMAC correlator -- SURVEY 8(f) rank 4 (last item).  PAPER.md eq. 3 (L98) and section 6.2.2
+ * (L172-178): "voltage data from every pair of antennas are combined to produce visibilities ...
+ * only the Conjugate Multiply Accumulate (CMAC) operation was developed ... partial results are
+ * summed together ... and the result is divided by the integration time and number of averaged
+ * frequency channels.  Visibilities are stored in a lower triangular matrix form for each
+ * integration interval and output frequency channel."  DESIGN.md reading R17 fixes what the paper
+ * leaves open (sample format and array order):
+ *   volt [F][A][Ns][2] int8: fine channel f, input a (tile x polarisation), time sample, (re, im);
+ *        MWA Phase I VCS samples are 4 + 4 bit, i.e. values in [-8, 7]; any value in [-127, 127] is allowed
+ *   interval t = samples [t n_t, (t+1) n_t), T = Ns / n_t;  output channel c = fine channels [c n_avg, (c+1) n_avg)
+ *   S[t][c][i][j] = sum_{f in c} sum_{s in t} x_i(f,s) conj(x_j(f,s))      for j <= i   (exact, 64-bit integers)
+ *   vis [T][C][A(A+1)/2] complex64, entry i(i+1)/2 + j = (float)S / (float)(n_t n_avg): ONE fp32 division of two
+ *        exactly representable integers (|S| < 2^24 whenever n_t n_avg max|x|^2 2 < 2^24; larger sums are first
+ *        rounded to fp32 by the int -> float conversion, on both sides)
+ * Pins (tests/test_oracle_corr_pins.py): hand-worked two-input case (tests/golden/cmac_two_inputs.txt);
+ * constant inputs -> c_i conj(c_j); autos real and = mean |x|^2; conjugate symmetry under swapping inputs;
+ * independent numpy einsum; averaging n_avg channels = mean of the single-channel results (exact sums);
+ * a common signal with per-input phase steps -> the phase differences; independent noise -> cross terms
+ * within 6 sigma of zero.
+ * ---------------------------------------------------------------------------------------- */
+int oracle_correlate(const int8_t *volt, int F, int A, int Ns, int n_t, int n_avg, float *vis)
+{
+    if (n_t < 1 || n_avg < 1 || Ns % n_t != 0 || F % n_avg != 0) return -1;
+    const int T = Ns / n_t, C = F / n_avg;
+    const size_t ntri = (size_t)A * (A + 1) / 2;
+    const float norm = (float)((long long)n_t * n_avg);
+    for (int t = 0; t < T; ++t)
+        for (int c = 0; c < C; ++c)
+            for (int i = 0; i < A; ++i)
+                for (int j = 0; j <= i; ++j) {
+                    long long sr = 0, si = 0;
+                    for (int f = c * n_avg; f < (c + 1) * n_avg; ++f) {
+                        const int8_t *xi = volt + 2 * (((size_t)f * A + i) * Ns + (size_t)t * n_t);
+                        const int8_t *xj = volt + 2 * (((size_t)f * A + j) * Ns + (size_t)t * n_t);
+                        for (int s = 0; s < n_t; ++s) {
+                            const long long ar = xi[2 * s], ai = xi[2 * s + 1], br = xj[2 * s], bi = xj[2 * s + 1];
+                            sr += ar * br + ai * bi;           /* (ar + i ai)(br - i bi) */
+                            si += ai * br - ar * bi;
+                        }
+                    }
+                    float *o = vis + 2 * (((size_t)t * C + c) * ntri + (size_t)i * (i + 1) / 2 + j);
+                    o[0] = (float)sr / norm;
+                    o[1] = (float)si / norm;
+                }
+    return 0;
+}
