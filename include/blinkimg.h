@@ -199,6 +199,23 @@ int blink_image_conv(const blink_c64 *vis, const float *uvw_m, const double *fre
                      void *workspace, size_t workspace_bytes, void *stream);
 int blink_conv_taps_host(double f, int support, double beta, float *w /* HOST [support] */, double *fit_error /* HOST, opt */);
 
+/*
+ * CMAC correlator (eq. 3; section 6.2.2: "only the Conjugate Multiply Accumulate (CMAC) operation
+ * was developed ... the result is divided by the integration time and number of averaged frequency channels.
+ * Visibilities are stored in a lower triangular matrix form for each integration interval and output frequency
+ * channel"; reading R17 for the sample format and array order the paper leaves open):
+ *   volt  in  [F][A][Ns][2] int8: fine channel, input (tile x polarisation), time sample, (re, im); values in
+ *             [-127, 127] (MWA Phase I VCS samples are 4 + 4 bit: [-8, 7]); 16-byte aligned
+ *   n_t       samples per integration interval: T = Ns / n_t intervals (Ns % n_t == 0; n_t a multiple of 8, >= 64)
+ *   n_avg     contiguous fine channels averaged into one output channel: C = F / n_avg (F % n_avg == 0)
+ *   vis   out [T][C][A(A+1)/2] complex64: entry i(i+1)/2 + j (j <= i, autocorrelations included) =
+ *             (float)(sum_{f,s} x_i conj(x_j)) / (float)(n_t n_avg); the integer sum is exact (int32 accumulators:
+ *             n_t * n_avg <= 66000), the division is one correctly rounded fp32 operation
+ * Runs on the int8 tensor cores (tcgen05.mma kind::i8, accumulators in TMEM), one persistent CTA per SM; needs no
+ * workspace.  BLINK_ERR_UNSUPPORTED for n_t not a multiple of 8 or below 64, A > 4096, n_t * n_avg > 66000.
+ */
+int blink_correlate(const int8_t *volt, int F, int A, int Ns, int n_t, int n_avg, blink_c64 *vis, void *stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -23,7 +23,7 @@ OPT_IMAGE_PATH, OPT_FUSED_CTAS, OPT_GRID_CHUNK_B, OPT_AVG_WSUM = 0, 1, 2, 3
 EXPORTS = ["blink_strerror", "blink_last_cuda_error", "blink_set_option", "blink_get_option",
            "blink_kernel_launches", "blink_workspace_bytes", "blink_grid", "blink_fft2d_inverse",
            "blink_image", "blink_image_host", "blink_image_avg", "blink_apply_gains", "blink_image_cal",
-           "blink_image_conv", "blink_conv_taps_host"]
+           "blink_image_conv", "blink_conv_taps_host", "blink_correlate"]
 
 
 class BlinkError(RuntimeError):
@@ -73,6 +73,8 @@ def lib():
         L.blink_image_conv.argtypes = [vp, vp, vp, i, i, i, i, i, d, i, d, vp, vp, vp, vp, sz, vp]
         L.blink_conv_taps_host.restype = i
         L.blink_conv_taps_host.argtypes = [d, i, d, vp, ctypes.POINTER(d)]
+        L.blink_correlate.restype = i
+        L.blink_correlate.argtypes = [vp, i, i, i, i, i, vp, vp]
         _lib = L
     return _lib
 
@@ -269,6 +271,21 @@ def blink_conv_taps_host(f: float, support: int, beta: float = 0.0):
     rc = lib().blink_conv_taps_host(float(f), int(support), float(beta), w.ctypes.data_as(ctypes.c_void_p), ctypes.byref(err))
     _check(rc, "blink_conv_taps_host")
     return w, err.value
+
+
+def blink_correlate(volt: torch.Tensor, n_t: int, n_avg: int, vis: Optional[torch.Tensor] = None):
+    """volt [F][A][Ns][2] int8 (CUDA) -> vis [T][C][A(A+1)/2] complex64: lower-triangular CMAC products per interval / channel."""
+    _dev(volt, torch.int8, "volt")
+    F, A, Ns, two = volt.shape
+    if two != 2:
+        raise BlinkError("volt must be [F][A][Ns][2] int8")
+    if Ns % n_t or F % n_avg:
+        raise BlinkError("Ns must be a multiple of n_t and F of n_avg")
+    if vis is None:
+        vis = torch.empty((Ns // n_t, F // n_avg, A * (A + 1) // 2), dtype=torch.complex64, device=volt.device)
+    rc = lib().blink_correlate(_ptr(volt), F, A, Ns, int(n_t), int(n_avg), _ptr(vis), _stream(volt.device))
+    _check(rc, "blink_correlate")
+    return vis
 
 
 def blink_image_host(vis_host: torch.Tensor, uvw_host: torch.Tensor, freqs_hz, n_pix: int, pixscale_rad: float,

@@ -254,3 +254,20 @@ def make_random(T: int, C: int, P: int, B: int, n_pix: int, weighting: int, seed
     return Workload(name="random", T=T, C=C, P=P, B=B, n_pix=n_pix, pixscale_rad=pix, weighting=weighting,
                     freqs_hz=freqs, uvw_m=torch.from_numpy(uvw).to(device),
                     vis=torch.from_numpy(vis).to(device), sources={}, meta={"seed": seed})
+
+
+def make_voltages(F: int, A: int, Ns: int, seed: int, device="cpu", amp: float = 2.0, lo: int = -8, hi: int = 7) -> torch.Tensor:
+    """Synthetic fine-channelised voltages shaped like MWA Phase I VCS data: [F][A][Ns][2] int8,
+    a common sky signal seen by every input with its own complex gain plus independent receiver noise, quantised to
+    the 4 + 4 bit range [-8, 7] (``lo`` / ``hi`` widen it for full-range tests).  No correlator arithmetic here."""
+    g = torch.Generator(device=device)
+    g.manual_seed(seed)
+    dev = torch.device(device)
+    sky = torch.randn((F, 1, Ns, 2), generator=g, device=dev)
+    ph = torch.rand((1, A, 1), generator=g, device=dev) * (2 * math.pi)
+    gr, gi = torch.cos(ph), torch.sin(ph)
+    x = torch.empty((F, A, Ns, 2), device=dev)
+    x[..., 0] = sky[..., 0] * gr - sky[..., 1] * gi
+    x[..., 1] = sky[..., 0] * gi + sky[..., 1] * gr
+    x = amp * (0.6 * x + torch.randn((F, A, Ns, 2), generator=g, device=dev))
+    return torch.clamp(torch.round(x), lo, hi).to(torch.int8)
