@@ -174,6 +174,7 @@ def main():
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-avg", action="store_true")
     ap.add_argument("--no-conv", action="store_true")
+    ap.add_argument("--no-corr", action="store_true")
     ap.add_argument("--conv-support", type=int, default=5, help="support of the gridding kernel timed in conv_mode (3, 5, 7)")
     ap.add_argument("--T", type=int, default=None, help="reduce timesteps (debug only; invalidates the headline)")
     args = ap.parse_args()
@@ -309,6 +310,50 @@ def main():
         except Exception as ex:  # report, never hide
             conv = {"error": str(ex)[:200]}
 
+    # ---- SURVEY 8(f) rank 4 (last item): CMAC correlator on the int8 tensor cores (blink_correlate) --------------
+    # one second of MWA Phase I voltages: 3072 fine channels of 10 kHz x 256 inputs x 10000
+    # samples, correlated at 20 ms / 40 kHz -> 50 x 768 lower-triangular matrices (the visibilities config 3 images)
+    corr = None
+    if not args.no_corr and args.T is None:
+        try:
+            Fc, Ac, Nsc, n_t, n_avg = 3072, 256, 10000, 200, 4
+            volt = torch.empty((Fc, Ac, Nsc, 2), dtype=torch.int8, device=dev)
+            for f0 in range(0, Fc, 256):
+                volt[f0:f0 + 256] = workloads.make_voltages(256, Ac, Nsc, seed=7000 + 100 * rank + f0, device=dev)
+            visc = torch.empty((Nsc // n_t, Fc // n_avg, Ac * (Ac + 1) // 2), dtype=torch.complex64, device=dev)
+            run_k = lambda: bk.blink_correlate(volt, n_t, n_avg, vis=visc)
+            for _ in range(args.warmup):
+                run_k()
+            barrier()
+            ek = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+            ek[0].record()
+            for _ in range(args.steps):
+                run_k()
+            ek[1].record()
+            barrier()
+            ms_k = torch.tensor([ek[0].elapsed_time(ek[1]) / args.steps], device=dev)
+            if world > 1:
+                dist.all_reduce(ms_k, op=dist.ReduceOp.MAX)
+            ms_k = float(ms_k.item())
+            n_mat = (Nsc // n_t) * (Fc // n_avg)
+            cmacs = n_mat * (Ac * (Ac + 1) // 2) * n_t * n_avg
+            # int8 multiply-adds the tensor cores are asked for: 3 tiles of 128 x 256 x (13 K-steps of 32 bytes per fine channel)
+            issued_ops = 2 * n_mat * 3 * 128 * 256 * (13 * 32) * n_avg
+            pk = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json"))) if os.path.exists(os.path.join(ROOT, "MEASURED_PEAKS.json")) else {}
+            i8_peak = 2.0 * float(pk.get("bf16_tflops", 2250.0 * 0.725))
+            corr = {"api": "blink_correlate (tcgen05.mma kind::i8; PAPER.md eq. 3, L172-178; DESIGN.md R17)",
+                    "workload": f"{Fc} fine channels x {Ac} inputs x {Nsc} samples (1 s of MWA Phase I VCS data), n_t {n_t}, n_avg {n_avg}",
+                    "ms_per_step": ms_k, "seconds_of_data_per_s": world / (ms_k * 1e-3),
+                    "tcmac_per_s": world * cmacs / (ms_k * 1e-3) / 1e12,
+                    "roofline": {"bound": "tensor", "achieved": world * issued_ops / (ms_k * 1e-3) / 1e12, "unit": "TOP/s (int8)",
+                                 "peak": i8_peak, "frac": issued_ops / (ms_k * 1e-3) / 1e12 / i8_peak,
+                                 "peak_source": "2 x MEASURED_PEAKS.json bf16_tflops (nominal int8 : bf16 ratio)",
+                                 "useful_frac": 8 * cmacs / (ms_k * 1e-3) / 1e12 / i8_peak},
+                    "hbm_gbs": (volt.numel() + visc.numel() * 8) / (ms_k * 1e-3) / 1e9}
+            del volt, visc
+        except Exception as ex:  # report, never hide
+            corr = {"error": str(ex)[:200]}
+
     # ---- end to end through the host-buffer entry point (rank-local, then max over ranks) -----------------
     e2e = None
     if not args.no_e2e:
@@ -387,7 +432,7 @@ def main():
                    (w.vis.numel() * 8 / 1e9, n_img * N * N * 4 / 1e9),
                    "image_path": args.path, "parallelism": f"independent batches x{world}"},
         "gvis_per_s": value * B / 1e9,
-        "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu, "avg_mode": avg, "conv_mode": conv,
+        "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu, "avg_mode": avg, "conv_mode": conv, "corr_mode": corr,
         "ms_per_step_each": per_step,
     }
     print(json.dumps(out))

@@ -14,7 +14,7 @@
 // One persistent CTA per SM; a unit = (t, c, tile (I, J <= I)) of the lower triangle.  Warp roles:
 //   warp 0      TMA producer: [128 rows][128 bytes] boxes of X_J (and X_I when I != J) into a 4-stage ring (128B swizzle);
 //               the K tail of an interval and rows beyond A are zero-filled by the tensor map's bounds
-//   warps 2-5   build the transformed rows b'' of every stage in shared memory (byte permute + per-byte negate)
+//   warps 2-5   build the transformed rows b'' of every stage in shared memory (byte permute + per-byte two's complement; -128 is outside the input contract)
 //   warp 1      one lane issues the MMAs (4 K-steps of 32 bytes per stage), tcgen05.commit frees the stage / publishes the tile
 //   warps 6-9   epilogue: tcgen05.ld the int32 tile (double-buffered in TMEM: 2 x 256 columns), convert, divide by the number
 //               of accumulated samples (one fp32 division, as the oracle), store the triangular matrix
@@ -73,13 +73,13 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&r)[32])
         : "memory");
 }
 
-// unit -> (t, c, I, J): the tiles of one (t, c) are consecutive units, so the CTAs working on them share X through L2
+// unit -> (t, c, I, J): the tiles of one (t, c) are consecutive units, so the CTAs working on them share X through L2;
 __device__ __forceinline__ void corr_unit(const CorrArgs &a, int u, int &t, int &c, int &I, int &J)
 {
     const int item = u / a.n_tiles;
     int k = u - item * a.n_tiles;
-    t = item / a.C;
-    c = item - t * a.C;
+    c = item / a.T;                                             // t fastest: the CTAs running at the same time read
+    t = item - c * a.T;                                         // neighbouring intervals of the same rows (DRAM pages)
     I = 0;
     while (k > I) { k -= I + 1; ++I; }                          // row I holds tiles J = 0..I
     J = k;
@@ -180,10 +180,12 @@ corr_kernel(const CorrArgs a, const __grid_constant__ CUtensorMap tmap)
 #pragma unroll
                 for (int k = 0; k < 8; ++k) v[k] = src[tx + k * 128];
 #pragma unroll
-                for (int k = 0; k < 8; ++k) {                   // (re, im) -> (-im, re), saturating negate; same swizzled slot
-                    auto xf = [](uint32_t w) {
-                        const uint32_t sw = __byte_perm(w, 0u, 0x2301);
-                        return (__vnegss4(sw) & 0x00FF00FFu) | (sw & 0xFF00FF00u);
+                for (int k = 0; k < 8; ++k) {                   // (re, im) -> (-im, re); same swizzled slot
+                    auto xf = [](uint32_t w) {                 // bytes (r0, i0, r1, i1) -> (-i0, r0, -i1, r1)
+                        const uint32_t sw = __byte_perm(w, 0u, 0x2301);                   // (i0, r0, i1, r1)
+                        const uint32_t n = ~sw;                                           // -x = ~x + 1 per byte, no carry across bytes
+                        const uint32_t neg = ((n & 0x7F7F7F7Fu) + 0x01010101u) ^ (n & 0x80808080u);
+                        return (neg & 0x00FF00FFu) | (sw & 0xFF00FF00u);
                     };
                     dst[tx + k * 128] = make_uint4(xf(v[k].x), xf(v[k].y), xf(v[k].z), xf(v[k].w));
                 }
