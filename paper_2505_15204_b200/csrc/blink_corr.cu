@@ -14,28 +14,30 @@
 // One persistent CTA per SM; a unit = (t, c, tile (I, J <= I)) of the lower triangle.  Warp roles:
 //   warp 0      TMA producer: [128 rows][128 bytes] boxes of X_J (and X_I when I != J) into a 4-stage ring (128B swizzle);
 //               the K tail of an interval and rows beyond A are zero-filled by the tensor map's bounds
-//   warps 2-5   build the transformed rows b'' of every stage in shared memory (byte permute + per-byte two's complement; -128 is outside the input contract)
+//   warps 2-9   build the transformed rows b'' of every stage in shared memory (byte permute + per-byte two's complement; -128 is outside the input contract)
 //   warp 1      one lane issues the MMAs (4 K-steps of 32 bytes per stage), tcgen05.commit frees the stage / publishes the tile
-//   warps 6-9   epilogue: tcgen05.ld the int32 tile (double-buffered in TMEM: 2 x 256 columns), convert, divide by the number
+//   warps 10-13 epilogue: tcgen05.ld the int32 tile (double-buffered in TMEM: 2 x 256 columns), convert, divide by the number
 //               of accumulated samples (one fp32 division, as the oracle), store the triangular matrix
 #include "blink_common.cuh"
 #include "blink_tma.cuh"
 
 namespace blink {
 
-constexpr int kCorrThreads = 320;
+constexpr int kCorrXfWarps = 8;                                  // warps that build the transformed rows
+constexpr int kCorrThreads = (2 + kCorrXfWarps + 4) * 32;
 constexpr int kCorrStages = 4;
 constexpr int kCorrTile = 128;                                  // rows / columns of an output tile
 constexpr int kCorrChunk = 128;                                 // K bytes per stage row (64 complex samples) = swizzle span
 constexpr int kCorrRowsBytes = kCorrTile * kCorrChunk;          // 16 KB: 128 rows x 128 bytes
 constexpr int kCorrStageBytes = 3 * kCorrRowsBytes;             // X_I | X_J | b''_J
-constexpr size_t kCorrSmem = (size_t)kCorrStages * kCorrStageBytes + 1024 /* alignment */ + 256 /* barriers */;
+constexpr int kCorrOutBytes = 32 * 33 * 8;                     // per epilogue warp: 32 x 32 complex64, rows padded to 33
+constexpr size_t kCorrSmem = (size_t)kCorrStages * kCorrStageBytes + 1024 /* alignment */ + 256 /* barriers */ + 4 * kCorrOutBytes;
 
 struct CorrArgs {
     int A, T, C, n_t, n_avg;
     int n_tiles_side, n_tiles, n_units;
     int nk, last_ksteps;                                        // chunks per (interval, fine channel); K steps of the last one
-    float norm;                                                 // n_t * n_avg
+    float norm, rnorm;                                          // n_t * n_avg and its correctly rounded reciprocal
     float2 *vis;
 };
 
@@ -100,7 +102,7 @@ corr_kernel(const CorrArgs a, const __grid_constant__ CUtensorMap tmap)
     if (threadIdx.x == 0) {
         for (int s = 0; s < kCorrStages; ++s) {
             mbar_init(&full_tma[s], 1);
-            mbar_init(&full_xf[s], 128);
+            mbar_init(&full_xf[s], kCorrXfWarps * 32);
             mbar_init(&empty[s], 1);
         }
         for (int b = 0; b < 2; ++b) {
@@ -167,8 +169,9 @@ corr_kernel(const CorrArgs a, const __grid_constant__ CUtensorMap tmap)
                 tc_commit(&tmem_full[b]);
             }
         }
-    } else if (warp < 6) {
-        const int tx = threadIdx.x - 64;                        // 0..127
+    } else if (warp < 2 + kCorrXfWarps) {
+        constexpr int XT = kCorrXfWarps * 32, XV = 1024 / XT;      // threads, 16-byte vectors per thread and stage
+        const int tx = threadIdx.x - 64;
         uint32_t it = 0;
         for (int u = blockIdx.x; u < a.n_units; u += gridDim.x) {
             for (int q = 0; q < chunks; ++q, ++it) {
@@ -176,26 +179,36 @@ corr_kernel(const CorrArgs a, const __grid_constant__ CUtensorMap tmap)
                 mbar_wait(&full_tma[s], ph);
                 const uint4 *src = reinterpret_cast<const uint4 *>(tiles + (size_t)s * kCorrStageBytes + kCorrRowsBytes);
                 uint4 *dst = reinterpret_cast<uint4 *>(tiles + (size_t)s * kCorrStageBytes + 2 * kCorrRowsBytes);
-                uint4 v[8];
+                uint4 v[XV];
 #pragma unroll
-                for (int k = 0; k < 8; ++k) v[k] = src[tx + k * 128];
+                for (int k = 0; k < XV; ++k) v[k] = src[tx + k * XT];
 #pragma unroll
-                for (int k = 0; k < 8; ++k) {                   // (re, im) -> (-im, re); same swizzled slot
+                for (int k = 0; k < XV; ++k) {                   // (re, im) -> (-im, re); same swizzled slot
                     auto xf = [](uint32_t w) {                 // bytes (r0, i0, r1, i1) -> (-i0, r0, -i1, r1)
                         const uint32_t sw = __byte_perm(w, 0u, 0x2301);                   // (i0, r0, i1, r1)
                         const uint32_t n = ~sw;                                           // -x = ~x + 1 per byte, no carry across bytes
                         const uint32_t neg = ((n & 0x7F7F7F7Fu) + 0x01010101u) ^ (n & 0x80808080u);
                         return (neg & 0x00FF00FFu) | (sw & 0xFF00FF00u);
                     };
-                    dst[tx + k * 128] = make_uint4(xf(v[k].x), xf(v[k].y), xf(v[k].z), xf(v[k].w));
+                    dst[tx + k * XT] = make_uint4(xf(v[k].x), xf(v[k].y), xf(v[k].z), xf(v[k].w));
                 }
                 fence_proxy_async();                            // generic-proxy writes -> the tensor core's async-proxy reads
                 mbar_arrive(&full_xf[s]);
             }
         }
     } else {
+        // sum / norm, correctly rounded, without the division subroutine: y = RN(1 / norm) from the host, q = RN(a y), then
+        // two residual corrections with exact remainders r = a - norm q (fma) -- the sequence IEEE division itself uses once
+        // range checks are out of the way (|a| < 2^31, 1 <= norm <= 66000: no overflow, underflow or subnormals; a = 0 gives +0)
+        const float nrm = a.norm, rn = a.rnorm;
+        auto div_norm = [nrm, rn](int v) {
+            const float x = (float)v;
+            float q = __fmul_rn(x, rn);
+            q = fmaf(fmaf(-nrm, q, x), rn, q);
+            return fmaf(fmaf(-nrm, q, x), rn, q);
+        };
         const int q4 = warp & 3;                                // TMEM lane quadrant this warp may read
-        const int row = q4 * 32 + lane;
+        float2 *stage = reinterpret_cast<float2 *>(reinterpret_cast<unsigned char *>(tmem_slot + 4) + (size_t)(warp - 2 - kCorrXfWarps) * kCorrOutBytes);
         const size_t ntri = (size_t)a.A * (a.A + 1) / 2;
         uint32_t n = 0;
         for (int u = blockIdx.x; u < a.n_units; u += gridDim.x, ++n) {
@@ -204,8 +217,7 @@ corr_kernel(const CorrArgs a, const __grid_constant__ CUtensorMap tmap)
             const uint32_t b = n & 1u;
             mbar_wait(&tmem_full[b], (n >> 1) & 1u);
             tc_fence_after();
-            const int gi = I * kCorrTile + row;
-            float2 *out = a.vis + ((size_t)t * a.C + c) * ntri + (size_t)gi * (gi + 1) / 2;
+            float2 *mat = a.vis + ((size_t)t * a.C + c) * ntri;
             for (int cj = 0; cj < 4; ++cj) {
                 if (I == J && cj > q4) break;                   // above the diagonal for every row of this warp
                 uint32_t re[32], im[32];
@@ -213,14 +225,18 @@ corr_kernel(const CorrArgs a, const __grid_constant__ CUtensorMap tmap)
                 tmem_ld32(taddr, re);
                 tmem_ld32(taddr + 128u, im);
                 asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-                if (gi < a.A) {
+                // a lane holds 32 columns of ONE row; the matrix wants a warp to write 32 consecutive columns of a row
+                // (256 contiguous bytes = 8 full sectors per store instead of 32 partial ones): transpose through shared memory
 #pragma unroll
-                    for (int k = 0; k < 32; ++k) {
-                        const int gj = J * kCorrTile + cj * 32 + k;
-                        if (gj <= gi)
-                            out[gj] = make_float2(__fdiv_rn((float)(int)re[k], a.norm), __fdiv_rn((float)(int)im[k], a.norm));
-                    }
+                for (int k = 0; k < 32; ++k) stage[lane * 33 + k] = make_float2(div_norm((int)re[k]), div_norm((int)im[k]));
+                __syncwarp();
+                const int gj = J * kCorrTile + cj * 32 + lane;
+#pragma unroll 8
+                for (int r = 0; r < 32; ++r) {
+                    const int gi = I * kCorrTile + q4 * 32 + r;
+                    if (gi < a.A && gj <= gi) mat[(size_t)gi * (gi + 1) / 2 + gj] = stage[r * 33 + lane];
                 }
+                __syncwarp();
             }
             tc_fence_before();
             mbar_arrive(&tmem_empty[b]);
@@ -259,6 +275,7 @@ extern "C" int blink_correlate(const int8_t *volt, int F, int A, int Ns, int n_t
     a.nk = (kbytes + kCorrChunk - 1) / kCorrChunk;
     a.last_ksteps = (kbytes - (a.nk - 1) * kCorrChunk + 31) / 32;
     a.norm = (float)((long long)n_t * n_avg);
+    a.rnorm = (float)(1.0 / (double)((long long)n_t * n_avg));
     a.vis = reinterpret_cast<float2 *>(vis);
     CUtensorMap tmap;
     // volt as bytes: [F][A][T][2 n_t], innermost first {2 n_t, T, A, F}; a box = 128 bytes x 1 interval x 128 inputs x 1 channel
