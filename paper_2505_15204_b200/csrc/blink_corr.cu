@@ -186,8 +186,9 @@ corr_kernel(const CorrArgs a, const __grid_constant__ CUtensorMap tmap)
                 for (int k = 0; k < XV; ++k) {                   // (re, im) -> (-im, re); same swizzled slot
                     auto xf = [](uint32_t w) {                 // bytes (r0, i0, r1, i1) -> (-i0, r0, -i1, r1)
                         const uint32_t sw = __byte_perm(w, 0u, 0x2301);                   // (i0, r0, i1, r1)
-                        const uint32_t n = ~sw;                                           // -x = ~x + 1 per byte, no carry across bytes
-                        const uint32_t neg = ((n & 0x7F7F7F7Fu) + 0x01010101u) ^ (n & 0x80808080u);
+                        // -x = ~x + 1 on bytes 0 and 2: with bytes 1 and 3 cleared first, each +1 carries at most into the
+                        // cleared byte above it and is masked away
+                        const uint32_t neg = (~sw & 0x00FF00FFu) + 0x00010001u;
                         return (neg & 0x00FF00FFu) | (sw & 0xFF00FF00u);
                     };
                     dst[tx + k * XT] = make_uint4(xf(v[k].x), xf(v[k].y), xf(v[k].z), xf(v[k].w));
