@@ -172,6 +172,9 @@ def test_conv_config3_full_size_sampled(bk, oracle_mod):
     """BASELINE.json config 3 at full size in the launch configuration bench.py --conv times (S = 5): wsum of every
     (t,c) exact, sampled images within tolerance, centre-pixel closed form for every image."""
     from paper_2505_15204_b200 import workloads
+    import gc
+    gc.collect()
+    torch.cuda.empty_cache()
     free, _ = torch.cuda.mem_get_info()
     if free < 60e9:
         pytest.skip("needs ~50 GB of device memory")

@@ -80,9 +80,12 @@ def test_correlate_one_second_sampled(bk, oracle_mod):
     10000 samples, 20 ms x 40 kHz -> 50 x 768 matrices of 32896 entries.  Sampled (t, c) against the oracle bit for bit,
     autocorrelations real and positive everywhere."""
     from paper_2505_15204_b200 import workloads
+    import gc
+    gc.collect()
+    torch.cuda.empty_cache()                                      # memory cached by earlier tests of the session
     free, _ = torch.cuda.mem_get_info()
-    if free < 120e9:
-        pytest.skip("needs ~100 GB of device memory (generation included)")
+    if free < 70e9:
+        pytest.skip("needs ~60 GB of device memory (generation included)")
     F, A, Ns, n_t, n_avg = 3072, 256, 10000, 200, 4
     volt = torch.empty((F, A, Ns, 2), dtype=torch.int8, device="cuda")
     for f0 in range(0, F, 256):
