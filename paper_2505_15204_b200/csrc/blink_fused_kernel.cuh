@@ -304,12 +304,16 @@ fused_image_kernel(const FusedArgs a, const __grid_constant__ ScaleBlock sc, con
                 // S taps of one column.  (Measured: fp32 atomicAdd on shared memory is a load + CAS spin loop per scalar on
                 // sm_100, yet an optimistic batch of 64-bit CAS on the (re, im) pairs -- S loads, S CAS in flight, retry only
                 // on interference -- was 1.4x (S = 5) to 2.1x (S = 7) SLOWER than the plain per-scalar adds below.)
+                // Odd lanes add the imaginary part first: one warp-wide atomic then touches even AND odd banks (the real parts
+                // alone live in the 16 even banks), which cuts the expected bank conflicts of 32 unrelated rows.
+                const int odd = lane & 1;
                 auto add_taps = [&](float2 *col, int row0, int dir, float ar, float ai) {
+                    const float first = odd ? ai : ar, second = odd ? ar : ai;
 #pragma unroll
                     for (int i = 0; i < S; ++i) {
-                        const int o = xsw(row0 + dir * i);
-                        atomicAdd(&col[o].x, wy[i] * ar);
-                        atomicAdd(&col[o].y, wy[i] * ai);
+                        float *cell = reinterpret_cast<float *>(&col[xsw(row0 + dir * i)]);
+                        atomicAdd(cell + odd, wy[i] * first);
+                        atomicAdd(cell + (odd ^ 1), wy[i] * second);
                     }
                 };
                 auto wx_of = [&](int jj) {                      // tap jj - R of the u axis (dynamic index: LDC)
