@@ -265,8 +265,12 @@ fused_image_kernel(const FusedArgs a, const __grid_constant__ ScaleBlock sc, con
                     if (sq.y >> 31) vv.y = -vv.y;
                     float2 *col = second ? c1 : c0;
                     const int o = xsw(iv + H);
-                    atomicAdd(&col[o].x, vv.x);
-                    atomicAdd(&col[o].y, vv.y);
+                    {                                           // odd lanes imaginary part first: even and odd banks per warp atomic
+                        const int odd = lane & 1;
+                        float *cell = reinterpret_cast<float *>(&col[o]);
+                        atomicAdd(cell + odd, odd ? vv.y : vv.x);
+                        atomicAdd(cell + (odd ^ 1), odd ? vv.x : vv.y);
+                    }
                     if (uniform) atomicAdd(second ? &n1[o] : &n0[o], 1u);
                     if (col0) {                                 // iu == 0: the conjugate lies in column 0 too
                         const int o2 = xsw(H - iv);
