@@ -47,6 +47,16 @@ def test_correlate_full_range_int8(bk, oracle_mod):
     _check(bk, oracle_mod, volt, 512, 2)
 
 
+def test_correlate_sums_beyond_2_24_and_many_tiles(bk, oracle_mod):
+    # full-range samples over 8192 x 2 accumulations: |sums| reach 2.6e8 > 2^24, so the int32 -> fp32 conversion rounds
+    # (identically on both sides) before the division; 520 inputs = 5 tile rows (15 tiles), the last one with 8 valid rows
+    from paper_2505_15204_b200 import workloads
+    volt = workloads.make_voltages(2, 520, 8192, seed=13, device="cuda", amp=90.0, lo=-127, hi=127)
+    _check(bk, oracle_mod, volt, 8192, 2)
+    ref_max = float(np.abs(oracle_mod.correlate(volt[:, :4].cpu().numpy(), 8192, 2)).max()) * 16384
+    assert ref_max > 2 ** 24
+
+
 def test_correlate_many_units(bk, oracle_mod):
     # 16 intervals x 48 channels x 3 tiles = 2304 units over 148 CTAs: stage ring and TMEM buffers wrap many times
     from paper_2505_15204_b200 import workloads
