@@ -323,6 +323,9 @@ def test_config3_full_size_sampled(bk, oracle_mod):
     cell indices of every (t,c,b) bit-exact, wsum of every (t,c) exact, 24 sampled images (spread over t and c,
     including the channels the dispersed transient crosses) within 1e-4 x peak, plus size-independent properties."""
     from paper_2505_15204_b200 import workloads
+    import gc
+    gc.collect()
+    torch.cuda.empty_cache()                                      # memory cached by earlier tests of the session
     free, _ = torch.cuda.mem_get_info()
     if free < 60e9:
         pytest.skip("needs ~50 GB of device memory")
@@ -446,6 +449,9 @@ def test_image_avg_config3_full_size(bk, oracle_mod):
     weight sums of all 38400 (t,c) exact; timestep 0's averaged image against the oracle's mean of its 768 images;
     every timestep against the mean of blink_image's own images."""
     from paper_2505_15204_b200 import workloads
+    import gc
+    gc.collect()
+    torch.cuda.empty_cache()                                      # memory cached by earlier tests of the session
     free, _ = torch.cuda.mem_get_info()
     if free < 60e9:
         pytest.skip("needs ~50 GB of device memory")
