@@ -69,6 +69,10 @@ def test_no_cpu_fallback_without_device(so_path):
     rc = L.blink_image(p, p, fr, 1, 1, 1, 4, 32, 0.01, 0, p, p, None, None, p, 64, None)
     assert rc == -4                                                      # BLINK_ERR_CUDA, and says why
     assert L.blink_last_cuda_error().decode() != ""
+    big = np.zeros(1 << 16, dtype=np.float32)
+    q = big.ctypes.data_as(ctypes.c_void_p)
+    assert L.blink_image_conv(q, q, fr, 1, 1, 1, 4, 256, 0.01, 5, 0.0, q, q, None, q, 1 << 18, None) == -4
+    assert L.blink_correlate(q, 2, 4, 128, 64, 1, q, None) == -4
 
 
 def test_conv_taps_host_logic_against_oracle(so_path, oracle_mod):
