@@ -16,9 +16,13 @@ def bk():
     return binding
 
 
-def _check(bk, oracle_mod, volt, n_t, n_avg):
-    vis = bk.blink_correlate(volt, n_t, n_avg)
-    torch.cuda.synchronize()
+def _check(bk, oracle_mod, volt, n_t, n_avg, path=0):
+    bk.set_option(bk.OPT_CORR_PATH, path)
+    try:
+        vis = bk.blink_correlate(volt, n_t, n_avg)
+        torch.cuda.synchronize()
+    finally:
+        bk.set_option(bk.OPT_CORR_PATH, 0)
     ref = oracle_mod.correlate(volt.cpu().numpy(), n_t, n_avg)
     got = vis.cpu().numpy()
     assert got.shape == ref.shape
@@ -55,6 +59,15 @@ def test_correlate_sums_beyond_2_24_and_many_tiles(bk, oracle_mod):
     _check(bk, oracle_mod, volt, 8192, 2)
     ref_max = float(np.abs(oracle_mod.correlate(volt[:, :4].cpu().numpy(), 8192, 2)).max()) * 16384
     assert ref_max > 2 ** 24
+
+
+@pytest.mark.parametrize("F,A,Ns,n_t,n_avg", [(8, 256, 1000, 200, 4), (4, 200, 1024, 64, 2), (48, 256, 16 * 64, 64, 1), (3, 129, 288, 72, 3)])
+def test_correlate_cluster_multicast(bk, oracle_mod, F, A, Ns, n_t, n_avg):
+    # BLINK_OPT_CORR_PATH = 2: 3-CTA clusters, one (t, c) matrix per cluster at a time, X_0 / X_1 loaded once by multicast TMA
+    # (129..256 inputs; other sizes fall back to the plain kernel); 768 matrices over <= 49 clusters wrap every ring many times
+    from paper_2505_15204_b200 import workloads
+    volt = workloads.make_voltages(F, A, Ns, seed=17 + A, device="cuda")
+    _check(bk, oracle_mod, volt, n_t, n_avg, path=2)
 
 
 def test_correlate_many_units(bk, oracle_mod):
