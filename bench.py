@@ -175,6 +175,7 @@ def main():
     ap.add_argument("--no-avg", action="store_true")
     ap.add_argument("--no-conv", action="store_true")
     ap.add_argument("--no-corr", action="store_true")
+    ap.add_argument("--no-cufft", action="store_true")
     ap.add_argument("--conv-support", type=int, default=5, help="support of the gridding kernel timed in conv_mode (3, 5, 7)")
     ap.add_argument("--T", type=int, default=None, help="reduce timesteps (debug only; invalidates the headline)")
     args = ap.parse_args()
@@ -278,6 +279,32 @@ def main():
             del ws_a, img_a
         except Exception as ex:  # report, never hide
             avg = {"error": str(ex)[:200]}
+
+    # ---- same-box context for the FFT step alone (the paper's FFT is the vendor library call, L194): cuFFT batched
+    # C2C inverse through torch.fft.ifft2 on already materialised grids; bench-only comparator, not linked into libblinkimg,
+    # not the oracle, no shift / normalisation / real part (those are extra passes for a library FFT)
+    cufft = None
+    if not args.no_cufft and rank == 0:
+        try:
+            nb = int(min(n_img, max(1, (4 << 30) // (N * N * 8))))
+            g = torch.randn((nb, N, N, 2), device=dev, dtype=torch.float32)
+            gc_ = torch.view_as_complex(g)
+            for _ in range(2):
+                torch.fft.ifft2(gc_)
+            torch.cuda.synchronize()
+            ef = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+            ef[0].record()
+            for _ in range(5):
+                out_f = torch.fft.ifft2(gc_)
+            ef[1].record()
+            torch.cuda.synchronize()
+            ms_f = ef[0].elapsed_time(ef[1]) / 5
+            cufft = {"api": "torch.fft.ifft2 (cuFFT batched C2C, complex64, out of place)", "batch": nb,
+                     "ms_per_batch": ms_f, "ms_per_step_extrapolated": ms_f * n_img / nb,
+                     "images_per_s": nb / (ms_f * 1e-3), "note": "FFT only, on materialised grids; context, not a target"}
+            del g, gc_, out_f
+        except Exception as ex:
+            cufft = {"error": str(ex)[:200]}
 
     # ---- convolutional gridding (blink_image_conv), same inputs and outputs -------------------
     conv = None
@@ -441,7 +468,7 @@ def main():
                    (w.vis.numel() * 8 / 1e9, n_img * N * N * 4 / 1e9),
                    "image_path": args.path, "parallelism": f"independent batches x{world}"},
         "gvis_per_s": value * B / 1e9,
-        "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu, "avg_mode": avg, "conv_mode": conv, "corr_mode": corr,
+        "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu, "avg_mode": avg, "conv_mode": conv, "corr_mode": corr, "cufft_context": cufft,
         "ms_per_step_each": per_step,
     }
     print(json.dumps(out))
