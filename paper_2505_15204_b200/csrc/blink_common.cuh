@@ -99,16 +99,19 @@ __device__ __forceinline__ int mirror_of(int cell, int n)
 // grid / counts by (tc - out_tc0) so that a chunk can land at the start of a workspace buffer.
 int grid_range(const float2 *vis, const float *uvw_m, const double *freqs_hz, double pixscale_rad, int T, int C,
                int P, int B, int n_pix, int weighting, int tc0, int ntc, int out_tc0, float2 *grid, float *wsum,
-               int32_t *cell_idx, uint32_t *counts, cudaStream_t st, bool half_only = false);
+               int32_t *cell_idx, uint32_t *counts, cudaStream_t st, bool half_only = false, int *row_extent = nullptr);
 bool grid_needs_global_counts(int B, int n_pix, int weighting);
 // hermitian: the grids come from the library's own gridders (G[-v][-u] = conj G[v][u], row / column -N/2 empty)
 // tw_generic: device array of n_pix complex64 (gfft_workspace_bytes) for sides that are not a power of two, else unused
+// row_extent (hermitian, generic sides only; written by grid_range): image i only has data in its rows v = 0 ..
+// row_extent[i / ext_div] - 1; the rows above are neither read nor transformed (they need not even be initialised)
 int fft2d_range(float2 *grid, int n_pix, int batch, const float *scale, int scale_div, int scale_img_base,
-                float *image, float *image_imag, cudaStream_t st, float2 *tw_generic = nullptr, bool hermitian = false);
+                float *image, float *image_imag, cudaStream_t st, float2 *tw_generic = nullptr, bool hermitian = false,
+                const int *row_extent = nullptr, int ext_div = 1);
 // image sides: even, 32..kMaxPix, only prime factors 2, 3, 5 (powers of two run the tuned kernels)
 bool size_supported(int n_pix);
 size_t gfft_workspace_bytes(int n_pix);
 int gfft2d_range(float2 *grid, int n, int batch, const float *scale, int scale_div, int img_base, float *image,
-                 float *image_imag, float2 *tw, cudaStream_t st, bool hermitian);
+                 float *image_imag, float2 *tw, cudaStream_t st, bool hermitian, const int *row_extent = nullptr, int ext_div = 1);
 
 }  // namespace blink

@@ -187,11 +187,12 @@ static int launch_fft2d(float2 *grid, int batch, const float *scale, int scale_d
 }
 
 int fft2d_range(float2 *grid, int n_pix, int batch, const float *scale, int scale_div, int img_base, float *image,
-                float *image_imag, cudaStream_t st, float2 *tw_generic, bool hermitian)
+                float *image_imag, cudaStream_t st, float2 *tw_generic, bool hermitian, const int *row_extent, int ext_div)
 {
     if (batch == 0) return BLINK_OK;
     if (!is_pow2(n_pix))
-        return size_supported(n_pix) ? gfft2d_range(grid, n_pix, batch, scale, scale_div, img_base, image, image_imag, tw_generic, st, hermitian)
+        return size_supported(n_pix) ? gfft2d_range(grid, n_pix, batch, scale, scale_div, img_base, image, image_imag, tw_generic, st, hermitian,
+                                                    row_extent, ext_div)
                                      : (int)BLINK_ERR_UNSUPPORTED;
     switch (n_pix) {
         case 32: return launch_fft2d<32>(grid, batch, scale, scale_div, img_base, image, image_imag, st);

@@ -156,9 +156,11 @@ __device__ __forceinline__ float2 *gfft_run(float2 *a, float2 *b, int nt, int ld
 template <int NN>
 __global__ void __launch_bounds__(kGRowThreads)
 gfft_rows_kernel(float2 *__restrict__ grid, long long n_rows, const GPlan pl, const float2 *__restrict__ tw, int nr, int rows_per_img,
-                 int row_off)
+                 int row_off, const int *__restrict__ ext, int ext_div)
 {
     // logical row L -> image L / rows_per_img, row row_off + L % rows_per_img (Hermitian grids: only the rows v >= 0)
+    // ext (optional): image i holds data only in its first ext[i / ext_div] logical rows; the others are all zero, so is
+    // their transform, and nobody reads them: they are skipped (not read, not written)
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int n = NN ? NN : pl.n, h = n / 2;
     float2 *a = reinterpret_cast<float2 *>(smem_raw), *b = a + (size_t)nr * n;
@@ -167,13 +169,22 @@ gfft_rows_kernel(float2 *__restrict__ grid, long long n_rows, const GPlan pl, co
     __syncthreads();
     for (long long base = (long long)blockIdx.x * nr; base < n_rows; base += (long long)gridDim.x * nr) {
         const int cnt = (int)(n_rows - base < nr ? n_rows - base : nr);
+        unsigned live = 0xffffffffu;                           // bit tr: row base + tr has to be transformed (same value in every thread)
+        if (ext != nullptr) {
+            live = 0u;
+            for (int tr = 0; tr < cnt; ++tr) {
+                const long long L = base + tr;
+                if ((int)(L % rows_per_img) < __ldg(ext + (L / rows_per_img) / ext_div)) live |= 1u << tr;
+            }
+            if (live == 0u) continue;
+        }
         for (int idx = threadIdx.x; idx < cnt * n; idx += kGRowThreads) {
             const int tr = idx / n, j = idx - tr * n;
             int q = j + h;                                     // transform index j lives in centred column (j + h) mod n
             if (q >= n) q -= n;
             const long long L = base + tr;
             const long long grow = (L / rows_per_img) * n + row_off + (L % rows_per_img);
-            a[(size_t)tr * n + j] = grid[grow * n + q];
+            a[(size_t)tr * n + j] = ((live >> tr) & 1u) ? grid[grow * n + q] : make_float2(0.f, 0.f);
         }
         __syncthreads();
         const float2 *res = gfft_run<NN>(a, b, cnt, n, pl, stw);
@@ -181,7 +192,7 @@ gfft_rows_kernel(float2 *__restrict__ grid, long long n_rows, const GPlan pl, co
             const int tr = idx / n, j = idx - tr * n;
             const long long L = base + tr;
             const long long grow = (L / rows_per_img) * n + row_off + (L % rows_per_img);
-            grid[grow * n + j] = res[(size_t)tr * n + j];                       // natural (unshifted) x order
+            if ((live >> tr) & 1u) grid[grow * n + j] = res[(size_t)tr * n + j];   // natural (unshifted) x order
         }
         __syncthreads();
     }
@@ -232,7 +243,7 @@ gfft_cols_kernel(const float2 *__restrict__ grid, const GPlan pl, const float2 *
 template <int NN>
 __global__ void __launch_bounds__(kGColThreads)
 gfft_cols_herm_kernel(const float2 *__restrict__ grid, const GPlan pl, const float2 *__restrict__ tw, int kc, const float *__restrict__ scale,
-                      int scale_div, int img_base, float *__restrict__ image)
+                      int scale_div, int img_base, float *__restrict__ image, const int *__restrict__ ext, int ext_div, int ext_base)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int n = NN ? NN : pl.n, h = n / 2, np = kc / 2;                // np column pairs = transforms per CTA
@@ -242,9 +253,11 @@ gfft_cols_herm_kernel(const float2 *__restrict__ grid, const GPlan pl, const flo
     for (int m = threadIdx.x; m < n; m += kGColThreads) stw[m] = tw[m];
     const int x0 = blockIdx.x * kc, img = blockIdx.y;
     const size_t img_off = (size_t)img * n * n;
+    const int vu = ext != nullptr ? __ldg(ext + (ext_base + img) / ext_div) : h;      // rows v >= vu are zero and are not read
     for (int idx = threadIdx.x; idx < h * np; idx += kGColThreads) {
         const int v = idx / np, p = idx - v * np;              // p fastest: consecutive 16-byte column pairs of one row
-        const float4 q = *reinterpret_cast<const float4 *>(grid + img_off + (size_t)(h + v) * n + x0 + 2 * p);
+        float4 q = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (v < vu) q = *reinterpret_cast<const float4 *>(grid + img_off + (size_t)(h + v) * n + x0 + 2 * p);
         a[(size_t)p * ld + v] = make_float2(q.x - q.w, q.y + q.z);                   // S1 + i S2
         if (v > 0) a[(size_t)p * ld + n - v] = make_float2(q.x + q.w, q.z - q.y);    // conj S1 + i conj S2
     }
@@ -280,7 +293,7 @@ bool size_supported(int n)
 size_t gfft_workspace_bytes(int n) { return is_pow2(n) ? 0 : align_up((size_t)n * sizeof(float2), 256); }
 
 int gfft2d_range(float2 *grid, int n, int batch, const float *scale, int scale_div, int img_base, float *image,
-                 float *image_imag, float2 *tw, cudaStream_t st, bool hermitian)
+                 float *image_imag, float2 *tw, cudaStream_t st, bool hermitian, const int *row_extent, int ext_div)
 {
     if (image_imag) hermitian = false;                          // the imaginary part is only defined for the general transform
     if (batch == 0) return BLINK_OK;
@@ -312,13 +325,15 @@ int gfft2d_range(float2 *grid, int n, int batch, const float *scale, int scale_d
     const int rows_per_img = hermitian ? n / 2 : n, row_off = hermitian ? n / 2 : 0;
     const long long n_rows = (long long)batch * rows_per_img;
     const long long want = (n_rows + nr - 1) / nr, cap = (long long)sm_count() * 8;
-    rows_k<<<(unsigned)(want < cap ? want : cap), kGRowThreads, nr * per + twb, st>>>(grid, n_rows, pl, tw, nr, rows_per_img, row_off);
+    rows_k<<<(unsigned)(want < cap ? want : cap), kGRowThreads, nr * per + twb, st>>>(grid, n_rows, pl, tw, nr, rows_per_img, row_off,
+                                                                                           hermitian ? row_extent : nullptr, ext_div);
     BLINK_LAUNCH_CHECK("gfft_rows_kernel");
     // Hermitian: kc columns are kc/2 transforms; keep two CTAs per SM when the arrays allow it
     int kch = 2;
     for (int c = 16; c >= 2; c >>= 1)
         if (n % c == 0 && (size_t)(c / 2) * per + twb <= 100 * 1024) { kch = c; break; }
     if (hermitian && (size_t)(kch / 2) * per > budget) hermitian = false;
+    if (!hermitian && row_extent) return BLINK_ERR_UNSUPPORTED;   // skipped rows are only defined for the Hermitian consumer (cannot happen: kch = 2 always fits)
     if (hermitian)
         BLINK_CUDA_TRY(cudaFuncSetAttribute(herm_k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)((kch / 2) * per + twb)));
     for (int b0 = 0; b0 < batch; b0 += 65535) {
@@ -326,7 +341,7 @@ int gfft2d_range(float2 *grid, int n, int batch, const float *scale, int scale_d
         if (hermitian)
             herm_k<<<dim3(n / kch, nb), kGColThreads, (kch / 2) * per + twb, st>>>(grid + (size_t)b0 * n * n, pl, tw, kch, scale,
                                                                                           scale_div, img_base + b0,
-                                                                                          image + (size_t)b0 * n * n);
+                                                                                          image + (size_t)b0 * n * n, row_extent, ext_div, b0);
         else
             cols_k<<<dim3(n / kc, nb), kGColThreads, kc * per + twb, st>>>(grid + (size_t)b0 * n * n, pl, tw, kc, scale, scale_div,
                                                                            img_base + b0, image + (size_t)b0 * n * n,

@@ -19,6 +19,8 @@ struct GridArgs {
     float2 *grid; float *wsum; int32_t *cell_idx; uint32_t *counts;     // wsum/cell_idx by absolute tc, grid/counts by tc - out_tc0
     int chunk_b, n_chunks, tile_cells, n_bands;
     int half_only;                                // the consumer only reads rows v >= 0 (Hermitian transform): skip the bands below
+    int *row_extent;                              // OPTIONAL [tc - out_tc0]: rows v = 0 .. row_extent-1 are the only ones the consumer has to read;
+                                                  // with half_only the (all-zero) bands above the last occupied one are not even stored
 };
 
 __global__ void __launch_bounds__(kGridThreads)
@@ -31,6 +33,7 @@ grid_tiles_kernel(const GridArgs a, const __grid_constant__ ScaleBlock sc)
     uint32_t *cur = off + a.n_bands + 1;                       // [n_bands]
     uint32_t *items = cur + a.n_bands;                         // [2 * chunk_b]
     __shared__ uint32_t red[kGridThreads / 32];
+    __shared__ int s_last;                                     // last band that holds a sample (-1: none)
 
     const int tc = a.tc0 + blockIdx.x;
     const int t = tc / a.C, c = tc - t * a.C;
@@ -52,6 +55,7 @@ grid_tiles_kernel(const GridArgs a, const __grid_constant__ ScaleBlock sc)
         const int b1 = min(B, b0 + a.chunk_b);
         // ---- phase 1: cell index of every baseline of the chunk, band histogram --------------------
         for (int i = threadIdx.x; i <= a.n_bands; i += kGridThreads) off[i] = 0;
+        if (threadIdx.x == 0) s_last = -1;
         __syncthreads();
         for (int b = b0 + threadIdx.x; b < b1; b += kGridThreads) {
             const int cell = cell_of(uvw[3 * b], uvw[3 * b + 1], s, n, h);
@@ -79,6 +83,12 @@ grid_tiles_kernel(const GridArgs a, const __grid_constant__ ScaleBlock sc)
             if (lane == 0) off[a.n_bands] = carry;
         }
         __syncthreads();
+        if (a.row_extent) {                                    // the occupied bands are mirror-symmetric: the last one bounds the rows v >= 0 in use
+            int mine = -1;
+            for (int i = threadIdx.x; i < a.n_bands; i += kGridThreads)
+                if (off[i + 1] > off[i]) mine = i;             // increasing i per thread
+            if (mine >= 0) atomicMax(&s_last, mine);
+        }
         // ---- phase 2: counting-sort the samples (and conjugates) by band ---------------------------
         for (int b = b0 + threadIdx.x; b < b1; b += kGridThreads) {
             const int cell = cell_of(uvw[3 * b], uvw[3 * b + 1], s, n, h);
@@ -97,6 +107,9 @@ grid_tiles_kernel(const GridArgs a, const __grid_constant__ ScaleBlock sc)
             const uint32_t k0 = off[band], k1 = off[band + 1];
             if (multi && ch > 0 && k0 == k1) continue;         // nothing to spill for this band (uniform branch)
             if (a.half_only && (size_t)(band + 1) * a.tile_cells <= (size_t)h * n) continue;   // rows v < 0 only: never read
+            // empty rows above the data are never read either; the band after the last occupied one is still stored because
+            // the last row in use may straddle the band boundary (bands are 8192 cells, not whole rows)
+            if (a.half_only && a.row_extent && band > s_last + 1) continue;
             for (int p = 0; p < a.P; ++p) {
                 for (int i = threadIdx.x; i < a.tile_cells; i += kGridThreads) {
                     tile[i] = make_float2(0.f, 0.f);
@@ -172,6 +185,17 @@ grid_tiles_kernel(const GridArgs a, const __grid_constant__ ScaleBlock sc)
             }
         }
     }
+    if (a.row_extent && threadIdx.x == 0) {
+        // rows v >= 0 (centred rows h .. h + extent - 1) that lie in bands 0 .. s_last; everything above is zero / not stored
+        int ext = h;
+        if (a.half_only) {
+            const long long last_cell = (long long)(s_last + 1) * a.tile_cells - 1;            // -1 when there is no sample at all
+            const long long r = last_cell < 0 ? -1 : last_cell / n;
+            ext = (int)(r - h + 1);
+            ext = ext < 0 ? 0 : (ext > h ? h : ext);
+        }
+        a.row_extent[otc] = ext;
+    }
     // ---- weight sum ----------------------------------------------------------------------------
     uint32_t val = uniform ? my_occ : my_in;
 #pragma unroll
@@ -219,7 +243,7 @@ bool grid_needs_global_counts(int B, int n_pix, int weighting)
 
 int grid_range(const float2 *vis, const float *uvw_m, const double *freqs_hz, double pixscale_rad, int T, int C, int P,
                int B, int n_pix, int weighting, int tc0, int ntc, int out_tc0, float2 *grid, float *wsum,
-               int32_t *cell_idx, uint32_t *counts, cudaStream_t st, bool half_only)
+               int32_t *cell_idx, uint32_t *counts, cudaStream_t st, bool half_only, int *row_extent)
 {
     (void)T;
     if (ntc <= 0) return BLINK_OK;
@@ -237,6 +261,7 @@ int grid_range(const float2 *vis, const float *uvw_m, const double *freqs_hz, do
     a.n_chunks = B > 0 ? (B + chunk - 1) / chunk : 1;
     if (a.n_chunks > 1 && weighting == BLINK_W_UNIFORM && counts == nullptr) return BLINK_ERR_WORKSPACE;
     a.half_only = (half_only && a.n_chunks == 1 && counts == nullptr) ? 1 : 0;
+    a.row_extent = row_extent;
     const size_t smem = grid_smem_bytes(a.tile_cells, a.n_bands, a.chunk_b);
     BLINK_CUDA_TRY(cudaFuncSetAttribute(grid_tiles_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     // sub-ranges that stay inside one timestep's block of <= 1024 channels (scales travel as a kernel parameter)

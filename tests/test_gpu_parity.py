@@ -601,6 +601,34 @@ def test_grid_and_image_non_pow2(bk, oracle_mod, n, weighting):
         _check_avg(bk, oracle_mod, w, True)
 
 
+@pytest.mark.parametrize("n,weighting,fill", [(240, 0, 0.2), (240, 1, 0.45), (360, 0, 0.07), (1200, 0, 0.3)])
+def test_non_pow2_row_extents_poisoned_workspace(bk, oracle_mod, n, weighting, fill):
+    """Sides that are not a power of two: the gridder reports how many rows v >= 0 of every (t,c) hold data and the
+    Hermitian transform skips the rest (never stored, never read).  The workspace is filled with NaN bit patterns first,
+    so a skipped row that IS read (or an extent that is too small) poisons the image; the channels span an octave, so
+    the extents differ from (t,c) to (t,c); one timestep has no baseline on the grid (W = 0, zero image) and one has a
+    single sample on the row v = 0."""
+    from paper_2505_15204_b200 import workloads
+    w = workloads.make_random(T=4, C=3, P=2, B=700, n_pix=n, weighting=weighting, seed=7000 + n + weighting, device="cuda", fill=fill)
+    w.freqs_hz = np.array([100e6, 150e6, 200e6])
+    uvw = w.uvw_m.clone()
+    uvw[2] = 1e7                                               # timestep 2: everything far off the grid
+    uvw[3, 1:] = 1e7                                           # timestep 3: one baseline, on the row v = 0
+    uvw[3, 0, 0], uvw[3, 0, 1] = 5.0, 0.0
+    w.uvw_m = uvw
+    rec, _ = bk.blink_workspace_bytes(bk.OP_IMAGE, w.T, w.C, w.P, w.B, n, weighting)
+    for nbytes in (rec, None):                                 # the recommended size, then a size that forces several chunks
+        if nbytes is None:
+            _, mn = bk.blink_workspace_bytes(bk.OP_IMAGE, w.T, w.C, w.P, w.B, n, weighting)
+            nbytes = mn + 4 * (rec - mn) // 12 // 256 * 256
+        ws = torch.full((nbytes // 4 + 4,), float("nan"), dtype=torch.float32, device="cuda").view(torch.uint8)[:max(nbytes, 16)]
+        res = bk.blink_image(w.vis, w.uvw_m, w.freqs_hz, n, w.pixscale_rad, weighting, workspace=ws)
+        torch.cuda.synchronize()
+        assert bool(torch.isfinite(res["image"]).all())
+        _check_images(bk, w, res, oracle_mod, [0, 5, 7, 10] if n == 1200 else None)
+        assert bool((res["image"][12:18] == 0).all()) and bool((res["wsum"][6:9] == 0).all())
+
+
 def test_image_1200_paper_size(bk, oracle_mod):
     """The paper's high-time-resolution image side (1200 x 1200): config-3 visibilities imaged at 1200,
     individually and channel-averaged, against the oracle."""
