@@ -19,12 +19,14 @@ size_t fused_conv_workspace_bytes(int T, int B, int n_pix, int ctas);           
 int counts_only(const float *uvw_m, const double *freqs_hz, double pixscale_rad, int T, int C, int B, int n_pix,
                 int tc0, int ntc, uint32_t *counts, cudaStream_t st);
 
+// sides that are not a power of two keep one row extent per (t,c) behind the grids (see image_device)
+static size_t ext_bytes(int n_pix) { return is_pow2(n_pix) ? 0 : 16; }
 static size_t unfused_bytes_per_tc(int P, int B, int n_pix, int weighting, bool have_counts)
 {
     const size_t n2 = (size_t)n_pix * n_pix;
     size_t b = (size_t)P * n2 * sizeof(float2);
     if (!have_counts && grid_needs_global_counts(B, n_pix, weighting)) b += n2 * sizeof(uint32_t);
-    return b + 16;                                             // + the (t,c)'s row extent (an int; 16 keeps the arrays aligned)
+    return b + ext_bytes(n_pix);                               // + the (t,c)'s row extent (an int; 16 keeps the arrays aligned)
 }
 
 static bool use_fused(int P, int B, int n_pix, int weighting)
@@ -57,12 +59,12 @@ static int image_device(const float2 *vis, const float *uvw_m, const double *fre
     workspace_bytes -= twb;
     const int chunk = (int)std::min<size_t>((size_t)ntc, workspace_bytes / per_tc);
     float2 *wgrid = static_cast<float2 *>(workspace);
-    const bool ws_counts = per_tc - 16 > (size_t)P * n2 * sizeof(float2);
+    const bool ws_counts = per_tc - ext_bytes(n_pix) > (size_t)P * n2 * sizeof(float2);
     uint32_t *wcounts = ws_counts ? reinterpret_cast<uint32_t *>(wgrid + (size_t)chunk * P * n2) : nullptr;
     // sides that are not a power of two: the gridder reports how many rows v >= 0 of each (t,c) hold data, and the
     // Hermitian transform neither reads nor transforms the rest (MWA-like uv coverage fills ~1/3 of a 1200 grid's rows)
     int *vrows = is_pow2(n_pix) ? nullptr
-                                : reinterpret_cast<int *>(static_cast<unsigned char *>(workspace) + (size_t)chunk * (per_tc - 16));
+                                : reinterpret_cast<int *>(static_cast<unsigned char *>(workspace) + (size_t)chunk * (per_tc - ext_bytes(n_pix)));
     for (int s = tc0; s < tc0 + ntc; s += chunk) {
         const int m = std::min(chunk, tc0 + ntc - s);
         // counts: caller's array (absolute index) or the workspace copy (chunk-relative)
