@@ -52,7 +52,8 @@ enum {
 
 /* Options for blink_set_option (process-wide tuning / test switches; defaults in brackets). */
 enum {
-    BLINK_OPT_IMAGE_PATH = 0,     /* [0] 0 = auto, 1 = force unfused (grid -> rows -> columns), 2 = force fused */
+    BLINK_OPT_IMAGE_PATH = 0,     /* [0] 0 = auto (fused where supported; batches of <= 8 Mi pixels take the unfused chain when the
+                                         workspace holds them), 1 = force unfused (grid -> rows -> columns), 2 = force fused */
     BLINK_OPT_FUSED_CTAS = 1,     /* [0] 0 = auto (one persistent CTA per SM), else CTAs for the fused kernel  */
     BLINK_OPT_GRID_CHUNK_B = 2,   /* [0] 0 = auto, else baselines per gridder chunk (tests the spill path)     */
     BLINK_OPT_AVG_WSUM = 3,       /* [0] blink_image_avg weight sums: 0 = auto, 1 = sort + binary search, 2 = ballot counting */

@@ -36,6 +36,13 @@ static bool use_fused(int P, int B, int n_pix, int weighting)
     return fused_supported(P, B, n_pix, weighting);
 }
 
+// auto path only: batches of at most 8 Mi pixels (128 images of 256^2, 32 of 512^2, 8 of 1024^2, 2 of 2048^2: the measured
+// cross-over of the two paths on a B200) go through the unfused chain
+static bool small_batch(int ntc, int P, int n_pix)
+{
+    return option(BLINK_OPT_IMAGE_PATH) == 0 && (size_t)ntc * P * n_pix * n_pix <= ((size_t)8 << 20);
+}
+
 static int image_device(const float2 *vis, const float *uvw_m, const double *freqs_hz, int T, int C, int P, int B,
                         int n_pix, double pixscale_rad, int weighting, int tc0, int ntc, float *image, float *wsum,
                         int32_t *cell_idx, uint32_t *counts, void *workspace, size_t workspace_bytes, cudaStream_t st,
@@ -44,7 +51,14 @@ static int image_device(const float2 *vis, const float *uvw_m, const double *fre
     // image / wsum / cell_idx / counts are indexed by ABSOLUTE tc; the range [tc0, tc0+ntc) is processed
     const size_t n2 = (size_t)n_pix * n_pix;
     if (cal.gains && !use_fused(P, B, n_pix, weighting)) return BLINK_ERR_UNSUPPORTED;   // gains are fused into the fused kernel only
-    if (use_fused(P, B, n_pix, weighting)) {
+    bool fused = use_fused(P, B, n_pix, weighting);
+    // A handful of images leaves most SMs idle under the fused kernel (one CTA per image: 144 us for ONE 256 x 256 image,
+    // config 1); the unfused chain spreads the rows and columns of an image over many CTAs (56 us).  Taken when the whole
+    // range fits the workspace as one chunk; otherwise the fused kernel runs as before.
+    if (fused && !cal.gains && small_batch(ntc, P, n_pix) &&
+        workspace_bytes >= gfft_workspace_bytes(n_pix) + (size_t)ntc * unfused_bytes_per_tc(P, B, n_pix, weighting, counts != nullptr))
+        fused = false;
+    if (fused) {
         int rc = fused_image(vis, uvw_m, freqs_hz, pixscale_rad, T, C, P, B, n_pix, weighting, tc0, ntc, image, wsum,
                              cell_idx, workspace, workspace_bytes, st, cal);
         if (rc != BLINK_OK) return rc;
@@ -149,6 +163,9 @@ extern "C" int blink_workspace_bytes(int op, int T, int C, int P, int B, int n_p
                 if (ctas <= 0) ctas = fused_default_ctas();
                 rec = fused_workspace_bytes(T, B, n_pix, ctas);
                 mn = fused_workspace_bytes(T, B, n_pix, 1);
+                const int ntc = op == BLINK_OP_IMAGE_HOST ? C : T * C;        // (t,c) per image_device call
+                if (small_batch(ntc, P, n_pix))                              // room for the small-batch route (see image_device)
+                    rec = std::max(rec, gfft_workspace_bytes(n_pix) + (size_t)ntc * unfused_bytes_per_tc(P, B, n_pix, weighting, false));
             } else {
                 const size_t per_tc = unfused_bytes_per_tc(P, B, n_pix, weighting, false);
                 mn = gfft_workspace_bytes(n_pix) + per_tc;

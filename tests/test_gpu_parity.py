@@ -136,7 +136,7 @@ def test_grid_collisions_single_cell(bk, oracle_mod):
 
 
 # --------------------------------------------------------------------------- blink_image
-@pytest.mark.parametrize("path", [0, 1])
+@pytest.mark.parametrize("path", [0, 1, 2])
 def test_image_config1_full(bk, oracle_mod, path):
     from paper_2505_15204_b200 import workloads
     w = workloads.make_config(1, device="cuda")
@@ -162,7 +162,7 @@ def test_image_config1_full(bk, oracle_mod, path):
 
 
 @pytest.mark.parametrize("cfg,T,C", [(2, 1, 3), (3, 2, 3), (4, 1, 2), (5, 1, 2)])
-@pytest.mark.parametrize("path", [0, 1])
+@pytest.mark.parametrize("path", [0, 1, 2])
 def test_image_reduced_configs(bk, oracle_mod, cfg, T, C, path):
     from paper_2505_15204_b200 import workloads
     w = workloads.make_config(cfg, device="cuda", T=T, C=C)
@@ -180,7 +180,7 @@ def test_image_reduced_configs(bk, oracle_mod, cfg, T, C, path):
 
 
 @pytest.mark.parametrize("weighting", [0, 1])
-@pytest.mark.parametrize("path", [0, 1])
+@pytest.mark.parametrize("path", [0, 1, 2])
 def test_image_random_ragged(bk, oracle_mod, weighting, path):
     # odd sizes everywhere: B not a multiple of anything, P = 3, off-grid samples, tiny workspace (forces chunking)
     from paper_2505_15204_b200 import workloads
@@ -565,6 +565,29 @@ def test_more_than_1024_channels(bk, oracle_mod, path):
     mean = res["image"].reshape(w.T, w.C, w.n_pix, w.n_pix).double().mean(dim=1)
     assert float((avg["image_avg"].double() - mean).abs().max() / mean.abs().max()) <= TOL
     assert torch.equal(avg["wsum"], res["wsum"])
+
+
+def test_small_batch_auto_route(bk, oracle_mod):
+    """Auto path, batches of <= 8 Mi pixels: the unfused chain when the workspace holds the whole range (recommended
+    size), the fused kernel when it does not (minimum size); both against the oracle, indices and weight sums bit-exact."""
+    from paper_2505_15204_b200 import workloads
+    for weighting in (0, 1):
+        w = workloads.make_config(1, device="cuda")
+        w.weighting = weighting
+        T, C, P, B = w.vis.shape
+        rec, mn = bk.blink_workspace_bytes(bk.OP_IMAGE, T, C, P, B, w.n_pix, weighting)
+        assert rec >= w.n_pix * w.n_pix * 8 and mn < rec
+        for nbytes in (rec, mn):
+            ws = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+            res = bk.blink_image(w.vis, w.uvw_m, w.freqs_hz, w.n_pix, w.pixscale_rad, weighting, want_cell_idx=True,
+                                 want_counts=True, workspace=ws)
+            torch.cuda.synchronize()
+            _check_images(bk, w, res, oracle_mod)
+            assert np.array_equal(res["cell_idx"].cpu().numpy(),
+                                  oracle_mod.cells(w.uvw_m.cpu().numpy(), w.freqs_hz, w.n_pix, w.pixscale_rad))
+            _, cn, _, _ = oracle_mod.grid_one(w.vis.cpu().numpy()[0, 0, 0], w.uvw_m.cpu().numpy()[0], w.freqs_hz[0], w.n_pix,
+                                              w.pixscale_rad, weighting)
+            assert np.array_equal(res["counts"].cpu().numpy().astype(np.uint32)[0], cn)
 
 
 # --------------------------------------------------------------------------- sides that are not a power of two
