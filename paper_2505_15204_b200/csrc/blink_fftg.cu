@@ -17,7 +17,22 @@ constexpr int kGRowThreads = 512, kGColThreads = 512;
 struct GPlan {
     int n, nst;
     int radix[16];
+    int toff[16];                                  // stage s reads its twiddles W_n^(k n / (P_s R_s)), k < P_s, at table[toff[s] + k]
 };
+
+// The N-entry table exp(2 pi i m / N) of the workspace is re-packed per CTA into one COMPACT run per stage (stage s: P_s
+// consecutive entries), because a warp of a stage reads the entries k * step for consecutive k: out of the full table that is
+// a stride of `step` complex numbers -- 16 at the radix-3 stage of 1200, i.e. every lane in the same bank (measured: 32
+// wavefronts per load, 19 % of the column kernel's shared-memory traffic); out of the compact run it is unit stride.
+__device__ __forceinline__ void stage_twiddles(float2 *__restrict__ stw, const float2 *__restrict__ tw, const GPlan &pl)
+{
+    int P = 1;
+    for (int s = 0; s < pl.nst; ++s) {
+        const int step = pl.n / (P * pl.radix[s]);
+        for (int k = threadIdx.x; k < P; k += blockDim.x) stw[pl.toff[s] + k] = tw[k * step];
+        P *= pl.radix[s];
+    }
+}
 
 __global__ void gfft_twiddle_kernel(float2 *tw, int n)
 {
@@ -69,7 +84,7 @@ __device__ __forceinline__ void gstage(const float2 *__restrict__ src, float2 *_
 {
     const int n = NN ? NN : n_rt, P = PP ? PP : p_rt;
     if constexpr (NN != 0 && PP != 0) {
-        constexpr int nb = NN / R, step = NN / (PP * R);
+        constexpr int nb = NN / R;
         for (int idx = threadIdx.x; idx < nt * nb; idx += blockDim.x) {
             const int tr = idx / nb, i = idx - tr * nb;
             const int k = i % PP;
@@ -78,7 +93,7 @@ __device__ __forceinline__ void gstage(const float2 *__restrict__ src, float2 *_
 #pragma unroll
             for (int r = 0; r < R; ++r) x[r] = s[r * nb];
             if constexpr (PP > 1) {
-                const float2 w1 = tw[k * step];
+                const float2 w1 = tw[k];                       // compact per-stage run (stage_twiddles)
                 x[1] = cmul(x[1], w1);
                 if constexpr (R >= 3) {
                     const float2 w2 = cmul(w1, w1);
@@ -97,7 +112,7 @@ __device__ __forceinline__ void gstage(const float2 *__restrict__ src, float2 *_
         }
         return;
     }
-    const int nb = n / R, step = n / (P * R);
+    const int nb = n / R;
     const float inv_nb = 1.0f / (float)nb, inv_p = 1.0f / (float)P;
     for (int idx = threadIdx.x; idx < nt * nb; idx += blockDim.x) {
         const int tr = fdiv_small(idx, nb, inv_nb), i = idx - tr * nb;
@@ -107,7 +122,7 @@ __device__ __forceinline__ void gstage(const float2 *__restrict__ src, float2 *_
 #pragma unroll
         for (int r = 0; r < R; ++r) x[r] = s[r * nb];
         if (P > 1) {                                           // one table read per butterfly; w^2.. are products (<= 2 extra roundings)
-            const float2 w1 = tw[k * step];
+            const float2 w1 = tw[k];                           // compact per-stage run (stage_twiddles)
             x[1] = cmul(x[1], w1);
             if constexpr (R >= 3) {
                 const float2 w2 = cmul(w1, w1);
@@ -131,20 +146,21 @@ template <int NN>
 __device__ __forceinline__ float2 *gfft_run(float2 *a, float2 *b, int nt, int ld, const GPlan &pl, const float2 *tw)
 {
     if constexpr (NN == 1200) {                                // 5 * 5 * 3 * 4 * 4, the plan gfft2d_range builds for 1200
-        gstage<5, 1200, 1>(a, b, nt, 1200, ld, 1, tw);   __syncthreads();
-        gstage<5, 1200, 5>(b, a, nt, 1200, ld, 5, tw);   __syncthreads();
-        gstage<3, 1200, 25>(a, b, nt, 1200, ld, 25, tw); __syncthreads();
-        gstage<4, 1200, 75>(b, a, nt, 1200, ld, 75, tw); __syncthreads();
-        gstage<4, 1200, 300>(a, b, nt, 1200, ld, 300, tw); __syncthreads();
+        gstage<5, 1200, 1>(a, b, nt, 1200, ld, 1, tw);   __syncthreads();               // toff = 0, 1, 6, 31, 106 (gfft2d_range)
+        gstage<5, 1200, 5>(b, a, nt, 1200, ld, 5, tw + 1);   __syncthreads();
+        gstage<3, 1200, 25>(a, b, nt, 1200, ld, 25, tw + 6); __syncthreads();
+        gstage<4, 1200, 75>(b, a, nt, 1200, ld, 75, tw + 31); __syncthreads();
+        gstage<4, 1200, 300>(a, b, nt, 1200, ld, 300, tw + 106); __syncthreads();
         return b;
     }
     int P = 1;
     for (int s = 0; s < pl.nst; ++s) {
         const int R = pl.radix[s];
-        if (R == 4) gstage<4>(a, b, nt, pl.n, ld, P, tw);
-        else if (R == 2) gstage<2>(a, b, nt, pl.n, ld, P, tw);
-        else if (R == 3) gstage<3>(a, b, nt, pl.n, ld, P, tw);
-        else gstage<5>(a, b, nt, pl.n, ld, P, tw);
+        const float2 *tws = tw + pl.toff[s];
+        if (R == 4) gstage<4>(a, b, nt, pl.n, ld, P, tws);
+        else if (R == 2) gstage<2>(a, b, nt, pl.n, ld, P, tws);
+        else if (R == 3) gstage<3>(a, b, nt, pl.n, ld, P, tws);
+        else gstage<5>(a, b, nt, pl.n, ld, P, tws);
         __syncthreads();
         float2 *t = a; a = b; b = t;
         P *= R;
@@ -165,7 +181,7 @@ gfft_rows_kernel(float2 *__restrict__ grid, long long n_rows, const GPlan pl, co
     const int n = NN ? NN : pl.n, h = n / 2;
     float2 *a = reinterpret_cast<float2 *>(smem_raw), *b = a + (size_t)nr * n;
     float2 *stw = b + (size_t)nr * n;                          // the twiddle table, staged once per CTA
-    for (int m = threadIdx.x; m < n; m += kGRowThreads) stw[m] = tw[m];
+    stage_twiddles(stw, tw, pl);
     __syncthreads();
     for (long long base = (long long)blockIdx.x * nr; base < n_rows; base += (long long)gridDim.x * nr) {
         const int cnt = (int)(n_rows - base < nr ? n_rows - base : nr);
@@ -209,7 +225,7 @@ gfft_cols_kernel(const float2 *__restrict__ grid, const GPlan pl, const float2 *
     const int ld = n + 1;                                      // odd leading dimension: the kc columns of a row fall in different banks
     float2 *a = reinterpret_cast<float2 *>(smem_raw), *b = a + (size_t)kc * ld;
     float2 *stw = b + (size_t)kc * ld;
-    for (int m = threadIdx.x; m < n; m += kGColThreads) stw[m] = tw[m];
+    stage_twiddles(stw, tw, pl);
     const int x0 = blockIdx.x * kc, img = blockIdx.y;
     const size_t img_off = (size_t)img * n * n;
     for (int idx = threadIdx.x; idx < n * kc; idx += kGColThreads) {
@@ -243,14 +259,15 @@ gfft_cols_kernel(const float2 *__restrict__ grid, const GPlan pl, const float2 *
 template <int NN>
 __global__ void __launch_bounds__(kGColThreads)
 gfft_cols_herm_kernel(const float2 *__restrict__ grid, const GPlan pl, const float2 *__restrict__ tw, int kc, const float *__restrict__ scale,
-                      int scale_div, int img_base, float *__restrict__ image, const int *__restrict__ ext, int ext_div, int ext_base)
+                      int scale_div, int img_base, float *__restrict__ image, const int *__restrict__ ext, int ext_div, int ext_base, int ld)
 {
+    // ld (herm_ld): the leading dimension that makes the transposing accesses below -- lane -> (row v + lane / np, pair lane % np),
+    // address pair * ld + row -- fall into every bank exactly twice (the minimum for 8-byte words)
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int n = NN ? NN : pl.n, h = n / 2, np = kc / 2;                // np column pairs = transforms per CTA
-    const int ld = n + 1;
     float2 *a = reinterpret_cast<float2 *>(smem_raw), *b = a + (size_t)np * ld;
     float2 *stw = b + (size_t)np * ld;
-    for (int m = threadIdx.x; m < n; m += kGColThreads) stw[m] = tw[m];
+    stage_twiddles(stw, tw, pl);
     const int x0 = blockIdx.x * kc, img = blockIdx.y;
     const size_t img_off = (size_t)img * n * n;
     const int vu = ext != nullptr ? __ldg(ext + (ext_base + img) / ext_div) : h;      // rows v >= vu are zero and are not read
@@ -290,6 +307,13 @@ bool size_supported(int n)
     while (n % 5 == 0) n /= 5;
     return n == 1;
 }
+// leading dimension of the Hermitian column kernel's arrays for np transforms per CTA: np * (ld mod 16) = 32 (mod 16 banks of
+// 8 bytes) spreads the np x (32 / np) lanes of a transposing access over all banks; np <= 2 needs nothing but keeps the odd pad
+static int herm_ld(int n, int np)
+{
+    const int want = np == 4 ? 8 : np == 8 ? 4 : 1;
+    return n + (want - n % 16 + 16) % 16;
+}
 size_t gfft_workspace_bytes(int n) { return is_pow2(n) ? 0 : align_up((size_t)n * sizeof(float2), 256); }
 
 int gfft2d_range(float2 *grid, int n, int batch, const float *scale, int scale_div, int img_base, float *image,
@@ -306,9 +330,10 @@ int gfft2d_range(float2 *grid, int n, int batch, const float *scale, int scale_d
     while (m % 4 == 0) { pl.radix[pl.nst++] = 4; m /= 4; }
     while (m % 2 == 0) { pl.radix[pl.nst++] = 2; m /= 2; }
     if (m != 1) return BLINK_ERR_UNSUPPORTED;
+    for (int s = 0, P = 1, off = 0; s < pl.nst; ++s) { pl.toff[s] = off; off += P; P *= pl.radix[s]; }   // sum of P_s < n: fits the n-entry array
     gfft_twiddle_kernel<<<(n + 255) / 256, 256, 0, st>>>(tw, n);
     BLINK_LAUNCH_CHECK("gfft_twiddle_kernel");
-    const size_t per = 2 * (size_t)(n + 1) * sizeof(float2);    // ping + pong of one transform (padded leading dimension)
+    const size_t per = 2 * (size_t)(n + 16) * sizeof(float2);   // ping + pong of one transform (padded leading dimension: n + 1, or herm_ld)
     const size_t twb = (size_t)n * sizeof(float2);              // + the twiddle table staged in shared memory
     const size_t budget = 200 * 1024 - twb;
     int nr = (int)std::min<size_t>(2, budget / per);
@@ -341,7 +366,8 @@ int gfft2d_range(float2 *grid, int n, int batch, const float *scale, int scale_d
         if (hermitian)
             herm_k<<<dim3(n / kch, nb), kGColThreads, (kch / 2) * per + twb, st>>>(grid + (size_t)b0 * n * n, pl, tw, kch, scale,
                                                                                           scale_div, img_base + b0,
-                                                                                          image + (size_t)b0 * n * n, row_extent, ext_div, b0);
+                                                                                          image + (size_t)b0 * n * n, row_extent, ext_div, b0,
+                                                                                          herm_ld(n, kch / 2));
         else
             cols_k<<<dim3(n / kc, nb), kGColThreads, kc * per + twb, st>>>(grid + (size_t)b0 * n * n, pl, tw, kc, scale, scale_div,
                                                                            img_base + b0, image + (size_t)b0 * n * n,
