@@ -55,6 +55,14 @@ def test_host_only_calls(so_path):
     # sides that are not a power of two need an N-entry twiddle table for the mixed-radix transform
     rec, mn = bk.blink_workspace_bytes(bk.OP_FFT2D, 1, 1, 1, 0, 1200, 0)
     assert rec == mn == 1200 * 8 + (-1200 * 8) % 256
+    # ... and blink_image at such a side keeps one row extent (16 bytes) per (t,c) behind the chunk's grids
+    twb = rec
+    rec, mn = bk.blink_workspace_bytes(bk.OP_IMAGE, 2, 768, 1, 8128, 1200, 0)
+    assert mn == twb + 1200 * 1200 * 8 + 16 and rec == twb + 256 * (1200 * 1200 * 8 + 16)
+    # small batches (<= 8 Mi pixels, auto path): the recommended size also holds the whole range for the unfused chain
+    for n, n_img in ((256, 128), (512, 32), (1024, 8), (2048, 2)):
+        rec, mn = bk.blink_workspace_bytes(bk.OP_IMAGE, 1, n_img, 1, 8128, n, 0)
+        assert rec >= n_img * n * n * 8 and mn <= rec
 
 
 def test_no_cpu_fallback_without_device(so_path):
