@@ -650,6 +650,15 @@ def test_non_pow2_row_extents_poisoned_workspace(bk, oracle_mod, n, weighting, f
         assert bool(torch.isfinite(res["image"]).all())
         _check_images(bk, w, res, oracle_mod, [0, 5, 7, 10] if n == 1200 else None)
         assert bool((res["image"][12:18] == 0).all()) and bool((res["wsum"][6:9] == 0).all())
+    if n <= 360:
+        # with the caller's counts array the gridder stores every band (no half plane, full extents): same images, exact counts
+        res = bk.blink_image(w.vis, w.uvw_m, w.freqs_hz, n, w.pixscale_rad, weighting, want_counts=True)
+        torch.cuda.synchronize()
+        _check_images(bk, w, res, oracle_mod)
+        vis, uvw = w.vis.cpu().numpy(), w.uvw_m.cpu().numpy()
+        for tc in (0, 4, 7, 9):
+            _, cn, _, _ = oracle_mod.grid_one(vis[tc // w.C, tc % w.C, 0], uvw[tc // w.C], w.freqs_hz[tc % w.C], n, w.pixscale_rad, weighting)
+            assert np.array_equal(res["counts"].cpu().numpy().astype(np.uint32)[tc], cn)
 
 
 def test_image_1200_paper_size(bk, oracle_mod):
