@@ -16,6 +16,7 @@ namespace blink {
 // 480 threads per column CTA: the 960 radix-5 butterflies of its 4 transforms are exactly 2 rounds (measured best of 400 ... 608
 // once the bank conflicts were gone: 14.4 vs 14.9 ms per 1536 images of 1200^2 at 512)
 constexpr int kGRowThreads = 512, kGColThreads = 480;
+constexpr int kGRowsMax = 2;                       // rows per round of a row-pass CTA
 struct GPlan {
     int n, nst;
     int radix[16];
@@ -187,30 +188,38 @@ gfft_rows_kernel(float2 *__restrict__ grid, long long n_rows, const GPlan pl, co
     __syncthreads();
     for (long long base = (long long)blockIdx.x * nr; base < n_rows; base += (long long)gridDim.x * nr) {
         const int cnt = (int)(n_rows - base < nr ? n_rows - base : nr);
-        unsigned live = 0xffffffffu;                           // bit tr: row base + tr has to be transformed (same value in every thread)
-        if (ext != nullptr) {
-            live = 0u;
-            for (int tr = 0; tr < cnt; ++tr) {
-                const long long L = base + tr;
-                if ((int)(L % rows_per_img) < __ldg(ext + (L / rows_per_img) / ext_div)) live |= 1u << tr;
+        // per row of this round (nr <= kGRowsMax): where it lives in the grid and whether it has to be transformed (bit tr of
+        // `live`, the same value in every thread).  The 64-bit divisions happen here, once per row -- inside the element loops
+        // below they were most of the kernel's instructions (ncu: 350 k thread instructions per 1200-point row).
+        float2 *grow[kGRowsMax];
+        unsigned live = 0u;
+#pragma unroll
+        for (int tr = 0; tr < kGRowsMax; ++tr) {
+            grow[tr] = grid;
+            if (tr < cnt) {
+                const long long L = base + tr, im = L / rows_per_img;
+                const int r = (int)(L - im * rows_per_img);
+                grow[tr] = grid + (im * n + row_off + r) * n;
+                if (ext == nullptr || r < __ldg(ext + im / ext_div)) live |= 1u << tr;
             }
-            if (live == 0u) continue;
         }
-        for (int idx = threadIdx.x; idx < cnt * n; idx += blockDim.x) {
-            const int tr = idx / n, j = idx - tr * n;
-            int q = j + h;                                     // transform index j lives in centred column (j + h) mod n
-            if (q >= n) q -= n;
-            const long long L = base + tr;
-            const long long grow = (L / rows_per_img) * n + row_off + (L % rows_per_img);
-            a[(size_t)tr * n + j] = ((live >> tr) & 1u) ? grid[grow * n + q] : make_float2(0.f, 0.f);
+        if (live == 0u) continue;
+#pragma unroll
+        for (int tr = 0; tr < kGRowsMax; ++tr) {
+            if (tr >= cnt) break;
+            const bool lv = (live >> tr) & 1u;
+            for (int j = threadIdx.x; j < n; j += blockDim.x) {
+                int q = j + h;                                 // transform index j lives in centred column (j + h) mod n
+                if (q >= n) q -= n;
+                a[(size_t)tr * n + j] = lv ? grow[tr][q] : make_float2(0.f, 0.f);
+            }
         }
         __syncthreads();
         const float2 *res = gfft_run<NN>(a, b, cnt, n, pl, stw);
-        for (int idx = threadIdx.x; idx < cnt * n; idx += blockDim.x) {
-            const int tr = idx / n, j = idx - tr * n;
-            const long long L = base + tr;
-            const long long grow = (L / rows_per_img) * n + row_off + (L % rows_per_img);
-            if ((live >> tr) & 1u) grid[grow * n + j] = res[(size_t)tr * n + j];   // natural (unshifted) x order
+#pragma unroll
+        for (int tr = 0; tr < kGRowsMax; ++tr) {
+            if (tr >= cnt || !((live >> tr) & 1u)) continue;
+            for (int j = threadIdx.x; j < n; j += blockDim.x) grow[tr][j] = res[(size_t)tr * n + j];   // natural (unshifted) x order
         }
         __syncthreads();
     }
@@ -273,8 +282,9 @@ gfft_cols_herm_kernel(const float2 *__restrict__ grid, const GPlan pl, const flo
     const int x0 = blockIdx.x * kc, img = blockIdx.y;
     const size_t img_off = (size_t)img * n * n;
     const int vu = ext != nullptr ? __ldg(ext + (ext_base + img) / ext_div) : h;      // rows v >= vu are zero and are not read
+    const int lg = 31 - __clz(np);                             // np is a power of two (gfft2d_range): shifts, not divisions
     for (int idx = threadIdx.x; idx < h * np; idx += blockDim.x) {
-        const int v = idx / np, p = idx - v * np;              // p fastest: consecutive 16-byte column pairs of one row
+        const int v = idx >> lg, p = idx & (np - 1);           // p fastest: consecutive 16-byte column pairs of one row
         float4 q = make_float4(0.f, 0.f, 0.f, 0.f);
         if (v < vu) q = *reinterpret_cast<const float4 *>(grid + img_off + (size_t)(h + v) * n + x0 + 2 * p);
         a[(size_t)p * ld + v] = make_float2(q.x - q.w, q.y + q.z);                   // S1 + i S2
@@ -289,7 +299,7 @@ gfft_cols_herm_kernel(const float2 *__restrict__ grid, const GPlan pl, const flo
         s = (w != 0.0f) ? 1.0f / w : 0.0f;
     }
     for (int idx = threadIdx.x; idx < n * np; idx += blockDim.x) {
-        const int j = idx / np, p = idx - j * np;
+        const int j = idx >> lg, p = idx & (np - 1);
         int y = j + h, x = x0 + 2 * p + h, x1 = x0 + 2 * p + 1 + h;      // fftshift of both axes
         if (y >= n) y -= n;
         if (x >= n) x -= n;
@@ -338,7 +348,7 @@ int gfft2d_range(float2 *grid, int n, int batch, const float *scale, int scale_d
     const size_t per = 2 * (size_t)(n + 16) * sizeof(float2);   // ping + pong of one transform (padded leading dimension: n + 1, or herm_ld)
     const size_t twb = (size_t)n * sizeof(float2);              // + the twiddle table staged in shared memory
     const size_t budget = 200 * 1024 - twb;
-    int nr = (int)std::min<size_t>(2, budget / per);
+    int nr = (int)std::min<size_t>(kGRowsMax, budget / per);
     int kc = 1;
     for (int c = 8; c >= 1; c >>= 1)
         if ((n / 2) % c == 0 && (size_t)c * per <= budget) { kc = c; break; }
