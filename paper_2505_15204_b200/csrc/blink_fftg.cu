@@ -305,8 +305,12 @@ gfft_cols_herm_kernel(const float2 *__restrict__ grid, const GPlan pl, const flo
         if (x >= n) x -= n;
         if (x1 >= n) x1 -= n;
         const float2 z = res[(size_t)p * ld + j];
-        image[img_off + (size_t)y * n + x] = z.x * s;
-        image[img_off + (size_t)y * n + x1] = z.y * s;
+        if ((h & 1) == 0) {                                    // x is even, x1 = x + 1 < n: one aligned 8-byte store
+            *reinterpret_cast<float2 *>(image + img_off + (size_t)y * n + x) = make_float2(z.x * s, z.y * s);
+        } else {
+            image[img_off + (size_t)y * n + x] = z.x * s;
+            image[img_off + (size_t)y * n + x1] = z.y * s;
+        }
     }
 }
 
