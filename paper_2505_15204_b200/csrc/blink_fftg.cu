@@ -239,8 +239,9 @@ gfft_cols_kernel(const float2 *__restrict__ grid, const GPlan pl, const float2 *
     stage_twiddles(stw, tw, pl);
     const int x0 = blockIdx.x * kc, img = blockIdx.y;
     const size_t img_off = (size_t)img * n * n;
+    const int lg = 31 - __clz(kc);                             // kc is a power of two (gfft2d_range): shifts, not divisions
     for (int idx = threadIdx.x; idx < n * kc; idx += blockDim.x) {
-        const int j = idx / kc, c = idx - j * kc;              // c fastest: kc consecutive columns of one row
+        const int j = idx >> lg, c = idx & (kc - 1);           // c fastest: kc consecutive columns of one row
         int r = j + h;                                         // transform index j lives in centred row (j + h) mod n
         if (r >= n) r -= n;
         a[(size_t)c * ld + j] = grid[img_off + (size_t)r * n + x0 + c];
@@ -253,7 +254,7 @@ gfft_cols_kernel(const float2 *__restrict__ grid, const GPlan pl, const float2 *
         s = (w != 0.0f) ? 1.0f / w : 0.0f;
     }
     for (int idx = threadIdx.x; idx < n * kc; idx += blockDim.x) {
-        const int j = idx / kc, c = idx - j * kc;
+        const int j = idx >> lg, c = idx & (kc - 1);
         int y = j + h, x = x0 + c + h;                         // fftshift of both axes
         if (y >= n) y -= n;
         if (x >= n) x -= n;
