@@ -192,6 +192,26 @@ def apply_gains(vis, gains, ant_pairs):
     return out
 
 
+def image_stokes_i(vis, uvw_m, freqs_hz, n_pix: int, pixscale_rad: float, weighting: int, tc_ids=None):
+    """vis [T][C][P][B] (P = 2: XX, YY; P = 4: XX, XY, YX, YY) -> ((I_XX + I_YY) / 2 float64 [n][N][N], wsum [n]); tc = t*C + c."""
+    v = _c64(vis)
+    uvw = np.ascontiguousarray(uvw_m, dtype=np.float32)
+    fr = np.ascontiguousarray(freqs_hz, dtype=np.float64)
+    T, C, P, B = v.shape
+    ids = np.ascontiguousarray(np.arange(T * C) if tc_ids is None else tc_ids, dtype=np.int64)
+    L = lib()
+    L.oracle_image_stokes_i.restype = ctypes.c_int
+    L.oracle_image_stokes_i.argtypes = [ctypes.c_void_p] * 3 + [ctypes.c_int] * 5 + [ctypes.c_double, ctypes.c_int,
+                                        ctypes.c_void_p, ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p]
+    out = np.empty((len(ids), n_pix, n_pix), dtype=np.float64)
+    wsum = np.empty(len(ids), dtype=np.float64)
+    rc = L.oracle_image_stokes_i(_p(v), _p(uvw), _p(fr), T, C, P, B, int(n_pix), float(pixscale_rad), int(weighting),
+                                 _p(ids), len(ids), _p(out), _p(wsum))
+    if rc != 0:
+        raise ValueError("oracle_image_stokes_i: P must be 2 or 4 and tc_ids inside the batch")
+    return out, wsum
+
+
 # ---- convolutional gridding (SURVEY 8(f) rank 2, DESIGN.md reading R16) ----------------------------------
 def _conv_protos():
     L = lib()

@@ -30,6 +30,8 @@
  *                                   closed form with an empty channel counted in the mean
  *   oracle_apply_gains            : identity for unit gains; pure phases rotate by phi_a1 - phi_a2; independent
  *                                   numpy evaluation; undoing a simulated corruption restores the image
+ *   oracle_image_stokes_i         : unit sources -> 1.0; YY = -XX -> 0; XX-only -> half the XX image; single-baseline
+ *                                   closed form; == the image of the averaged visibilities (linearity)
  * Nothing here is "parity unpinned".
  *
  * Build: gcc -O2 -ffp-contract=off -fPIC -shared -pthread -o liboracle.so blink_oracle.c -lm
@@ -402,6 +404,40 @@ int oracle_image_avg(const float *vis, const float *uvw_m, const double *freqs_h
     const double inv = 1.0 / (avg_time ? (double)T * C : (double)C);
     for (size_t k = 0; k < n_out * n2; ++k) out[k] *= inv;
     free(img);
+    return 0;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * Stokes I images ("BLINK currently images only the XX polarisation ... does not form Stokes I";
+ * L351 lists it as future work, reading R18): the plain definition --
+ * image the XX plane (p = 0) and the YY plane (p = P-1; P = 2: XX, YY; P = 4: XX, XY, YX, YY) of every (t, c) with
+ * oracle_image_one and take I = (I_XX + I_YY) / 2 pixel by pixel.  out [n_ids][N][N], wsum [n_ids] (the W the two
+ * planes share); tc_ids index (t, c) pairs, tc = t*C + c.
+ * Pins (tests/test_oracle_pins.py): unit sources in XX and YY -> 1.0 at the centre; YY = -XX -> zero image;
+ * XX-only signal -> half the XX image; a single baseline against the closed-form cosine of the mean visibility;
+ * equals one image of the averaged visibilities (linearity, evaluated through oracle_image_one independently).
+ * ---------------------------------------------------------------------------------------- */
+int oracle_image_stokes_i(const float *vis, const float *uvw_m, const double *freqs_hz,
+                          int T, int C, int P, int B, int n_pix, double pixscale_rad, int weighting,
+                          const int64_t *tc_ids, int n_ids, double *out, double *wsum)
+{
+    const size_t n2 = (size_t)n_pix * n_pix;
+    if (P != 2 && P != 4) return -1;
+    double *xx = (double *)malloc(sizeof(double) * n2), *yy = (double *)malloc(sizeof(double) * n2);
+    if (!xx || !yy) { free(xx); free(yy); return -1; }
+    for (int k = 0; k < n_ids; ++k) {
+        const int64_t tc = tc_ids[k];
+        const int t = (int)(tc / C), c = (int)(tc % C);
+        if (t < 0 || t >= T) { free(xx); free(yy); return -1; }
+        const float *vxx = vis + 2 * ((((size_t)t * C + c) * P + 0) * (size_t)B);
+        const float *vyy = vis + 2 * ((((size_t)t * C + c) * P + (P - 1)) * (size_t)B);
+        const float *uvw = uvw_m + (size_t)t * B * 3;
+        const double W = oracle_image_one(vxx, uvw, freqs_hz[c], B, n_pix, pixscale_rad, weighting, xx, NULL, NULL, NULL, NULL);
+        oracle_image_one(vyy, uvw, freqs_hz[c], B, n_pix, pixscale_rad, weighting, yy, NULL, NULL, NULL, NULL);
+        for (size_t q = 0; q < n2; ++q) out[(size_t)k * n2 + q] = 0.5 * (xx[q] + yy[q]);
+        wsum[k] = W;
+    }
+    free(xx); free(yy);
     return 0;
 }
 

@@ -515,3 +515,82 @@ def test_non_pow2_single_cell_closed_form_and_unit_source(oracle_mod):
     r = oracle_mod.image_one(np.ones(200, np.complex64), uvw, 150e6, n, 1.0 / n, 0)
     assert abs(r["image"][n // 2, n // 2] - 1.0) < 1e-12 and r["image"].max() <= r["image"][n // 2, n // 2] + 1e-12
     assert r["W"] == 2 * np.count_nonzero(r["cell_idx"] >= 0)
+
+
+# ---------------------------------------------------------------------------------------------
+# Stokes I images, I = (XX + YY) / 2 (reading R18)
+# ---------------------------------------------------------------------------------------------
+def _stokes_inputs(seed, P, B=60, N=32, T=2, C=2):
+    rng = np.random.default_rng(seed)
+    uvw = rng.uniform(-25, 25, (T, B, 3)).astype(np.float32)
+    vis = (rng.normal(size=(T, C, P, B)) + 1j * rng.normal(size=(T, C, P, B))).astype(np.complex64)
+    freqs = 150e6 + 1e6 * np.arange(C)
+    return vis, uvw, freqs, N, 1.0 / N
+
+
+@pytest.mark.parametrize("P", [2, 4])
+@pytest.mark.parametrize("weighting", [0, 1])
+def test_stokes_i_special_cases(oracle_mod, P, weighting):
+    vis, uvw, freqs, N, pix = _stokes_inputs(70 + P, P)
+    h = N // 2
+    # unit sources in XX and YY (whatever sits in XY / YX is ignored): exactly 1.0 at the phase centre
+    v1 = vis.copy()
+    v1[:, :, 0] = 1.0
+    v1[:, :, P - 1] = 1.0
+    img, W = oracle_mod.image_stokes_i(v1, uvw, freqs, N, pix, weighting)
+    assert np.all(np.abs(img[:, h, h] - 1.0) < 1e-12) and np.all(W > 0)
+    # YY = -XX: the two images cancel pixel by pixel
+    v2 = vis.copy()
+    v2[:, :, P - 1] = -v2[:, :, 0]
+    img, _ = oracle_mod.image_stokes_i(v2, uvw, freqs, N, pix, weighting)
+    assert np.max(np.abs(img)) < 1e-12
+    # signal in XX only: half the XX image, and W is the (t, c)'s weight sum
+    v3 = vis.copy()
+    v3[:, :, P - 1] = 0
+    img, W = oracle_mod.image_stokes_i(v3, uvw, freqs, N, pix, weighting, tc_ids=[3, 0])
+    for k, tc in enumerate([3, 0]):
+        t, c = divmod(tc, vis.shape[1])
+        r = oracle_mod.image_one(vis[t, c, 0], uvw[t], freqs[c], N, pix, weighting)
+        assert np.max(np.abs(img[k] - 0.5 * r["image"])) < 1e-13 and W[k] == r["W"]
+
+
+def test_stokes_i_single_baseline_closed_form(oracle_mod):
+    # one baseline on cell (ku, kv): I = (2 / W) |Vm| cos(2 pi (ku x' + kv y') / N + arg Vm) with Vm = (V_XX + V_YY) / 2, W = 2
+    N, ku, kv = 32, 5, -3
+    f = 150e6
+    s = float(oracle_mod.scale(f, N, 1.0 / N))
+    uvw = np.array([[[ku / s, kv / s, 0.0]]], dtype=np.float32)
+    vxx, vyy = 0.8 - 0.3j, -0.2 + 1.1j
+    vis = np.zeros((1, 1, 4, 1), dtype=np.complex64)
+    vis[0, 0, 0, 0], vis[0, 0, 3, 0] = vxx, vyy
+    vis[0, 0, 1, 0], vis[0, 0, 2, 0] = 9.0, -7.0j                      # XY, YX must not leak in
+    img, W = oracle_mod.image_stokes_i(vis, uvw, [f], N, 1.0 / N, 0)
+    assert W[0] == 2.0
+    vm = 0.5 * (np.complex64(vxx).astype(np.complex128) + np.complex64(vyy).astype(np.complex128))
+    want = _closed_form_single_cell(N, ku, kv, vm) / 2.0
+    assert np.max(np.abs(img[0] - want)) < 1e-12
+
+
+@pytest.mark.parametrize("weighting", [0, 1])
+def test_stokes_i_equals_image_of_mean_visibilities(oracle_mod, weighting):
+    # linearity: gridding, weighting (shared W and counts) and the transform are linear in V
+    vis, uvw, freqs, N, pix = _stokes_inputs(77, 2, B=200)
+    img, W = oracle_mod.image_stokes_i(vis, uvw, freqs, N, pix, weighting)
+    for tc in range(4):
+        t, c = divmod(tc, 2)
+        vm = (0.5 * (vis[t, c, 0].astype(np.complex128) + vis[t, c, 1].astype(np.complex128)))
+        # float64 mean visibilities through an independent numpy gridding + numpy.fft (the oracle takes complex64 inputs)
+        ci = oracle_mod.cells(uvw[t:t + 1], freqs[c:c + 1], N, pix)[0, 0]
+        g = np.zeros(N * N, dtype=np.complex128)
+        cnt = np.zeros(N * N)
+        ok = ci >= 0
+        mir = (N - ci[ok] // N) * N + (N - ci[ok] % N)
+        np.add.at(g, ci[ok], vm[ok]); np.add.at(g, mir, np.conj(vm[ok]))
+        np.add.at(cnt, ci[ok], 1); np.add.at(cnt, mir, 1)
+        if weighting == 1:
+            g[cnt > 0] /= cnt[cnt > 0]
+            Wn = np.count_nonzero(cnt)
+        else:
+            Wn = cnt.sum()
+        ref = np.fft.fftshift(np.fft.ifft2(np.fft.ifftshift(g.reshape(N, N)))).real * N * N / Wn
+        assert W[tc] == Wn and np.max(np.abs(img[tc] - ref)) < 1e-12 * max(1.0, np.max(np.abs(ref)))
