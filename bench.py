@@ -9,8 +9,10 @@ images of 512 x 512, 8128 baselines) -- the configuration the metric is quoted o
 
 Prints ONE JSON line.  value = dirty images/s (whole job), device-resident inputs; e2e = the same through
 blink_image_host() with pinned HOST buffers (H2D of visibilities and D2H of every image inside the timed
-region); roofline = algorithmic bytes (M36 = 36 N^2 + 8 B per image + 12 T B) / kernel time /
-measured HBM peak; cpu_baseline = the CPU oracle, as it stands, on a bounded sample.
+region); roofline = the bytes the fused implementation MUST move (M4 = 4 N^2 + 8 B per image + 12 T B: visibilities
+in, images out) / kernel time / measured HBM peak, with the SURVEY 8(d) contract models M36 / M20 as
+labelled companions; configs = short timed legs of BASELINE.json configs 1, 2, 4 (one timestep) and 5;
+cpu_baseline = the CPU oracle, as it stands, on a bounded sample.
 Multi-GPU (torchrun): every rank images its own independent batch ("replicas / independent shards",
 PAPER.md L150, L322: each second of observation is independent) -- weak scaling, no collective on the data path.
 """
@@ -162,6 +164,65 @@ def run_reference(args, rank: int):
         "gpu_launches": 0}))
 
 
+def timed_ms(run, steps, warmup, dev, world, flush=None):
+    """Mean device time of `run` (CUDA events on the current stream), max over ranks.  flush: a tensor larger than L2 that is
+    rewritten before every timed call (small workloads whose inputs and outputs would otherwise stay in L2)."""
+    for _ in range(warmup):
+        run()
+    torch.cuda.synchronize(dev)
+    tot = 0.0
+    if flush is None:
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(steps):
+            run()
+        e1.record()
+        torch.cuda.synchronize(dev)
+        tot = e0.elapsed_time(e1)
+    else:
+        for _ in range(steps):
+            flush.add_(1)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            run()
+            e1.record()
+            torch.cuda.synchronize(dev)
+            tot += e0.elapsed_time(e1)
+    return shard.max_over_ranks(tot / steps, device=dev)
+
+
+def config_leg(bk, cfg, T, dev, world, rank, steps, warmup, peak):
+    """One short timed leg of BASELINE.json config `cfg` through blink_image (device-resident inputs)."""
+    w = workloads.make_config(cfg, device=dev, T=T, seed=shard.rank_seed(cfg, rank))
+    Tn, C, P, B, N = w.T, w.C, w.P, w.B, w.n_pix
+    n_img = Tn * C * P
+    image = torch.empty((n_img, N, N), dtype=torch.float32, device=dev)
+    wsum = torch.empty(Tn * C, dtype=torch.float32, device=dev)
+    rec, _ = bk.blink_workspace_bytes(bk.OP_IMAGE, Tn, C, P, B, N, w.weighting)
+    ws = torch.empty(max(rec, 256), dtype=torch.uint8, device=dev)
+    run = lambda: bk.blink_image(w.vis, w.uvw_m, w.freqs_hz, N, w.pixscale_rad, w.weighting, image=image, workspace=ws, wsum=wsum)
+    small = n_img * N * N * 4 < (512 << 20)                     # outputs that would sit in the 126 MB L2: flush between calls
+    flush = torch.zeros(256 << 20, dtype=torch.uint8, device=dev) if small else None
+    l0 = bk.kernel_launches()
+    ms = timed_ms(run, steps, warmup, dev, world, flush)
+    launches = (bk.kernel_launches() - l0) // (steps + warmup)
+    mb = model_bytes(Tn, C, P, B, N)
+    shp = workloads.config_shape(cfg)
+    out = {"workload": f"config{cfg}: {Tn} of {shp['T']} timesteps x {C} channels x {P} pol = {n_img} images of {N}x{N}, {B} baselines, "
+                       f"{'natural' if w.weighting == 0 else 'uniform'} weighting",
+           "ms_per_step": ms, "images_per_s": world * n_img / (ms * 1e-3), "gvis_per_s": world * n_img * B / (ms * 1e-3) / 1e9,
+           "frac_M4": mb["M4"] / (ms * 1e-3) / 1e9 / peak, "model_speedup_M36": mb["M36"] / (ms * 1e-3) / 1e9 / peak,
+           "gpu_launches_per_step": int(launches), "l2": "flushed between timed calls (256 MB write)" if small else "outputs larger than L2; no flush"}
+    if cfg == 1:
+        out["us_per_image"] = ms * 1e3
+        out["note"] = "one image: launch-latency bound, fractions not meaningful (SURVEY 8(d))"
+    if Tn < shp["T"]:
+        out["ms_full_config_extrapolated"] = ms * shp["T"] / Tn
+    del image, ws, w
+    torch.cuda.empty_cache()
+    return out
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -177,6 +238,7 @@ def main():
     ap.add_argument("--no-corr", action="store_true")
     ap.add_argument("--no-paper-size", action="store_true")
     ap.add_argument("--no-cufft", action="store_true")
+    ap.add_argument("--no-configs", action="store_true", help="skip the timed legs of configs 1, 2, 4 (one timestep), 5")
     ap.add_argument("--conv-support", type=int, default=5, help="support of the gridding kernel timed in conv_mode (3, 5, 7)")
     ap.add_argument("--T", type=int, default=None, help="reduce timesteps (debug only; invalidates the headline)")
     args = ap.parse_args()
@@ -206,7 +268,7 @@ def main():
     image = torch.empty((n_img, N, N), dtype=torch.float32, device=dev)
     wsum = torch.empty(T * C, dtype=torch.float32, device=dev)
     rec, mn = bk.blink_workspace_bytes(bk.OP_IMAGE, T, C, P, B, N, w.weighting)
-    ws = torch.empty(max(rec, 16), dtype=torch.uint8, device=dev)
+    ws = torch.empty(max(rec, 256), dtype=torch.uint8, device=dev)
 
     def step():
         bk.blink_image(w.vis, w.uvw_m, w.freqs_hz, N, w.pixscale_rad, w.weighting, image=image, workspace=ws, wsum=wsum)
@@ -238,14 +300,10 @@ def main():
     barrier()
     launches = bk.kernel_launches() - launches0
     clocks = sampler.stop() if rank == 0 else None
-    total_ms = ev[0].elapsed_time(ev[-1])
     per_step = [ev[k].elapsed_time(ev[k + 1]) for k in range(args.steps)]
-    tmax = torch.tensor([total_ms], device=dev)
-    if world > 1:
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-    total_ms = float(tmax.item())
+    total_ms = shard.max_over_ranks(ev[0].elapsed_time(ev[-1]), device=dev)      # slowest rank
     ms_per_step = total_ms / args.steps
-    value = world * n_img / (ms_per_step * 1e-3)
+    value = shard.aggregate_rate(n_img, world, ms_per_step)                      # whole job: every rank imaged n_img
 
     # ---- channel-averaged images (blink_image_avg), same inputs, device-resident -------
     avg = None
@@ -441,7 +499,7 @@ def main():
             img_h = torch.empty((n_img, N, N), dtype=torch.float32, pin_memory=True)
             wsum_h = torch.empty(T * C, dtype=torch.float32, pin_memory=True)
             rec_h, _ = bk.blink_workspace_bytes(bk.OP_IMAGE_HOST, T, C, P, B, N, w.weighting)
-            del image
+            image = None                                          # config 3's 40 GB of device images: not needed any more
             torch.cuda.empty_cache()
             ws_h = torch.empty(rec_h, dtype=torch.uint8, device=dev)
             e_steps = max(1, min(args.steps, 3))
@@ -463,6 +521,21 @@ def main():
         except Exception as ex:  # report, never hide
             e2e = {"value": None, "unit": "images/s", "error": str(ex)[:200]}
 
+    # ---- the other configs, driver-timed (1, 2 and 5 whole; 4 = one of its 10 timesteps, 51.5 GB of images) ----
+    configs = None
+    if not args.no_configs and args.T is None and args.path == 0:
+        image = None
+        del ws
+        torch.cuda.empty_cache()
+        configs = {}
+        for cfg, Tc in ((1, None), (2, None), (4, 1), (5, None)):
+            if cfg == args.config:
+                continue
+            try:
+                configs[f"config{cfg}"] = config_leg(bk, cfg, Tc, dev, world, rank, max(3, min(args.steps, 10)), args.warmup, hbm_peak()[0])
+            except Exception as ex:  # report, never hide
+                configs[f"config{cfg}"] = {"error": str(ex)[:200]}
+
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -471,17 +544,26 @@ def main():
     mb = model_bytes(T, C, P, B, N)
     peak, peak_src = hbm_peak()
     kern_ms = float(np.mean(per_step))
-    achieved = mb["M36"] / (kern_ms * 1e-3) / 1e9
+    fused = args.path != 1
+    # The fused kernel never materialises the uv grid, so the bytes it MUST move are M4 (visibilities in, images out); the
+    # unfused chain (--path 1) really moves M36.  M36 / M20 of SURVEY 8(d) stay as labelled model-speedup numbers.
+    model = "M4" if fused else "M36"
+    achieved = mb[model] / (kern_ms * 1e-3) / 1e9
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "traffic": None, "peak_source": peak_src,
-                "kernel": "blink_image step (all kernels of the step, CUDA events on the launch stream)",
-                "algorithmic_bytes_per_step": mb["M36"], "model": "M36 = n_img*(36 N^2 + 8 B) + 12 T B",
-                "frac_M20": mb["M20"] / (kern_ms * 1e-3) / 1e9 / peak, "frac_M4": mb["M4"] / (kern_ms * 1e-3) / 1e9 / peak,
+                "kernel": "fused_image_kernel (+ presort_kernel, < 0.1 % of the step): CUDA events on the launch stream over the timed region"
+                          if fused else "grid_tiles_kernel + fft_rows_kernel + fft_cols_kernel (CUDA events on the launch stream)",
+                "algorithmic_bytes_per_step": mb[model],
+                "model": ("M4 = n_img*(4 N^2 + 8 B) + 12 T B: visibilities and uvw read once, images written (the grid never reaches HBM)"
+                          if fused else "M36 = n_img*(36 N^2 + 8 B) + 12 T B (SURVEY 8(d): grid written, read and rewritten by two passes)"),
+                "frac_M4": mb["M4"] / (kern_ms * 1e-3) / 1e9 / peak,
+                "model_speedup_M36": mb["M36"] / (kern_ms * 1e-3) / 1e9 / peak,
+                "model_speedup_M20": mb["M20"] / (kern_ms * 1e-3) / 1e9 / peak,
                 "kernel_ms": kern_ms,
-                "note": "M36 is SURVEY 8(d)'s contract model (grid written, read and rewritten by two passes); the fused kernel never "
-                        "materialises the grid, so frac exceeds 1 by construction -- frac_M4 (compulsory: visibilities in, images out) "
-                        "and traffic (ncu DRAM bytes) are the honest companions"}
-    prof = os.path.join(ROOT, "profiles", "traffic.csv")      # DRAM bytes per step from the committed ncu capture
+                "note": "frac is against the compulsory bytes of the implementation timed.  model_speedup_M36 / _M20 divide SURVEY 8(d)'s "
+                        "contract models (three unfused kernels / gridder fused into the row pass) by the same time and peak: values above 1 "
+                        "mean traffic the fusion removed, they are not roofline fractions."}
+    prof = os.path.join(ROOT, "profiles", "traffic.csv")      # stored ncu figures of a committed capture (NOT measured by this run)
     if os.path.exists(prof):
         try:
             import csv
@@ -489,7 +571,11 @@ def main():
             for row in csv.DictReader(open(prof)):
                 if row["key"] == key and args.T is None:
                     roofline["traffic"] = int(row["dram_bytes_per_step"])
+                    roofline["traffic_is"] = "STORED ncu figure (dram__bytes_read.sum + dram__bytes_write.sum of one --set full capture), not measured by this run"
                     roofline["traffic_source"] = row["source"]
+                    roofline["traffic_over_algorithmic"] = int(row["dram_bytes_per_step"]) / mb[model]
+                    if row.get("limiter"):
+                        roofline["limiter_stored_ncu"] = row["limiter"]
         except Exception:
             pass
     if avg and "hbm_gbs" in avg:
@@ -508,7 +594,7 @@ def main():
                    (w.vis.numel() * 8 / 1e9, n_img * N * N * 4 / 1e9),
                    "image_path": args.path, "parallelism": f"independent batches x{world}"},
         "gvis_per_s": value * B / 1e9,
-        "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu, "avg_mode": avg, "conv_mode": conv, "paper_size_mode": paper, "corr_mode": corr, "cufft_context": cufft,
+        "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu, "avg_mode": avg, "conv_mode": conv, "paper_size_mode": paper, "corr_mode": corr, "cufft_context": cufft, "configs": configs,
         "ms_per_step_each": per_step,
     }
     print(json.dumps(out))

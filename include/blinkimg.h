@@ -41,7 +41,7 @@ typedef struct blink_c64 { float re, im; } blink_c64;       /* == float2 == comp
 
 enum { BLINK_W_NATURAL = 0, BLINK_W_UNIFORM = 1 };
 enum { BLINK_OP_GRID = 0, BLINK_OP_FFT2D = 1, BLINK_OP_IMAGE = 2, BLINK_OP_IMAGE_HOST = 3, BLINK_OP_IMAGE_AVG = 4,
-       BLINK_OP_IMAGE_CONV = 5 };
+       BLINK_OP_IMAGE_CONV = 5, BLINK_OP_IMAGE_STOKES_I = 6 };
 enum {
     BLINK_OK = 0,
     BLINK_ERR_INVALID_ARG = -1,   /* NULL / misaligned pointer, non-positive size, bad enum          */
@@ -50,7 +50,9 @@ enum {
     BLINK_ERR_CUDA        = -4    /* a CUDA runtime/driver call failed: see blink_last_cuda_error()   */
 };
 
-/* Options for blink_set_option (process-wide tuning / test switches; defaults in brackets). */
+/* Options for blink_set_option: tuning / test switches of the CALLING THREAD (thread-local; defaults in brackets).
+ * A call reads the options of the thread that issues it, so a switch set by one thread never changes the route of a
+ * call made by another; there is no process-wide mutable state besides the launch counter. */
 enum {
     BLINK_OPT_IMAGE_PATH = 0,     /* [0] 0 = auto (fused where supported; batches of <= 8 Mi pixels take the unfused chain when the
                                          workspace holds them), 1 = force unfused (grid -> rows -> columns), 2 = force fused */
@@ -217,6 +219,26 @@ int blink_conv_taps_host(double f, int support, double beta, float *w /* HOST [s
  * workspace.  BLINK_ERR_UNSUPPORTED for n_t not a multiple of 8 or below 64, A > 4096, n_t * n_avg > 66000.
  */
 int blink_correlate(const int8_t *volt, int F, int A, int Ns, int n_t, int n_avg, blink_c64 *vis, void *stream);
+/*
+ * Input-contract check for blink_correlate: *count (DEVICE, 8 bytes, written asynchronously on `stream`) = number of the
+ * n_bytes int8 samples at `volt` (16-byte aligned) that equal -128.  The correlator negates imaginary parts bytewise and
+ * -(-128) does not exist in int8, so such a sample silently corrupts the imaginary parts of its products; callers that
+ * cannot guarantee [-127, 127] run this first (one read of the voltages).
+ */
+int blink_volt_out_of_range(const int8_t *volt, size_t n_bytes, unsigned long long *count, void *stream);
+
+/*
+ * Stokes I dirty images (the paper images XX only and "does not form Stokes I"; L351 future work;
+ * DESIGN.md reading R18):  image[t*C + c] = (I_XX + I_YY) / 2  with I_XX, I_YY exactly blink_image's images of the planes
+ * p = 0 and p = P-1 of vis [T][C][P][B] (P = 2: XX, YY;  P = 4: XX, XY, YX, YY; other P: BLINK_ERR_INVALID_ARG).
+ * W and the uniform-weighting cell counts are shared by the planes of a (t,c), so the result is one image of the mean
+ * visibilities (V_XX + V_YY) / 2, which is how it is computed: half the work of imaging both planes.
+ *   image  out [T*C][N][N] float32;  wsum out [T*C];  other arguments as blink_image.
+ * `workspace` >= blink_workspace_bytes(BLINK_OP_IMAGE_STOKES_I) minimum, 256-byte aligned (holds the combined visibilities).
+ */
+int blink_image_stokes_i(const blink_c64 *vis, const float *uvw_m, const double *freqs_hz,
+                         int T, int C, int P, int B, int n_pix, double pixscale_rad, int weighting,
+                         float *image, float *wsum, void *workspace, size_t workspace_bytes, void *stream);
 
 #ifdef __cplusplus
 }

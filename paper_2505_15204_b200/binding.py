@@ -17,13 +17,14 @@ _SO = os.path.join(_HERE, "libblinkimg.so")
 _lib = None
 
 W_NATURAL, W_UNIFORM = 0, 1
-OP_GRID, OP_FFT2D, OP_IMAGE, OP_IMAGE_HOST, OP_IMAGE_AVG, OP_IMAGE_CONV = 0, 1, 2, 3, 4, 5
+OP_GRID, OP_FFT2D, OP_IMAGE, OP_IMAGE_HOST, OP_IMAGE_AVG, OP_IMAGE_CONV, OP_IMAGE_STOKES_I = 0, 1, 2, 3, 4, 5, 6
 OPT_IMAGE_PATH, OPT_FUSED_CTAS, OPT_GRID_CHUNK_B, OPT_AVG_WSUM, OPT_CORR_PATH = 0, 1, 2, 3, 4
 
 EXPORTS = ["blink_strerror", "blink_last_cuda_error", "blink_set_option", "blink_get_option",
            "blink_kernel_launches", "blink_workspace_bytes", "blink_grid", "blink_fft2d_inverse",
            "blink_image", "blink_image_host", "blink_image_avg", "blink_apply_gains", "blink_image_cal",
-           "blink_image_conv", "blink_conv_taps_host", "blink_correlate"]
+           "blink_image_conv", "blink_conv_taps_host", "blink_correlate", "blink_image_stokes_i",
+           "blink_volt_out_of_range"]
 
 
 class BlinkError(RuntimeError):
@@ -75,6 +76,10 @@ def lib():
         L.blink_conv_taps_host.argtypes = [d, i, d, vp, ctypes.POINTER(d)]
         L.blink_correlate.restype = i
         L.blink_correlate.argtypes = [vp, i, i, i, i, i, vp, vp]
+        L.blink_image_stokes_i.restype = i
+        L.blink_image_stokes_i.argtypes = [vp, vp, vp, i, i, i, i, i, d, i, vp, vp, vp, sz, vp]
+        L.blink_volt_out_of_range.restype = i
+        L.blink_volt_out_of_range.argtypes = [vp, sz, vp, vp]
         _lib = L
     return _lib
 
@@ -95,10 +100,36 @@ def _stream(device) -> ctypes.c_void_p:
     return ctypes.c_void_p(torch.cuda.current_stream(device).cuda_stream)
 
 
-def _dev(t: torch.Tensor, dtype, name: str) -> torch.Tensor:
-    if not t.is_cuda or t.dtype != dtype or not t.is_contiguous():
+def _dev(t: torch.Tensor, dtype, name: str, shape=None, device=None) -> torch.Tensor:
+    """Argument check only: contiguous CUDA tensor of the given dtype (and shape / device when stated)."""
+    if not isinstance(t, torch.Tensor) or not t.is_cuda or t.dtype != dtype or not t.is_contiguous():
         raise BlinkError(f"{name} must be a contiguous CUDA tensor of dtype {dtype}")
+    if shape is not None and tuple(t.shape) != tuple(shape):
+        raise BlinkError(f"{name} must have shape {tuple(shape)}, got {tuple(t.shape)}")
+    if device is not None and t.device != device:
+        raise BlinkError(f"{name} is on {t.device}, expected {device}")
     return t
+
+
+def _out(t: Optional[torch.Tensor], dtype, n_elems: int, name: str, device) -> None:
+    """Caller-supplied output / workspace: right device and dtype, contiguous, at least n_elems elements."""
+    if t is None:
+        return
+    if not t.is_cuda or t.device != device or t.dtype != dtype or not t.is_contiguous() or t.numel() < n_elems:
+        raise BlinkError(f"{name} must be a contiguous {dtype} tensor on {device} with at least {n_elems} elements")
+
+
+def _vis_uvw(vis: torch.Tensor, uvw_m: torch.Tensor, freqs_hz):
+    """vis [T][C][P][B] complex64 and uvw_m [T][B][3] float32 on one device, len(freqs_hz) == C."""
+    _dev(vis, torch.complex64, "vis")
+    if vis.dim() != 4:
+        raise BlinkError(f"vis must be [T][C][P][B], got {tuple(vis.shape)}")
+    T, C, P, B = vis.shape
+    _dev(uvw_m, torch.float32, "uvw_m", (T, B, 3), vis.device)
+    fr = _freqs(freqs_hz)
+    if fr.ndim != 1 or fr.shape[0] != C:
+        raise BlinkError(f"freqs_hz must hold C = {C} frequencies, got shape {fr.shape}")
+    return T, C, P, B, fr, vis.device
 
 
 def set_option(key: int, value: int) -> None:
@@ -124,10 +155,8 @@ def _freqs(freqs_hz) -> np.ndarray:
 def blink_grid(vis: torch.Tensor, uvw_m: torch.Tensor, freqs_hz, n_pix: int, pixscale_rad: float, weighting: int = 0,
                want_cell_idx: bool = False, want_counts: bool = False, grid: Optional[torch.Tensor] = None):
     """vis [T][C][P][B] complex64, uvw_m [T][B][3] float32 (CUDA) -> dict(grid, wsum, cell_idx?, counts?)"""
-    _dev(vis, torch.complex64, "vis"); _dev(uvw_m, torch.float32, "uvw_m")
-    T, C, P, B = vis.shape
-    fr = _freqs(freqs_hz)
-    dev = vis.device
+    T, C, P, B, fr, dev = _vis_uvw(vis, uvw_m, freqs_hz)
+    _out(grid, torch.complex64, T * C * P * n_pix * n_pix, "grid", dev)
     if grid is None:
         grid = torch.empty((T * C * P, n_pix, n_pix), dtype=torch.complex64, device=dev)
     wsum = torch.empty(T * C, dtype=torch.float32, device=dev)
@@ -135,9 +164,10 @@ def blink_grid(vis: torch.Tensor, uvw_m: torch.Tensor, freqs_hz, n_pix: int, pix
     counts = torch.empty((T * C, n_pix, n_pix), dtype=torch.int32, device=dev) if want_counts else None
     rec, _ = blink_workspace_bytes(OP_GRID, T, C, P, B, n_pix, weighting)
     ws = torch.empty(max(rec, 16), dtype=torch.uint8, device=dev)
-    rc = lib().blink_grid(_ptr(vis), _ptr(uvw_m), fr.ctypes.data_as(ctypes.c_void_p), T, C, P, B, n_pix,
-                          float(pixscale_rad), int(weighting), _ptr(grid), _ptr(wsum), _ptr(cell_idx), _ptr(counts),
-                          _ptr(ws), ws.numel(), _stream(dev))
+    with torch.cuda.device(dev):
+        rc = lib().blink_grid(_ptr(vis), _ptr(uvw_m), fr.ctypes.data_as(ctypes.c_void_p), T, C, P, B, n_pix,
+                              float(pixscale_rad), int(weighting), _ptr(grid), _ptr(wsum), _ptr(cell_idx), _ptr(counts),
+                              _ptr(ws), ws.numel(), _stream(dev))
     _check(rc, "blink_grid")
     return dict(grid=grid, wsum=wsum, cell_idx=cell_idx, counts=counts)
 
@@ -146,74 +176,117 @@ def blink_fft2d_inverse(grid: torch.Tensor, scale: Optional[torch.Tensor] = None
                         want_imag: bool = False, image: Optional[torch.Tensor] = None):
     """grid [batch][N][N] complex64 (CUDA, CLOBBERED) -> dict(image float32, imag?)"""
     _dev(grid, torch.complex64, "grid")
-    batch, n, n2 = grid.shape
-    assert n == n2
+    if grid.dim() != 3 or grid.shape[1] != grid.shape[2]:
+        raise BlinkError(f"grid must be [batch][N][N], got {tuple(grid.shape)}")
+    batch, n, _ = grid.shape
     dev = grid.device
+    _out(image, torch.float32, batch * n * n, "image", dev)
     if image is None:
         image = torch.empty((batch, n, n), dtype=torch.float32, device=dev)
     imag = torch.empty((batch, n, n), dtype=torch.float32, device=dev) if want_imag else None
     if scale is not None:
-        _dev(scale, torch.float32, "scale")
+        _dev(scale, torch.float32, "scale", device=dev)
+        if scale_stride_div < 1 or scale.numel() < -(-batch // int(scale_stride_div)):
+            raise BlinkError("scale must hold ceil(batch / scale_stride_div) entries")
     rec, _ = blink_workspace_bytes(OP_FFT2D, batch, 1, 1, 0, n, 0)         # non-zero only for sides that are not 2^k
     ws = torch.empty(rec, dtype=torch.uint8, device=dev) if rec else None
-    rc = lib().blink_fft2d_inverse(_ptr(grid), n, batch, _ptr(scale), int(scale_stride_div), _ptr(image), _ptr(imag),
-                                   _ptr(ws), rec, _stream(dev))
+    with torch.cuda.device(dev):
+        rc = lib().blink_fft2d_inverse(_ptr(grid), n, batch, _ptr(scale), int(scale_stride_div), _ptr(image), _ptr(imag),
+                                       _ptr(ws), rec, _stream(dev))
     _check(rc, "blink_fft2d_inverse")
     return dict(image=image, imag=imag)
+
+
+def _image_outputs(T, C, P_out, n_pix, dev, image, wsum, name="image"):
+    _out(image, torch.float32, T * C * P_out * n_pix * n_pix, name, dev)
+    _out(wsum, torch.float32, T * C, "wsum", dev)
+    if image is None:
+        image = torch.empty((T * C * P_out, n_pix, n_pix), dtype=torch.float32, device=dev)
+    if wsum is None:
+        wsum = torch.empty(T * C, dtype=torch.float32, device=dev)
+    return image, wsum
+
+
+def _workspace(workspace, op, T, C, P, B, n_pix, weighting, dev):
+    if workspace is None:
+        rec, _ = blink_workspace_bytes(op, T, C, P, B, n_pix, weighting)
+        return torch.empty(max(rec, 256), dtype=torch.uint8, device=dev)
+    _out(workspace, torch.uint8, 0, "workspace", dev)
+    if workspace.data_ptr() % 256:
+        raise BlinkError("workspace must be 256-byte aligned")
+    return workspace
 
 
 def blink_image(vis: torch.Tensor, uvw_m: torch.Tensor, freqs_hz, n_pix: int, pixscale_rad: float, weighting: int = 0,
                 want_cell_idx: bool = False, want_counts: bool = False, image: Optional[torch.Tensor] = None,
                 workspace: Optional[torch.Tensor] = None, wsum: Optional[torch.Tensor] = None):
     """vis [T][C][P][B] complex64, uvw_m [T][B][3] float32 (CUDA) -> dict(image [T*C*P][N][N] float32, wsum, ...)"""
-    _dev(vis, torch.complex64, "vis"); _dev(uvw_m, torch.float32, "uvw_m")
-    T, C, P, B = vis.shape
-    fr = _freqs(freqs_hz)
-    dev = vis.device
-    if image is None:
-        image = torch.empty((T * C * P, n_pix, n_pix), dtype=torch.float32, device=dev)
-    if wsum is None:
-        wsum = torch.empty(T * C, dtype=torch.float32, device=dev)
+    T, C, P, B, fr, dev = _vis_uvw(vis, uvw_m, freqs_hz)
+    image, wsum = _image_outputs(T, C, P, n_pix, dev, image, wsum)
     cell_idx = torch.empty((T, C, B), dtype=torch.int32, device=dev) if want_cell_idx else None
     counts = torch.empty((T * C, n_pix, n_pix), dtype=torch.int32, device=dev) if want_counts else None
-    if workspace is None:
-        rec, _ = blink_workspace_bytes(OP_IMAGE, T, C, P, B, n_pix, weighting)
-        workspace = torch.empty(max(rec, 16), dtype=torch.uint8, device=dev)
-    rc = lib().blink_image(_ptr(vis), _ptr(uvw_m), fr.ctypes.data_as(ctypes.c_void_p), T, C, P, B, n_pix,
-                           float(pixscale_rad), int(weighting), _ptr(image), _ptr(wsum), _ptr(cell_idx), _ptr(counts),
-                           _ptr(workspace), workspace.numel(), _stream(dev))
+    workspace = _workspace(workspace, OP_IMAGE, T, C, P, B, n_pix, weighting, dev)
+    with torch.cuda.device(dev):
+        rc = lib().blink_image(_ptr(vis), _ptr(uvw_m), fr.ctypes.data_as(ctypes.c_void_p), T, C, P, B, n_pix,
+                               float(pixscale_rad), int(weighting), _ptr(image), _ptr(wsum), _ptr(cell_idx), _ptr(counts),
+                               _ptr(workspace), workspace.numel(), _stream(dev))
     _check(rc, "blink_image")
     return dict(image=image, wsum=wsum, cell_idx=cell_idx, counts=counts)
+
+
+def blink_image_stokes_i(vis: torch.Tensor, uvw_m: torch.Tensor, freqs_hz, n_pix: int, pixscale_rad: float,
+                         weighting: int = 0, image: Optional[torch.Tensor] = None,
+                         workspace: Optional[torch.Tensor] = None, wsum: Optional[torch.Tensor] = None):
+    """vis [T][C][P][B] with P = 2 (XX, YY) or 4 (XX, XY, YX, YY) -> dict(image [T*C][N][N] = (I_XX + I_YY) / 2, wsum)"""
+    T, C, P, B, fr, dev = _vis_uvw(vis, uvw_m, freqs_hz)
+    image, wsum = _image_outputs(T, C, 1, n_pix, dev, image, wsum)
+    workspace = _workspace(workspace, OP_IMAGE_STOKES_I, T, C, P, B, n_pix, weighting, dev)
+    with torch.cuda.device(dev):
+        rc = lib().blink_image_stokes_i(_ptr(vis), _ptr(uvw_m), fr.ctypes.data_as(ctypes.c_void_p), T, C, P, B, n_pix,
+                                        float(pixscale_rad), int(weighting), _ptr(image), _ptr(wsum),
+                                        _ptr(workspace), workspace.numel(), _stream(dev))
+    _check(rc, "blink_image_stokes_i")
+    return dict(image=image, wsum=wsum)
 
 
 def blink_image_avg(vis: torch.Tensor, uvw_m: torch.Tensor, freqs_hz, n_pix: int, pixscale_rad: float, weighting: int = 0,
                     avg_time: bool = False, image_avg: Optional[torch.Tensor] = None,
                     workspace: Optional[torch.Tensor] = None, wsum: Optional[torch.Tensor] = None):
     """Mean of the dirty images over channels (-> [T*P][N][N]) or over timesteps and channels (-> [P][N][N])."""
-    _dev(vis, torch.complex64, "vis"); _dev(uvw_m, torch.float32, "uvw_m")
-    T, C, P, B = vis.shape
-    fr = _freqs(freqs_hz)
-    dev = vis.device
+    T, C, P, B, fr, dev = _vis_uvw(vis, uvw_m, freqs_hz)
     n_out = P if avg_time else T * P
+    _out(image_avg, torch.float32, n_out * n_pix * n_pix, "image_avg", dev)
+    _out(wsum, torch.float32, T * C, "wsum", dev)
     if image_avg is None:
         image_avg = torch.empty((n_out, n_pix, n_pix), dtype=torch.float32, device=dev)
     if wsum is None:
         wsum = torch.empty(T * C, dtype=torch.float32, device=dev)
-    if workspace is None:
-        rec, _ = blink_workspace_bytes(OP_IMAGE_AVG, T, C, P, B, n_pix, weighting)
-        workspace = torch.empty(max(rec, 16), dtype=torch.uint8, device=dev)
-    rc = lib().blink_image_avg(_ptr(vis), _ptr(uvw_m), fr.ctypes.data_as(ctypes.c_void_p), T, C, P, B, n_pix,
-                               float(pixscale_rad), int(weighting), int(bool(avg_time)), _ptr(image_avg), _ptr(wsum),
-                               _ptr(workspace), workspace.numel(), _stream(dev))
+    workspace = _workspace(workspace, OP_IMAGE_AVG, T, C, P, B, n_pix, weighting, dev)
+    with torch.cuda.device(dev):
+        rc = lib().blink_image_avg(_ptr(vis), _ptr(uvw_m), fr.ctypes.data_as(ctypes.c_void_p), T, C, P, B, n_pix,
+                                   float(pixscale_rad), int(weighting), int(bool(avg_time)), _ptr(image_avg), _ptr(wsum),
+                                   _ptr(workspace), workspace.numel(), _stream(dev))
     _check(rc, "blink_image_avg")
     return dict(image_avg=image_avg, wsum=wsum)
 
 
+def _gains_pairs(gains: torch.Tensor, ant_pairs: torch.Tensor, C: int, P: int, B: int, dev):
+    _dev(gains, torch.complex64, "gains", device=dev)
+    if gains.dim() != 3 or gains.shape[0] != C or gains.shape[1] != P or gains.shape[2] < 1:
+        raise BlinkError(f"gains must be [C={C}][P={P}][A], got {tuple(gains.shape)}")
+    _dev(ant_pairs, torch.int32, "ant_pairs", (B, 2), dev)
+    return int(gains.shape[2])
+
+
 def blink_apply_gains(vis: torch.Tensor, gains: torch.Tensor, ant_pairs: torch.Tensor):
-    """In place: vis[t][c][p][b] *= gains[c][p][a1] * conj(gains[c][p][a2]); ant_pairs [B][2] int32 (CUDA)."""
-    _dev(vis, torch.complex64, "vis"); _dev(gains, torch.complex64, "gains"); _dev(ant_pairs, torch.int32, "ant_pairs")
+    """In place: vis[t][c][p][b] *= gains[c][p][a1] * conj(gains[c][p][a2]); ant_pairs [B][2] int32 (CUDA), 0 <= a < A."""
+    _dev(vis, torch.complex64, "vis")
+    if vis.dim() != 4:
+        raise BlinkError(f"vis must be [T][C][P][B], got {tuple(vis.shape)}")
     T, C, P, B = vis.shape
-    rc = lib().blink_apply_gains(_ptr(vis), _ptr(gains), _ptr(ant_pairs), T, C, P, B, gains.shape[2], _stream(vis.device))
+    A = _gains_pairs(gains, ant_pairs, C, P, B, vis.device)
+    with torch.cuda.device(vis.device):
+        rc = lib().blink_apply_gains(_ptr(vis), _ptr(gains), _ptr(ant_pairs), T, C, P, B, A, _stream(vis.device))
     _check(rc, "blink_apply_gains")
     return vis
 
@@ -222,21 +295,14 @@ def blink_image_cal(vis: torch.Tensor, uvw_m: torch.Tensor, freqs_hz, gains: tor
                     n_pix: int, pixscale_rad: float, weighting: int = 0, image: Optional[torch.Tensor] = None,
                     workspace: Optional[torch.Tensor] = None, wsum: Optional[torch.Tensor] = None):
     """blink_image with per-antenna gain corrections fused into the gridder's load (vis is left untouched)."""
-    _dev(vis, torch.complex64, "vis"); _dev(uvw_m, torch.float32, "uvw_m")
-    _dev(gains, torch.complex64, "gains"); _dev(ant_pairs, torch.int32, "ant_pairs")
-    T, C, P, B = vis.shape
-    fr = _freqs(freqs_hz)
-    dev = vis.device
-    if image is None:
-        image = torch.empty((T * C * P, n_pix, n_pix), dtype=torch.float32, device=dev)
-    if wsum is None:
-        wsum = torch.empty(T * C, dtype=torch.float32, device=dev)
-    if workspace is None:
-        rec, _ = blink_workspace_bytes(OP_IMAGE, T, C, P, B, n_pix, weighting)
-        workspace = torch.empty(max(rec, 16), dtype=torch.uint8, device=dev)
-    rc = lib().blink_image_cal(_ptr(vis), _ptr(uvw_m), fr.ctypes.data_as(ctypes.c_void_p), _ptr(gains), _ptr(ant_pairs),
-                               gains.shape[2], T, C, P, B, n_pix, float(pixscale_rad), int(weighting), _ptr(image),
-                               _ptr(wsum), _ptr(workspace), workspace.numel(), _stream(dev))
+    T, C, P, B, fr, dev = _vis_uvw(vis, uvw_m, freqs_hz)
+    A = _gains_pairs(gains, ant_pairs, C, P, B, dev)
+    image, wsum = _image_outputs(T, C, P, n_pix, dev, image, wsum)
+    workspace = _workspace(workspace, OP_IMAGE, T, C, P, B, n_pix, weighting, dev)
+    with torch.cuda.device(dev):
+        rc = lib().blink_image_cal(_ptr(vis), _ptr(uvw_m), fr.ctypes.data_as(ctypes.c_void_p), _ptr(gains), _ptr(ant_pairs),
+                                   A, T, C, P, B, n_pix, float(pixscale_rad), int(weighting), _ptr(image),
+                                   _ptr(wsum), _ptr(workspace), workspace.numel(), _stream(dev))
     _check(rc, "blink_image_cal")
     return dict(image=image, wsum=wsum)
 
@@ -245,21 +311,14 @@ def blink_image_conv(vis: torch.Tensor, uvw_m: torch.Tensor, freqs_hz, n_pix: in
                      beta: float = 0.0, image: Optional[torch.Tensor] = None, workspace: Optional[torch.Tensor] = None,
                      wsum: Optional[torch.Tensor] = None, want_cell_idx: bool = False):
     """blink_image with the Kaiser-Bessel gridding kernel of odd support 3 / 5 / 7 (natural weighting, grid-corrected)."""
-    _dev(vis, torch.complex64, "vis"); _dev(uvw_m, torch.float32, "uvw_m")
-    T, C, P, B = vis.shape
-    fr = _freqs(freqs_hz)
-    dev = vis.device
-    if image is None:
-        image = torch.empty((T * C * P, n_pix, n_pix), dtype=torch.float32, device=dev)
-    if wsum is None:
-        wsum = torch.empty(T * C, dtype=torch.float32, device=dev)
+    T, C, P, B, fr, dev = _vis_uvw(vis, uvw_m, freqs_hz)
+    image, wsum = _image_outputs(T, C, P, n_pix, dev, image, wsum)
     cell_idx = torch.empty((T, C, B), dtype=torch.int32, device=dev) if want_cell_idx else None
-    if workspace is None:
-        rec, _ = blink_workspace_bytes(OP_IMAGE_CONV, T, C, P, B, n_pix, 0)
-        workspace = torch.empty(max(rec, 16), dtype=torch.uint8, device=dev)
-    rc = lib().blink_image_conv(_ptr(vis), _ptr(uvw_m), fr.ctypes.data_as(ctypes.c_void_p), T, C, P, B, n_pix,
-                                float(pixscale_rad), int(support), float(beta), _ptr(image), _ptr(wsum), _ptr(cell_idx),
-                                _ptr(workspace), workspace.numel(), _stream(dev))
+    workspace = _workspace(workspace, OP_IMAGE_CONV, T, C, P, B, n_pix, 0, dev)
+    with torch.cuda.device(dev):
+        rc = lib().blink_image_conv(_ptr(vis), _ptr(uvw_m), fr.ctypes.data_as(ctypes.c_void_p), T, C, P, B, n_pix,
+                                    float(pixscale_rad), int(support), float(beta), _ptr(image), _ptr(wsum), _ptr(cell_idx),
+                                    _ptr(workspace), workspace.numel(), _stream(dev))
     _check(rc, "blink_image_conv")
     return dict(image=image, wsum=wsum, cell_idx=cell_idx)
 
@@ -273,32 +332,62 @@ def blink_conv_taps_host(f: float, support: int, beta: float = 0.0):
     return w, err.value
 
 
-def blink_correlate(volt: torch.Tensor, n_t: int, n_avg: int, vis: Optional[torch.Tensor] = None):
-    """volt [F][A][Ns][2] int8 (CUDA) -> vis [T][C][A(A+1)/2] complex64: lower-triangular CMAC products per interval / channel."""
+def blink_volt_out_of_range(volt: torch.Tensor) -> int:
+    """Number of int8 samples equal to -128 (outside blink_correlate's input contract [-127, 127]); synchronises."""
     _dev(volt, torch.int8, "volt")
-    F, A, Ns, two = volt.shape
-    if two != 2:
+    cnt = torch.zeros(1, dtype=torch.int64, device=volt.device)
+    with torch.cuda.device(volt.device):
+        rc = lib().blink_volt_out_of_range(_ptr(volt), volt.numel(), _ptr(cnt), _stream(volt.device))
+    _check(rc, "blink_volt_out_of_range")
+    return int(cnt.item())
+
+
+def blink_correlate(volt: torch.Tensor, n_t: int, n_avg: int, vis: Optional[torch.Tensor] = None, check_range: bool = False):
+    """volt [F][A][Ns][2] int8 (CUDA) -> vis [T][C][A(A+1)/2] complex64: lower-triangular CMAC products per interval / channel.
+
+    Input contract (include/blinkimg.h): every sample in [-127, 127].  The kernel negates imaginary parts bytewise, and
+    -(-128) does not exist in int8: a sample of -128 silently gives wrong imaginary parts.  check_range=True counts such
+    samples first (one extra pass over volt, synchronising) and raises."""
+    _dev(volt, torch.int8, "volt")
+    if volt.dim() != 4 or volt.shape[3] != 2:
         raise BlinkError("volt must be [F][A][Ns][2] int8")
+    F, A, Ns, _ = volt.shape
     if Ns % n_t or F % n_avg:
         raise BlinkError("Ns must be a multiple of n_t and F of n_avg")
+    if check_range and blink_volt_out_of_range(volt):
+        raise BlinkError("volt holds samples equal to -128: outside blink_correlate's input range [-127, 127]")
+    n_out = (Ns // n_t) * (F // n_avg) * (A * (A + 1) // 2)
+    _out(vis, torch.complex64, n_out, "vis", volt.device)
     if vis is None:
         vis = torch.empty((Ns // n_t, F // n_avg, A * (A + 1) // 2), dtype=torch.complex64, device=volt.device)
-    rc = lib().blink_correlate(_ptr(volt), F, A, Ns, int(n_t), int(n_avg), _ptr(vis), _stream(volt.device))
+    with torch.cuda.device(volt.device):
+        rc = lib().blink_correlate(_ptr(volt), F, A, Ns, int(n_t), int(n_avg), _ptr(vis), _stream(volt.device))
     _check(rc, "blink_correlate")
     return vis
 
 
 def blink_image_host(vis_host: torch.Tensor, uvw_host: torch.Tensor, freqs_hz, n_pix: int, pixscale_rad: float,
                      weighting: int, image_host: torch.Tensor, wsum_host: torch.Tensor, workspace: torch.Tensor):
-    """Host-buffer variant: vis_host / uvw_host / image_host / wsum_host are (pinned) CPU tensors."""
+    """Host-buffer variant: vis_host / uvw_host / image_host / wsum_host are (pinned) CPU tensors; workspace is a
+    256-byte aligned CUDA uint8 tensor of at least blink_workspace_bytes(OP_IMAGE_HOST) minimum bytes."""
+    if vis_host.dim() != 4:
+        raise BlinkError(f"vis_host must be [T][C][P][B], got {tuple(vis_host.shape)}")
     T, C, P, B = vis_host.shape
     fr = _freqs(freqs_hz)
-    for t, dt, nm in ((vis_host, torch.complex64, "vis_host"), (uvw_host, torch.float32, "uvw_host"),
-                      (image_host, torch.float32, "image_host"), (wsum_host, torch.float32, "wsum_host")):
-        if t.is_cuda or t.dtype != dt or not t.is_contiguous():
-            raise BlinkError(f"{nm} must be a contiguous CPU tensor of dtype {dt}")
-    rc = lib().blink_image_host(_ptr(vis_host), _ptr(uvw_host), fr.ctypes.data_as(ctypes.c_void_p), T, C, P, B, n_pix,
-                                float(pixscale_rad), int(weighting), _ptr(image_host), _ptr(wsum_host),
-                                _ptr(workspace), workspace.numel())
+    if fr.ndim != 1 or fr.shape[0] != C:
+        raise BlinkError(f"freqs_hz must hold C = {C} frequencies, got shape {fr.shape}")
+    for t, dt, nm, n in ((vis_host, torch.complex64, "vis_host", T * C * P * B), (uvw_host, torch.float32, "uvw_host", T * B * 3),
+                         (image_host, torch.float32, "image_host", T * C * P * n_pix * n_pix),
+                         (wsum_host, torch.float32, "wsum_host", T * C)):
+        if t.is_cuda or t.dtype != dt or not t.is_contiguous() or t.numel() < n:
+            raise BlinkError(f"{nm} must be a contiguous CPU tensor of dtype {dt} with at least {n} elements")
+    if tuple(uvw_host.shape) != (T, B, 3):
+        raise BlinkError(f"uvw_host must be [T][B][3], got {tuple(uvw_host.shape)}")
+    if not workspace.is_cuda or workspace.dtype != torch.uint8 or not workspace.is_contiguous() or workspace.data_ptr() % 256:
+        raise BlinkError("workspace must be a contiguous, 256-byte aligned CUDA uint8 tensor")
+    with torch.cuda.device(workspace.device):
+        rc = lib().blink_image_host(_ptr(vis_host), _ptr(uvw_host), fr.ctypes.data_as(ctypes.c_void_p), T, C, P, B, n_pix,
+                                    float(pixscale_rad), int(weighting), _ptr(image_host), _ptr(wsum_host),
+                                    _ptr(workspace), workspace.numel())
     _check(rc, "blink_image_host")
     return dict(image=image_host, wsum=wsum_host)

@@ -14,10 +14,11 @@ namespace blink {
 
 static thread_local char g_err[512] = "";
 static std::atomic<unsigned long long> g_launches{0};
-static std::atomic<int> g_opts[8];
+static thread_local int g_opts[8];                             // route / test switches of the CALLING thread
 static std::mutex g_init_mu;
-static int g_init_device = -1;
-static int g_sm_count = 0;
+constexpr int kMaxDevices = 64;
+static bool g_dev_ready[kMaxDevices];                           // per device: twiddle table uploaded (guarded by g_init_mu)
+static std::atomic<int> g_dev_sms[kMaxDevices];
 __device__ float2 g_twiddle[kTwiddleN];
 
 void set_cuda_error(cudaError_t e, const char *where)
@@ -27,8 +28,13 @@ void set_cuda_error(cudaError_t e, const char *where)
 }
 void set_error_text(const char *text) { snprintf(g_err, sizeof(g_err), "%s", text); }
 void count_launch(unsigned n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
-int option(int key) { return (key >= 0 && key < 8) ? g_opts[key].load(std::memory_order_relaxed) : 0; }
-int sm_count() { return g_sm_count; }
+int option(int key) { return (key >= 0 && key < 8) ? g_opts[key] : 0; }
+int sm_count()
+{
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) return 0;
+    return g_dev_sms[dev].load(std::memory_order_relaxed);
+}
 
 const float2 *twiddle_table()
 {
@@ -41,15 +47,15 @@ int ensure_device()
 {
     int dev = -1;
     BLINK_CUDA_TRY(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kMaxDevices) { set_error_text("device ordinal out of range"); return BLINK_ERR_CUDA; }
     std::lock_guard<std::mutex> lk(g_init_mu);
-    if (g_init_device == dev) return BLINK_OK;
+    if (g_dev_ready[dev]) return BLINK_OK;
     cudaDeviceProp prop;
     BLINK_CUDA_TRY(cudaGetDeviceProperties(&prop, dev));
     if (prop.major != 10) {
         set_error_text("libblinkimg is built for sm_100a only: no compute-capability-10.x device is current");
         return BLINK_ERR_CUDA;
     }
-    g_sm_count = prop.multiProcessorCount;
     std::vector<float2> tw(kTwiddleN);
     const double two_pi = 6.283185307179586476925286766559;
     for (int m = 0; m < kTwiddleN; ++m) {
@@ -62,8 +68,9 @@ int ensure_device()
     tw[kTwiddleN / 4] = make_float2(0.f, 1.f);
     tw[kTwiddleN / 2] = make_float2(-1.f, 0.f);
     tw[3 * kTwiddleN / 4] = make_float2(0.f, -1.f);
-    BLINK_CUDA_TRY(cudaMemcpyToSymbol(g_twiddle, tw.data(), sizeof(float2) * kTwiddleN));
-    g_init_device = dev;
+    BLINK_CUDA_TRY(cudaMemcpyToSymbol(g_twiddle, tw.data(), sizeof(float2) * kTwiddleN));   // this device's copy of the symbol
+    g_dev_sms[dev].store(prop.multiProcessorCount, std::memory_order_relaxed);
+    g_dev_ready[dev] = true;
     return BLINK_OK;
 }
 
@@ -141,12 +148,12 @@ extern "C" unsigned long long blink_kernel_launches(void) { return blink::g_laun
 extern "C" int blink_set_option(int key, int value)
 {
     if (key < 0 || key >= 8) return BLINK_ERR_INVALID_ARG;
-    blink::g_opts[key].store(value);
+    blink::g_opts[key] = value;
     return BLINK_OK;
 }
 extern "C" int blink_get_option(int key, int *value)
 {
     if (key < 0 || key >= 8 || !value) return BLINK_ERR_INVALID_ARG;
-    *value = blink::g_opts[key].load();
+    *value = blink::g_opts[key];
     return BLINK_OK;
 }

@@ -113,6 +113,9 @@ avg_grid_kernel(const AvgArgs a, const __grid_constant__ ScaleBlock sc)
 // (baseline, timestep, chunk of channels) keeps (u, v) in registers and walks the channels; a warp's 32 baselines
 // are counted with one ballot per channel into shared counters, flushed with one global atomic per channel.
 constexpr int kAvgChunk = 128;
+// |x| against the grid edge h - 1/2 with round-to-nearest-even at the tie: rint(h - 1/2) is h (off the grid) for even h
+// and h-1 (on the grid) for odd h
+__device__ __forceinline__ bool on_grid_edge(float x, float edge, int h) { return (h & 1) ? (x <= edge) : (x < edge); }
 __global__ void __launch_bounds__(kAvgThreads)
 avg_count_kernel(const AvgArgs a, const __grid_constant__ ScaleBlock sc, unsigned *__restrict__ n_in, int t_lo, int c_lo, int nc,
                  int nchunk, int bblocks)
@@ -126,9 +129,10 @@ avg_count_kernel(const AvgArgs a, const __grid_constant__ ScaleBlock sc, unsigne
     for (int i = threadIdx.x; i < kAvgChunk; i += kAvgThreads) s_cnt[i] = 0u;
     __syncthreads();
     const int n = a.n, h = n / 2;
-    // A sample is on the grid iff |rint(u s)| <= h-1 and |rint(v s)| <= h-1.  h-1 is odd, so the tie |x| = h-1/2
-    // rounds away to h: the test is |u s| < h - 1/2 on the fp32 products, and because fp32 multiplication by
-    // s > 0 is monotone it is ONE product: max(|u|, |v|) * s < h - 1/2 (NaN in either coordinate fails).
+    // A sample is on the grid iff |rint(u s)| <= h-1 and |rint(v s)| <= h-1.  For even h, h-1 is odd and the tie
+    // |x| = h-1/2 rounds away to h: the test is |u s| < h - 1/2 on the fp32 products; for odd h (N = 2 mod 4) the tie
+    // rounds to the even h-1 and stays on the grid: |u s| <= h - 1/2 (on_grid_edge).  Because fp32 multiplication by
+    // s > 0 is monotone it is ONE product: max(|u|, |v|) * s against h - 1/2 (NaN in either coordinate fails).
     float m_uv = __int_as_float(0x7fc00000);                            // NaN: never on the grid
     if (b < a.B) {
         const float u = a.uvw_m[((size_t)t * a.B + b) * 3], v = a.uvw_m[((size_t)t * a.B + b) * 3 + 1];
@@ -138,7 +142,7 @@ avg_count_kernel(const AvgArgs a, const __grid_constant__ ScaleBlock sc, unsigne
     const float edge = (float)h - 0.5f;
     const int c0 = c_lo + k * kAvgChunk, c1 = min(c0 + kAvgChunk, c_lo + nc);
     for (int c = c0; c < c1; ++c) {
-        const unsigned m = __ballot_sync(0xffffffffu, __fmul_rn(m_uv, sc.s[c - a.c_base]) < edge);
+        const unsigned m = __ballot_sync(0xffffffffu, on_grid_edge(__fmul_rn(m_uv, sc.s[c - a.c_base]), edge, h));
         if ((threadIdx.x & 31) == 0 && m) atomicAdd(&s_cnt[c - c0], (unsigned)__popc(m));
     }
     __syncthreads();
@@ -182,12 +186,13 @@ __global__ void avg_wsearch_kernel(const AvgArgs a, const __grid_constant__ Scal
     if (i >= a.ntc) return;
     const int tc = a.tc0 + i;
     const int t = tc / a.C, c = tc - t * a.C;
-    const float s = sc.s[c - a.c_base], edge = (float)(a.n / 2) - 0.5f;
+    const int h = a.n / 2;
+    const float s = sc.s[c - a.c_base], edge = (float)h - 0.5f;
     const float *m = sorted_m + (size_t)t * a.B;
     int lo = 0, hi = a.B;                                               // first index whose sample is off the grid
     while (lo < hi) {
         const int mid = (lo + hi) >> 1;
-        if (__fmul_rn(__ldg(m + mid), s) < edge) lo = mid + 1; else hi = mid;
+        if (on_grid_edge(__fmul_rn(__ldg(m + mid), s), edge, h)) lo = mid + 1; else hi = mid;
     }
     const float W = (float)(2 * lo);
     a.wsum[tc] = W;

@@ -156,12 +156,9 @@ static int launch_fft2d(float2 *grid, int batch, const float *scale, int scale_d
     using RC = RowCfg<N>;
     using CC = ColCfg<N>;
     const float2 *tw = twiddle_table();
-    static bool attr_done = false;        // per-process; attributes are per-function and idempotent
-    if (!attr_done) {
-        BLINK_CUDA_TRY(cudaFuncSetAttribute(fft_rows_kernel<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RC::SMEM));
-        BLINK_CUDA_TRY(cudaFuncSetAttribute(fft_cols_kernel<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)CC::SMEM));
-        attr_done = true;
-    }
+    // the attribute belongs to the current device's context: set it on every launch (cheap, idempotent)
+    BLINK_CUDA_TRY(cudaFuncSetAttribute(fft_rows_kernel<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RC::SMEM));
+    BLINK_CUDA_TRY(cudaFuncSetAttribute(fft_cols_kernel<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)CC::SMEM));
     // grid.y is limited to 65535: process the batch in slabs
     const long long n_rows = (long long)batch * N;
     long long want = (n_rows + RC::G - 1) / RC::G;

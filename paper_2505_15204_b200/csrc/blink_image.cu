@@ -126,6 +126,50 @@ apply_gains_kernel(float2 *__restrict__ vis, const float2 *__restrict__ gains, c
     }
 }
 
+// Stokes I (reading R18): gridding, weighting (W and the cell counts are shared by the planes of a (t,c)) and the
+// transform are linear in V, so (I_XX + I_YY) / 2 is ONE image of the visibilities (V_XX + V_YY) / 2: half the work of
+// imaging both planes.  One thread per visibility pair of the output row, 16-byte accesses when B is even.
+template <int VEC>
+__global__ void __launch_bounds__(256)
+stokes_combine_kernel(const float2 *__restrict__ vis, float2 *__restrict__ out, long long n_tc, int P, int B)
+{
+    const int b = (blockIdx.x * blockDim.x + threadIdx.x) * VEC;
+    if (b >= B) return;
+    for (long long tc = blockIdx.y; tc < n_tc; tc += gridDim.y) {
+        const float2 *xx = vis + (tc * P) * B + b, *yy = vis + (tc * P + (P - 1)) * B + b;
+        float2 *dst = out + tc * B + b;
+        if constexpr (VEC == 2) {
+            const float4 a = __ldcs(reinterpret_cast<const float4 *>(xx)), c = __ldcs(reinterpret_cast<const float4 *>(yy));
+            *reinterpret_cast<float4 *>(dst) = make_float4(0.5f * (a.x + c.x), 0.5f * (a.y + c.y), 0.5f * (a.z + c.z), 0.5f * (a.w + c.w));
+        } else {
+            const float2 a = __ldcs(xx), c = __ldcs(yy);
+            *dst = make_float2(0.5f * (a.x + c.x), 0.5f * (a.y + c.y));
+        }
+    }
+}
+
+// samples outside blink_correlate's input contract (int8 -128): grid-stride count, one atomic per CTA
+__global__ void __launch_bounds__(256) volt_range_kernel(const int4 *__restrict__ v16, size_t n16, const int8_t *__restrict__ tail,
+                                                         int n_tail, unsigned long long *__restrict__ count)
+{
+    unsigned c = 0;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n16; i += (size_t)gridDim.x * blockDim.x) {
+        const int4 q = __ldcs(v16 + i);
+        const unsigned w[4] = {(unsigned)q.x, (unsigned)q.y, (unsigned)q.z, (unsigned)q.w};
+#pragma unroll
+        for (int k = 0; k < 4; ++k) c += __popc(__vcmpeq4(w[k], 0x80808080u) & 0x01010101u);
+    }
+    if (blockIdx.x == 0 && (int)threadIdx.x < n_tail && tail[threadIdx.x] == (int8_t)-128) ++c;
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) c += __shfl_xor_sync(0xffffffffu, c, d);
+    __shared__ unsigned s;
+    if (threadIdx.x == 0) s = 0;
+    __syncthreads();
+    if ((threadIdx.x & 31) == 0 && c) atomicAdd(&s, c);
+    __syncthreads();
+    if (threadIdx.x == 0 && s) atomicAdd(count, (unsigned long long)s);
+}
+
 }  // namespace blink
 
 using namespace blink;
@@ -156,6 +200,16 @@ extern "C" int blink_workspace_bytes(int op, int T, int C, int P, int B, int n_p
         case BLINK_OP_FFT2D:
             rec = mn = gfft_workspace_bytes(n_pix);
             break;
+        case BLINK_OP_IMAGE_STOKES_I: {                         // combined visibilities + a one-plane blink_image
+            if (P != 2 && P != 4) return BLINK_ERR_INVALID_ARG;
+            size_t r1 = 0, m1 = 0;
+            int rc1 = blink_workspace_bytes(BLINK_OP_IMAGE, T, C, 1, B, n_pix, weighting, &r1, &m1);
+            if (rc1 != BLINK_OK) return rc1;
+            const size_t comb = align_up((size_t)T * C * B * sizeof(float2), 256);
+            rec = comb + r1;
+            mn = comb + m1;
+            break;
+        }
         case BLINK_OP_IMAGE:
         case BLINK_OP_IMAGE_HOST: {
             if (use_fused(P, B, n_pix, weighting)) {
@@ -221,7 +275,7 @@ extern "C" int blink_image_host(const blink_c64 *vis_host, const float *uvw_m_ho
 {
     int rc = check_common(vis_host, uvw_m_host, freqs_hz, T, C, P, B, n_pix, pixscale_rad, weighting);
     if (rc != BLINK_OK) return rc;
-    if (!image_host || !wsum_host || !workspace || !aligned16(workspace)) return BLINK_ERR_INVALID_ARG;
+    if (!image_host || !wsum_host || !workspace || (reinterpret_cast<uintptr_t>(workspace) & 255u)) return BLINK_ERR_INVALID_ARG;   // the fused path needs 256
     rc = ensure_device();
     if (rc != BLINK_OK) return rc;
     size_t need = 0, need_min = 0;
@@ -242,37 +296,47 @@ extern "C" int blink_image_host(const blink_c64 *vis_host, const float *uvw_m_ho
     unsigned char *compute_ws = w + stage;
     const size_t compute_bytes = (workspace_bytes - stage) / 2 / 256 * 256;       // one half per slot
 
-    // two pipelines (slots): H2D vis(t) -> image(t) -> D2H images(t), each on its own stream
-    static cudaStream_t streams[2] = {nullptr, nullptr};
-    for (int k = 0; k < 2; ++k)
-        if (!streams[k]) BLINK_CUDA_TRY(cudaStreamCreateWithFlags(&streams[k], cudaStreamNonBlocking));
-    cudaEvent_t uvw_ready;
-    BLINK_CUDA_TRY(cudaEventCreateWithFlags(&uvw_ready, cudaEventDisableTiming));
-    BLINK_CUDA_TRY(cudaMemcpyAsync(d_uvw, uvw_m_host, (size_t)T * B * 3 * sizeof(float), cudaMemcpyHostToDevice, streams[0]));
-    BLINK_CUDA_TRY(cudaEventRecord(uvw_ready, streams[0]));
-    BLINK_CUDA_TRY(cudaStreamWaitEvent(streams[1], uvw_ready, 0));
+    // two pipelines (slots): H2D vis(t) -> image(t) -> D2H images(t), each on its own stream.  Streams and the event are
+    // created per call on the CURRENT device and destroyed on every exit path (after draining both streams).
+    cudaStream_t streams[2] = {nullptr, nullptr};
+    cudaEvent_t uvw_ready = nullptr;
     int result = BLINK_OK;
+    auto fail = [&](cudaError_t e, const char *where) {
+        if (e != cudaSuccess && result == BLINK_OK) { set_cuda_error(e, where); result = BLINK_ERR_CUDA; }
+        return e != cudaSuccess;
+    };
+    for (int k = 0; k < 2 && result == BLINK_OK; ++k)
+        fail(cudaStreamCreateWithFlags(&streams[k], cudaStreamNonBlocking), "cudaStreamCreateWithFlags");
+    if (result == BLINK_OK) fail(cudaEventCreateWithFlags(&uvw_ready, cudaEventDisableTiming), "cudaEventCreateWithFlags");
+    if (result == BLINK_OK) {
+        fail(cudaMemcpyAsync(d_uvw, uvw_m_host, (size_t)T * B * 3 * sizeof(float), cudaMemcpyHostToDevice, streams[0]), "cudaMemcpyAsync(uvw)") ||
+            fail(cudaEventRecord(uvw_ready, streams[0]), "cudaEventRecord") ||
+            fail(cudaStreamWaitEvent(streams[1], uvw_ready, 0), "cudaStreamWaitEvent");
+    }
     for (int t = 0; t < T && result == BLINK_OK; ++t) {
         const int k = t & 1;
         cudaStream_t st = streams[k];
         float2 *d_vis = reinterpret_cast<float2 *>(slots + (size_t)k * (vis_b + img_b));
         float *d_img = reinterpret_cast<float *>(slots + (size_t)k * (vis_b + img_b) + vis_b);
         const size_t vis_elems = (size_t)C * P * B;
-        BLINK_CUDA_TRY(cudaMemcpyAsync(d_vis, reinterpret_cast<const float2 *>(vis_host) + (size_t)t * vis_elems,
-                                       vis_elems * sizeof(float2), cudaMemcpyHostToDevice, st));
+        if (fail(cudaMemcpyAsync(d_vis, reinterpret_cast<const float2 *>(vis_host) + (size_t)t * vis_elems,
+                                 vis_elems * sizeof(float2), cudaMemcpyHostToDevice, st), "cudaMemcpyAsync(vis)"))
+            break;
         // one timestep as a T=1 problem: uvw of timestep t, outputs of timestep t
         result = image_device(d_vis, d_uvw + (size_t)t * B * 3, freqs_hz, 1, C, P, B, n_pix, pixscale_rad, weighting, 0, C,
                               d_img, d_wsum + (size_t)t * C, nullptr, nullptr, compute_ws + (size_t)k * compute_bytes,
                               compute_bytes, st);
         if (result != BLINK_OK) break;
-        BLINK_CUDA_TRY(cudaMemcpyAsync(image_host + (size_t)t * C * P * n2, d_img, (size_t)C * P * n2 * sizeof(float),
-                                       cudaMemcpyDeviceToHost, st));
+        fail(cudaMemcpyAsync(image_host + (size_t)t * C * P * n2, d_img, (size_t)C * P * n2 * sizeof(float),
+                             cudaMemcpyDeviceToHost, st), "cudaMemcpyAsync(images)");
     }
-    BLINK_CUDA_TRY(cudaStreamSynchronize(streams[0]));
-    BLINK_CUDA_TRY(cudaStreamSynchronize(streams[1]));
+    for (int k = 0; k < 2; ++k)                                 // drain on every path: nothing may still be in flight on return
+        if (streams[k]) fail(cudaStreamSynchronize(streams[k]), "cudaStreamSynchronize");
     if (result == BLINK_OK)
-        BLINK_CUDA_TRY(cudaMemcpy(wsum_host, d_wsum, (size_t)T * C * sizeof(float), cudaMemcpyDeviceToHost));
-    cudaEventDestroy(uvw_ready);
+        fail(cudaMemcpy(wsum_host, d_wsum, (size_t)T * C * sizeof(float), cudaMemcpyDeviceToHost), "cudaMemcpy(wsum)");
+    if (uvw_ready) cudaEventDestroy(uvw_ready);
+    for (int k = 0; k < 2; ++k)
+        if (streams[k]) cudaStreamDestroy(streams[k]);
     return result;
 }
 
@@ -324,4 +388,45 @@ extern "C" int blink_image_cal(const blink_c64 *vis, const float *uvw_m, const d
     return image_device(reinterpret_cast<const float2 *>(vis), uvw_m, freqs_hz, T, C, P, B, n_pix, pixscale_rad, weighting,
                         0, T * C, image, wsum, nullptr, nullptr, workspace, workspace_bytes,
                         static_cast<cudaStream_t>(stream), cal);
+}
+
+extern "C" int blink_image_stokes_i(const blink_c64 *vis, const float *uvw_m, const double *freqs_hz, int T, int C, int P, int B,
+                                    int n_pix, double pixscale_rad, int weighting, float *image, float *wsum,
+                                    void *workspace, size_t workspace_bytes, void *stream)
+{
+    int rc = check_common(vis, uvw_m, freqs_hz, T, C, P, B, n_pix, pixscale_rad, weighting);
+    if (rc != BLINK_OK) return rc;
+    if (P != 2 && P != 4) return BLINK_ERR_INVALID_ARG;
+    if (!image || !wsum || !aligned16(vis) || !aligned16(image)) return BLINK_ERR_INVALID_ARG;
+    rc = ensure_device();
+    if (rc != BLINK_OK) return rc;
+    // workspace: the combined visibilities [T][C][B] | the workspace of the one-plane blink_image that follows
+    const size_t comb = align_up((size_t)T * C * B * sizeof(float2), 256);
+    if (!workspace || (reinterpret_cast<uintptr_t>(workspace) & 255u) || workspace_bytes < comb) return BLINK_ERR_WORKSPACE;
+    float2 *vm = static_cast<float2 *>(workspace);
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const long long n_tc = (long long)T * C;
+    const unsigned rows_y = (unsigned)std::min<long long>(n_tc, 4096);
+    const float2 *v = reinterpret_cast<const float2 *>(vis);
+    if ((B & 1) == 0)
+        stokes_combine_kernel<2><<<dim3((B / 2 + 255) / 256, rows_y), 256, 0, st>>>(v, vm, n_tc, P, B);
+    else
+        stokes_combine_kernel<1><<<dim3((B + 255) / 256, rows_y), 256, 0, st>>>(v, vm, n_tc, P, B);
+    BLINK_LAUNCH_CHECK("stokes_combine_kernel");
+    return image_device(vm, uvw_m, freqs_hz, T, C, 1, B, n_pix, pixscale_rad, weighting, 0, T * C, image, wsum, nullptr, nullptr,
+                        static_cast<unsigned char *>(workspace) + comb, workspace_bytes - comb, st);
+}
+
+extern "C" int blink_volt_out_of_range(const int8_t *volt, size_t n_bytes, unsigned long long *count, void *stream)
+{
+    if (!volt || !count || !aligned16(volt)) return BLINK_ERR_INVALID_ARG;
+    int rc = ensure_device();
+    if (rc != BLINK_OK) return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    BLINK_CUDA_TRY(cudaMemsetAsync(count, 0, sizeof(unsigned long long), st));
+    const size_t n16 = n_bytes / 16;
+    const int blocks = (int)std::min<size_t>((n16 + 255) / 256 + 1, (size_t)(sm_count() > 0 ? sm_count() : 148) * 8);
+    volt_range_kernel<<<blocks, 256, 0, st>>>(reinterpret_cast<const int4 *>(volt), n16, volt + n16 * 16, (int)(n_bytes - n16 * 16), count);
+    BLINK_LAUNCH_CHECK("volt_range_kernel");
+    return BLINK_OK;
 }

@@ -1,12 +1,12 @@
 """GPU parity of blink_image_conv (convolutional gridding, reading R16) against the
 CPU oracle, through the C ABI.
 
-Bars: wsum and the nearest-cell index of every baseline bit-exact.  Images: north_star's rule (max abs error
-<= 1e-4 x peak) applies to what the transform produces, i.e. BEFORE the grid correction 1 / (c(y) c(x)) -- the
-correction is an exact per-pixel factor that grows towards the image edge (up to ~3000x in the corners for
-S = 7) and scales the fp32 rounding error of that pixel with it.  So the test compares
-    max |I_gpu - I_oracle| c(y) c(x)  <=  1e-4 * max |I_oracle| c(y) c(x)
-and, in the central half of the field (where the correction is below ~4), the plain rule as well.
+Bars: wsum and the nearest-cell index of every baseline bit-exact.  Images: north_star's PLAIN rule over the WHOLE image,
+    max |I_gpu - I_oracle|  <=  1e-4 * max |I_oracle|,
+grid correction included.  (Round 1 asserted a taper-weighted form because the correction 1 / (c(y) c(x)) grows to ~2600 in
+the corners for S = 7 and multiplies the transform's fp32 rounding error there; measured in round 2 the plain rule holds
+with margin -- worst over config 1 at 256^2 and config 3 at 512^2: 1.9e-7 (S = 3), 9.0e-7 (S = 5), 5.0e-6 (S = 7) -- so
+it is the assertion and the weighted form is gone.)
 """
 import numpy as np
 import pytest
@@ -40,18 +40,14 @@ def _check_conv(w, res, oracle_mod, S, beta=0.0, ids=None, check_cells=True):
     ref, wref = oracle_mod.image_conv_batch(vis, uvw, w.freqs_hz, n, w.pixscale_rad, S, b, ids, nthreads=8)
     img = res["image"][torch.as_tensor(ids, device=res["image"].device)].cpu().numpy().astype(np.float64)
     wsum = res["wsum"].cpu().numpy()
-    c = oracle_mod.conv_taper(n, S, b)
-    cc = np.outer(c, c)
-    q = slice(h - n // 4, h + n // 4)
-    worst = worst_c = 0.0
+    worst = 0.0
     for k, i in enumerate(ids):
         assert wsum[i // w.P] == np.float32(wref[k]), (i, wsum[i // w.P], wref[k])
         if wref[k] == 0:
             assert np.all(img[k] == 0)
             continue
-        worst = max(worst, float(np.max(np.abs(img[k] - ref[k]) * cc) / np.max(np.abs(ref[k]) * cc)))
-        worst_c = max(worst_c, float(np.max(np.abs(img[k] - ref[k])[q, q]) / np.max(np.abs(ref[k][q, q]))))
-    assert worst <= TOL and worst_c <= TOL, (worst, worst_c)
+        worst = max(worst, float(np.max(np.abs(img[k] - ref[k])) / np.max(np.abs(ref[k]))))     # whole image, corners included
+    assert worst <= TOL, worst
     if check_cells and res.get("cell_idx") is not None:
         ci = res["cell_idx"].cpu().numpy()
         for t in range(w.T):
@@ -191,21 +187,18 @@ def test_conv_config3_full_size_sampled(bk, oracle_mod):
     rng = np.random.default_rng(35)
     ids = np.unique([0, T * C - 1] + [int(i) for i in rng.choice(T * C, 8, replace=False)])
     sel = torch.as_tensor(ids, device="cuda")
-    c = oracle_mod.conv_taper(N, S, _beta(S))
-    cc = np.outer(c, c)
     img_s = res["image"][sel].cpu().numpy().astype(np.float64)
     vis_s = w.vis.reshape(T * C, B)[sel].cpu().numpy()
     worst = 0.0
     for k, i in enumerate(ids):
         t, cch = divmod(int(i), C)
         ref = oracle_mod.image_conv_one(vis_s[k], uvw[t], w.freqs_hz[cch], N, w.pixscale_rad, S, _beta(S))["image"]
-        worst = max(worst, float(np.max(np.abs(img_s[k] - ref) * cc) / np.max(np.abs(ref) * cc)))
+        worst = max(worst, float(np.max(np.abs(img_s[k] - ref)) / np.max(np.abs(ref))))
     assert worst <= TOL, worst
     # closed form for EVERY image: taps sum to 1 and c(0) = 1, so the centre pixel is sum(2 Re V_in) / W
     centre = res["image"][:, h, h].double().cpu().numpy()
     inr_t = torch.as_tensor(inr, device="cuda").reshape(T * C, B)
     want = (2.0 * (w.vis.reshape(T * C, B).real.double() * inr_t).sum(dim=1) / (2.0 * inr_t.sum(dim=1))).cpu().numpy()
-    q = slice(h - N // 4, h + N // 4)
-    peak = res["image"][:, q, q].reshape(T * C, -1).abs().amax(dim=1).double().cpu().numpy()
+    peak = res["image"].reshape(T * C, -1).abs().amax(dim=1).double().cpu().numpy()
     assert np.max(np.abs(centre - want) / peak) <= TOL
     assert bool(torch.isfinite(res["image"]).all())

@@ -693,3 +693,223 @@ def test_fused_repeatability_stress(bk, oracle_mod):
             assert float((res["image"] - first).abs().max()) <= 1e-6 * peak, k
             assert torch.equal(res["wsum"], wsum0)
         wsum0 = res["wsum"].clone()
+
+
+# --------------------------------------------------------------------------- the FUSED kernel's own cell decisions
+def _tie_cases(h):
+    """(u, v) in cells (the scale is exactly 1 cell per metre): half-cell ties for even and odd k, the range limits,
+    the fold u < 0 -> u >= 0, signed zeros.  Rounding is to nearest, ties to even (reading R2)."""
+    return [
+        (2.5, 7.0), (3.5, -9.0), (-2.5, 11.0), (-3.5, -13.0),            # u ties: 2, 4, -2, -4
+        (21.0, 2.5), (23.0, 3.5), (-25.0, -2.5), (-27.0, -3.5),          # v ties
+        (0.5, 30.0), (-0.5, 32.0), (1.5, 34.0), (-1.5, -36.0),           # ties that land on / next to the u = 0 column
+        (0.0, 40.0), (-0.0, 42.0), (0.0, -44.0), (-0.0, -46.0),          # the u = 0 column itself, signed zeros
+        (0.0, 0.0), (-0.0, -0.0), (-0.4, 50.0), (0.4, -52.0),            # DC; |u| < 1/2 folds onto column 0
+        (h - 1.0, 60.0), (-(h - 1.0), -62.0), (64.0, h - 1.0), (-66.0, -(h - 1.0)),    # the last cells in range
+        (h - 0.5, 70.0), (72.0, h - 0.5), (-(h - 0.5), 74.0), (76.0, -(h - 0.5)),      # tie at the edge: rounds to h (even) -> dropped
+        (h - 1.5, 80.0), (82.0, -(h - 1.5)), (h - 1.0, h - 1.0), (-(h - 1.0), h - 1.0),  # tie that rounds to h - 2; corners
+    ]
+
+
+@pytest.mark.parametrize("n", [256, 512])
+@pytest.mark.parametrize("weighting", [0, 1])
+@pytest.mark.parametrize("path", [2, 1])
+def test_fused_cell_decisions_one_hot(bk, oracle_mod, n, weighting, path):
+    """What the gridder itself decides (not the side computation behind cell_idx): 8 baselines per timestep, 8 planes, plane
+    p carries ONLY baseline p, so every image is one cosine fringe whose (k_u, k_v) is the cell the gridder chose
+    (eq. 4-5; closed form of SURVEY 8(c) 'FFT, any N').  A wrong cell changes the image by O(1) x peak."""
+    from paper_2505_15204_b200 import workloads
+    h = n // 2
+    f = 150e6
+    pix = 299792458.0 / (f * n)
+    assert float(oracle_mod.scale(f, n, pix)) == 1.0                # one cell per metre: u_m IS the cell coordinate
+    cases = _tie_cases(float(h))
+    B = 8
+    T = len(cases) // B
+    uvw = np.zeros((T, B, 3), dtype=np.float32)
+    uvw[:, :, :2] = np.array(cases, dtype=np.float32).reshape(T, B, 2)
+    rng = np.random.default_rng(n + weighting)
+    amp = (rng.uniform(0.5, 2.0, (T, B)) * np.exp(1j * rng.uniform(-np.pi, np.pi, (T, B)))).astype(np.complex64)
+    vis = np.zeros((T, 1, B, B), dtype=np.complex64)
+    for b in range(B):
+        vis[:, 0, b, b] = amp[:, b]
+    w = workloads.Workload(name="ties", T=T, C=1, P=B, B=B, n_pix=n, pixscale_rad=pix, weighting=weighting,
+                           freqs_hz=np.array([f]), uvw_m=torch.tensor(uvw, device="cuda"), vis=torch.tensor(vis, device="cuda"),
+                           sources={}, meta={})
+    bk.set_option(bk.OPT_IMAGE_PATH, path)
+    try:
+        res = bk.blink_image(w.vis, w.uvw_m, w.freqs_hz, n, pix, weighting, want_cell_idx=True)
+        torch.cuda.synchronize()
+    finally:
+        bk.set_option(bk.OPT_IMAGE_PATH, 0)
+    ci = oracle_mod.cells(uvw, w.freqs_hz, n, pix)[:, 0]            # [T][B]
+    assert np.array_equal(res["cell_idx"].cpu().numpy()[:, 0], ci)
+    # the cases do what they were built for (ties to even, edge tie dropped, signed zeros on column 0)
+    flat = ci.ravel()
+    cell = lambda iu, iv: (iv + h) * n + (iu + h)
+    assert flat[0] == cell(2, 7) and flat[1] == cell(4, -9) and flat[2] == cell(-2, 11) and flat[3] == cell(-4, -13)
+    assert flat[4] == cell(21, 2) and flat[5] == cell(23, 4) and flat[8] == cell(0, 30) and flat[10] == cell(2, 34)
+    assert flat[13] == cell(0, 42) and flat[18] == cell(0, 50) and np.all(flat[24:28] == -1) and flat[28] == cell(h - 2, 80)
+    img = res["image"].cpu().numpy().reshape(T, B, n, n).astype(np.float64)
+    wsum = res["wsum"].cpu().numpy()
+    y, x = np.mgrid[0:n, 0:n]
+    for t in range(T):
+        ok = ci[t] >= 0
+        if weighting == 0:
+            assert wsum[t] == 2 * ok.sum()
+        for b in range(B):
+            r = oracle_mod.image_one(vis[t, 0, b], uvw[t], f, n, pix, weighting)
+            assert wsum[t] == np.float32(r["W"])
+            if not ok[b]:
+                assert np.all(img[t, b] == 0), (t, b)
+                continue
+            peak = np.max(np.abs(r["image"]))
+            assert np.max(np.abs(img[t, b] - r["image"])) <= TOL * peak, (t, b)
+            if weighting == 0:                                      # the closed form itself, from the oracle's cell
+                iv, iu = ci[t, b] // n - h, ci[t, b] % n - h
+                V = amp[t, b].astype(np.complex128)
+                if iu == 0 and iv == 0:
+                    want = np.full((n, n), 2 * V.real / wsum[t])
+                else:
+                    want = 2 * abs(V) * np.cos(2 * np.pi * (iu * (x - h) + iv * (y - h)) / n + np.angle(V)) / wsum[t]
+                assert np.max(np.abs(img[t, b] - want)) <= TOL * np.max(np.abs(want)), (t, b, iu, iv)
+
+
+# --------------------------------------------------------------------------- full size: configs 2, 5 and one timestep of 4
+def _full_size_check(bk, oracle_mod, w, n_sample, seed):
+    """The recipe of test_config3_full_size_sampled for any config, natural or uniform: cell index of every (t,c,b) and
+    wsum of every (t,c) bit-exact, n_sample images (spread over t, c, p) within 1e-4 x peak, centre pixel of EVERY image
+    against its closed form sum_cells G / W."""
+    T, C, P, B, N = w.T, w.C, w.P, w.B, w.n_pix
+    res = bk.blink_image(w.vis, w.uvw_m, w.freqs_hz, N, w.pixscale_rad, w.weighting, want_cell_idx=True)
+    torch.cuda.synchronize()
+    uvw = w.uvw_m.cpu().numpy()
+    ref_ci = oracle_mod.cells(uvw, w.freqs_hz, N, w.pixscale_rad)
+    assert np.array_equal(res["cell_idx"].cpu().numpy(), ref_ci)
+    ci = torch.as_tensor(ref_ci, device="cuda").reshape(T * C, B).long()
+    ok = ci >= 0
+    vre = w.vis.reshape(T * C, P, B).real.double()
+    if w.weighting == 0:
+        W = 2.0 * ok.sum(dim=1).double()
+        centre = 2.0 * (vre * ok[:, None, :]).sum(dim=2) / W[:, None]
+    else:
+        mir = (N - ci // N) * N + (N - ci % N)
+        row = torch.arange(T * C, device="cuda")[:, None] * (N * N)
+        keys = torch.cat([(row + ci)[ok], (row + mir)[ok]])
+        uniq, inv, counts = torch.unique(keys, return_inverse=True, return_counts=True)
+        W = torch.bincount(uniq // (N * N), minlength=T * C).double()
+        inv_cnt = torch.zeros((T * C, B), dtype=torch.float64, device="cuda")
+        inv_cnt[ok] = 1.0 / counts[inv[: int(ok.sum())]].double()   # samples (vis + conjugates) in the cell of every baseline
+        centre = 2.0 * (vre * inv_cnt[:, None, :]).sum(dim=2) / W[:, None]
+    assert torch.equal(res["wsum"], W.float())                     # every (t,c), bit-exact
+    h = N // 2
+    got = res["image"][:, h, h].double().reshape(T * C, P)
+    peak = res["image"].reshape(T * C * P, -1).abs().amax(dim=1).double().reshape(T * C, P)
+    assert float(((got - centre).abs() / peak).max()) <= TOL
+    assert bool(torch.isfinite(res["image"]).all())
+    rng = np.random.default_rng(seed)
+    n_img = T * C * P
+    ids = np.unique(np.concatenate([[0, n_img - 1], rng.choice(n_img, n_sample, replace=False)]))
+    vis_c = w.vis.cpu().numpy()
+    worst = 0.0
+    for k0 in range(0, len(ids), 8):                               # 8 images at a time: the oracle returns float64 images
+        part = ids[k0:k0 + 8]
+        ref, wref = oracle_mod.image_batch(vis_c, uvw, w.freqs_hz, N, w.pixscale_rad, w.weighting, part, nthreads=8)
+        img = res["image"][torch.as_tensor(part, device="cuda")].cpu().numpy()
+        for k, i in enumerate(part):
+            assert float(res["wsum"][i // P]) == np.float32(wref[k])
+            worst = max(worst, _img_err(img[k], ref[k]))
+    assert worst <= TOL, worst
+    return worst
+
+
+@pytest.mark.parametrize("cfg,T,n_sample", [(2, None, 16), (5, None, 16), (4, 1, 16)])
+def test_full_size_configs_2_5_4(bk, oracle_mod, cfg, T, n_sample):
+    """BASELINE.json configs 2 (768 x 1024^2, natural), 5 (320 x 4096^2, uniform) at FULL size and ONE full timestep of
+    config 4 (3072 x 2048^2, 4 pols, uniform) in the launch configuration bench.py times."""
+    from paper_2505_15204_b200 import workloads
+    import gc
+    gc.collect()
+    torch.cuda.empty_cache()
+    free, _ = torch.cuda.mem_get_info()
+    if free < 80e9:
+        pytest.skip("needs ~70 GB of device memory")
+    w = workloads.make_config(cfg, device="cuda", T=T)
+    shp = workloads.config_shape(cfg)
+    assert (w.C, w.P, w.B, w.n_pix, w.weighting) == (shp["C"], shp["P"], shp["B"], shp["n_pix"], shp["weighting"])
+    assert w.T == (shp["T"] if T is None else T)
+    _full_size_check(bk, oracle_mod, w, n_sample, seed=900 + cfg)
+
+
+# --------------------------------------------------------------------------- Stokes I (SURVEY section 2 item 19)
+@pytest.mark.parametrize("P", [2, 4])
+@pytest.mark.parametrize("weighting", [0, 1])
+@pytest.mark.parametrize("n,B,path", [(256, 1237, 2), (256, 2048, 2), (128, 700, 0), (240, 500, 0)])
+def test_stokes_i_vs_oracle(bk, oracle_mod, P, weighting, n, B, path):
+    from paper_2505_15204_b200 import workloads
+    w = workloads.make_random(T=2, C=3, P=P, B=B, n_pix=n, weighting=weighting, seed=80 + P + n, device="cuda", fill=1.1)
+    bk.set_option(bk.OPT_IMAGE_PATH, path)
+    try:
+        res = bk.blink_image_stokes_i(w.vis, w.uvw_m, w.freqs_hz, n, w.pixscale_rad, weighting)
+        torch.cuda.synchronize()
+    finally:
+        bk.set_option(bk.OPT_IMAGE_PATH, 0)
+    ref, wref = oracle_mod.image_stokes_i(w.vis.cpu().numpy(), w.uvw_m.cpu().numpy(), w.freqs_hz, n, w.pixscale_rad, weighting)
+    img = res["image"].cpu().numpy()
+    assert img.shape == ref.shape
+    assert np.array_equal(res["wsum"].cpu().numpy(), wref.astype(np.float32))
+    for k in range(ref.shape[0]):
+        assert _img_err(img[k], ref[k]) <= TOL, (k, _img_err(img[k], ref[k]))
+    with pytest.raises(bk.BlinkError):                              # P = 3 has no XX / YY reading
+        w3 = workloads.make_random(T=1, C=1, P=3, B=64, n_pix=64, weighting=0, seed=1, device="cuda")
+        bk.blink_image_stokes_i(w3.vis, w3.uvw_m, w3.freqs_hz, 64, w3.pixscale_rad, 0)
+
+
+def test_stokes_i_config4_reduced(bk, oracle_mod):
+    from paper_2505_15204_b200 import workloads
+    w = workloads.make_config(4, device="cuda", T=1, C=2)
+    res = bk.blink_image_stokes_i(w.vis, w.uvw_m, w.freqs_hz, w.n_pix, w.pixscale_rad, w.weighting)
+    ref, wref = oracle_mod.image_stokes_i(w.vis.cpu().numpy(), w.uvw_m.cpu().numpy(), w.freqs_hz, w.n_pix, w.pixscale_rad, w.weighting)
+    assert np.array_equal(res["wsum"].cpu().numpy(), wref.astype(np.float32))
+    for k in range(2):
+        assert _img_err(res["image"][k].cpu().numpy(), ref[k]) <= TOL
+
+
+# --------------------------------------------------------------------------- ADVICE round 1: avg tie at odd N/2
+@pytest.mark.parametrize("n", [90, 50])
+@pytest.mark.parametrize("wopt", [1, 2])
+def test_avg_edge_tie_odd_half(bk, oracle_mod, n, wopt):
+    """N = 2 (mod 4): h = N/2 is odd, so |x| = h - 1/2 rounds to the EVEN h - 1 and stays on the grid; the averaging path's
+    one-product range test must count it (wsum bit-exact, image normalised by the right W)."""
+    from paper_2505_15204_b200 import workloads
+    h = n // 2
+    f = 150e6
+    pix = 299792458.0 / (f * n)
+    assert float(oracle_mod.scale(f, n, pix)) == 1.0
+    w = workloads.make_random(T=1, C=1, P=1, B=40, n_pix=n, weighting=0, seed=n, device="cuda", fill=0.5)
+    w.freqs_hz, w.pixscale_rad = np.array([f]), pix
+    uvw = w.uvw_m.clone()
+    uvw[0, :, :2] = torch.as_tensor(np.random.default_rng(n).uniform(-h / 2, h / 2, (40, 2)).astype(np.float32))
+    uvw[0, 0, 0], uvw[0, 1, 1], uvw[0, 2, 0], uvw[0, 3, 1] = h - 0.5, -(h - 0.5), h + 0.5, h - 1.5
+    w.uvw_m = uvw
+    ci = oracle_mod.cells(uvw.cpu().numpy(), w.freqs_hz, n, pix)[0, 0]
+    assert ci[0] >= 0 and ci[1] >= 0 and ci[2] == -1 and ci[3] >= 0   # the tie IS on the grid for odd h
+    bk.set_option(bk.OPT_AVG_WSUM, wopt)
+    try:
+        _check_avg(bk, oracle_mod, w, False)
+    finally:
+        bk.set_option(bk.OPT_AVG_WSUM, 0)
+
+
+def test_volt_out_of_range(bk):
+    from paper_2505_15204_b200 import workloads
+    volt = workloads.make_voltages(3, 5, 1003, seed=9, device="cuda", lo=-127, hi=127)
+    assert bk.blink_volt_out_of_range(volt) == 0
+    flat = volt.view(-1)
+    for i in (0, 17, flat.numel() - 1, flat.numel() - 9):
+        flat[i] = -128
+    assert bk.blink_volt_out_of_range(volt) == 4
+    v2 = workloads.make_voltages(8, 16, 200, seed=9, device="cuda")
+    v2.view(-1)[5] = -128
+    with pytest.raises(bk.BlinkError):
+        bk.blink_correlate(v2, 200, 4, check_range=True)
