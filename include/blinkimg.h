@@ -41,7 +41,7 @@ typedef struct blink_c64 { float re, im; } blink_c64;       /* == float2 == comp
 
 enum { BLINK_W_NATURAL = 0, BLINK_W_UNIFORM = 1 };
 enum { BLINK_OP_GRID = 0, BLINK_OP_FFT2D = 1, BLINK_OP_IMAGE = 2, BLINK_OP_IMAGE_HOST = 3, BLINK_OP_IMAGE_AVG = 4,
-       BLINK_OP_IMAGE_CONV = 5, BLINK_OP_IMAGE_STOKES_I = 6 };
+       BLINK_OP_IMAGE_CONV = 5, BLINK_OP_IMAGE_STOKES_I = 6, BLINK_OP_IMAGE_CAL = 7 };
 enum {
     BLINK_OK = 0,
     BLINK_ERR_INVALID_ARG = -1,   /* NULL / misaligned pointer, non-positive size, bad enum          */
@@ -163,9 +163,11 @@ int blink_image_avg(const blink_c64 *vis, const float *uvw_m, const double *freq
  *   gains      in  [C][P][A] complex64 (a per-antenna phase carries the cable-length and geometric delays)
  *   ant_pairs  in  [B][2] int32, (a1, a2) of every baseline, 0 <= a < A; 8-byte aligned
  * blink_apply_gains corrects `vis` IN PLACE, one thread per visibility (the paper's own form).
- * blink_image_cal is blink_image with the correction fused into the gridder's load: `vis` is not modified and
- * never written.  It needs the fused kernel (256 <= n_pix <= 4096, B <= 16384), else BLINK_ERR_UNSUPPORTED --
- * use blink_apply_gains followed by blink_image there.  Other arguments as blink_image.
+ * blink_image_cal is blink_image of the corrected visibilities; `vis` is not modified and never written.  Where the fused
+ * kernel runs (n_pix a power of two in [256, 4096], B <= 16384) the correction is fused into the gridder's load; for every
+ * other supported size (the paper's 1200 and 8192 among them) the corrected visibilities are written to the head of the
+ * workspace and imaged by the unfused chain.  `workspace` >= blink_workspace_bytes(BLINK_OP_IMAGE_CAL) minimum, 256-byte
+ * aligned.  Other arguments as blink_image.
  */
 int blink_apply_gains(blink_c64 *vis, const blink_c64 *gains, const int32_t *ant_pairs,
                       int T, int C, int P, int B, int A, void *stream);

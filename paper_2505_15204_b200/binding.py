@@ -17,7 +17,7 @@ _SO = os.path.join(_HERE, "libblinkimg.so")
 _lib = None
 
 W_NATURAL, W_UNIFORM = 0, 1
-OP_GRID, OP_FFT2D, OP_IMAGE, OP_IMAGE_HOST, OP_IMAGE_AVG, OP_IMAGE_CONV, OP_IMAGE_STOKES_I = 0, 1, 2, 3, 4, 5, 6
+OP_GRID, OP_FFT2D, OP_IMAGE, OP_IMAGE_HOST, OP_IMAGE_AVG, OP_IMAGE_CONV, OP_IMAGE_STOKES_I, OP_IMAGE_CAL = 0, 1, 2, 3, 4, 5, 6, 7
 OPT_IMAGE_PATH, OPT_FUSED_CTAS, OPT_GRID_CHUNK_B, OPT_AVG_WSUM, OPT_CORR_PATH = 0, 1, 2, 3, 4
 
 EXPORTS = ["blink_strerror", "blink_last_cuda_error", "blink_set_option", "blink_get_option",
@@ -298,7 +298,7 @@ def blink_image_cal(vis: torch.Tensor, uvw_m: torch.Tensor, freqs_hz, gains: tor
     T, C, P, B, fr, dev = _vis_uvw(vis, uvw_m, freqs_hz)
     A = _gains_pairs(gains, ant_pairs, C, P, B, dev)
     image, wsum = _image_outputs(T, C, P, n_pix, dev, image, wsum)
-    workspace = _workspace(workspace, OP_IMAGE, T, C, P, B, n_pix, weighting, dev)
+    workspace = _workspace(workspace, OP_IMAGE_CAL, T, C, P, B, n_pix, weighting, dev)
     with torch.cuda.device(dev):
         rc = lib().blink_image_cal(_ptr(vis), _ptr(uvw_m), fr.ctypes.data_as(ctypes.c_void_p), _ptr(gains), _ptr(ant_pairs),
                                    A, T, C, P, B, n_pix, float(pixscale_rad), int(weighting), _ptr(image),

@@ -1,7 +1,8 @@
 // Centred inverse 2D transform for image sides that are NOT a power of two (N even, N = 2^a 3^b 5^c; the paper
 // images at 1200 x 1200).  Same definition as blink_fft2d.cu (sign +, unnormalised, fftshift,
 // 1/scale, real part; readings R5-R7), different machinery: a mixed-radix Stockham transform whose every stage
-// goes through shared memory (two ping-pong arrays), radices 4, 2, 3, 5, twiddles from an N-entry table
+// goes through shared memory (two ping-pong arrays), radices 15, 16 (register-resident 3 x 5 / 4 x 4 butterflies), 5, 3, 4, 2,
+// twiddles from an N-entry table
 // exp(+2 pi i m / N) that an init kernel writes (in double) into the caller's workspace.
 //   pass 1 (gfft_rows_kernel): rows, in place, input taken at the centred column (n + h) mod N, output in natural x;
 //   pass 2 (gfft_cols_kernel): KC columns per CTA, output row / column moved by h again, scaled, real part stored.
@@ -10,13 +11,18 @@
 
 #include "blink_common.cuh"
 #include "blink_fft.cuh"
+#include "blink_fftg.cuh"
 
 namespace blink {
 
-// 480 threads per column CTA: the 960 radix-5 butterflies of its 4 transforms are exactly 2 rounds (measured best of 400 ... 608
-// once the bank conflicts were gone: 14.4 vs 14.9 ms per 1536 images of 1200^2 at 512)
-constexpr int kGRowThreads = 512, kGColThreads = 480;
-constexpr int kGRowsMax = 2;                       // rows per round of a row-pass CTA
+// Threads per CTA.  The paper's side 1200 runs as 15 x 5 x 16 (register-resident radix-15 and radix-16 butterflies: three
+// stages and three CTA barriers per transform instead of the five of 5 x 5 x 3 x 4 x 4 -- the barriers between stages were
+// the measured bound of round 1's column pass: 3.3 warps waiting at one per issuing warp).  Four transforms per CTA are then
+// 320 + 960 + 300 butterflies: with 320 threads that is 1 + 3 + 1 rounds with (almost) every thread busy.
+constexpr int kGRowThreads = 512, kGColThreads = 480, kGThreads1200 = 320;
+template <int NN> __host__ __device__ constexpr int grow_threads() { return NN == 1200 ? kGThreads1200 : kGRowThreads; }
+template <int NN> __host__ __device__ constexpr int gcol_threads() { return NN == 1200 ? kGThreads1200 : kGColThreads; }
+constexpr int kGRowsMax = 4;                       // rows per round of a row-pass CTA
 struct GPlan {
     int n, nst;
     int radix[16];
@@ -46,29 +52,11 @@ __global__ void gfft_twiddle_kernel(float2 *tw, int n)
     tw[m] = make_float2((float)c, (float)s);
 }
 
-__device__ __forceinline__ void gdft3(float2 &x0, float2 &x1, float2 &x2)
+int gfft_fill_twiddles(float2 *dst, int n, cudaStream_t st)
 {
-    const float2 t = cadd(x1, x2), d = csub(x1, x2);
-    const float2 m = make_float2(x0.x - 0.5f * t.x, x0.y - 0.5f * t.y);
-    const float2 q = make_float2(0.86602540378443864676f * d.x, 0.86602540378443864676f * d.y);
-    x0 = cadd(x0, t);
-    x1 = make_float2(m.x - q.y, m.y + q.x);                    // m + i q
-    x2 = make_float2(m.x + q.y, m.y - q.x);                    // m - i q
-}
-__device__ __forceinline__ void gdft5(float2 &x0, float2 &x1, float2 &x2, float2 &x3, float2 &x4)
-{
-    const float c1 = 0.30901699437494742410f, c2 = -0.80901699437494742410f;      // cos(2 pi / 5), cos(4 pi / 5)
-    const float s1 = 0.95105651629515357212f, s2 = 0.58778525229247312917f;       // sin(2 pi / 5), sin(4 pi / 5)
-    const float2 a1 = cadd(x1, x4), a2 = cadd(x2, x3), b1 = csub(x1, x4), b2 = csub(x2, x3);
-    const float2 p1 = make_float2(x0.x + c1 * a1.x + c2 * a2.x, x0.y + c1 * a1.y + c2 * a2.y);
-    const float2 p2 = make_float2(x0.x + c2 * a1.x + c1 * a2.x, x0.y + c2 * a1.y + c1 * a2.y);
-    const float2 q1 = make_float2(s1 * b1.x + s2 * b2.x, s1 * b1.y + s2 * b2.y);
-    const float2 q2 = make_float2(s2 * b1.x - s1 * b2.x, s2 * b1.y - s1 * b2.y);
-    x0 = cadd(x0, cadd(a1, a2));
-    x1 = make_float2(p1.x - q1.y, p1.y + q1.x);                // p1 + i q1
-    x4 = make_float2(p1.x + q1.y, p1.y - q1.x);
-    x2 = make_float2(p2.x - q2.y, p2.y + q2.x);                // p2 + i q2
-    x3 = make_float2(p2.x + q2.y, p2.y - q2.x);
+    gfft_twiddle_kernel<<<(n + 255) / 256, 256, 0, st>>>(dst, n);
+    BLINK_LAUNCH_CHECK("gfft_twiddle_kernel");
+    return BLINK_OK;
 }
 
 // exact i / d for 0 <= i < 2^16 by a float reciprocal ((i + 1/2) / d is at least 1/(2d) away from an integer, far
@@ -95,20 +83,8 @@ __device__ __forceinline__ void gstage(const float2 *__restrict__ src, float2 *_
             float2 x[R];
 #pragma unroll
             for (int r = 0; r < R; ++r) x[r] = s[r * nb];
-            if constexpr (PP > 1) {
-                const float2 w1 = tw[k];                       // compact per-stage run (stage_twiddles)
-                x[1] = cmul(x[1], w1);
-                if constexpr (R >= 3) {
-                    const float2 w2 = cmul(w1, w1);
-                    x[2] = cmul(x[2], w2);
-                    if constexpr (R >= 4) x[3] = cmul(x[3], cmul(w1, w2));
-                    if constexpr (R >= 5) x[4] = cmul(x[4], cmul(w2, w2));
-                }
-            }
-            if constexpr (R == 2) dft2(x[0], x[1]);
-            if constexpr (R == 3) gdft3(x[0], x[1], x[2]);
-            if constexpr (R == 4) dft4(x[0], x[1], x[2], x[3]);
-            if constexpr (R == 5) gdft5(x[0], x[1], x[2], x[3], x[4]);
+            if constexpr (PP > 1) gtwiddle<R>(x, tw[k]);      // compact per-stage run (stage_twiddles)
+            gbutterfly<R>(x);
             float2 *d = dst + (size_t)tr * ld + (i - k) * R + k;
 #pragma unroll
             for (int r = 0; r < R; ++r) d[r * PP] = x[r];
@@ -124,20 +100,8 @@ __device__ __forceinline__ void gstage(const float2 *__restrict__ src, float2 *_
         float2 x[R];
 #pragma unroll
         for (int r = 0; r < R; ++r) x[r] = s[r * nb];
-        if (P > 1) {                                           // one table read per butterfly; w^2.. are products (<= 2 extra roundings)
-            const float2 w1 = tw[k];                           // compact per-stage run (stage_twiddles)
-            x[1] = cmul(x[1], w1);
-            if constexpr (R >= 3) {
-                const float2 w2 = cmul(w1, w1);
-                x[2] = cmul(x[2], w2);
-                if constexpr (R >= 4) x[3] = cmul(x[3], cmul(w1, w2));
-                if constexpr (R >= 5) x[4] = cmul(x[4], cmul(w2, w2));
-            }
-        }
-        if constexpr (R == 2) dft2(x[0], x[1]);
-        if constexpr (R == 3) gdft3(x[0], x[1], x[2]);
-        if constexpr (R == 4) dft4(x[0], x[1], x[2], x[3]);
-        if constexpr (R == 5) gdft5(x[0], x[1], x[2], x[3], x[4]);
+        if (P > 1) gtwiddle<R>(x, tw[k]);                      // one table read per butterfly; w^2.. are products
+        gbutterfly<R>(x);
         float2 *d = dst + (size_t)tr * ld + (i - k) * R + k;
 #pragma unroll
         for (int r = 0; r < R; ++r) d[r * P] = x[r];
@@ -148,19 +112,19 @@ __device__ __forceinline__ void gstage(const float2 *__restrict__ src, float2 *_
 template <int NN>
 __device__ __forceinline__ float2 *gfft_run(float2 *a, float2 *b, int nt, int ld, const GPlan &pl, const float2 *tw)
 {
-    if constexpr (NN == 1200) {                                // 5 * 5 * 3 * 4 * 4, the plan gfft2d_range builds for 1200
-        gstage<5, 1200, 1>(a, b, nt, 1200, ld, 1, tw);   __syncthreads();               // toff = 0, 1, 6, 31, 106 (gfft2d_range)
-        gstage<5, 1200, 5>(b, a, nt, 1200, ld, 5, tw + 1);   __syncthreads();
-        gstage<3, 1200, 25>(a, b, nt, 1200, ld, 25, tw + 6); __syncthreads();
-        gstage<4, 1200, 75>(b, a, nt, 1200, ld, 75, tw + 31); __syncthreads();
-        gstage<4, 1200, 300>(a, b, nt, 1200, ld, 300, tw + 106); __syncthreads();
+    if constexpr (NN == 1200) {                                // 15 * 5 * 16, the plan gfft2d_range builds for 1200
+        gstage<15, 1200, 1>(a, b, nt, 1200, ld, 1, tw);       __syncthreads();          // toff = 0, 1, 16 (gfft2d_range)
+        gstage<5, 1200, 15>(b, a, nt, 1200, ld, 15, tw + 1);  __syncthreads();
+        gstage<16, 1200, 75>(a, b, nt, 1200, ld, 75, tw + 16); __syncthreads();
         return b;
     }
     int P = 1;
     for (int s = 0; s < pl.nst; ++s) {
         const int R = pl.radix[s];
         const float2 *tws = tw + pl.toff[s];
-        if (R == 4) gstage<4>(a, b, nt, pl.n, ld, P, tws);
+        if (R == 16) gstage<16>(a, b, nt, pl.n, ld, P, tws);
+        else if (R == 15) gstage<15>(a, b, nt, pl.n, ld, P, tws);
+        else if (R == 4) gstage<4>(a, b, nt, pl.n, ld, P, tws);
         else if (R == 2) gstage<2>(a, b, nt, pl.n, ld, P, tws);
         else if (R == 3) gstage<3>(a, b, nt, pl.n, ld, P, tws);
         else gstage<5>(a, b, nt, pl.n, ld, P, tws);
@@ -173,7 +137,7 @@ __device__ __forceinline__ float2 *gfft_run(float2 *a, float2 *b, int nt, int ld
 
 // ------------------------------------------------------------------------------------------ rows
 template <int NN>
-__global__ void __launch_bounds__(kGRowThreads)
+__global__ void __launch_bounds__(grow_threads<NN>())
 gfft_rows_kernel(float2 *__restrict__ grid, long long n_rows, const GPlan pl, const float2 *__restrict__ tw, int nr, int rows_per_img,
                  int row_off, const int *__restrict__ ext, int ext_div)
 {
@@ -227,7 +191,7 @@ gfft_rows_kernel(float2 *__restrict__ grid, long long n_rows, const GPlan pl, co
 
 // ------------------------------------------------------------------------------------------ columns + epilogue
 template <int NN>
-__global__ void __launch_bounds__(kGColThreads)
+__global__ void __launch_bounds__(gcol_threads<NN>())
 gfft_cols_kernel(const float2 *__restrict__ grid, const GPlan pl, const float2 *__restrict__ tw, int kc, const float *__restrict__ scale,
                  int scale_div, int img_base, float *__restrict__ image, float *__restrict__ image_imag)
 {
@@ -269,7 +233,7 @@ gfft_cols_kernel(const float2 *__restrict__ grid, const GPlan pl, const float2 *
 // x1, x2 become ONE complex transform Z[v] = R[v][x1] + i R[v][x2], Z[-v] = conj R[v][x1] + i conj R[v][x2] whose
 // real part is image column x1 and imaginary part image column x2.  Half the reads, half the transforms.
 template <int NN>
-__global__ void __launch_bounds__(kGColThreads)
+__global__ void __launch_bounds__(gcol_threads<NN>())
 gfft_cols_herm_kernel(const float2 *__restrict__ grid, const GPlan pl, const float2 *__restrict__ tw, int kc, const float *__restrict__ scale,
                       int scale_div, int img_base, float *__restrict__ image, const int *__restrict__ ext, int ext_div, int ext_base, int ld)
 {
@@ -342,8 +306,10 @@ int gfft2d_range(float2 *grid, int n, int batch, const float *scale, int scale_d
     GPlan pl{};
     pl.n = n;
     int m = n;
-    while (m % 5 == 0) { pl.radix[pl.nst++] = 5; m /= 5; }     // odd radices first (see gstage)
+    while (m % 15 == 0) { pl.radix[pl.nst++] = 15; m /= 15; }  // odd radices first (see gstage); 15 and 16 in registers
+    while (m % 5 == 0) { pl.radix[pl.nst++] = 5; m /= 5; }
     while (m % 3 == 0) { pl.radix[pl.nst++] = 3; m /= 3; }
+    while (m % 16 == 0) { pl.radix[pl.nst++] = 16; m /= 16; }
     while (m % 4 == 0) { pl.radix[pl.nst++] = 4; m /= 4; }
     while (m % 2 == 0) { pl.radix[pl.nst++] = 2; m /= 2; }
     if (m != 1) return BLINK_ERR_UNSUPPORTED;
@@ -353,7 +319,8 @@ int gfft2d_range(float2 *grid, int n, int batch, const float *scale, int scale_d
     const size_t per = 2 * (size_t)(n + 16) * sizeof(float2);   // ping + pong of one transform (padded leading dimension: n + 1, or herm_ld)
     const size_t twb = (size_t)n * sizeof(float2);              // + the twiddle table staged in shared memory
     const size_t budget = 200 * 1024 - twb;
-    int nr = (int)std::min<size_t>(kGRowsMax, budget / per);
+    // rows per round: the paper's side takes 4 (two CTAs of 320 threads per SM), the others 2 as before
+    int nr = (int)std::min<size_t>(n == 1200 ? 4 : 2, n == 1200 ? (100 * 1024 - twb) / per : budget / per);
     int kc = 1;
     for (int c = 8; c >= 1; c >>= 1)
         if ((n / 2) % c == 0 && (size_t)c * per <= budget) { kc = c; break; }
@@ -367,7 +334,9 @@ int gfft2d_range(float2 *grid, int n, int batch, const float *scale, int scale_d
     const int rows_per_img = hermitian ? n / 2 : n, row_off = hermitian ? n / 2 : 0;
     const long long n_rows = (long long)batch * rows_per_img;
     const long long want = (n_rows + nr - 1) / nr, cap = (long long)sm_count() * 8;
-    rows_k<<<(unsigned)(want < cap ? want : cap), kGRowThreads, nr * per + twb, st>>>(grid, n_rows, pl, tw, nr, rows_per_img, row_off,
+    const int row_threads = n == 1200 ? grow_threads<1200>() : grow_threads<0>();
+    const int col_threads = n == 1200 ? gcol_threads<1200>() : gcol_threads<0>();
+    rows_k<<<(unsigned)(want < cap ? want : cap), row_threads, nr * per + twb, st>>>(grid, n_rows, pl, tw, nr, rows_per_img, row_off,
                                                                                            hermitian ? row_extent : nullptr, ext_div);
     BLINK_LAUNCH_CHECK("gfft_rows_kernel");
     // Hermitian: kc columns are kc/2 transforms; keep two CTAs per SM when the arrays allow it
@@ -381,12 +350,12 @@ int gfft2d_range(float2 *grid, int n, int batch, const float *scale, int scale_d
     for (int b0 = 0; b0 < batch; b0 += 65535) {
         const int nb = batch - b0 < 65535 ? batch - b0 : 65535;
         if (hermitian)
-            herm_k<<<dim3(n / kch, nb), kGColThreads, (kch / 2) * per + twb, st>>>(grid + (size_t)b0 * n * n, pl, tw, kch, scale,
+            herm_k<<<dim3(n / kch, nb), col_threads, (kch / 2) * per + twb, st>>>(grid + (size_t)b0 * n * n, pl, tw, kch, scale,
                                                                                           scale_div, img_base + b0,
                                                                                           image + (size_t)b0 * n * n, row_extent, ext_div, b0,
                                                                                           herm_ld(n, kch / 2));
         else
-            cols_k<<<dim3(n / kc, nb), kGColThreads, kc * per + twb, st>>>(grid + (size_t)b0 * n * n, pl, tw, kc, scale, scale_div,
+            cols_k<<<dim3(n / kc, nb), col_threads, kc * per + twb, st>>>(grid + (size_t)b0 * n * n, pl, tw, kc, scale, scale_div,
                                                                            img_base + b0, image + (size_t)b0 * n * n,
                                                                            image_imag ? image_imag + (size_t)b0 * n * n : nullptr);
         BLINK_LAUNCH_CHECK("gfft_cols_kernel");

@@ -90,11 +90,19 @@ __global__ void counts_kernel(const float *__restrict__ uvw_m, const ScaleBlock 
     atomicAdd(&dst[mirror_of(cell, n)], 1u);
 }
 
+// the fused kernel of the paper's own side, 1200 x 1200 (blink_fused_g.cu)
+bool fused_g_supported(int B, int n_pix);
+size_t fused_g_workspace_bytes(int T, int B, int ctas);
+int fused_g_image(const float2 *vis, const float *uvw_m, const double *freqs_hz, double pixscale_rad, int T, int C, int P, int B,
+                  int weighting, int tc0, int ntc, float *image, float *wsum, int32_t *cell_idx, void *workspace,
+                  size_t workspace_bytes, cudaStream_t st, GainRef cal);
+
 // ------------------------------------------------------------------------------------------ host
 bool fused_supported(int P, int B, int n_pix, int weighting)
 {
     (void)P;
     if (B > kSortMaxB) return false;
+    if (n_pix == 1200) return fused_g_supported(B, n_pix);
     const bool uni = weighting == BLINK_W_UNIFORM;
     switch (n_pix) {
         case 256: return fused_stages<256>(B, uni) > 0;
@@ -119,6 +127,7 @@ int presort_launch(const float *uvw_m, int T, int B, float *su, uint2 *svb, cuda
 }
 size_t fused_workspace_bytes(int T, int B, int n_pix, int ctas)
 {
+    if (n_pix == 1200) return fused_g_workspace_bytes(T, B, ctas);
     return sort_bytes(T, B) + (size_t)ctas * (n_pix / 2) * n_pix * sizeof(float2);
 }
 int fused_default_ctas() { return sm_count() > 0 ? sm_count() : 148; }
@@ -137,6 +146,8 @@ int fused_image(const float2 *vis, const float *uvw_m, const double *freqs_hz, d
         case 1024: return launch_fused<1024>(a, freqs_hz, pixscale_rad, workspace, workspace_bytes, st);
         case 2048: return launch_fused<2048>(a, freqs_hz, pixscale_rad, workspace, workspace_bytes, st);
         case 4096: return launch_fused<4096>(a, freqs_hz, pixscale_rad, workspace, workspace_bytes, st);
+        case 1200: return fused_g_image(vis, uvw_m, freqs_hz, pixscale_rad, T, C, P, B, weighting, tc0, ntc, image, wsum, cell_idx,
+                                        workspace, workspace_bytes, st, cal);
         default: return BLINK_ERR_UNSUPPORTED;
     }
 }

@@ -1,0 +1,377 @@
+// Fused imaging kernel for the paper's own image side, 1200 x 1200 (Table 6): visibilities ->
+// dirty images with the uv grid never materialised, the design of blink_fused.cu carried over to a side that is not a
+// power of two (1200 = 15 x 5 x 16).
+//
+//   * presort (blink_fused.cu): per timestep the baselines sorted by |u_m|, folded into the half plane u >= 0, so that for
+//     every channel the samples of a u-column are one contiguous range of the list;
+//   * one persistent CTA per SM walks over (t,c); it holds FG_G transform groups of 160 threads that run DECOUPLED behind
+//     their own named barriers.  A group owns one shared-memory array of 2 x 1200 complex64 and works on TWO transforms at
+//     a time: 80 + 80 radix-15 butterflies, 240 + 240 radix-5 butterflies (three rounds), 75 + 75 radix-16 butterflies --
+//     every stage register-resident (blink_fftg.cuh), in place in the array (read -> barrier -> write -> barrier);
+//   * pass 1, per column pair (u0, u0+1): grid the pair's samples into the (zeroed) array with native 64-bit exchanges
+//     (cell_add_exch), divide by the cell counts for uniform weighting while loading the first stage, transform along v,
+//     and store the result TRANSPOSED, HT[ky][u], to the per-CTA scratch straight from the registers of the last stage;
+//   * pass 2, per two row pairs (ky, ky+1), (ky+2, ky+3): Z[u] = HT[ky][u] + i HT[ky+1][u], Z[N-u] = conj + i conj (the
+//     Hermitian packing of blink_fused.cu); the four rows -- only the columns u < ulim hold anything -- arrive in a
+//     per-group staging buffer by bulk async copies issued one unit ahead, are transformed along u, and stored as two real image rows from the
+//     registers of the last stage with the shift, 1/W and the real part folded in (centred index = (j + N/2) mod N).
+// Steps a0-a5 of include/blinkimg.h; PAPER.md L190-194 (gridding, inverse 2D FFT, shift), L150 (fp32).
+#include <algorithm>
+
+#include "blink_fused_kernel.cuh"
+#include "blink_fftg.cuh"
+
+namespace blink {
+
+constexpr int FG_N = 1200, FG_H = 600;
+constexpr int FG_TG = 160;                                      // threads per group (5 warps)
+constexpr int FG_G = 4;                                         // groups per CTA
+constexpr int FG_THREADS = FG_TG * FG_G;                        // 640
+constexpr int FG_LD = 1208;                                     // leading dimension of a group's two arrays (complex64)
+constexpr int FG_TW = 1 + 15 + 75;                              // compact twiddle runs of the three stages
+constexpr int kFgMaxB = 15000;                                 // the staged visibility row must fit next to the arrays
+
+// shared memory: arrays | twiddle runs | column offsets | mbarriers | U = union( pass 1: visibility row + 16-bit cell counts,
+//                                                                               pass 2: per-group staging of 4 rows of HT )
+struct FgSmem {
+    static constexpr size_t ARR = (size_t)FG_G * 2 * FG_LD * sizeof(float2);          // 77.3 KB
+    static constexpr size_t CNT = (size_t)FG_G * 2 * (FG_N / 2) * sizeof(uint32_t);    // 19.2 KB: 16-bit counts, two per word
+    static constexpr size_t TW = ((size_t)FG_TW * sizeof(float2) + 15) & ~(size_t)15;
+    static constexpr size_t COFF = ((size_t)(FG_H + 2) * 4 + 15) & ~(size_t)15;
+    static constexpr size_t BARS = 64;                                                 // visbar + FG_G staging barriers
+    static constexpr size_t STG_G = (size_t)4 * FG_H * sizeof(float2);                 // 19.2 KB per group: 4 rows x 600 columns
+    static constexpr size_t HEAD = ARR + TW + COFF + BARS;
+    __host__ __device__ static size_t front(int B) { return ((size_t)B * 8 + 15) & ~(size_t)15; }
+    __host__ __device__ static size_t uni(int B) { return front(B) + CNT > FG_G * STG_G ? front(B) + CNT : FG_G * STG_G; }
+    static size_t bytes(int B) { return HEAD + uni(B) + 16; }
+};
+
+// One in-place Stockham stage of the group's two transforms (radix R, sub-transform length P; see gstage in blink_fftg.cu):
+//   input  element n of transform tr:  load(tr, n)           (FIRST)  or  arr[tr * LD + n]
+//   output element j of transform tr:  emit(tr, j, value)    (LAST)   or  arr[tr * LD + j]
+// Butterfly i reads n = i + r N/R and writes j = (i - k) R + k + r P, k = i mod P.  All of a thread's butterflies (ROUNDS of
+// them) are loaded before the barrier that separates the stage's reads from its writes.
+struct FgNoHook { __device__ __forceinline__ void operator()() const {} };
+template <int R, int P, bool FIRST, bool LAST, class Sync, class Load, class Emit, class Hook = FgNoHook>
+__device__ __forceinline__ void fg_stage(float2 *arr, const float2 *__restrict__ tw, int tid, Sync gsync, Load load, Emit emit,
+                                         Hook hook = Hook())
+{
+    constexpr int nb = FG_N / R, total = 2 * nb, ROUNDS = (total + FG_TG - 1) / FG_TG;
+    float2 x[ROUNDS][R];
+#pragma unroll
+    for (int q = 0; q < ROUNDS; ++q) {
+        const int idx = tid + q * FG_TG;
+        if (idx < total) {
+            const int tr = idx >= nb, i = idx - tr * nb;
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                if constexpr (FIRST) x[q][r] = load(tr, i + r * nb);
+                else x[q][r] = arr[tr * FG_LD + i + r * nb];
+            }
+            if constexpr (P > 1) gtwiddle<R>(x[q], tw[i % P]);
+            gbutterfly<R>(x[q]);
+        }
+    }
+    if constexpr (!LAST) {
+        gsync();                                               // every read of the array is done (also the previous unit's)
+        hook();                                                // FIRST: the stage's inputs are in registers
+#pragma unroll
+        for (int q = 0; q < ROUNDS; ++q) {
+            const int idx = tid + q * FG_TG;
+            if (idx < total) {
+                const int tr = idx >= nb, i = idx - tr * nb, k = i % P;
+                float2 *d = arr + tr * FG_LD + (i - k) * R + k;
+#pragma unroll
+                for (int r = 0; r < R; ++r) d[r * P] = x[q][r];
+            }
+        }
+        gsync();
+    } else {
+#pragma unroll
+        for (int q = 0; q < ROUNDS; ++q) {
+            const int idx = tid + q * FG_TG;
+            if (idx < total) {
+                const int tr = idx >= nb, i = idx - tr * nb, k = i % P;
+#pragma unroll
+                for (int r = 0; r < R; ++r) emit(tr, (i - k) * R + k + r * P, x[q][r]);
+            }
+        }
+    }
+}
+
+// the three stages of 1200 = 15 x 5 x 16; twiddle runs at tw + 0 (unused), + 1 (P = 15), + 16 (P = 75)
+template <class Sync, class Load, class Emit, class Hook = FgNoHook>
+__device__ __forceinline__ void fg_transform2(float2 *arr, const float2 *tw, int tid, Sync gsync, Load load, Emit emit, Hook hook = Hook())
+{
+    auto no_load = [](int, int) { return make_float2(0.f, 0.f); };
+    auto no_emit = [](int, int, float2) {};
+    fg_stage<15, 1, true, false>(arr, tw, tid, gsync, load, no_emit, hook);
+    fg_stage<5, 15, false, false>(arr, tw + 1, tid, gsync, no_load, no_emit);
+    fg_stage<16, 75, false, true>(arr, tw + 16, tid, gsync, no_load, emit);
+}
+
+__global__ void __launch_bounds__(FG_THREADS, 1)
+fused_g_kernel(const FusedArgs a, const __grid_constant__ ScaleBlock sc, const float2 *__restrict__ tw_full)
+{
+    constexpr int N = FG_N, H = FG_H;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const bool uniform = a.weighting == BLINK_W_UNIFORM;
+    const int B = a.B;
+    const int g = threadIdx.x / FG_TG, tid = threadIdx.x % FG_TG, lane = threadIdx.x & 31;
+
+    unsigned char *q = smem_raw + ((16 - (smem_u32(smem_raw) & 15u)) & 15u);
+    float2 *arr_all = reinterpret_cast<float2 *>(q);             q += FgSmem::ARR;
+    float2 *stw = reinterpret_cast<float2 *>(q);                 q += FgSmem::TW;
+    uint32_t *coff = reinterpret_cast<uint32_t *>(q);            q += FgSmem::COFF;
+    uint64_t *visbar = reinterpret_cast<uint64_t *>(q);          q += FgSmem::BARS;
+    uint64_t *stbar = visbar + 1 + g;                            // this group's staging barrier
+    float2 *visrow = reinterpret_cast<float2 *>(q);                                               // U, pass 1: [B]
+    uint32_t *cnt_all = reinterpret_cast<uint32_t *>(q + FgSmem::front(B));
+    float2 *stg = reinterpret_cast<float2 *>(q + (size_t)g * FgSmem::STG_G);                      // U, pass 2: [4][ulim]
+    float2 *arr = arr_all + (size_t)g * 2 * FG_LD;
+    uint32_t *cnt = cnt_all + (size_t)g * 2 * (N / 2);           // cnt[tr * 600 + (n >> 1)], 16 bits per cell
+    __shared__ int s_nin, s_occ, s_ncol;
+
+    float2 *HT = a.scratch + (size_t)blockIdx.x * N * H;         // [N ky][H u], transposed pass-1 output
+    auto gsync = [g] { asm volatile("bar.sync %0, %1;" ::"r"(g + 1), "n"(FG_TG) : "memory"); };
+    const float lim = (float)(H - 1);
+
+    // compact per-stage twiddle runs: stage with sub-transform length P reads W_N^(k N / (P R)), k < P
+    for (int k = threadIdx.x; k < FG_TW; k += FG_THREADS) {
+        int step, kk;
+        if (k < 1) { step = 0; kk = 0; }
+        else if (k < 16) { step = N / (15 * 5); kk = k - 1; }
+        else { step = N / (75 * 16); kk = k - 16; }
+        stw[k] = tw_full[kk * step];
+    }
+    if (threadIdx.x == 0) {
+        for (int k = 0; k <= FG_G; ++k) mbar_init(visbar + k, 1);
+        fence_mbar_init();
+    }
+    uint32_t vph = 0, sph = 0;
+    const bool bulk = (B & 1) == 0;
+    const int tc_end = a.tc0 + a.ntc;
+    __syncthreads();
+    auto clear_group = [&] {                                    // this group's arrays (and counts): zero for the next gridding
+        float4 *z = reinterpret_cast<float4 *>(arr);
+        for (int i = tid; i < 2 * FG_LD / 2; i += FG_TG) z[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (uniform) for (int i = tid; i < 2 * (N / 2); i += FG_TG) cnt[i] = 0u;
+    };
+
+    for (int tc = a.tc0 + blockIdx.x; tc < tc_end; tc += gridDim.x) {
+        const int t = tc / a.C, c = tc - t * a.C;
+        const float s = sc.s[c - a.c_base];
+        const float *su = a.su + (size_t)t * B;
+        const uint2 *svb = a.svb + (size_t)t * B;
+        auto col_of = [&](float x) -> int {                     // column of sorted sample value x = |u_m| (H = off the grid, NaN too)
+            int i;
+            const float xr = rint_rne(__fmul_rn(x, s), i);
+            return (xr <= lim) ? i : H;
+        };
+        int n_cp = 0, ulim = 0;
+        float wsum_val = 0.f;
+
+        for (int p = 0; p < a.P; ++p) {
+            const size_t img_idx = (size_t)tc * a.P + p;
+            float *img = a.image + img_idx * N * N;
+            __syncthreads();                                    // (C) every group has finished the previous pass 2: U is free
+            if (bulk) {
+                if (threadIdx.x == 0) {                         // the image's visibility row, by one bulk async copy
+                    fence_proxy_async();
+                    mbar_expect_tx(visbar, (uint32_t)B * 8u);
+                    bulk_load_1d(visrow, a.vis + img_idx * B, (uint32_t)B * 8u, visbar);
+                }
+            } else {
+                const float2 *vrow = a.vis + img_idx * B;       // odd B: rows are only 8-byte aligned
+                for (int i = threadIdx.x; i < B; i += FG_THREADS) visrow[i] = vrow[i];
+            }
+            clear_group();
+            if (p == 0) {
+                if (threadIdx.x == 0) { s_nin = 0; s_occ = 0; }
+                // column offsets: coff[u] = first sorted sample whose column is >= u, u = 0..H+1 (sample B = sentinel of column H+1)
+                for (int j = threadIdx.x; j <= B; j += FG_THREADS) {
+                    const int cj = j < B ? col_of(__ldg(su + j)) : H + 1;
+                    const int cq = j > 0 ? col_of(__ldg(su + j - 1)) : -1;
+                    for (int u = cq + 1; u <= cj; ++u) coff[u] = (uint32_t)j;
+                    if (cj >= H && cq < H) s_ncol = cq + 1;      // occupied columns are [0, cq]
+                }
+                if (a.cell_idx) {
+                    const float *uvw = a.uvw_m + (size_t)t * B * 3;
+                    for (int b = threadIdx.x; b < B; b += FG_THREADS)
+                        a.cell_idx[(size_t)tc * B + b] = cell_of(uvw[3 * b], uvw[3 * b + 1], s, N, H);
+                }
+            }
+            __syncthreads();                                    // (A)
+            if (p == 0) {
+                n_cp = (s_ncol + 1) / 2;
+                ulim = 2 * n_cp;
+            }
+            if (bulk) { mbar_wait(visbar, vph); vph ^= 1u; }
+            if (a.cal.gains) {                                  // corrections fused into the load (R15)
+                const float2 *gc = a.cal.gains + ((size_t)c * a.P + p) * a.cal.A;
+                for (int i = threadIdx.x; i < B; i += FG_THREADS) {
+                    const int2 ap = __ldg(a.cal.ant + i);
+                    const float2 g1 = __ldg(gc + ap.x), g2 = __ldg(gc + ap.y);
+                    visrow[i] = cmul(visrow[i], cmul(g1, make_float2(g2.x, -g2.y)));
+                }
+                __syncthreads();
+            }
+
+            // ================= pass 1: column pairs (2cp, 2cp+1): grid, transform along v, store transposed ==========
+            int my_in = 0, my_occ = 0;
+            for (int cp = g; cp < n_cp; cp += FG_G) {
+                const int u0 = 2 * cp;
+                const int k0 = (int)coff[u0], k1 = (int)coff[u0 + 1], k2 = (int)coff[u0 + 2];
+                gsync();                                        // the arrays are zero (clear_group of the previous unit / image)
+                for (int j = k0 + tid; j < k2; j += FG_TG) {
+                    const uint2 sq = __ldg(svb + j);
+                    int iv;
+                    const float yr = rint_rne(__fmul_rn(__uint_as_float(sq.x), s), iv);
+                    if (fabsf(yr) <= lim) {                     // NaN fails; |iu| <= H-1 by construction
+                        float2 vv = visrow[sq.y & 0x7fffffffu];
+                        if (sq.y >> 31) vv.y = -vv.y;
+                        const int tr = j >= k1;
+                        const int n = iv < 0 ? iv + N : iv;     // transform index of centred row iv + H
+                        cell_add_exch(&arr[tr * FG_LD + n], vv);
+                        if (uniform) atomicAdd(&cnt[tr * (N / 2) + (n >> 1)], 1u << ((n & 1) * 16));
+                        if (u0 == 0 && !tr) {                   // iu == 0: the conjugate lies in column 0 too, at row -iv
+                            const int n2 = iv > 0 ? N - iv : -iv;
+                            cell_add_exch(&arr[n2], make_float2(vv.x, -vv.y));
+                            if (uniform) atomicAdd(&cnt[n2 >> 1], 1u << ((n2 & 1) * 16));
+                        }
+                        ++my_in;
+                    }
+                }
+                gsync();
+                auto load = [&](int tr, int n) -> float2 {      // a3: divide by the cell count (uniform weighting)
+                    float2 v = arr[tr * FG_LD + n];
+                    if (uniform) {
+                        const uint32_t cn = (cnt[tr * (N / 2) + (n >> 1)] >> ((n & 1) * 16)) & 0xffffu;
+                        if (cn) {
+                            v.x = __fdiv_rn(v.x, (float)cn);
+                            v.y = __fdiv_rn(v.y, (float)cn);
+                            my_occ += (u0 + tr == 0) ? 1 : 2;   // the mirror image of a u > 0 cell is occupied too
+                        }
+                    }
+                    return v;
+                };
+                auto emit = [&](int tr, int ky, float2 v) { HT[(size_t)ky * H + u0 + tr] = v; };
+                fg_transform2(arr, stw, tid, gsync, load, emit);
+                gsync();                                        // the last stage's reads are done: zero for the next unit
+                clear_group();
+            }
+            if (p == 0) {
+#pragma unroll
+                for (int d = 16; d > 0; d >>= 1) {
+                    my_occ += __shfl_xor_sync(0xffffffffu, my_occ, d);
+                    my_in += __shfl_xor_sync(0xffffffffu, my_in, d);
+                }
+                if (lane == 0) { atomicAdd(&s_occ, my_occ); atomicAdd(&s_nin, my_in); }
+            }
+            // HT stores (generic proxy) must be visible to the bulk copies (async proxy) of pass 2
+            __threadfence();
+            asm volatile("fence.proxy.async;" ::: "memory");
+            __syncthreads();                                    // (B) pass 1 is over: U turns into the staging buffers
+            if (p == 0) wsum_val = uniform ? (float)s_occ : (float)(2 * s_nin);
+            if (wsum_val == 0.f) {
+                for (int i = threadIdx.x; i < N * N / 4; i += FG_THREADS)
+                    reinterpret_cast<float4 *>(img)[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+                continue;
+            }
+            const float inv_w = 1.0f / wsum_val;
+
+            // ================= pass 2: two row pairs per unit -> four real image rows ===================================
+            // The four rows HT[ky0 .. ky0+3][0 .. ulim) of a unit are staged by bulk async copies into the group's buffer one
+            // unit ahead: the request for unit k+1 goes out right after the barrier that follows unit k's first-stage reads
+            // (the only reads of the buffer), so it lands while unit k runs its remaining stages and stores.
+            const uint32_t row_bytes = (uint32_t)ulim * 8u;     // ulim is even: a multiple of 16 bytes
+            auto request = [&](int unit) {
+                fence_proxy_async();
+                mbar_expect_tx(stbar, 4u * row_bytes);
+#pragma unroll
+                for (int r = 0; r < 4; ++r) bulk_load_1d(stg + (size_t)r * ulim, HT + (size_t)(4 * unit + r) * H, row_bytes, stbar);
+            };
+            if (tid == 0 && g < N / 4) request(g);
+            for (int unit = g; unit < N / 4; unit += FG_G) {
+                const int ky0 = 4 * unit;
+                mbar_wait(stbar, sph);
+                sph ^= 1u;
+                auto load = [&](int tr, int n) -> float2 {
+                    const float2 *r0 = stg + (size_t)(2 * tr) * ulim, *r1 = r0 + ulim;
+                    if (n < H) {                                // Z[u] = S1 + i S2
+                        if (n >= ulim) return make_float2(0.f, 0.f);
+                        const float2 s1 = r0[n], s2 = r1[n];
+                        return make_float2(s1.x - s2.y, s1.y + s2.x);
+                    }
+                    const int u = N - n;                        // Z[N - u] = conj(S1) + i conj(S2); u = H is the empty column
+                    if (u >= ulim || n == H) return make_float2(0.f, 0.f);
+                    const float2 s1 = r0[u], s2 = r1[u];
+                    return make_float2(s1.x + s2.y, s2.x - s1.y);
+                };
+                auto emit = [&](int tr, int j, float2 z) {
+                    const int ky = ky0 + 2 * tr;
+                    const int y0 = ky < H ? ky + H : ky - H, y1 = ky + 1 < H ? ky + 1 + H : ky + 1 - H;
+                    const int x = j < H ? j + H : j - H;        // fftshift of both axes
+                    __stcs(img + (size_t)y0 * N + x, z.x * inv_w);
+                    __stcs(img + (size_t)y1 * N + x, z.y * inv_w);
+                };
+                auto after_first_reads = [&] {                  // runs right after the first stage's read -> write barrier
+                    if (tid == 0 && unit + FG_G < N / 4) request(unit + FG_G);
+                };
+                fg_transform2(arr, stw, tid, gsync, load, emit, after_first_reads);
+            }
+        }
+        if (threadIdx.x == 0) a.wsum[tc] = wsum_val;
+    }
+}
+
+// ------------------------------------------------------------------------------------------ host
+bool fused_g_supported(int B, int n_pix)
+{
+    return n_pix == FG_N && B <= kFgMaxB && B <= 16384 && FgSmem::bytes(B) <= kSmemLimit;
+}
+size_t fused_g_workspace_bytes(int T, int B, int ctas)
+{
+    return sort_bytes(T, B) + align_up((size_t)FG_N * sizeof(float2), 256) + (size_t)ctas * FG_N * FG_H * sizeof(float2);
+}
+int gfft_fill_twiddles(float2 *dst, int n, cudaStream_t st);      // blink_fftg.cu: dst[m] = exp(2 pi i m / n), evaluated in double
+
+int fused_g_image(const float2 *vis, const float *uvw_m, const double *freqs_hz, double pixscale_rad, int T, int C, int P, int B,
+                  int weighting, int tc0, int ntc, float *image, float *wsum, int32_t *cell_idx, void *workspace,
+                  size_t workspace_bytes, cudaStream_t st, GainRef cal)
+{
+    const size_t per_cta = (size_t)FG_N * FG_H * sizeof(float2);
+    const size_t twb = align_up((size_t)FG_N * sizeof(float2), 256);
+    const size_t sortb = sort_bytes(T, B);
+    if (!workspace || (reinterpret_cast<uintptr_t>(workspace) & 255u) || workspace_bytes < sortb + twb + per_cta) return BLINK_ERR_WORKSPACE;
+    int ctas = option(BLINK_OPT_FUSED_CTAS);
+    if (ctas <= 0) ctas = fused_default_ctas();
+    ctas = (int)std::min<size_t>((size_t)ctas, (workspace_bytes - sortb - twb) / per_cta);
+    unsigned char *wsp = static_cast<unsigned char *>(workspace);
+    float *su = reinterpret_cast<float *>(wsp);
+    uint2 *svb = reinterpret_cast<uint2 *>(wsp + sortb / 3);
+    float2 *tw = reinterpret_cast<float2 *>(wsp + sortb);
+    float2 *scratch = reinterpret_cast<float2 *>(wsp + sortb + twb);
+    int rc = presort_launch(uvw_m, T, B, su, svb, st);
+    if (rc != BLINK_OK) return rc;
+    rc = gfft_fill_twiddles(tw, FG_N, st);
+    if (rc != BLINK_OK) return rc;
+    const size_t smem = FgSmem::bytes(B);
+    BLINK_CUDA_TRY(cudaFuncSetAttribute(fused_g_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    FusedArgs base{};
+    base.cal = cal;
+    base.vis = vis; base.uvw_m = uvw_m; base.T = T; base.C = C; base.P = P; base.B = B; base.weighting = weighting;
+    base.image = image; base.wsum = wsum; base.cell_idx = cell_idx;
+    return for_channel_blocks(C, tc0, ntc, freqs_hz, FG_N, pixscale_rad,
+                              [&](int s0, int m, int c_base, const ScaleBlock &sc) -> int {
+                                  FusedArgs a = base;
+                                  a.tc0 = s0; a.ntc = m; a.c_base = c_base;
+                                  a.scratch = scratch; a.su = su; a.svb = svb;
+                                  const int grid = m < ctas ? m : ctas;
+                                  fused_g_kernel<<<grid, FG_THREADS, smem, st>>>(a, sc, tw);
+                                  BLINK_LAUNCH_CHECK("fused_g_kernel");
+                                  return (int)BLINK_OK;
+                              });
+}
+
+}  // namespace blink

@@ -50,7 +50,7 @@ static int image_device(const float2 *vis, const float *uvw_m, const double *fre
 {
     // image / wsum / cell_idx / counts are indexed by ABSOLUTE tc; the range [tc0, tc0+ntc) is processed
     const size_t n2 = (size_t)n_pix * n_pix;
-    if (cal.gains && !use_fused(P, B, n_pix, weighting)) return BLINK_ERR_UNSUPPORTED;   // gains are fused into the fused kernel only
+    if (cal.gains && !use_fused(P, B, n_pix, weighting)) return BLINK_ERR_UNSUPPORTED;   // callers apply the gains first there (blink_image_cal)
     bool fused = use_fused(P, B, n_pix, weighting);
     // A handful of images leaves most SMs idle under the fused kernel (one CTA per image: 144 us for ONE 256 x 256 image,
     // config 1); the unfused chain spreads the rows and columns of an image over many CTAs (56 us).  Taken when the whole
@@ -101,7 +101,7 @@ __device__ __forceinline__ float2 gain_factor(const float2 *gc, int2 ap)
 }
 template <int VEC>
 __global__ void __launch_bounds__(256)
-apply_gains_kernel(float2 *__restrict__ vis, const float2 *__restrict__ gains, const int2 *__restrict__ ant, long long n_rows,
+apply_gains_kernel(float2 *vis, const float2 *src, const float2 *__restrict__ gains, const int2 *__restrict__ ant, long long n_rows,
                    int C, int P, int B, int A)
 {
     const int b = (blockIdx.x * blockDim.x + threadIdx.x) * VEC;
@@ -113,14 +113,15 @@ apply_gains_kernel(float2 *__restrict__ vis, const float2 *__restrict__ gains, c
         const int p = (int)(row % P), c = (int)((row / P) % C);
         const float2 *gc = gains + ((size_t)c * P + p) * A;
         float2 *dst = vis + row * B + b;
+        const float2 *in = src + row * B + b;                                                  // src == vis: in place
         if constexpr (VEC == 2) {
             const float2 f0 = gain_factor(gc, ap[0]), f1 = gain_factor(gc, ap[1]);
-            float4 v = *reinterpret_cast<float4 *>(dst);
+            float4 v = *reinterpret_cast<const float4 *>(in);
             v = make_float4(f0.x * v.x - f0.y * v.y, f0.x * v.y + f0.y * v.x, f1.x * v.z - f1.y * v.w, f1.x * v.w + f1.y * v.z);
             *reinterpret_cast<float4 *>(dst) = v;
         } else {
             const float2 f = gain_factor(gc, ap[0]);
-            const float2 v = *dst;
+            const float2 v = *in;
             *dst = make_float2(f.x * v.x - f.y * v.y, f.x * v.y + f.y * v.x);
         }
     }
@@ -200,6 +201,15 @@ extern "C" int blink_workspace_bytes(int op, int T, int C, int P, int B, int n_p
         case BLINK_OP_FFT2D:
             rec = mn = gfft_workspace_bytes(n_pix);
             break;
+        case BLINK_OP_IMAGE_CAL: {                              // fused sizes: as blink_image; else + the corrected copy
+            size_t r1 = 0, m1 = 0;
+            int rc1 = blink_workspace_bytes(BLINK_OP_IMAGE, T, C, P, B, n_pix, weighting, &r1, &m1);
+            if (rc1 != BLINK_OK) return rc1;
+            const size_t corr = use_fused(P, B, n_pix, weighting) ? 0 : align_up((size_t)T * C * P * B * sizeof(float2), 256);
+            rec = corr + r1;
+            mn = corr + m1;
+            break;
+        }
         case BLINK_OP_IMAGE_STOKES_I: {                         // combined visibilities + a one-plane blink_image
             if (P != 2 && P != 4) return BLINK_ERR_INVALID_ARG;
             size_t r1 = 0, m1 = 0;
@@ -348,6 +358,18 @@ static int check_gains(const void *gains, const void *ant_pairs, int A)
     return BLINK_OK;
 }
 
+static int launch_gains(float2 *dst, const float2 *src, const float2 *g, const int2 *ap, int T, int C, int P, int B, int A, cudaStream_t st)
+{
+    const long long n_rows = (long long)T * C * P;
+    const unsigned rows_y = (unsigned)std::min<long long>(n_rows, 2048);
+    if ((B & 1) == 0 && aligned16(dst) && aligned16(src))
+        apply_gains_kernel<2><<<dim3((B / 2 + 255) / 256, rows_y), 256, 0, st>>>(dst, src, g, ap, n_rows, C, P, B, A);
+    else
+        apply_gains_kernel<1><<<dim3((B + 255) / 256, rows_y), 256, 0, st>>>(dst, src, g, ap, n_rows, C, P, B, A);
+    BLINK_LAUNCH_CHECK("apply_gains_kernel");
+    return BLINK_OK;
+}
+
 extern "C" int blink_apply_gains(blink_c64 *vis, const blink_c64 *gains, const int32_t *ant_pairs, int T, int C, int P, int B,
                                  int A, void *stream)
 {
@@ -356,18 +378,9 @@ extern "C" int blink_apply_gains(blink_c64 *vis, const blink_c64 *gains, const i
     if (rc != BLINK_OK) return rc;
     rc = ensure_device();
     if (rc != BLINK_OK) return rc;
-    const long long n_rows = (long long)T * C * P;
-    const unsigned rows_y = (unsigned)std::min<long long>(n_rows, 2048);
     float2 *v = reinterpret_cast<float2 *>(vis);
-    const float2 *g = reinterpret_cast<const float2 *>(gains);
-    const int2 *ap = reinterpret_cast<const int2 *>(ant_pairs);
-    cudaStream_t st = static_cast<cudaStream_t>(stream);
-    if ((B & 1) == 0 && aligned16(vis))
-        apply_gains_kernel<2><<<dim3((B / 2 + 255) / 256, rows_y), 256, 0, st>>>(v, g, ap, n_rows, C, P, B, A);
-    else
-        apply_gains_kernel<1><<<dim3((B + 255) / 256, rows_y), 256, 0, st>>>(v, g, ap, n_rows, C, P, B, A);
-    BLINK_LAUNCH_CHECK("apply_gains_kernel");
-    return BLINK_OK;
+    return launch_gains(v, v, reinterpret_cast<const float2 *>(gains), reinterpret_cast<const int2 *>(ant_pairs), T, C, P, B, A,
+                        static_cast<cudaStream_t>(stream));
 }
 
 extern "C" int blink_image_cal(const blink_c64 *vis, const float *uvw_m, const double *freqs_hz, const blink_c64 *gains,
@@ -385,9 +398,21 @@ extern "C" int blink_image_cal(const blink_c64 *vis, const float *uvw_m, const d
     cal.gains = reinterpret_cast<const float2 *>(gains);
     cal.ant = reinterpret_cast<const int2 *>(ant_pairs);
     cal.A = A;
-    return image_device(reinterpret_cast<const float2 *>(vis), uvw_m, freqs_hz, T, C, P, B, n_pix, pixscale_rad, weighting,
-                        0, T * C, image, wsum, nullptr, nullptr, workspace, workspace_bytes,
-                        static_cast<cudaStream_t>(stream), cal);
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const float2 *v = reinterpret_cast<const float2 *>(vis);
+    if (!use_fused(P, B, n_pix, weighting)) {
+        // sizes the fused kernel does not cover (the paper's 1200 and 8192 among them): the corrected visibilities go to the
+        // head of the workspace (out of place: `vis` stays untouched here too) and the unfused chain images them
+        const size_t corr = align_up((size_t)T * C * P * B * sizeof(float2), 256);
+        if (!workspace || (reinterpret_cast<uintptr_t>(workspace) & 255u) || workspace_bytes < corr) return BLINK_ERR_WORKSPACE;
+        float2 *vc = static_cast<float2 *>(workspace);
+        rc = launch_gains(vc, v, cal.gains, cal.ant, T, C, P, B, A, st);
+        if (rc != BLINK_OK) return rc;
+        return image_device(vc, uvw_m, freqs_hz, T, C, P, B, n_pix, pixscale_rad, weighting, 0, T * C, image, wsum, nullptr, nullptr,
+                            static_cast<unsigned char *>(workspace) + corr, workspace_bytes - corr, st);
+    }
+    return image_device(v, uvw_m, freqs_hz, T, C, P, B, n_pix, pixscale_rad, weighting, 0, T * C, image, wsum, nullptr, nullptr,
+                        workspace, workspace_bytes, st, cal);
 }
 
 extern "C" int blink_image_stokes_i(const blink_c64 *vis, const float *uvw_m, const double *freqs_hz, int T, int C, int P, int B,
