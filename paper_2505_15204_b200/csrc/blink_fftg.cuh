@@ -6,33 +6,36 @@
 
 namespace blink {
 
+// The butterflies below use the packed fp32 pair instructions of sm_100 (blink_fft.cuh: add / mul / fma.f32x2 on a 64-bit
+// register pair = one complex number), half the issue slots of the scalar forms.
+__device__ __forceinline__ float2 bcast(float c) { return make_float2(c, c); }
 __device__ __forceinline__ void gdft3(float2 &x0, float2 &x1, float2 &x2)
 {
+    const float c = 0.86602540378443864676f;                   // sin(2 pi / 3)
     const float2 t = cadd(x1, x2), d = csub(x1, x2);
-    const float2 m = make_float2(x0.x - 0.5f * t.x, x0.y - 0.5f * t.y);
-    const float2 q = make_float2(0.86602540378443864676f * d.x, 0.86602540378443864676f * d.y);
+    const float2 m = pk_fma(t, bcast(-0.5f), x0);              // x0 - t / 2
     x0 = cadd(x0, t);
-    x1 = make_float2(m.x - q.y, m.y + q.x);                    // m + i q
-    x2 = make_float2(m.x + q.y, m.y - q.x);                    // m - i q
+    x1 = pk_fma(make_float2(d.y, d.x), make_float2(-c, c), m); // m + i c d
+    x2 = pk_fma(make_float2(d.y, d.x), make_float2(c, -c), m); // m - i c d
 }
 __device__ __forceinline__ void gdft5(float2 &x0, float2 &x1, float2 &x2, float2 &x3, float2 &x4)
 {
     const float c1 = 0.30901699437494742410f, c2 = -0.80901699437494742410f;      // cos(2 pi / 5), cos(4 pi / 5)
     const float s1 = 0.95105651629515357212f, s2 = 0.58778525229247312917f;       // sin(2 pi / 5), sin(4 pi / 5)
     const float2 a1 = cadd(x1, x4), a2 = cadd(x2, x3), b1 = csub(x1, x4), b2 = csub(x2, x3);
-    const float2 p1 = make_float2(x0.x + c1 * a1.x + c2 * a2.x, x0.y + c1 * a1.y + c2 * a2.y);
-    const float2 p2 = make_float2(x0.x + c2 * a1.x + c1 * a2.x, x0.y + c2 * a1.y + c1 * a2.y);
-    const float2 q1 = make_float2(s1 * b1.x + s2 * b2.x, s1 * b1.y + s2 * b2.y);
-    const float2 q2 = make_float2(s2 * b1.x - s1 * b2.x, s2 * b1.y - s1 * b2.y);
+    const float2 p1 = pk_fma(a2, bcast(c2), pk_fma(a1, bcast(c1), x0));
+    const float2 p2 = pk_fma(a2, bcast(c1), pk_fma(a1, bcast(c2), x0));
+    const float2 q1 = pk_fma(b2, bcast(s2), pk_mul(b1, bcast(s1)));
+    const float2 q2 = pk_fma(b2, bcast(-s1), pk_mul(b1, bcast(s2)));
     x0 = cadd(x0, cadd(a1, a2));
-    x1 = make_float2(p1.x - q1.y, p1.y + q1.x);                // p1 + i q1
-    x4 = make_float2(p1.x + q1.y, p1.y - q1.x);
-    x2 = make_float2(p2.x - q2.y, p2.y + q2.x);                // p2 + i q2
-    x3 = make_float2(p2.x + q2.y, p2.y - q2.x);
+    x1 = add_i(p1, q1);                                        // p1 + i q1
+    x4 = sub_i(p1, q1);
+    x2 = add_i(p2, q2);                                        // p2 + i q2
+    x3 = sub_i(p2, q2);
 }
 
 // x * exp(+2 pi i m / n) for compile-time constants (c, s) = (cos, sin)(2 pi m / n)
-__device__ __forceinline__ float2 cmulc(float2 x, float c, float s) { return make_float2(x.x * c - x.y * s, x.x * s + x.y * c); }
+__device__ __forceinline__ float2 cmulc(float2 x, float c, float s) { return cmul(x, make_float2(c, s)); }
 
 // 16-point inverse DFT in registers, natural order in and out: 4 x 4 decimation in time.
 //   A[k1][n2] = sum_n1 x[n2 + 4 n1] W4^(n1 k1);  X[k1 + 4 k2] = sum_n2 (W16^(n2 k1) A[k1][n2]) W4^(n2 k2)

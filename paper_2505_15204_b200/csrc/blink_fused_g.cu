@@ -24,22 +24,29 @@
 namespace blink {
 
 constexpr int FG_N = 1200, FG_H = 600;
-constexpr int FG_TG = 160;                                      // threads per group (5 warps)
-constexpr int FG_G = 4;                                         // groups per CTA
+#ifndef BLINK_FG_NT
+#define BLINK_FG_NT 2
+#endif
+constexpr int FG_NT = BLINK_FG_NT;                              // transforms a group works on at a time (2: a column / row-pair PAIR)
+constexpr int FG_TG = FG_NT == 2 ? 160 : 96;                    // threads per group (5 or 3 warps): 80 radix-15 butterflies per transform
+#ifndef BLINK_FG_GROUPS
+#define BLINK_FG_GROUPS 4
+#endif
+constexpr int FG_G = BLINK_FG_GROUPS;                           // groups per CTA
 constexpr int FG_THREADS = FG_TG * FG_G;                        // 640
-constexpr int FG_LD = 1208;                                     // leading dimension of a group's two arrays (complex64)
+constexpr int FG_LD = 1208;                                     // leading dimension of a group's arrays (complex64)
 constexpr int FG_TW = 1 + 15 + 75;                              // compact twiddle runs of the three stages
 constexpr int kFgMaxB = 15000;                                 // the staged visibility row must fit next to the arrays
 
 // shared memory: arrays | twiddle runs | column offsets | mbarriers | U = union( pass 1: visibility row + 16-bit cell counts,
 //                                                                               pass 2: per-group staging of 4 rows of HT )
 struct FgSmem {
-    static constexpr size_t ARR = (size_t)FG_G * 2 * FG_LD * sizeof(float2);          // 77.3 KB
-    static constexpr size_t CNT = (size_t)FG_G * 2 * (FG_N / 2) * sizeof(uint32_t);    // 19.2 KB: 16-bit counts, two per word
+    static constexpr size_t ARR = (size_t)FG_G * FG_NT * FG_LD * sizeof(float2);      // 77.3 KB
+    static constexpr size_t CNT = (size_t)FG_G * FG_NT * (FG_N / 2) * sizeof(uint32_t);  // 19.2 KB: 16-bit counts, two per word
     static constexpr size_t TW = ((size_t)FG_TW * sizeof(float2) + 15) & ~(size_t)15;
     static constexpr size_t COFF = ((size_t)(FG_H + 2) * 4 + 15) & ~(size_t)15;
-    static constexpr size_t BARS = 64;                                                 // visbar + FG_G staging barriers
-    static constexpr size_t STG_G = (size_t)4 * FG_H * sizeof(float2);                 // 19.2 KB per group: 4 rows x 600 columns
+    static constexpr size_t BARS = 128;                                                // visbar + 2 staging barriers per group
+    static constexpr size_t STG_G = (size_t)2 * FG_NT * FG_H * sizeof(float2);         // 19.2 KB per group: 4 rows x 600 columns
     static constexpr size_t HEAD = ARR + TW + COFF + BARS;
     __host__ __device__ static size_t front(int B) { return ((size_t)B * 8 + 15) & ~(size_t)15; }
     __host__ __device__ static size_t uni(int B) { return front(B) + CNT > FG_G * STG_G ? front(B) + CNT : FG_G * STG_G; }
@@ -56,7 +63,7 @@ template <int R, int P, bool FIRST, bool LAST, class Sync, class Load, class Emi
 __device__ __forceinline__ void fg_stage(float2 *arr, const float2 *__restrict__ tw, int tid, Sync gsync, Load load, Emit emit,
                                          Hook hook = Hook())
 {
-    constexpr int nb = FG_N / R, total = 2 * nb, ROUNDS = (total + FG_TG - 1) / FG_TG;
+    constexpr int nb = FG_N / R, total = FG_NT * nb, ROUNDS = (total + FG_TG - 1) / FG_TG;
     float2 x[ROUNDS][R];
 #pragma unroll
     for (int q = 0; q < ROUNDS; ++q) {
@@ -124,12 +131,12 @@ fused_g_kernel(const FusedArgs a, const __grid_constant__ ScaleBlock sc, const f
     float2 *stw = reinterpret_cast<float2 *>(q);                 q += FgSmem::TW;
     uint32_t *coff = reinterpret_cast<uint32_t *>(q);            q += FgSmem::COFF;
     uint64_t *visbar = reinterpret_cast<uint64_t *>(q);          q += FgSmem::BARS;
-    uint64_t *stbar = visbar + 1 + g;                            // this group's staging barrier
+    uint64_t *stbar = visbar + 1 + 2 * g;                        // this group's two staging barriers
     float2 *visrow = reinterpret_cast<float2 *>(q);                                               // U, pass 1: [B]
     uint32_t *cnt_all = reinterpret_cast<uint32_t *>(q + FgSmem::front(B));
     float2 *stg = reinterpret_cast<float2 *>(q + (size_t)g * FgSmem::STG_G);                      // U, pass 2: [4][ulim]
-    float2 *arr = arr_all + (size_t)g * 2 * FG_LD;
-    uint32_t *cnt = cnt_all + (size_t)g * 2 * (N / 2);           // cnt[tr * 600 + (n >> 1)], 16 bits per cell
+    float2 *arr = arr_all + (size_t)g * FG_NT * FG_LD;
+    uint32_t *cnt = cnt_all + (size_t)g * FG_NT * (N / 2);           // cnt[tr * 600 + (n >> 1)], 16 bits per cell
     __shared__ int s_nin, s_occ, s_ncol;
 
     float2 *HT = a.scratch + (size_t)blockIdx.x * N * H;         // [N ky][H u], transposed pass-1 output
@@ -145,17 +152,17 @@ fused_g_kernel(const FusedArgs a, const __grid_constant__ ScaleBlock sc, const f
         stw[k] = tw_full[kk * step];
     }
     if (threadIdx.x == 0) {
-        for (int k = 0; k <= FG_G; ++k) mbar_init(visbar + k, 1);
+        for (int k = 0; k <= 2 * FG_G; ++k) mbar_init(visbar + k, 1);
         fence_mbar_init();
     }
-    uint32_t vph = 0, sph = 0;
+    uint32_t vph = 0, sph = 0;                                   // sph: phase bits of the two staging barriers
     const bool bulk = (B & 1) == 0;
     const int tc_end = a.tc0 + a.ntc;
     __syncthreads();
     auto clear_group = [&] {                                    // this group's arrays (and counts): zero for the next gridding
         float4 *z = reinterpret_cast<float4 *>(arr);
-        for (int i = tid; i < 2 * FG_LD / 2; i += FG_TG) z[i] = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (uniform) for (int i = tid; i < 2 * (N / 2); i += FG_TG) cnt[i] = 0u;
+        for (int i = tid; i < FG_NT * FG_LD / 2; i += FG_TG) z[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (uniform) for (int i = tid; i < FG_NT * (N / 2); i += FG_TG) cnt[i] = 0u;
     };
 
     for (int tc = a.tc0 + blockIdx.x; tc < tc_end; tc += gridDim.x) {
@@ -219,18 +226,26 @@ fused_g_kernel(const FusedArgs a, const __grid_constant__ ScaleBlock sc, const f
 
             // ================= pass 1: column pairs (2cp, 2cp+1): grid, transform along v, store transposed ==========
             int my_in = 0, my_occ = 0;
-            for (int cp = g; cp < n_cp; cp += FG_G) {
-                const int u0 = 2 * cp;
-                const int k0 = (int)coff[u0], k1 = (int)coff[u0 + 1], k2 = (int)coff[u0 + 2];
-                gsync();                                        // the arrays are zero (clear_group of the previous unit / image)
-                for (int j = k0 + tid; j < k2; j += FG_TG) {
-                    const uint2 sq = __ldg(svb + j);
+            // the first FG_TG samples of a unit are fetched one unit ahead (one register pair per thread), the rest in the loop
+            const int n_un = ulim / FG_NT;                      // units of FG_NT columns (the last column may be an empty one)
+            auto first_sample = [&](int cp_) -> uint2 {
+                if (cp_ < n_un) {
+                    const int j = (int)coff[FG_NT * cp_] + tid;
+                    if (j < (int)coff[FG_NT * cp_ + FG_NT]) return __ldg(svb + j);
+                }
+                return make_uint2(0u, 0u);
+            };
+            uint2 sq_next = first_sample(g);
+            for (int cp = g; cp < n_un; cp += FG_G) {
+                const int u0 = FG_NT * cp;
+                const int k0 = (int)coff[u0], k1 = (int)coff[u0 + 1], k2 = (int)coff[u0 + FG_NT];
+                auto grid_one = [&](uint2 sq, int j) {
                     int iv;
                     const float yr = rint_rne(__fmul_rn(__uint_as_float(sq.x), s), iv);
                     if (fabsf(yr) <= lim) {                     // NaN fails; |iu| <= H-1 by construction
                         float2 vv = visrow[sq.y & 0x7fffffffu];
                         if (sq.y >> 31) vv.y = -vv.y;
-                        const int tr = j >= k1;
+                        const int tr = FG_NT == 2 && j >= k1;
                         const int n = iv < 0 ? iv + N : iv;     // transform index of centred row iv + H
                         cell_add_exch(&arr[tr * FG_LD + n], vv);
                         if (uniform) atomicAdd(&cnt[tr * (N / 2) + (n >> 1)], 1u << ((n & 1) * 16));
@@ -241,7 +256,11 @@ fused_g_kernel(const FusedArgs a, const __grid_constant__ ScaleBlock sc, const f
                         }
                         ++my_in;
                     }
-                }
+                };
+                gsync();                                        // the arrays are zero (clear_group of the previous unit / image)
+                if (k0 + tid < k2) grid_one(sq_next, k0 + tid);
+                for (int j = k0 + tid + FG_TG; j < k2; j += FG_TG) grid_one(__ldg(svb + j), j);
+                sq_next = first_sample(cp + FG_G);              // lands while this unit is transformed
                 gsync();
                 auto load = [&](int tr, int n) -> float2 {      // a3: divide by the cell count (uniform weighting)
                     float2 v = arr[tr * FG_LD + n];
@@ -285,19 +304,29 @@ fused_g_kernel(const FusedArgs a, const __grid_constant__ ScaleBlock sc, const f
             // unit ahead: the request for unit k+1 goes out right after the barrier that follows unit k's first-stage reads
             // (the only reads of the buffer), so it lands while unit k runs its remaining stages and stores.
             const uint32_t row_bytes = (uint32_t)ulim * 8u;     // ulim is even: a multiple of 16 bytes
-            auto request = [&](int unit) {
+            // the buffer holds four rows of up to 600 columns: with ulim <= 300 (the paper's MWA coverage fills ~200) it is
+            // split into two halves and the requests run TWO units ahead
+            const int nbuf = ulim <= H / 2 ? 2 : 1;
+            constexpr int RU = 2 * FG_NT, NU = N / RU;          // rows of HT per unit, units per image
+            auto request = [&](int unit, int b) {
                 fence_proxy_async();
-                mbar_expect_tx(stbar, 4u * row_bytes);
+                mbar_expect_tx(stbar + b, (uint32_t)RU * row_bytes);
 #pragma unroll
-                for (int r = 0; r < 4; ++r) bulk_load_1d(stg + (size_t)r * ulim, HT + (size_t)(4 * unit + r) * H, row_bytes, stbar);
+                for (int r = 0; r < RU; ++r)
+                    bulk_load_1d(stg + (size_t)(RU * b + r) * ulim, HT + (size_t)(RU * unit + r) * H, row_bytes, stbar + b);
             };
-            if (tid == 0 && g < N / 4) request(g);
-            for (int unit = g; unit < N / 4; unit += FG_G) {
-                const int ky0 = 4 * unit;
-                mbar_wait(stbar, sph);
-                sph ^= 1u;
+            if (tid == 0)
+                for (int b = 0; b < nbuf; ++b)
+                    if (g + b * FG_G < NU) request(g + b * FG_G, b);
+            int it = 0;
+            for (int unit = g; unit < NU; unit += FG_G, ++it) {
+                const int ky0 = RU * unit;
+                const int b = nbuf == 2 ? (it & 1) : 0;
+                mbar_wait(stbar + b, (sph >> b) & 1u);
+                sph ^= 1u << b;
+                const float2 *sb = stg + (size_t)(RU * b) * ulim;
                 auto load = [&](int tr, int n) -> float2 {
-                    const float2 *r0 = stg + (size_t)(2 * tr) * ulim, *r1 = r0 + ulim;
+                    const float2 *r0 = sb + (size_t)(2 * tr) * ulim, *r1 = r0 + ulim;
                     if (n < H) {                                // Z[u] = S1 + i S2
                         if (n >= ulim) return make_float2(0.f, 0.f);
                         const float2 s1 = r0[n], s2 = r1[n];
@@ -316,7 +345,7 @@ fused_g_kernel(const FusedArgs a, const __grid_constant__ ScaleBlock sc, const f
                     __stcs(img + (size_t)y1 * N + x, z.y * inv_w);
                 };
                 auto after_first_reads = [&] {                  // runs right after the first stage's read -> write barrier
-                    if (tid == 0 && unit + FG_G < N / 4) request(unit + FG_G);
+                    if (tid == 0 && unit + nbuf * FG_G < NU) request(unit + nbuf * FG_G, b);
                 };
                 fg_transform2(arr, stw, tid, gsync, load, emit, after_first_reads);
             }
