@@ -18,7 +18,7 @@ _lib = None
 
 W_NATURAL, W_UNIFORM = 0, 1
 OP_GRID, OP_FFT2D, OP_IMAGE, OP_IMAGE_HOST, OP_IMAGE_AVG, OP_IMAGE_CONV, OP_IMAGE_STOKES_I, OP_IMAGE_CAL = 0, 1, 2, 3, 4, 5, 6, 7
-OPT_IMAGE_PATH, OPT_FUSED_CTAS, OPT_GRID_CHUNK_B, OPT_AVG_WSUM, OPT_CORR_PATH = 0, 1, 2, 3, 4
+OPT_IMAGE_PATH, OPT_FUSED_CTAS, OPT_GRID_CHUNK_B, OPT_AVG_WSUM, OPT_CORR_PATH, OPT_FUSED_TEAM = 0, 1, 2, 3, 4, 5
 
 EXPORTS = ["blink_strerror", "blink_last_cuda_error", "blink_set_option", "blink_get_option",
            "blink_kernel_launches", "blink_workspace_bytes", "blink_grid", "blink_fft2d_inverse",

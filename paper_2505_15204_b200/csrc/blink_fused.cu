@@ -128,7 +128,8 @@ int presort_launch(const float *uvw_m, int T, int B, float *su, uint2 *svb, cuda
 size_t fused_workspace_bytes(int T, int B, int n_pix, int ctas)
 {
     if (n_pix == 1200) return fused_g_workspace_bytes(T, B, ctas);
-    return sort_bytes(T, B) + (size_t)ctas * (n_pix / 2) * n_pix * sizeof(float2);
+    // at least two scratch slots so that a team (two slots in turn) can run when the caller grants the recommended size
+    return sort_bytes(T, B) + kTeamBytes + (size_t)ctas * (n_pix / 2) * n_pix * sizeof(float2);
 }
 int fused_default_ctas() { return sm_count() > 0 ? sm_count() : 148; }
 

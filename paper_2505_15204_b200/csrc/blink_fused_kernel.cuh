@@ -39,7 +39,14 @@ struct FusedArgs {
     const float *su; const uint2 *svb;                         // per timestep: baselines sorted by |u| (presort_kernel)
     const float2 *tw;
     GainRef cal;                                               // optional per-antenna gains applied at the load
+    // teams: `team` consecutive CTAs image one (t,c) together (column pairs and pass-2 tiles dealt round-robin over the ranks;
+    // one scratch shared by the team, double-buffered; one global-memory barrier per image).  team == 1: a CTA per image.
+    int team;
+    unsigned *team_ctr;                                        // [n_teams] arrivals so far (monotonic)
+    unsigned *team_w;                                          // [n_teams][2 parities][2] running totals of (occupied cells, samples)
 };
+
+constexpr size_t kTeamBytes = 4096;                            // team_ctr + team_w of up to 148 teams, 256-aligned
 
 // Convolutional gridding (reading R16): the NORMALISED tap weight of tap j = -R..R of one axis,
 //   w_j(f) = k(j - f) / sum_i k(i - f),  f = x - rint(x) in [-1/2, 1/2],  k = Kaiser-Bessel window of support S = 2R+1,
@@ -137,7 +144,7 @@ int presort_launch(const float *uvw_m, int T, int B, float *su, uint2 *svb, cuda
 size_t sort_bytes(int T, int B);
 
 // ------------------------------------------------------------------------------------------ fused kernel
-template <int N, int NS, int R = 0>
+template <int N, int NS, int R = 0, bool TEAM = false>
 __global__ void __launch_bounds__(kFusedThreads, 1)
 fused_image_kernel(const FusedArgs a, const __grid_constant__ ScaleBlock sc, const __grid_constant__ CUtensorMap tmap,
                    const __grid_constant__ ConvPoly cpoly)
@@ -170,7 +177,11 @@ fused_image_kernel(const FusedArgs a, const __grid_constant__ ScaleBlock sc, con
     __shared__ int s_nin, s_occ, s_ncol;
     __shared__ unsigned s_done[4];                             // per stage buffer: groups that have released it (running count)
 
-    float2 *scratch = a.scratch + (size_t)blockIdx.x * H * N;
+    // TEAM == false compiles to the one-CTA-per-image kernel (K = 1, rank = 0: the compiler folds the team arithmetic away)
+    const int K = TEAM ? a.team : 1, team_id = (int)blockIdx.x / K, rank = (int)blockIdx.x - team_id * K, n_teams = (int)gridDim.x / K;
+    unsigned tcs = 0;                                          // (t,c) items this team has imaged so far
+    __shared__ unsigned s_prev[4];                             // thread 0: team totals (occ, nin) at the last use of each parity
+    if (threadIdx.x == 0) s_prev[0] = s_prev[1] = s_prev[2] = s_prev[3] = 0u;
     // barrier over ONE transform group (its columns / exchange array are private to it)
     auto gsync = [g] {
         if constexpr (TG == 32) __syncwarp();
@@ -197,12 +208,12 @@ fused_image_kernel(const FusedArgs a, const __grid_constant__ ScaleBlock sc, con
     const bool bulk = (B & 1) == 0;
     const int tc_end = a.tc0 + a.ntc;
     __syncthreads();
-    if (bulk && threadIdx.x == 0 && a.tc0 + (int)blockIdx.x < tc_end) {
+    if (bulk && threadIdx.x == 0 && a.tc0 + team_id < tc_end) {
         mbar_expect_tx(visbar, (uint32_t)B * 8u);
-        bulk_load_1d(visrow, a.vis + (size_t)(a.tc0 + blockIdx.x) * a.P * B, (uint32_t)B * 8u, visbar);
+        bulk_load_1d(visrow, a.vis + (size_t)(a.tc0 + team_id) * a.P * B, (uint32_t)B * 8u, visbar);
     }
 
-    for (int tc = a.tc0 + blockIdx.x; tc < tc_end; tc += gridDim.x) {
+    for (int tc = a.tc0 + team_id; tc < tc_end; tc += n_teams, ++tcs) {
         const int t = tc / a.C, c = tc - t * a.C;
         const float s = sc.s[c - a.c_base];
         const float *su = a.su + (size_t)t * B;
@@ -217,8 +228,13 @@ fused_image_kernel(const FusedArgs a, const __grid_constant__ ScaleBlock sc, con
         float wsum_val = 0.f;
 
         for (int p = 0; p < a.P; ++p) {
+            const unsigned seq = tcs * (unsigned)a.P + (unsigned)p;   // planes this team has imaged so far
             const size_t img_idx = (size_t)tc * a.P + p;
             float *img = a.image + img_idx * N * N;
+            // scratch slot: a CTA's own (team of one), else the team's two slots in turn -- the slot read by pass 2 of plane
+            // seq is rewritten by pass 1 of plane seq + 2, after every CTA has passed the barrier of plane seq + 1
+            const int slot = K == 1 ? (int)blockIdx.x : 2 * team_id + (int)(seq & 1u);
+            float2 *scratch = a.scratch + (size_t)slot * H * N;
             __syncthreads();                                    // (C) every group has finished the previous pass 2
             {                                                   // the region was last used by pass 2: clear the columns
                 const int n16 = (Cfg::COL_BYTES + (uniform ? Cfg::COL_BYTES / 2 : 0)) / 16;
@@ -249,7 +265,7 @@ fused_image_kernel(const FusedArgs a, const __grid_constant__ ScaleBlock sc, con
                     }
                 }
                 // ---- optional output: cell index of every baseline, in baseline order (a1) ---------------
-                if (a.cell_idx) {
+                if (a.cell_idx && rank == 0) {
                     const float *uvw = a.uvw_m + (size_t)t * B * 3;
                     for (int b = threadIdx.x; b < B; b += kFusedThreads)
                         a.cell_idx[(size_t)tc * B + b] = cell_of(uvw[3 * b], uvw[3 * b + 1], s, N, H, R);
@@ -385,8 +401,8 @@ fused_image_kernel(const FusedArgs a, const __grid_constant__ ScaleBlock sc, con
                     }
                 }
             };
-            if constexpr (R == 0) prefetch(g);
-            for (int cp = g; cp < n_cp; cp += G) {
+            if constexpr (R == 0) prefetch(g + G * rank);
+            for (int cp = g + G * rank; cp < n_cp; cp += G * K) {
                 const int u0 = 2 * cp;
                 if constexpr (R == 0) {
                     const int k0 = (int)coff[u0], k1 = (int)coff[u0 + 1], k2 = (int)coff[u0 + 2];
@@ -398,7 +414,7 @@ fused_image_kernel(const FusedArgs a, const __grid_constant__ ScaleBlock sc, con
                         if (j < k2) grid_one(pre[m * TG + tid], j >= k1, u0 == 0 && j < k1);
                     }
                     for (int j = k0 + tid + kPre * TG; j < k2; j += TG) grid_one(__ldg(svb + j), j >= k1, u0 == 0 && j < k1);
-                    prefetch(cp + G);                           // lands while this unit is transformed
+                    prefetch(cp + G * K);                       // lands while this unit is transformed
                 } else {
                     // samples whose support reaches columns u0, u0+1: nearest columns [u0-R, u0+1+R]; the mirrored
                     // taps come from nearest columns [0, R-u0], a subset (coff[H] = first sample beyond the range)
@@ -454,9 +470,35 @@ fused_image_kernel(const FusedArgs a, const __grid_constant__ ScaleBlock sc, con
             __threadfence();
             asm volatile("fence.proxy.async;" ::: "memory");
             __syncthreads();                                    // (B)
+            if (TEAM && K > 1) {
+                // team barrier: every CTA's share of H[u][ky] (and of the weight sum) is in global memory before anyone's pass 2
+                if (threadIdx.x == 0) {
+                    unsigned *tw = a.team_w + (size_t)team_id * 4 + (tcs & 1u) * 2;
+                    if (p == 0) { atomicAdd(tw, (unsigned)s_occ); atomicAdd(tw + 1, (unsigned)s_nin); }
+                    __threadfence();
+                    atomicAdd(a.team_ctr + team_id, 1u);
+                    const unsigned target = (seq + 1u) * (unsigned)K;
+                    unsigned seen;
+                    do {
+                        asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(a.team_ctr + team_id) : "memory");
+                    } while ((int)(seen - target) < 0);
+                    if (p == 0) {                               // the (t,c)'s totals = running totals minus their value two items ago
+                        unsigned occ, nin;
+                        asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(occ) : "l"(tw) : "memory");
+                        asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(nin) : "l"(tw + 1) : "memory");
+                        const unsigned o = (tcs & 1u) * 2u;
+                        s_occ = (int)(occ - s_prev[o]);
+                        s_nin = (int)(nin - s_prev[o + 1]);
+                        s_prev[o] = occ;
+                        s_prev[o + 1] = nin;
+                    }
+                }
+                __syncthreads();
+                asm volatile("fence.proxy.async;" ::: "memory"); // the other CTAs' scratch stores before this CTA's TMA loads
+            }
             if (bulk && threadIdx.x == 0) {                     // prefetch the next image's visibility row
                 size_t nxt = img_idx + 1;
-                if (p + 1 == a.P) nxt = (tc + (int)gridDim.x < tc_end) ? (size_t)(tc + gridDim.x) * a.P : (size_t)-1;
+                if (p + 1 == a.P) nxt = (tc + n_teams < tc_end) ? (size_t)(tc + n_teams) * a.P : (size_t)-1;
                 if (nxt != (size_t)-1) {
                     mbar_expect_tx(visbar, (uint32_t)B * 8u);
                     bulk_load_1d(visrow, a.vis + nxt * B, (uint32_t)B * 8u, visbar);
@@ -482,12 +524,12 @@ fused_image_kernel(const FusedArgs a, const __grid_constant__ ScaleBlock sc, con
                 for (int sb_ = 0; sb_ < Cfg::NSUB; ++sb_)
                     for (int bx = 0; bx < n_box; ++bx)
                         tma_load_3d(dst + (size_t)sb_ * Cfg::SUB_BYTES + (size_t)bx * Cfg::BOX_ROWS * Cfg::ROWB, &tmap, bar,
-                                    2 * (it * Cfg::KYS + sb_ * Cfg::KY), bx * Cfg::BOX_ROWS, (int)blockIdx.x);
+                                    2 * (it * Cfg::KYS + sb_ * Cfg::KY), bx * Cfg::BOX_ROWS, slot);
             };
-            if (threadIdx.x == 0)
-                for (int it = 0; it < NS && it < Cfg::NIT; ++it) request(it, (cs + (uint32_t)it) % (uint32_t)NS);
+            if (threadIdx.x == 0)                               // this CTA's tiles: it = rank, rank + K, ...
+                for (int i = 0; i < NS && rank + i * K < Cfg::NIT; ++i) request(rank + i * K, (cs + (uint32_t)i) % (uint32_t)NS);
             const int sub = g / Cfg::PPS, pair = g % Cfg::PPS;
-            for (int it = 0; it < Cfg::NIT; ++it) {
+            for (int it = rank; it < Cfg::NIT; it += K) {
                 mbar_wait(&full[cs], ck & 1u);
                 const uint32_t st_used = cs;
                 float2 z[1][kE];
@@ -520,7 +562,7 @@ fused_image_kernel(const FusedArgs a, const __grid_constant__ ScaleBlock sc, con
                         __threadfence_block();                  // the group's reads (ordered by its barrier) before the count
                         const unsigned old = atomicAdd(&s_done[st_used], 1u);
                         __threadfence_block();
-                        if (old % (unsigned)G == (unsigned)(G - 1) && it + NS < Cfg::NIT) request(it + NS, st_used);
+                        if (old % (unsigned)G == (unsigned)(G - 1) && it + NS * K < Cfg::NIT) request(it + NS * K, st_used);
                     }
                 };
                 ExchangePadded1 xch{xbuf};
@@ -544,8 +586,39 @@ fused_image_kernel(const FusedArgs a, const __grid_constant__ ScaleBlock sc, con
                 }
             }
         }
-        if (threadIdx.x == 0) a.wsum[tc] = wsum_val;
+        if (threadIdx.x == 0 && rank == 0) a.wsum[tc] = wsum_val;
     }
+}
+
+// Team size for ntc (t,c) items on `ctas` resident CTAs.  Cost model, in units of one plane imaged by one CTA alone:
+//   K = 1: rounds(1);   K > 1: rounds(K) / K * (1 + c + K f),   rounds(K) = ceil(ntc / (ctas / K)),
+// c = what team mode costs whatever its size (the barrier per plane, the totals), f = the per-plane work every member repeats
+// (column-offset scan, clearing, pipeline fill) as a fraction of a plane's work.  Fitted to a sweep of K = 1 .. 74 over
+// BASELINE.json configs 2, 4 (one timestep) and 5 on a B200: N = 1024: c ~ 0, f = 0.025; 2048: c = 0.06,
+// f = 0.007; 4096: c = 0.07, f = 0.002.  Sizes that leave a rank less than ~two rounds of column-pair units (K G > N / 16)
+// are not considered; a team is taken only when the model saves >= 3 %.
+template <int N>
+static int choose_team(int ntc, int ctas)
+{
+    const int forced = option(BLINK_OPT_FUSED_TEAM);
+    const int cand[] = {2, 3, 4, 6, 8, 12, 16, 37, 74, 148};
+    if (forced > 0) return forced <= ctas && forced <= FusedCfg<N>::NIT ? forced : 1;
+    const double c = N >= 4096 ? 0.07 : N >= 2048 ? 0.06 : N >= 1024 ? 0.0 : 0.05;
+    const double f = N >= 4096 ? 0.002 : N >= 2048 ? 0.007 : N >= 1024 ? 0.025 : N >= 512 ? 0.04 : 0.08;
+    auto cost = [&](int k) {
+        const int teams = ctas / k;
+        const double r = (double)((ntc + teams - 1) / teams) / k;
+        return k == 1 ? r : r * (1.0 + c + k * f);
+    };
+    int best = 1;
+    double best_c = cost(1);
+    for (int k : cand) {
+        if (k > ctas || k * FusedCfg<N>::G > N / 16 || k > FusedCfg<N>::NIT) continue;
+        const double ck = cost(k);
+        if (ck < best_c) { best = k; best_c = ck; }
+    }
+    if (best_c > 0.97 * cost(1)) best = 1;
+    return best;
 }
 
 // sub-ranges of flattened (t,c) that stay inside one block of <= 1024 channels
@@ -576,16 +649,17 @@ static int launch_fused(const FusedArgs &base, const double *freqs_hz, double pi
 {
     using Cfg = FusedCfg<N>;
     const size_t per_cta = (size_t)Cfg::H * N * sizeof(float2);
-    const size_t sortb = sort_bytes(base.T, base.B) + extra;
+    const size_t sortb = sort_bytes(base.T, base.B) + extra + kTeamBytes;
     if (!workspace || (reinterpret_cast<uintptr_t>(workspace) & 255u) || workspace_bytes < sortb + per_cta)
         return BLINK_ERR_WORKSPACE;
     int ctas = option(BLINK_OPT_FUSED_CTAS);
     if (ctas <= 0) ctas = fused_default_ctas();
-    ctas = (int)std::min<size_t>((size_t)ctas, (workspace_bytes - sortb) / per_cta);
+    const int slots_max = (int)std::min<size_t>((size_t)ctas, (workspace_bytes - sortb) / per_cta);   // scratch slots that fit
     // workspace: su | svb (baselines of every timestep sorted by |u|) | per-CTA scratch
     unsigned char *wsp = static_cast<unsigned char *>(workspace);
     float *su = reinterpret_cast<float *>(wsp);
-    uint2 *svb = reinterpret_cast<uint2 *>(wsp + (sortb - extra) / 3);
+    uint2 *svb = reinterpret_cast<uint2 *>(wsp + (sortb - extra - kTeamBytes) / 3);
+    unsigned *team_mem = reinterpret_cast<unsigned *>(wsp + sortb - kTeamBytes);
     void *scratch = wsp + sortb;
     {
         int rc = presort_launch(base.uvw_m, base.T, base.B, su, svb, st);
@@ -597,13 +671,16 @@ static int launch_fused(const FusedArgs &base, const double *freqs_hz, double pi
     const int ns = fused_stages<N>(base.B, uni);
     if (ns == 0) return BLINK_ERR_UNSUPPORTED;
     const size_t smem = fused_smem_bytes<N>(base.B, uni, ns);
-    if (ns == 3)
+    if (ns == 3) {
         BLINK_CUDA_TRY(cudaFuncSetAttribute(fused_image_kernel<N, 3, R>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    else
+        BLINK_CUDA_TRY(cudaFuncSetAttribute(fused_image_kernel<N, 3, R, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    } else {
         BLINK_CUDA_TRY(cudaFuncSetAttribute(fused_image_kernel<N, 2, R>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        BLINK_CUDA_TRY(cudaFuncSetAttribute(fused_image_kernel<N, 2, R, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    }
     CUtensorMap tmap;
-    // scratch viewed as float32 [ctas][H rows (u)][2N (ky re/im)]; boxes of [BOX_ROWS u][KY ky]
-    int rc = encode_tensor_map_3d_f32(&tmap, scratch, 2ull * N, (uint64_t)Cfg::H, (uint64_t)ctas, (uint64_t)N * 8,
+    // scratch viewed as float32 [slots][H rows (u)][2N (ky re/im)]; boxes of [BOX_ROWS u][KY ky]
+    int rc = encode_tensor_map_3d_f32(&tmap, scratch, 2ull * N, (uint64_t)Cfg::H, (uint64_t)slots_max, (uint64_t)N * 8,
                                       (uint64_t)Cfg::H * N * 8, 2 * Cfg::KY, Cfg::BOX_ROWS, 1,
                                       Cfg::ROWB >= 32 ? Cfg::ROWB : 0);
     if (rc != 0) { set_error_text("cuTensorMapEncodeTiled failed (fused scratch)"); return BLINK_ERR_CUDA; }
@@ -614,9 +691,27 @@ static int launch_fused(const FusedArgs &base, const double *freqs_hz, double pi
                                   a.scratch = static_cast<float2 *>(scratch);
                                   a.su = su; a.svb = svb;
                                   a.tw = twiddle_table();
-                                  const int grid = ntc < ctas ? ntc : ctas;
-                                  if (ns == 3) fused_image_kernel<N, 3, R><<<grid, kFusedThreads, smem, st>>>(a, sc, tmap, cpoly);
-                                  else fused_image_kernel<N, 2, R><<<grid, kFusedThreads, smem, st>>>(a, sc, tmap, cpoly);
+                                  // team size for this launch; a team of K needs two scratch slots (K > 1) or one per CTA (K == 1)
+                                  int team = choose_team<N>(ntc, ctas);
+                                  while (team > 1 && slots_max < 2) team = 1;
+                                  int grid;
+                                  if (team == 1) {
+                                      grid = std::min(ntc, std::min(ctas, slots_max));
+                                  } else {
+                                      const int teams = std::min(std::min(ctas / team, slots_max / 2), ntc);
+                                      grid = teams * team;
+                                      if (cudaMemsetAsync(team_mem, 0, kTeamBytes, st) != cudaSuccess) return (int)BLINK_ERR_CUDA;
+                                  }
+                                  a.team = team;
+                                  a.team_ctr = team_mem;
+                                  a.team_w = team_mem + 256;
+                                  if (team > 1) {
+                                      if (ns == 3) fused_image_kernel<N, 3, R, true><<<grid, kFusedThreads, smem, st>>>(a, sc, tmap, cpoly);
+                                      else fused_image_kernel<N, 2, R, true><<<grid, kFusedThreads, smem, st>>>(a, sc, tmap, cpoly);
+                                  } else {
+                                      if (ns == 3) fused_image_kernel<N, 3, R><<<grid, kFusedThreads, smem, st>>>(a, sc, tmap, cpoly);
+                                      else fused_image_kernel<N, 2, R><<<grid, kFusedThreads, smem, st>>>(a, sc, tmap, cpoly);
+                                  }
                                   BLINK_LAUNCH_CHECK("fused_image_kernel");
                                   return (int)BLINK_OK;
                               });

@@ -19,7 +19,7 @@ def bk():
     from paper_2505_15204_b200 import binding
     binding.lib()                     # raises if the .so is missing: no fallback
     yield binding
-    for k in (binding.OPT_IMAGE_PATH, binding.OPT_FUSED_CTAS, binding.OPT_GRID_CHUNK_B, binding.OPT_AVG_WSUM):
+    for k in (binding.OPT_IMAGE_PATH, binding.OPT_FUSED_CTAS, binding.OPT_GRID_CHUNK_B, binding.OPT_AVG_WSUM, binding.OPT_FUSED_TEAM):
         binding.set_option(k, 0)
 
 
@@ -782,6 +782,53 @@ def test_fused_cell_decisions_one_hot(bk, oracle_mod, n, weighting, path):
                 else:
                     want = 2 * abs(V) * np.cos(2 * np.pi * (iu * (x - h) + iv * (y - h)) / n + np.angle(V)) / wsum[t]
                 assert np.max(np.abs(img[t, b] - want)) <= TOL * np.max(np.abs(want)), (t, b, iu, iv)
+
+
+# --------------------------------------------------------------------------- teams of CTAs per image (fused kernel)
+@pytest.mark.parametrize("n,team,ctas,weighting", [(512, 2, 6, 0), (512, 3, 7, 1), (1024, 4, 8, 1), (2048, 5, 10, 0), (256, 2, 4, 1)])
+def test_fused_teams(bk, oracle_mod, n, team, ctas, weighting):
+    """BLINK_OPT_FUSED_TEAM: `team` CTAs image one (t,c) together (column pairs and pass-2 tiles dealt over the ranks, one
+    double-buffered scratch per team, a global-memory barrier per plane, weight sums added up across the team).  Forced team
+    sizes with fewer CTAs than items, P = 3 planes, samples off the grid, an empty (t,c) (W = 0) in the middle, and a grid that
+    is not a multiple of the team size."""
+    from paper_2505_15204_b200 import workloads
+    w = workloads.make_random(T=3, C=3, P=3 if n <= 512 else 1, B=1500, n_pix=n, weighting=weighting, seed=n + team, device="cuda", fill=1.1)
+    w.uvw_m[1, :, :] = 1e7                                      # timestep 1: nothing on the grid
+    w.uvw_m[2, 3, 0] = float("nan")
+    bk.set_option(bk.OPT_IMAGE_PATH, 2)
+    bk.set_option(bk.OPT_FUSED_TEAM, team)
+    bk.set_option(bk.OPT_FUSED_CTAS, ctas)
+    try:
+        res = bk.blink_image(w.vis, w.uvw_m, w.freqs_hz, n, w.pixscale_rad, weighting, want_cell_idx=True)
+        torch.cuda.synchronize()
+        res2 = bk.blink_image(w.vis, w.uvw_m, w.freqs_hz, n, w.pixscale_rad, weighting)       # again: counters start from zero
+        torch.cuda.synchronize()
+    finally:
+        for k in (bk.OPT_IMAGE_PATH, bk.OPT_FUSED_TEAM, bk.OPT_FUSED_CTAS):
+            bk.set_option(k, 0)
+    n_img = w.T * w.C * w.P
+    ids = np.arange(n_img) if n <= 512 else np.array([0, 2, 4, 6, 8])
+    _check_images(bk, w, res, oracle_mod, ids)
+    assert np.array_equal(res["cell_idx"].cpu().numpy(), oracle_mod.cells(w.uvw_m.cpu().numpy(), w.freqs_hz, n, w.pixscale_rad))
+    assert bool((res["image"][3 * w.P:6 * w.P] == 0).all()) and bool((res["wsum"][3:6] == 0).all())
+    assert torch.equal(res["wsum"], res2["wsum"])
+    peak = float(res["image"].abs().max())
+    assert float((res["image"] - res2["image"]).abs().max()) <= 1e-6 * peak
+
+
+def test_fused_teams_auto_config5_like(bk, oracle_mod):
+    """Auto team size: 6 images of 2048 x 2048 on a full GPU leave one-CTA-per-image 96 % idle; the launcher picks a team."""
+    from paper_2505_15204_b200 import workloads
+    w = workloads.make_config(4, device="cuda", T=1, C=6)
+    w.vis = w.vis[:, :, :1].contiguous()
+    w.P = 1
+    bk.set_option(bk.OPT_IMAGE_PATH, 2)
+    try:
+        res = bk.blink_image(w.vis, w.uvw_m, w.freqs_hz, w.n_pix, w.pixscale_rad, w.weighting, want_cell_idx=True)
+        torch.cuda.synchronize()
+    finally:
+        bk.set_option(bk.OPT_IMAGE_PATH, 0)
+    _check_images(bk, w, res, oracle_mod, [0, 3, 5])
 
 
 # --------------------------------------------------------------------------- the fused kernel of the paper's side, 1200
