@@ -9,6 +9,7 @@
 // mirrored into the gridded half plane as the conjugate sample's taps, and 1 / (c(y) c(x)) rides on the image store.
 // Host side (this file): the polynomial form of the normalised tap weights, the taper table kernel, the C ABI.
 #include <math.h>
+#include <algorithm>
 
 #include "blink_fused_kernel.cuh"
 
@@ -141,6 +142,129 @@ static int launch_conv(const FusedArgs &a, int R, const double *freqs_hz, double
     }
 }
 
+// ---- every other supported size (the paper's 1200 and 8192 among them): the plain form --------------------------------
+// One thread per (baseline, (t,c)) evaluates the sample's taps once and adds them, and the mirrored conjugate taps, to the
+// full complex grids of the P planes with global vector atomics (red.global.add.v2.f32); the unfused transform
+// (blink_fft2d.cu / blink_fftg.cu) follows and one elementwise pass applies the grid correction.  A fallback, not a tuned
+// path: it exists so that the convolutional gridder covers every side blink_image covers.
+template <int R>
+__global__ void __launch_bounds__(256)
+conv_scatter_kernel(const float2 *__restrict__ vis, const float *__restrict__ uvw_m, const __grid_constant__ ScaleBlock sc,
+                    const __grid_constant__ ConvPoly poly, int C, int P, int B, int n, int tc0, int c_base, float2 *__restrict__ grid,
+                    unsigned *__restrict__ n_in, int32_t *__restrict__ cell_idx)
+{
+    constexpr int S = 2 * R + 1;
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= B) return;
+    const int tc = tc0 + blockIdx.y, t = tc / C, c = tc - t * C, h = n / 2;
+    const float s = sc.s[c - c_base];
+    const float *q = uvw_m + ((size_t)t * B + b) * 3;
+    int iu0, iv0;
+    const float x = __fmul_rn(q[0], s), y = __fmul_rn(q[1], s);
+    const float xr = rint_rne(x, iu0), yr = rint_rne(y, iv0);
+    const float lim = (float)(h - 1 - R);
+    const bool ok = fabsf(xr) <= lim && fabsf(yr) <= lim;       // NaN fails: the whole support stays on the grid (R16)
+    if (cell_idx) cell_idx[(size_t)tc * B + b] = ok ? (iv0 + h) * n + (iu0 + h) : -1;
+    if (!ok) return;
+    const float fx = __fsub_rn(x, xr), fy = __fsub_rn(y, yr);
+    float wx[S], wy[S];
+#pragma unroll
+    for (int i = 0; i < S; ++i) {
+        float a = poly.c[i][kConvTerms - 1], d = a;
+#pragma unroll
+        for (int k = kConvTerms - 2; k >= 0; --k) { a = fmaf(a, fx, poly.c[i][k]); d = fmaf(d, fy, poly.c[i][k]); }
+        wx[i] = a;
+        wy[i] = d;
+    }
+    atomicAdd(&n_in[tc], 1u);
+    for (int p = 0; p < P; ++p) {
+        const float2 v = __ldg(vis + ((size_t)tc * P + p) * B + b);
+        float2 *g = grid + ((size_t)blockIdx.y * P + p) * n * n;
+#pragma unroll
+        for (int i = 0; i < S; ++i) {
+            const int r0 = iv0 - R + i;
+#pragma unroll
+            for (int j = 0; j < S; ++j) {
+                const int q0 = iu0 - R + j;
+                const float w = wy[i] * wx[j];
+                atomicAdd(g + (size_t)(r0 + h) * n + (q0 + h), make_float2(w * v.x, w * v.y));
+                atomicAdd(g + (size_t)(h - r0) * n + (h - q0), make_float2(w * v.x, -w * v.y));     // conjugate sample: mirrored taps
+            }
+        }
+    }
+}
+__global__ void conv_wsum_kernel(const unsigned *__restrict__ n_in, float *__restrict__ wsum, int tc0, int m)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < m) wsum[tc0 + i] = (float)(2u * n_in[tc0 + i]);
+}
+// image[i][y][x] *= inv_c[y] inv_c[x]  (n is even: float2 accesses)
+__global__ void __launch_bounds__(256) conv_correct_kernel(float *__restrict__ image, const float *__restrict__ inv_c, int n, size_t n_rows)
+{
+    const int half = n / 2;
+    for (size_t row = blockIdx.x; row < n_rows; row += gridDim.x) {
+        const float cy = inv_c[row % n];
+        float2 *r = reinterpret_cast<float2 *>(image + row * n);
+        for (int k = threadIdx.x; k < half; k += blockDim.x) {
+            float2 v = r[k];
+            v.x *= cy * inv_c[2 * k];
+            v.y *= cy * inv_c[2 * k + 1];
+            r[k] = v;
+        }
+    }
+}
+
+static size_t conv_unfused_fixed(int T, int C, int n_pix)
+{
+    return gfft_workspace_bytes(n_pix) + taper_bytes(n_pix) + align_up((size_t)T * C * sizeof(unsigned), 256);
+}
+size_t conv_unfused_workspace_bytes(int T, int C, int P, int n_pix, bool minimum)
+{
+    const size_t per_tc = (size_t)P * n_pix * n_pix * sizeof(float2);
+    return conv_unfused_fixed(T, C, n_pix) + per_tc * (minimum ? 1 : std::min<size_t>((size_t)T * C, 256));
+}
+
+static int conv_unfused(const float2 *vis, const float *uvw_m, const double *freqs_hz, int T, int C, int P, int B, int n_pix,
+                        double pixscale_rad, int support, double beta, const ConvPoly &poly_in, float *image, float *wsum,
+                        int32_t *cell_idx, void *workspace, size_t workspace_bytes, cudaStream_t st)
+{
+    const size_t n2 = (size_t)n_pix * n_pix, per_tc = (size_t)P * n2 * sizeof(float2);
+    const size_t fixed = conv_unfused_fixed(T, C, n_pix);
+    if (!workspace || (reinterpret_cast<uintptr_t>(workspace) & 255u) || workspace_bytes < fixed + per_tc) return BLINK_ERR_WORKSPACE;
+    unsigned char *w = static_cast<unsigned char *>(workspace);
+    float2 *tw_generic = gfft_workspace_bytes(n_pix) ? reinterpret_cast<float2 *>(w) : nullptr;
+    float *inv_c = reinterpret_cast<float *>(w + gfft_workspace_bytes(n_pix));
+    unsigned *n_in = reinterpret_cast<unsigned *>(w + gfft_workspace_bytes(n_pix) + taper_bytes(n_pix));
+    float2 *wgrid = reinterpret_cast<float2 *>(w + fixed);
+    const int chunk = (int)std::min<size_t>((size_t)T * C, std::min<size_t>((workspace_bytes - fixed) / per_tc, 65535));
+    conv_taper_kernel<<<(n_pix + 255) / 256, 256, 0, st>>>(inv_c, n_pix, support, beta);
+    BLINK_LAUNCH_CHECK("conv_taper_kernel");
+    BLINK_CUDA_TRY(cudaMemsetAsync(n_in, 0, (size_t)T * C * sizeof(unsigned), st));
+    ConvPoly poly = poly_in;
+    poly.inv_taper = inv_c;
+    const int R = (support - 1) / 2;
+    return for_channel_blocks(C, 0, T * C, freqs_hz, n_pix, pixscale_rad, [&](int s0, int m, int c_base, const ScaleBlock &sc) -> int {
+        for (int s = s0; s < s0 + m; s += chunk) {
+            const int mm = std::min(chunk, s0 + m - s);
+            BLINK_CUDA_TRY(cudaMemsetAsync(wgrid, 0, (size_t)mm * per_tc, st));
+            const dim3 g((B + 255) / 256, mm);
+            if (R == 1) conv_scatter_kernel<1><<<g, 256, 0, st>>>(vis, uvw_m, sc, poly, C, P, B, n_pix, s, c_base, wgrid, n_in, cell_idx);
+            else if (R == 2) conv_scatter_kernel<2><<<g, 256, 0, st>>>(vis, uvw_m, sc, poly, C, P, B, n_pix, s, c_base, wgrid, n_in, cell_idx);
+            else conv_scatter_kernel<3><<<g, 256, 0, st>>>(vis, uvw_m, sc, poly, C, P, B, n_pix, s, c_base, wgrid, n_in, cell_idx);
+            BLINK_LAUNCH_CHECK("conv_scatter_kernel");
+            conv_wsum_kernel<<<(mm + 255) / 256, 256, 0, st>>>(n_in, wsum, s, mm);
+            BLINK_LAUNCH_CHECK("conv_wsum_kernel");
+            float *img = image + (size_t)s * P * n2;
+            int rc = fft2d_range(wgrid, n_pix, mm * P, wsum, P, s * P, img, nullptr, st, tw_generic, /*hermitian=*/true);
+            if (rc != BLINK_OK) return rc;
+            const size_t n_rows = (size_t)mm * P * n_pix;
+            conv_correct_kernel<<<(unsigned)std::min<size_t>(n_rows, (size_t)148 * 16), 256, 0, st>>>(img, inv_c, n_pix, n_rows);
+            BLINK_LAUNCH_CHECK("conv_correct_kernel");
+        }
+        return (int)BLINK_OK;
+    });
+}
+
 }  // namespace blink
 
 using namespace blink;
@@ -183,9 +307,15 @@ extern "C" int blink_image_conv(const blink_c64 *vis, const float *uvw_m, const 
     int rc = conv_check(support, beta);
     if (rc != BLINK_OK) return rc;
     if ((long long)T * C * P > 0x3fffffffLL) return BLINK_ERR_UNSUPPORTED;
-    if (!is_pow2(n_pix) || !fused_supported(P, B, n_pix, BLINK_W_NATURAL)) return BLINK_ERR_UNSUPPORTED;
+    if (!size_supported(n_pix) || B > kMaxBaselines) return BLINK_ERR_UNSUPPORTED;
     rc = ensure_device();
     if (rc != BLINK_OK) return rc;
+    if (!is_pow2(n_pix) || !fused_supported(P, B, n_pix, BLINK_W_NATURAL)) {       // outside the fused kernel: the plain form
+        ConvPoly poly_u;
+        conv_fit_taps(support, beta, &poly_u);
+        return conv_unfused(reinterpret_cast<const float2 *>(vis), uvw_m, freqs_hz, T, C, P, B, n_pix, pixscale_rad, support, beta,
+                            poly_u, image, wsum, cell_idx, workspace, workspace_bytes, static_cast<cudaStream_t>(stream));
+    }
     const size_t extra = taper_bytes(n_pix);
     if (!workspace || (reinterpret_cast<uintptr_t>(workspace) & 255u) ||
         workspace_bytes < fused_conv_workspace_bytes(T, B, n_pix, 1))

@@ -16,6 +16,7 @@ int fused_image(const float2 *vis, const float *uvw_m, const double *freqs_hz, d
                 int32_t *cell_idx, void *workspace, size_t workspace_bytes, cudaStream_t st, GainRef cal);
 size_t avg_workspace_bytes(int T, int C, int P, int B, int n_pix, int weighting, bool minimum);   // blink_avg.cu
 size_t fused_conv_workspace_bytes(int T, int B, int n_pix, int ctas);                               // blink_fused_conv.cu
+size_t conv_unfused_workspace_bytes(int T, int C, int P, int n_pix, bool minimum);
 int counts_only(const float *uvw_m, const double *freqs_hz, double pixscale_rad, int T, int C, int B, int n_pix,
                 int tc0, int ntc, uint32_t *counts, cudaStream_t st);
 
@@ -249,7 +250,11 @@ extern "C" int blink_workspace_bytes(int op, int T, int C, int P, int B, int n_p
             mn = avg_workspace_bytes(T, C, P, B, n_pix, weighting, true);
             break;
         case BLINK_OP_IMAGE_CONV: {
-            if (!is_pow2(n_pix) || !fused_supported(P, B, n_pix, BLINK_W_NATURAL)) return BLINK_ERR_UNSUPPORTED;
+            if (!is_pow2(n_pix) || !fused_supported(P, B, n_pix, BLINK_W_NATURAL)) {
+                rec = conv_unfused_workspace_bytes(T, C, P, n_pix, false);
+                mn = conv_unfused_workspace_bytes(T, C, P, n_pix, true);
+                break;
+            }
             int ctas = option(BLINK_OPT_FUSED_CTAS);
             if (ctas <= 0) ctas = fused_default_ctas();
             rec = fused_conv_workspace_bytes(T, B, n_pix, ctas);

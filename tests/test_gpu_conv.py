@@ -122,6 +122,26 @@ def test_conv_large_sides(bk, oracle_mod, n, S):
     _check_conv(w, res, oracle_mod, S, ids=[1])
 
 
+@pytest.mark.parametrize("n,S,B", [(64, 3, 700), (128, 7, 1500), (240, 5, 1237), (1200, 5, 900)])
+def test_conv_sizes_outside_the_fused_kernel(bk, oracle_mod, n, S, B):
+    """Sides the fused kernel does not cover (below 256, not a power of two -- the paper's 1200 among them): the plain form
+    (global-atomic scatter of the taps, unfused transform, correction pass), recommended and minimum workspaces (chunking)."""
+    from paper_2505_15204_b200 import workloads
+    w = workloads.make_random(T=2, C=3, P=2, B=B, n_pix=n, weighting=0, seed=300 + n + S, device="cuda", fill=1.1)
+    w.uvw_m[1, 5, 0] = float("nan")
+    w.uvw_m[0, 6, :2] = 0.0                                         # DC: sample and conjugate taps overlap
+    ids = None if n <= 240 else [0, 7, 11]
+    res = bk.blink_image_conv(w.vis, w.uvw_m, w.freqs_hz, n, w.pixscale_rad, S, want_cell_idx=True)
+    torch.cuda.synchronize()
+    _check_conv(w, res, oracle_mod, S, ids=ids)
+    _, mn = bk.blink_workspace_bytes(bk.OP_IMAGE_CONV, w.T, w.C, w.P, w.B, n, 0)
+    ws = torch.empty(mn + 3 * w.P * n * n * 8, dtype=torch.uint8, device="cuda")          # four (t,c) per chunk
+    res1 = bk.blink_image_conv(w.vis, w.uvw_m, w.freqs_hz, n, w.pixscale_rad, S, workspace=ws)
+    torch.cuda.synchronize()
+    _check_conv(w, res1, oracle_mod, S, ids=ids, check_cells=False)
+    assert torch.equal(res["wsum"], res1["wsum"])
+
+
 def test_conv_two_stage_pipeline_and_beta(bk, oracle_mod):
     # B = 13000 leaves room for two pass-2 stage buffers only (NS = 2); a caller-chosen beta
     from paper_2505_15204_b200 import workloads
@@ -159,7 +179,7 @@ def test_conv_error_codes(bk):
     call = lambda n, S, beta, ws=4 << 20: L.blink_image_conv(p(x), p(x), f, 1, 1, 1, 4, n, 0.01, S, beta, p(x), p(x), None,
                                                               p(x), ws, None)
     assert call(256, 4, 0.0) == -2 and call(256, 9, 0.0) == -2 and call(256, 1, 0.0) == -2
-    assert call(128, 3, 0.0) == -2 and call(1200, 3, 0.0) == -2     # fused kernel only
+    assert call(98, 3, 0.0) == -2 and call(16, 3, 0.0) == -2        # sides blink_image does not support either
     assert call(256, 5, 6.0) == -1                                  # beta below 1.7 S
     assert call(256, 5, 0.0, ws=1024) == -3
 
