@@ -55,10 +55,14 @@ def test_host_only_calls(so_path):
     # sides that are not a power of two need an N-entry twiddle table for the mixed-radix transform
     rec, mn = bk.blink_workspace_bytes(bk.OP_FFT2D, 1, 1, 1, 0, 1200, 0)
     assert rec == mn == 1200 * 8 + (-1200 * 8) % 256
-    # ... and blink_image at such a side keeps one row extent (16 bytes) per (t,c) behind the chunk's grids
-    twb = rec
+    # ... and blink_image through the unfused chain at such a side keeps one row extent (16 bytes) per (t,c) behind the chunk's grids
+    rec, mn = bk.blink_workspace_bytes(bk.OP_IMAGE, 2, 768, 1, 8128, 240, 0)
+    twb = 240 * 8 + (-240 * 8) % 256
+    assert mn == twb + 240 * 240 * 8 + 16 and rec == twb + 256 * (240 * 240 * 8 + 16)
+    # the paper's side 1200 has a fused kernel: sorted baselines, the twiddle table, one transposed half plane per CTA
     rec, mn = bk.blink_workspace_bytes(bk.OP_IMAGE, 2, 768, 1, 8128, 1200, 0)
-    assert mn == twb + 1200 * 1200 * 8 + 16 and rec == twb + 256 * (1200 * 1200 * 8 + 16)
+    sortb = 3 * (2 * 8128 * 4 + (-2 * 8128 * 4) % 256)
+    assert mn == sortb + 9728 + 1200 * 600 * 8 and (rec - sortb - 9728) % (1200 * 600 * 8) == 0 and rec > mn
     # small batches (<= 8 Mi pixels, auto path): the recommended size also holds the whole range for the unfused chain
     for n, n_img in ((256, 128), (512, 32), (1024, 8), (2048, 2)):
         rec, mn = bk.blink_workspace_bytes(bk.OP_IMAGE, 1, n_img, 1, 8128, n, 0)
@@ -112,7 +116,11 @@ def test_conv_argument_checks(so_path):
     rec, mn = bk.blink_workspace_bytes(bk.OP_IMAGE_CONV, 50, 768, 1, 8128, 512, 0)
     rec0, mn0 = bk.blink_workspace_bytes(bk.OP_IMAGE, 50, 768, 1, 8128, 512, 0)
     assert rec == rec0 + 2048 and mn == mn0 + 2048                        # + the 512-entry correction table
+    # outside the fused kernel (the paper's 1200, sides below 256): twiddles + correction table + counters + the chunk's grids
+    rec, mn = bk.blink_workspace_bytes(bk.OP_IMAGE_CONV, 2, 300, 1, 100, 1200, 0)
+    fixed = 9728 + 4864 + 2560
+    assert mn == fixed + 1200 * 1200 * 8 and rec == fixed + 256 * 1200 * 1200 * 8
+    rec, mn = bk.blink_workspace_bytes(bk.OP_IMAGE_CONV, 1, 1, 2, 100, 128, 0)
+    assert rec == mn == 512 + 256 + 2 * 128 * 128 * 8
     with pytest.raises(bk.BlinkError):
-        bk.blink_workspace_bytes(bk.OP_IMAGE_CONV, 1, 1, 1, 100, 1200, 0)  # fused kernel only: powers of two
-    with pytest.raises(bk.BlinkError):
-        bk.blink_workspace_bytes(bk.OP_IMAGE_CONV, 1, 1, 1, 100, 128, 0)
+        bk.blink_workspace_bytes(bk.OP_IMAGE_CONV, 1, 1, 1, 100, 98, 0)    # 2 * 7^2
