@@ -191,6 +191,12 @@ def timed_ms(run, steps, warmup, dev, world, flush=None):
     return shard.max_over_ranks(tot / steps, device=dev)
 
 
+def bk_team_text(bk):
+    v = __import__("ctypes").c_int(0)
+    bk.lib().blink_get_option(bk.OPT_FUSED_TEAM, __import__("ctypes").byref(v))
+    return "auto (cost model of blink_fused_kernel.cuh)" if v.value == 0 else f"forced {v.value} CTAs per image"
+
+
 def config_leg(bk, cfg, T, dev, world, rank, steps, warmup, peak):
     """One short timed leg of BASELINE.json config `cfg` through blink_image (device-resident inputs)."""
     w = workloads.make_config(cfg, device=dev, T=T, seed=shard.rank_seed(cfg, rank))
@@ -212,7 +218,7 @@ def config_leg(bk, cfg, T, dev, world, rank, steps, warmup, peak):
                        f"{'natural' if w.weighting == 0 else 'uniform'} weighting",
            "ms_per_step": ms, "images_per_s": world * n_img / (ms * 1e-3), "gvis_per_s": world * n_img * B / (ms * 1e-3) / 1e9,
            "frac_M4": mb["M4"] / (ms * 1e-3) / 1e9 / peak, "model_speedup_M36": mb["M36"] / (ms * 1e-3) / 1e9 / peak,
-           "gpu_launches_per_step": int(launches), "l2": "flushed between timed calls (256 MB write)" if small else "outputs larger than L2; no flush"}
+           "team": bk_team_text(bk), "gpu_launches_per_step": int(launches), "l2": "flushed between timed calls (256 MB write)" if small else "outputs larger than L2; no flush"}
     if cfg == 1:
         out["us_per_image"] = ms * 1e3
         out["note"] = "one image: launch-latency bound, fractions not meaningful (SURVEY 8(d))"
@@ -240,6 +246,7 @@ def main():
     ap.add_argument("--no-cufft", action="store_true")
     ap.add_argument("--no-configs", action="store_true", help="skip the timed legs of configs 1, 2, 4 (one timestep), 5")
     ap.add_argument("--conv-support", type=int, default=5, help="support of the gridding kernel timed in conv_mode (3, 5, 7)")
+    ap.add_argument("--team", type=int, default=0, help="BLINK_OPT_FUSED_TEAM: CTAs per image in the fused kernel (0 = auto)")
     ap.add_argument("--T", type=int, default=None, help="reduce timesteps (debug only; invalidates the headline)")
     args = ap.parse_args()
 
@@ -260,6 +267,7 @@ def main():
         dist.init_process_group("nccl", device_id=dev)
     bk.lib()
     bk.set_option(bk.OPT_IMAGE_PATH, args.path)
+    bk.set_option(bk.OPT_FUSED_TEAM, args.team)
 
     # independent batch per rank ("each second of observation can be processed independently")
     w = workloads.make_config(args.config, device=dev, T=args.T, seed=shard.rank_seed(args.config, rank))
@@ -425,10 +433,10 @@ def main():
             n_p = TP * C * P
             m36 = n_p * (36 * NP * NP + 8 * B) + 12 * TP * B
             m4 = n_p * (4 * NP * NP + 8 * B) + 12 * TP * B
-            paper = {"api": "blink_image at n_pix = 1200 (generic mixed-radix chain: half-plane gridder, row pass, Hermitian column pass)",
+            paper = {"api": "blink_image at n_pix = 1200 (fused kernel of the paper's side, blink_fused_g.cu: 15 x 5 x 16 register-resident stages)",
                      "images_per_run": n_p, "ms_per_run": ms_p, "images_per_s": world * n_p / (ms_p * 1e-3),
                      "s_per_second_of_data": ms_p * 1e-3 * (T / TP),
-                     "frac_M36": m36 / (ms_p * 1e-3) / 1e9 / hbm_peak()[0], "frac_M4": m4 / (ms_p * 1e-3) / 1e9 / hbm_peak()[0],
+                     "frac_M4": m4 / (ms_p * 1e-3) / 1e9 / hbm_peak()[0], "model_speedup_M36": m36 / (ms_p * 1e-3) / 1e9 / hbm_peak()[0],
                      "paper_context": "PAPER.md Table 6 (L339-340), gridding + 2D FFT of 38400 images of 1200^2: 1.77 s on an H100 (cuFFT), "
                                       "7.09 s on an MI250X GCD (rocFFT); other machines: context, not a target"}
             del ws_p, vis_p, uvw_p, img_p

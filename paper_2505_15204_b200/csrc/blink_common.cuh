@@ -61,6 +61,9 @@ struct GainRef {
 struct ScaleBlock { float s[1024]; };
 
 #ifdef __CUDACC__
+#ifndef BLINK_GRID_EXCH
+#define BLINK_GRID_EXCH 1
+#endif
 // Round to nearest, ties to even, WITHOUT the quarter-rate conversion unit (FRND / F2I): adding and subtracting
 // 1.5 * 2^23 with two correctly rounded fp32 adds (never contracted into an fma) gives exactly rint(x) for
 // |x| < 2^22, and the integer sits in the mantissa of the intermediate sum.  For larger |x| (and inf / NaN) the
@@ -87,6 +90,27 @@ __device__ __forceinline__ int cell_of(float u_m, float v_m, float s, int n, int
     if (!cell_coords(u_m, v_m, s, h, iu, iv, r)) return -1;
     return (iv + h) * n + (iu + h);
 }
+// Accumulate one complex sample into a shared-memory cell WITHOUT floating-point atomics.  fp32 atomicAdd on shared memory
+// is a load + compare-and-swap spin loop per scalar on sm_100 (ATOMS.CAST.SPIN; profiles/r1_fused_v2.md: 17 wavefronts per
+// warp instruction), but the 64-bit exchange ATOMS.EXCH.64 is native.  Cells start at zero and almost every cell of a
+// nearest-cell grid receives ONE sample (1.04-1.22 per occupied cell), so: put the sample and look at what
+// came out.  Zero bits: the cell was empty, done -- one instruction.  Otherwise the value that came out is now this
+// thread's to re-add: take whatever is in the cell (exchange with zero), add, put the sum back; repeat while a put
+// displaces a non-zero value.  Invariant: cell + values in flight = sum of the samples; a value is in flight in exactly one
+// thread; every exit leaves nothing in flight.  Bit-identical samples are handled like any other (no tags, no compares of
+// values).  A displaced -0.0 merely costs one more round.
+__device__ __forceinline__ void cell_add_exch(float2 *cell, float2 v)
+{
+    unsigned long long *p = reinterpret_cast<unsigned long long *>(cell);
+    unsigned long long out = atomicExch(p, *reinterpret_cast<unsigned long long *>(&v));
+    while (out != 0ull) {
+        const unsigned long long cur = atomicExch(p, 0ull);
+        const float2 a = *reinterpret_cast<float2 *>(&out), b = *reinterpret_cast<const float2 *>(&cur);
+        float2 sum = make_float2(a.x + b.x, a.y + b.y);
+        out = atomicExch(p, *reinterpret_cast<unsigned long long *>(&sum));
+    }
+}
+
 __device__ __forceinline__ int mirror_of(int cell, int n)
 {
     const int r = cell / n, q = cell - r * n;

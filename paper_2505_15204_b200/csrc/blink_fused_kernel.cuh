@@ -56,28 +56,6 @@ constexpr int kConvTerms = 14;
 constexpr int kConvMaxSupport = 7;
 struct ConvPoly { float c[kConvMaxSupport][kConvTerms]; const float *inv_taper; };     // c[j + R][k] multiplies f^k
 
-// Accumulate one complex sample into a shared-memory cell WITHOUT floating-point atomics.  fp32 atomicAdd on shared memory
-// is a load + compare-and-swap spin loop per scalar on sm_100 (ATOMS.CAST.SPIN; profiles/r1_fused_v2.md: 17 wavefronts per
-// warp instruction), but the 64-bit exchange ATOMS.EXCH.64 is native.  Cells start at zero and almost every cell of a
-// nearest-cell grid receives ONE sample (1.04-1.22 per occupied cell), so: put the sample and look at what
-// came out.  Zero bits: the cell was empty, done -- one instruction.  Otherwise the value that came out is now this
-// thread's to re-add: take whatever is in the cell (exchange with zero), add, put the sum back; repeat while a put
-// displaces a non-zero value.  Invariant: cell + values in flight = sum of the samples; a value is in flight in exactly one
-// thread; every exit leaves nothing in flight.  Bit-identical samples are handled like any other (no tags, no compares of
-// values).  A displaced -0.0 merely costs one more round.
-#ifndef BLINK_GRID_EXCH
-#define BLINK_GRID_EXCH 1
-#endif
-__device__ __forceinline__ void cell_add_exch(float2 *cell, float2 v)
-{
-    unsigned long long *p = reinterpret_cast<unsigned long long *>(cell);
-    unsigned long long out = atomicExch(p, pk_bits(v));
-    while (out != 0ull) {
-        const unsigned long long cur = atomicExch(p, 0ull);
-        out = atomicExch(p, pk_bits(cadd(pk_f2(out), pk_f2(cur))));
-    }
-}
-
 struct ExchangePadded2 {
     float2 *c0, *c1;
     __device__ __forceinline__ void put(int w, const float2 (&v)[2]) const

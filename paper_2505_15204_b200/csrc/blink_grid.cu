@@ -122,8 +122,7 @@ grid_tiles_kernel(const GridArgs a, const __grid_constant__ ScaleBlock sc)
                     const int cl = it & 8191u;
                     float2 v = __ldg(vrow + (it >> 14));
                     if (it & (1u << 13)) v.y = -v.y;           // Hermitian conjugate sample
-                    atomicAdd(&tile[cl].x, v.x);
-                    atomicAdd(&tile[cl].y, v.y);
+                    cell_add_exch(&tile[cl], v);              // native 64-bit exchanges instead of two fp32 CAS loops (blink_common.cuh)
                     if (p == 0) atomicAdd(&cnt[cl], 1u);
                 }
                 __syncthreads();
