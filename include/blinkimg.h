@@ -199,7 +199,7 @@ int blink_image_cal(const blink_c64 *vis, const float *uvw_m, const double *freq
  * prime factors 2, 3, 5: the paper's 1200 and 8192 among them) takes the plain form -- taps scattered into full grids with
  * global vector atomics, the unfused transform, one elementwise correction pass -- in chunks that fit the workspace.
  * `workspace` >= blink_workspace_bytes(BLINK_OP_IMAGE_CONV) minimum, 256-byte aligned.  Other arguments as blink_image.
- * The tap weights are evaluated as degree-13 polynomials in the offset, fitted on the host at every call;
+ * The tap weights are evaluated as degree-11 polynomials in the offset, fitted on the host at every call;
  * blink_conv_taps_host (HOST pointers, no GPU needed) returns the weights exactly as the kernel evaluates them for
  * one offset f in [-1/2, 1/2], plus the largest deviation of the fit from the window's definition (tests).
  */

@@ -111,6 +111,21 @@ __device__ __forceinline__ void cell_add_exch(float2 *cell, float2 v)
     }
 }
 
+// The same without the optimistic first put, for cells that usually hold a value already (convolutional gridding: a cell is
+// hit ~S^2 times): take what is there (exchange with zero), add, put the sum back; a non-zero value coming out of the put
+// arrived in between and is re-added the same way.  Two native atomics per complex tap instead of two load + CAS spin loops.
+__device__ __forceinline__ void cell_add_take(float2 *cell, float2 v)
+{
+    unsigned long long *p = reinterpret_cast<unsigned long long *>(cell);
+    for (;;) {
+        const unsigned long long cur = atomicExch(p, 0ull);
+        const float2 c = *reinterpret_cast<const float2 *>(&cur);
+        float2 sum = make_float2(v.x + c.x, v.y + c.y);
+        const unsigned long long out = atomicExch(p, *reinterpret_cast<unsigned long long *>(&sum));
+        if (out == 0ull) break;
+        v = *reinterpret_cast<const float2 *>(&out);
+    }
+}
 __device__ __forceinline__ int mirror_of(int cell, int n)
 {
     const int r = cell / n, q = cell - r * n;

@@ -52,7 +52,10 @@ constexpr size_t kTeamBytes = 4096;                            // team_ctr + tea
 //   w_j(f) = k(j - f) / sum_i k(i - f),  f = x - rint(x) in [-1/2, 1/2],  k = Kaiser-Bessel window of support S = 2R+1,
 // is a smooth function of f and is evaluated as a polynomial in f (Horner, fp32).  The coefficients are fitted on the
 // host in double (Chebyshev interpolation, conv_fit_taps in blink_fused_conv.cu) and travel as a kernel parameter.
-constexpr int kConvTerms = 14;
+#ifndef BLINK_CONV_TERMS
+#define BLINK_CONV_TERMS 12
+#endif
+constexpr int kConvTerms = BLINK_CONV_TERMS;
 constexpr int kConvMaxSupport = 7;
 struct ConvPoly { float c[kConvMaxSupport][kConvTerms]; const float *inv_taper; };     // c[j + R][k] multiplies f^k
 
@@ -334,8 +337,16 @@ fused_image_kernel(const FusedArgs a, const __grid_constant__ ScaleBlock sc, con
                 // on interference -- was 1.4x (S = 5) to 2.1x (S = 7) SLOWER than the plain per-scalar adds below.)
                 // Odd lanes add the imaginary part first: one warp-wide atomic then touches even AND odd banks (the real parts
                 // alone live in the 16 even banks), which cuts the expected bank conflicts of 32 unrelated rows.
+#ifndef BLINK_CONV_TAKE
+#define BLINK_CONV_TAKE 1
+#endif
                 const int odd = lane & 1;
                 auto add_taps = [&](float2 *col, int row0, int dir, float ar, float ai) {
+#if BLINK_CONV_TAKE
+                    (void)odd;
+#pragma unroll
+                    for (int i = 0; i < S; ++i) cell_add_take(&col[xsw(row0 + dir * i)], make_float2(wy[i] * ar, wy[i] * ai));
+#else
                     const float first = odd ? ai : ar, second = odd ? ar : ai;
 #pragma unroll
                     for (int i = 0; i < S; ++i) {
@@ -343,6 +354,7 @@ fused_image_kernel(const FusedArgs a, const __grid_constant__ ScaleBlock sc, con
                         atomicAdd(cell + odd, wy[i] * first);
                         atomicAdd(cell + (odd ^ 1), wy[i] * second);
                     }
+#endif
                 };
                 auto wx_of = [&](int jj) {                      // tap jj - R of the u axis (dynamic index: LDC)
                     float w = cpoly.c[jj][kConvTerms - 1];
