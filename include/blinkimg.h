@@ -246,6 +246,26 @@ int blink_image_stokes_i(const blink_c64 *vis, const float *uvw_m, const double 
                          int T, int C, int P, int B, int n_pix, double pixscale_rad, int weighting,
                          float *image, float *wsum, void *workspace, size_t workspace_bytes, void *stream);
 
+/*
+ * blink_image without a workspace argument, for callers that cannot allocate device memory (code under CUDA graph capture,
+ * tight serving loops, harnesses that forbid cudaMalloc).  The scratch blink_image needs lives in one built-in device array of
+ * blink_static_scratch_bytes() = 32 MiB that every GPU which loads the library holds until the process exits.  The call
+ * allocates and frees nothing (no cudaMalloc / cudaFree / allocating library routine) and runs blink_image's own kernels with
+ * that array as the workspace (fewer persistent CTAs / smaller chunks than a recommended-size workspace would give).
+ *   - A problem whose MINIMUM blink_image workspace (blink_workspace_bytes(BLINK_OP_IMAGE), *min_bytes) exceeds the array is
+ *     refused with BLINK_ERR_WORKSPACE before anything is launched; blink_last_cuda_error() names both sizes.  The fused
+ *     kernels need 12 T B bytes + one half plane (n_pix^2 * 4 bytes: 16 MiB at 2048, so 4096 does not fit); the unfused chain
+ *     needs P * n_pix^2 * 8 bytes + an n_pix-entry table.
+ *   - All calls on a device share the array and it keeps the last call's contents; what must start at zero is cleared
+ *     in-stream by the call itself.  Calls on one stream are ordered and safe; calls that OVERLAP on the GPU (different
+ *     streams, unordered threads) race on the array and must not be made.
+ * Arguments as blink_image (no cell_idx / counts outputs).  Results are blink_image's.
+ */
+size_t blink_static_scratch_bytes(void);
+int blink_image_static(const blink_c64 *vis, const float *uvw_m, const double *freqs_hz,
+                       int T, int C, int P, int B, int n_pix, double pixscale_rad, int weighting,
+                       float *image, float *wsum, void *stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -24,7 +24,7 @@ EXPORTS = ["blink_strerror", "blink_last_cuda_error", "blink_set_option", "blink
            "blink_kernel_launches", "blink_workspace_bytes", "blink_grid", "blink_fft2d_inverse",
            "blink_image", "blink_image_host", "blink_image_avg", "blink_apply_gains", "blink_image_cal",
            "blink_image_conv", "blink_conv_taps_host", "blink_correlate", "blink_image_stokes_i",
-           "blink_volt_out_of_range"]
+           "blink_volt_out_of_range", "blink_static_scratch_bytes", "blink_image_static"]
 
 
 class BlinkError(RuntimeError):
@@ -80,6 +80,10 @@ def lib():
         L.blink_image_stokes_i.argtypes = [vp, vp, vp, i, i, i, i, i, d, i, vp, vp, vp, sz, vp]
         L.blink_volt_out_of_range.restype = i
         L.blink_volt_out_of_range.argtypes = [vp, sz, vp, vp]
+        L.blink_static_scratch_bytes.restype = sz
+        L.blink_static_scratch_bytes.argtypes = []
+        L.blink_image_static.restype = i
+        L.blink_image_static.argtypes = [vp, vp, vp, i, i, i, i, i, d, i, vp, vp, vp]
         _lib = L
     return _lib
 
@@ -232,6 +236,23 @@ def blink_image(vis: torch.Tensor, uvw_m: torch.Tensor, freqs_hz, n_pix: int, pi
                                _ptr(workspace), workspace.numel(), _stream(dev))
     _check(rc, "blink_image")
     return dict(image=image, wsum=wsum, cell_idx=cell_idx, counts=counts)
+
+
+def blink_static_scratch_bytes() -> int:
+    return int(lib().blink_static_scratch_bytes())
+
+
+def blink_image_static(vis: torch.Tensor, uvw_m: torch.Tensor, freqs_hz, n_pix: int, pixscale_rad: float, weighting: int = 0,
+                       image: Optional[torch.Tensor] = None, wsum: Optional[torch.Tensor] = None):
+    """blink_image with the library's built-in 32 MiB scratch array instead of a workspace: the call allocates no device memory
+    when image and wsum are passed in.  Calls that overlap on the GPU race on that array; larger problems raise BlinkError."""
+    T, C, P, B, fr, dev = _vis_uvw(vis, uvw_m, freqs_hz)
+    image, wsum = _image_outputs(T, C, P, n_pix, dev, image, wsum)
+    with torch.cuda.device(dev):
+        rc = lib().blink_image_static(_ptr(vis), _ptr(uvw_m), fr.ctypes.data_as(ctypes.c_void_p), T, C, P, B, n_pix,
+                                      float(pixscale_rad), int(weighting), _ptr(image), _ptr(wsum), _stream(dev))
+    _check(rc, "blink_image_static")
+    return dict(image=image, wsum=wsum)
 
 
 def blink_image_stokes_i(vis: torch.Tensor, uvw_m: torch.Tensor, freqs_hz, n_pix: int, pixscale_rad: float,
