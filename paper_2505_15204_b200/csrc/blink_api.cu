@@ -116,7 +116,7 @@ int encode_tensor_map_3d_f32(CUtensorMap *out, const void *base, uint64_t d0, ui
 // 4D uint8 tensor map, 128-byte swizzle (the correlator's voltage tiles).  dims / box in BYTES-as-elements, innermost
 // first; strides in bytes for dims 1..3 (multiples of 16).
 int encode_tensor_map_4d_u8(CUtensorMap *out, const void *base, const uint64_t dims[4], const uint64_t strides[3],
-                            const uint32_t box[4])
+                            const uint32_t box[4], int swizzle_bytes)
 {
     EncodeTiledFn fn = encode_fn();
     if (!fn) return -1;
@@ -125,8 +125,9 @@ int encode_tensor_map_4d_u8(CUtensorMap *out, const void *base, const uint64_t d
     cuuint32_t b[4] = {box[0], box[1], box[2], box[3]};
     cuuint32_t estr[4] = {1, 1, 1, 1};
     CUresult r = fn(out, CU_TENSOR_MAP_DATA_TYPE_UINT8, 4, const_cast<void *>(base), d, st, b, estr,
-                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
-                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+                    CU_TENSOR_MAP_INTERLEAVE_NONE,
+                    swizzle_bytes == 32 ? CU_TENSOR_MAP_SWIZZLE_32B : swizzle_bytes == 64 ? CU_TENSOR_MAP_SWIZZLE_64B : CU_TENSOR_MAP_SWIZZLE_128B,
+                    CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     return (int)r;
 }
 

@@ -37,6 +37,7 @@ struct CorrArgs {
     int A, T, C, n_t, n_avg;
     int n_tiles_side, n_tiles, n_units;
     int nk, last_ksteps;                                        // chunks per (interval, fine channel); K steps of the last one
+    int tail_box;                                               // bytes per row staged for the last chunk: 32, 64 or 128
     float norm, rnorm;                                          // n_t * n_avg and its correctly rounded reciprocal
     float2 *vis;
 };
@@ -47,10 +48,12 @@ __device__ __forceinline__ void tc_commit(uint64_t *bar)
 {
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
-// K-major operand tile, 128-byte swizzle: rows of 128 bytes, 8-row groups 1024 bytes apart (SBO), version 1
-__device__ __forceinline__ uint64_t umma_desc_k128(uint32_t saddr)
+// K-major operand tile whose rows are `span` = 128 / 64 / 32 bytes in the swizzle of that width: 8-row groups span x 8 bytes
+// apart (SBO), layout type 2 / 4 / 6 (bits 61-63), descriptor version 1 (bit 46); LBO is unused for swizzled K-major tiles
+__device__ __forceinline__ uint64_t umma_desc_k(uint32_t saddr, uint32_t span)
 {
-    return (uint64_t)((saddr & 0x3FFFFu) >> 4) | (1ull << 16) | (64ull << 32) | (1ull << 46) | (2ull << 61);
+    const uint64_t type = span == 128u ? 2ull : span == 64u ? 4ull : 6ull;
+    return (uint64_t)((saddr & 0x3FFFFu) >> 4) | (1ull << 16) | ((uint64_t)(span >> 1) << 32) | (1ull << 46) | (type << 61);
 }
 __device__ __forceinline__ void umma_i8(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate)
 {
@@ -75,36 +78,6 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&r)[32])
         : "memory");
 }
 
-// ---- cluster variant (MC): three CTAs of a cluster take the three tiles (0,0), (1,0), (1,1) of the SAME (t, c) matrix and every
-// staged block leaves L2 once: the CTA of tile (0,0) loads X_0 with a multicast to itself and to the CTA of (1,0), the CTA of
-// (1,1) loads X_1 to itself and to (1,0).  Measured without it: the loads alone (each block fetched by the two tiles that use
-// it, ~8 TB/s out of L2) are the floor of the kernel.
-__device__ __forceinline__ uint32_t cluster_rank()
-{
-    uint32_t r;
-    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
-    return r;
-}
-__device__ __forceinline__ void cluster_sync_all()
-{
-    asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
-    asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
-}
-__device__ __forceinline__ void tc_commit_mc(uint64_t *bar, uint16_t mask)
-{
-    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
-                 ::"r"(smem_u32(bar)), "h"(mask) : "memory");
-}
-__device__ __forceinline__ void tma_load_4d_mc(void *smem_dst, const CUtensorMap *map, uint64_t *bar, int c0, int c1, int c2, int c3,
-                                               uint16_t mask)
-{
-    asm volatile(
-        "cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.multicast::cluster"
-        " [%0], [%1, {%3, %4, %5, %6}], [%2], %7;"
-        ::"r"(smem_u32(smem_dst)), "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "h"(mask)
-        : "memory");
-}
-
 // unit -> (t, c, I, J): the tiles of one (t, c) are consecutive units, so the CTAs working on them share X through L2;
 __device__ __forceinline__ void corr_unit(const CorrArgs &a, int u, int &t, int &c, int &I, int &J)
 {
@@ -117,29 +90,17 @@ __device__ __forceinline__ void corr_unit(const CorrArgs &a, int u, int &t, int 
     J = k;
 }
 
-// k-th tile of this CTA: plain variant = unit blockIdx.x + k gridDim.x; cluster variant = tile `rank` of item cluster + k n_clusters
-template <bool MC>
-__device__ __forceinline__ bool corr_tile(const CorrArgs &a, int k, uint32_t rank, int &t, int &c, int &I, int &J)
+// k-th tile of this CTA: unit blockIdx.x + k gridDim.x
+__device__ __forceinline__ bool corr_tile(const CorrArgs &a, int k, int &t, int &c, int &I, int &J)
 {
-    if constexpr (MC) {
-        const int item = (int)(blockIdx.x / 3) + k * (int)(gridDim.x / 3);
-        if (item >= a.T * a.C) return false;
-        c = item / a.T;
-        t = item - c * a.T;
-        I = rank == 0 ? 0 : 1;
-        J = rank == 2 ? 1 : 0;
-        return true;
-    } else {
-        const long long u = (long long)blockIdx.x + (long long)k * gridDim.x;
-        if (u >= a.n_units) return false;
-        corr_unit(a, (int)u, t, c, I, J);
-        return true;
-    }
+    const long long u = (long long)blockIdx.x + (long long)k * gridDim.x;
+    if (u >= a.n_units) return false;
+    corr_unit(a, (int)u, t, c, I, J);
+    return true;
 }
 
-template <bool MC>
 __global__ void __launch_bounds__(kCorrThreads, 1)
-corr_kernel(const CorrArgs a, const __grid_constant__ CUtensorMap tmap)
+corr_kernel(const CorrArgs a, const __grid_constant__ CUtensorMap tmap, const __grid_constant__ CUtensorMap tmap_tail)
 {
     extern __shared__ __align__(16) unsigned char corr_smem[];
     const uint32_t base = smem_u32(corr_smem);
@@ -149,17 +110,16 @@ corr_kernel(const CorrArgs a, const __grid_constant__ CUtensorMap tmap)
     uint64_t *tmem_full = bars + 3 * kCorrStages, *tmem_empty = tmem_full + 2;
     uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(tmem_empty + 2);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const uint32_t rank = MC ? cluster_rank() : 0u;
-    // stage slots (16 KB each).  plain: A block | X_J | b''_J.  cluster: rank 0: - | X_0 | b''_0;  rank 1: X_1 | X_0 | b''_0;
-    // rank 2: X_1 | b''_1 | - (X_1 must sit at the same offset in ranks 1 and 2: one multicast writes both)
-    const uint32_t xj_off = (MC && rank == 2) ? 0u : (uint32_t)kCorrRowsBytes;     // X_J, followed by its transformed copy
+    // stage slots (16 KB each): A block X_I | X_J | b''_J
+    constexpr uint32_t xj_off = (uint32_t)kCorrRowsBytes;      // X_J, followed by its transformed copy
+    // the last chunk of an (interval, fine channel) holds a.tail_box bytes per row (32 / 64: narrower swizzle; 128: like the rest)
+    const uint32_t tail_rows_bytes = (uint32_t)kCorrTile * (uint32_t)a.tail_box;
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < kCorrStages; ++s) {
             mbar_init(&full_tma[s], 1);
             mbar_init(&full_xf[s], kCorrXfWarps * 32);
-            // cluster: a loading CTA may refill stage s only when its own MMAs AND those of the CTA of tile (1,0) are done with it
-            mbar_init(&empty[s], (MC && rank != 1) ? 2 : 1);
+            mbar_init(&empty[s], 1);
         }
         for (int b = 0; b < 2; ++b) {
             mbar_init(&tmem_full[b], 1);
@@ -167,6 +127,7 @@ corr_kernel(const CorrArgs a, const __grid_constant__ CUtensorMap tmap)
         }
         fence_mbar_init();
         tma_prefetch_desc(&tmap);
+        tma_prefetch_desc(&tmap_tail);
     }
     if (warp == 1) {                                            // TMEM: all 512 columns (two 128 x 256 int32 accumulators)
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)), "r"(512) : "memory");
@@ -174,7 +135,6 @@ corr_kernel(const CorrArgs a, const __grid_constant__ CUtensorMap tmap)
     }
     tc_fence_before();
     __syncthreads();
-    if constexpr (MC) cluster_sync_all();                       // every CTA's barriers exist before a peer arrives on them
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot;
     const int chunks = a.n_avg * a.nk;
@@ -183,25 +143,19 @@ corr_kernel(const CorrArgs a, const __grid_constant__ CUtensorMap tmap)
         if (lane == 0) {
             uint32_t it = 0;
             int t, c, I, J;
-            for (int k = 0; corr_tile<MC>(a, k, rank, t, c, I, J); ++k) {
+            for (int k = 0; corr_tile(a, k, t, c, I, J); ++k) {
                 for (int q = 0; q < chunks; ++q, ++it) {
                     const uint32_t s = it % kCorrStages, ph = (it / kCorrStages) & 1u;
                     mbar_wait(&empty[s], ph ^ 1u);
                     const int fi = q / a.nk, kc = q - fi * a.nk;
                     const int f = c * a.n_avg + fi;
                     unsigned char *st = tiles + (size_t)s * kCorrStageBytes;
-                    if constexpr (MC) {
-                        // every CTA arms its own barrier with the bytes it will RECEIVE; ranks 0 and 2 load for two CTAs each
-                        mbar_expect_tx(&full_tma[s], rank == 1 ? 2 * kCorrRowsBytes : kCorrRowsBytes);
-                        if (rank == 0)
-                            tma_load_4d_mc(st + kCorrRowsBytes, &tmap, &full_tma[s], kc * kCorrChunk, t, 0, f, (uint16_t)0x3);
-                        else if (rank == 2)
-                            tma_load_4d_mc(st, &tmap, &full_tma[s], kc * kCorrChunk, t, kCorrTile, f, (uint16_t)0x6);
-                    } else {
-                        mbar_expect_tx(&full_tma[s], I == J ? kCorrRowsBytes : 2 * kCorrRowsBytes);
-                        tma_load_4d(st + kCorrRowsBytes, &tmap, &full_tma[s], kc * kCorrChunk, t, J * kCorrTile, f);
-                        if (I != J) tma_load_4d(st, &tmap, &full_tma[s], kc * kCorrChunk, t, I * kCorrTile, f);
-                    }
+                    const bool tail = kc == a.nk - 1;
+                    const CUtensorMap *map = tail ? &tmap_tail : &tmap;
+                    const uint32_t rows_bytes = tail ? tail_rows_bytes : (uint32_t)kCorrRowsBytes;
+                    mbar_expect_tx(&full_tma[s], I == J ? rows_bytes : 2 * rows_bytes);
+                    tma_load_4d(st + kCorrRowsBytes, map, &full_tma[s], kc * kCorrChunk, t, J * kCorrTile, f);
+                    if (I != J) tma_load_4d(st, map, &full_tma[s], kc * kCorrChunk, t, I * kCorrTile, f);
                 }
             }
         }
@@ -211,7 +165,7 @@ corr_kernel(const CorrArgs a, const __grid_constant__ CUtensorMap tmap)
             const uint32_t idesc = (2u << 4) | (1u << 7) | (1u << 10) | ((256u >> 3) << 17) | ((128u >> 4) << 24);
             uint32_t it = 0, n = 0;
             int t, c, I, J;
-            for (int k = 0; corr_tile<MC>(a, k, rank, t, c, I, J); ++k, ++n) {
+            for (int k = 0; corr_tile(a, k, t, c, I, J); ++k, ++n) {
                 const uint32_t b = n & 1u;
                 mbar_wait(&tmem_empty[b], ((n >> 1) & 1u) ^ 1u);
                 tc_fence_after();
@@ -222,42 +176,51 @@ corr_kernel(const CorrArgs a, const __grid_constant__ CUtensorMap tmap)
                     mbar_wait(&full_xf[s], ph);
                     tc_fence_after();
                     const uint32_t st = smem_u32(tiles + (size_t)s * kCorrStageBytes);
-                    const uint64_t adesc = umma_desc_k128(I == J ? st + xj_off : st);
-                    const uint64_t bdesc = umma_desc_k128(st + xj_off);
                     const int kc = q % a.nk;
-                    const int ksteps = kc == a.nk - 1 ? a.last_ksteps : 4;
+                    const bool tail = kc == a.nk - 1;
+                    const uint64_t adesc = umma_desc_k(I == J ? st + xj_off : st, tail ? (uint32_t)a.tail_box : 128u);
+                    const uint64_t bdesc = umma_desc_k(st + xj_off, tail ? (uint32_t)a.tail_box : 128u);
+                    const int ksteps = tail ? a.last_ksteps : 4;
                     for (int ks = 0; ks < ksteps; ++ks)         // 32 bytes of K per instruction: +2 in units of 16 bytes
                         umma_i8(d, adesc + 2u * ks, bdesc + 2u * ks, idesc, (q | ks) != 0);
-                    if (MC && rank == 1) tc_commit_mc(&empty[s], (uint16_t)0x7);      // frees the slot for both loading CTAs and itself
-                    else tc_commit(&empty[s]);
+                    tc_commit(&empty[s]);
                 }
                 tc_commit(&tmem_full[b]);
             }
         }
     } else if (warp < 2 + kCorrXfWarps) {
-        constexpr int XT = kCorrXfWarps * 32, XV = 1024 / XT;      // threads, 16-byte vectors per thread and stage
+        constexpr int XT = kCorrXfWarps * 32, XV = 1024 / XT;      // threads, 16-byte vectors per thread and full stage
         const int tx = threadIdx.x - 64;
+        const int tail_vec = (int)(tail_rows_bytes / 16u);      // 16-byte vectors of a tail block (256 / 512 / 1024)
+        auto xf = [](uint32_t w) {                              // bytes (r0, i0, r1, i1) -> (-i0, r0, -i1, r1)
+            const uint32_t sw = __byte_perm(w, 0u, 0x2301);                   // (i0, r0, i1, r1)
+            // -x = ~x + 1 on bytes 0 and 2: with bytes 1 and 3 cleared first, each +1 carries at most into the
+            // cleared byte above it and is masked away
+            const uint32_t neg = (~sw & 0x00FF00FFu) + 0x00010001u;
+            return (neg & 0x00FF00FFu) | (sw & 0xFF00FF00u);
+        };
         uint32_t it = 0;
         int t, c, I, J;
-        for (int k = 0; corr_tile<MC>(a, k, rank, t, c, I, J); ++k) {
+        for (int k = 0; corr_tile(a, k, t, c, I, J); ++k) {
             for (int q = 0; q < chunks; ++q, ++it) {
                 const uint32_t s = it % kCorrStages, ph = (it / kCorrStages) & 1u;
                 mbar_wait(&full_tma[s], ph);
+                // (re, im) -> (-im, re), same (swizzled) slot of the block that follows X_J: the B operand is 256 rows in a row,
+                // so the transformed rows of a narrow tail block start right after its 128 x tail_box bytes
+                const int nvec = (q % a.nk == a.nk - 1) ? tail_vec : 1024;
                 const uint4 *src = reinterpret_cast<const uint4 *>(tiles + (size_t)s * kCorrStageBytes + xj_off);
-                uint4 *dst = reinterpret_cast<uint4 *>(tiles + (size_t)s * kCorrStageBytes + xj_off + kCorrRowsBytes);
-                uint4 v[XV];
+                uint4 *dst = const_cast<uint4 *>(src) + nvec;
+                if (nvec == 1024) {
+                    uint4 v[XV];
 #pragma unroll
-                for (int k = 0; k < XV; ++k) v[k] = src[tx + k * XT];
+                    for (int m = 0; m < XV; ++m) v[m] = src[tx + m * XT];
 #pragma unroll
-                for (int k = 0; k < XV; ++k) {                   // (re, im) -> (-im, re); same swizzled slot
-                    auto xf = [](uint32_t w) {                 // bytes (r0, i0, r1, i1) -> (-i0, r0, -i1, r1)
-                        const uint32_t sw = __byte_perm(w, 0u, 0x2301);                   // (i0, r0, i1, r1)
-                        // -x = ~x + 1 on bytes 0 and 2: with bytes 1 and 3 cleared first, each +1 carries at most into the
-                        // cleared byte above it and is masked away
-                        const uint32_t neg = (~sw & 0x00FF00FFu) + 0x00010001u;
-                        return (neg & 0x00FF00FFu) | (sw & 0xFF00FF00u);
-                    };
-                    dst[tx + k * XT] = make_uint4(xf(v[k].x), xf(v[k].y), xf(v[k].z), xf(v[k].w));
+                    for (int m = 0; m < XV; ++m) dst[tx + m * XT] = make_uint4(xf(v[m].x), xf(v[m].y), xf(v[m].z), xf(v[m].w));
+                } else {
+                    for (int i = tx; i < nvec; i += XT) {
+                        const uint4 v = src[i];
+                        dst[i] = make_uint4(xf(v.x), xf(v.y), xf(v.z), xf(v.w));
+                    }
                 }
                 fence_proxy_async();                            // generic-proxy writes -> the tensor core's async-proxy reads
                 mbar_arrive(&full_xf[s]);
@@ -279,7 +242,7 @@ corr_kernel(const CorrArgs a, const __grid_constant__ CUtensorMap tmap)
         const size_t ntri = (size_t)a.A * (a.A + 1) / 2;
         uint32_t n = 0;
         int t, c, I, J;
-        for (int k = 0; corr_tile<MC>(a, k, rank, t, c, I, J); ++k, ++n) {
+        for (int k = 0; corr_tile(a, k, t, c, I, J); ++k, ++n) {
             const uint32_t b = n & 1u;
             mbar_wait(&tmem_full[b], (n >> 1) & 1u);
             tc_fence_after();
@@ -310,7 +273,6 @@ corr_kernel(const CorrArgs a, const __grid_constant__ CUtensorMap tmap)
     }
     tc_fence_before();
     __syncthreads();
-    if constexpr (MC) cluster_sync_all();                       // no CTA leaves while a peer may still write into it or signal it
     if (warp == 1) {
         tc_fence_after();
         asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(512) : "memory");
@@ -344,52 +306,26 @@ extern "C" int blink_correlate(const int8_t *volt, int F, int A, int Ns, int n_t
     a.norm = (float)((long long)n_t * n_avg);
     a.rnorm = (float)(1.0 / (double)((long long)n_t * n_avg));
     a.vis = reinterpret_cast<float2 *>(vis);
-    CUtensorMap tmap;
+    // the K tail of an (interval, fine channel): 2 n_t = (nk - 1) 128 + tail bytes.  A tail of at most 32 / 64 bytes is staged as
+    // 32 / 64-byte rows (tensor map and UMMA descriptor in the swizzle of that width): the paper's 20 ms interval is 400 bytes =
+    // 3 x 128 + 16, and a fourth full-width chunk would stage and transform 128 bytes per row for 16 valid ones
+    const int tail_bytes = kbytes - (a.nk - 1) * kCorrChunk;
+    a.tail_box = tail_bytes <= 32 ? 32 : tail_bytes <= 64 ? 64 : 128;
+    CUtensorMap tmap, tmap_tail;
     // volt as bytes: [F][A][T][2 n_t], innermost first {2 n_t, T, A, F}; a box = 128 bytes x 1 interval x 128 inputs x 1 channel
     const uint64_t dims[4] = {(uint64_t)kbytes, (uint64_t)a.T, (uint64_t)A, (uint64_t)F};
     const uint64_t strides[3] = {(uint64_t)kbytes, (uint64_t)Ns * 2, (uint64_t)A * Ns * 2};
     const uint32_t box[4] = {(uint32_t)kCorrChunk, 1u, (uint32_t)kCorrTile, 1u};
-    if (encode_tensor_map_4d_u8(&tmap, volt, dims, strides, box) != 0) {
+    const uint32_t box_tail[4] = {(uint32_t)a.tail_box, 1u, (uint32_t)kCorrTile, 1u};
+    if (encode_tensor_map_4d_u8(&tmap, volt, dims, strides, box, kCorrChunk) != 0 ||
+        encode_tensor_map_4d_u8(&tmap_tail, volt, dims, strides, box_tail, a.tail_box) != 0) {
         set_error_text("cuTensorMapEncodeTiled failed (correlator voltages)");
         return BLINK_ERR_CUDA;
     }
     int ctas = sm_count() > 0 ? sm_count() : 148;
-    const int path = option(BLINK_OPT_CORR_PATH);
-    if (a.n_tiles_side == 2 && path == 2) {
-        // 3-CTA clusters, one per (t, c) matrix at a time
-        BLINK_CUDA_TRY(cudaFuncSetAttribute(corr_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kCorrSmem));
-        BLINK_CUDA_TRY(cudaFuncSetAttribute(corr_kernel<true>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
-        int clusters = ctas / 3;
-        {   // persistent clusters: launch no more than can be resident at once (45 on the B200s measured, not 148 / 3 = 49)
-            int maxc = 0;
-            cudaLaunchConfig_t q = {};
-            q.gridDim = dim3(3 * clusters); q.blockDim = dim3(kCorrThreads); q.dynamicSmemBytes = kCorrSmem;
-            cudaLaunchAttribute qa[1];
-            qa[0].id = cudaLaunchAttributeClusterDimension;
-            qa[0].val.clusterDim.x = 3; qa[0].val.clusterDim.y = 1; qa[0].val.clusterDim.z = 1;
-            q.attrs = qa; q.numAttrs = 1;
-            if (cudaOccupancyMaxActiveClusters(&maxc, corr_kernel<true>, &q) == cudaSuccess && maxc > 0 && maxc < clusters)
-                clusters = maxc;
-            (void)cudaGetLastError();
-        }
-        if (clusters > a.T * a.C) clusters = a.T * a.C;
-        cudaLaunchConfig_t cfg = {};
-        cfg.gridDim = dim3(3 * clusters);
-        cfg.blockDim = dim3(kCorrThreads);
-        cfg.dynamicSmemBytes = kCorrSmem;
-        cfg.stream = static_cast<cudaStream_t>(stream);
-        cudaLaunchAttribute at[1];
-        at[0].id = cudaLaunchAttributeClusterDimension;
-        at[0].val.clusterDim.x = 3; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
-        cfg.attrs = at;
-        cfg.numAttrs = 1;
-        BLINK_CUDA_TRY(cudaLaunchKernelEx(&cfg, corr_kernel<true>, a, tmap));
-        BLINK_LAUNCH_CHECK("corr_kernel<cluster>");
-        return BLINK_OK;
-    }
-    BLINK_CUDA_TRY(cudaFuncSetAttribute(corr_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kCorrSmem));
+    BLINK_CUDA_TRY(cudaFuncSetAttribute(corr_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kCorrSmem));
     if (ctas > a.n_units) ctas = a.n_units;
-    corr_kernel<false><<<ctas, kCorrThreads, kCorrSmem, static_cast<cudaStream_t>(stream)>>>(a, tmap);
+    corr_kernel<<<ctas, kCorrThreads, kCorrSmem, static_cast<cudaStream_t>(stream)>>>(a, tmap, tmap_tail);
     BLINK_LAUNCH_CHECK("corr_kernel");
     return BLINK_OK;
 }

@@ -85,6 +85,6 @@ int encode_tensor_map_3d_f32(CUtensorMap *out, const void *base, uint64_t d0, ui
                              int swizzle_bytes /*0,32,64,128*/);
 
 int encode_tensor_map_4d_u8(CUtensorMap *out, const void *base, const uint64_t dims[4], const uint64_t strides[3],
-                            const uint32_t box[4]);
+                            const uint32_t box[4], int swizzle_bytes);   // swizzle 32 / 64 / 128 = box[0] bytes
 
 }  // namespace blink

@@ -61,13 +61,14 @@ def test_correlate_sums_beyond_2_24_and_many_tiles(bk, oracle_mod):
     assert ref_max > 2 ** 24
 
 
-@pytest.mark.parametrize("F,A,Ns,n_t,n_avg", [(8, 256, 1000, 200, 4), (4, 200, 1024, 64, 2), (48, 256, 16 * 64, 64, 1), (3, 129, 288, 72, 3)])
-def test_correlate_cluster_multicast(bk, oracle_mod, F, A, Ns, n_t, n_avg):
-    # BLINK_OPT_CORR_PATH = 2: 3-CTA clusters, one (t, c) matrix per cluster at a time, X_0 / X_1 loaded once by multicast TMA
-    # (129..256 inputs; other sizes fall back to the plain kernel); 768 matrices over <= 49 clusters wrap every ring many times
+@pytest.mark.parametrize("n_t", [72, 80, 88, 96, 104, 120, 136, 200])
+def test_correlate_k_tails(bk, oracle_mod, n_t):
+    # 2 n_t bytes per (interval, fine channel) = full 128-byte chunks + a tail of 16 .. 112 bytes: tails of at most 32 / 64
+    # bytes are staged as 32 / 64-byte rows in the swizzle of that width (own tensor map, own UMMA descriptor), wider ones
+    # as a zero-filled 128-byte chunk; 200 inputs = a full and a partial tile row, 3 intervals x 2 output channels
     from paper_2505_15204_b200 import workloads
-    volt = workloads.make_voltages(F, A, Ns, seed=17 + A, device="cuda")
-    _check(bk, oracle_mod, volt, n_t, n_avg, path=2)
+    volt = workloads.make_voltages(6, 200, 3 * n_t, seed=23 + n_t, device="cuda")
+    _check(bk, oracle_mod, volt, n_t, 3)
 
 
 def test_correlate_many_units(bk, oracle_mod):
