@@ -59,7 +59,7 @@ enum {
     BLINK_OPT_FUSED_CTAS = 1,     /* [0] 0 = auto (one persistent CTA per SM), else CTAs for the fused kernel  */
     BLINK_OPT_GRID_CHUNK_B = 2,   /* [0] 0 = auto, else baselines per gridder chunk (tests the spill path)     */
     BLINK_OPT_AVG_WSUM = 3,       /* [0] blink_image_avg weight sums: 0 = auto, 1 = sort + binary search, 2 = ballot counting */
-    BLINK_OPT_CORR_PATH = 4,      /* [0] blink_correlate: 0 = auto, 1 = one CTA per tile; 2 is reserved (round 1's 3-CTA multicast variant was never faster and is gone) */
+    BLINK_OPT_CORR_PATH = 4,      /* [0] blink_correlate: 0 = auto, 1 = one CTA per tile; 2 is reserved (the 3-CTA multicast and the cta_group::2 pair kernels were measured slower and are gone: profiles/r2_corr.md) */
     BLINK_OPT_FUSED_TEAM = 5      /* [0] fused kernel: CTAs that image one (t,c) together: 0 = auto (1 for large batches; more when the batch
                                          leaves the last round of one-CTA-per-image half empty), else the team size */
 };

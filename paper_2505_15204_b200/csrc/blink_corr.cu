@@ -291,308 +291,6 @@ corr_kernel(const CorrArgs a, const __grid_constant__ CUtensorMap tmap, const __
 }
 
 
-// =====================================================================================================================
-// CTA-pair variant (tcgen05 cta_group::2) for 129..256 inputs (two tile rows: MWA Phase I).  A cluster of two CTAs on the two
-// SMs of a TPC runs ONE M = 256 x N = 256 MMA per K step: all 256 inputs against column tile J (Re | Im), i.e. the tiles (0,J) and
-// (1,J) at once; a unit = (t, c, J), two per matrix (of unit J = 1 the tile (0,1) lies above the diagonal and is dropped).  Why: the
-// one-CTA kernel is bound by shared-memory bandwidth (each SM stages, transforms and feeds the tensor core 96-112 KB per 128-byte
-// K chunk and tile); a pair shares the B operand, so per chunk an SM handles 64 KB for TWO tiles' worth of rows:
-//   CTA r stages rows 64 r .. 64 r + 63 of BOTH row tiles: [X_other half | X_J half | transformed X_J half], 3 x 8 KB;
-//   its A operand (128 rows) is the first 16 KB, its half of the B operand (128 of the N = 256 rows) the last 16 KB -- the rows of
-//   tile J are A rows and B rows at the same time, so nothing is loaded twice within a unit;
-//   TMEM lanes 0..63 = rows of tile 1 - J, lanes 64..127 = rows of tile J (diagonal tile); columns (N index) 128 r' + [0, 64) = Re and
-//   128 r' + [64, 128) = Im of the J tile's columns 64 r' .. 64 r' + 63 (r' = the CTA that staged those B rows).
-// Barriers: the loads of X_J complete on a LOCAL barrier (the CTA's own transform warps wait for it), the loads of X_other and the
-// transform warps' arrivals go to the LEADER's barriers (rank 0 issues every MMA), tcgen05.commit multicasts the stage / accumulator
-// releases to both CTAs, and both CTAs' epilogue warps release an accumulator on the leader's barrier.
-#ifndef BLINK_CORR_DIAG
-#define BLINK_CORR_DIAG 0
-#endif
-#ifndef BLINK_CORR_DIAGX
-#define BLINK_CORR_DIAGX 0
-#endif
-#ifndef BLINK_C2_STAGES
-#define BLINK_C2_STAGES 6
-#endif
-constexpr int kC2Stages = BLINK_C2_STAGES;
-constexpr int kC2Half = 64;                                     // rows per staged block
-constexpr int kC2StageBytes = 3 * kC2Half * kCorrChunk;         // 24 KB
-constexpr int kC2XfWarps = 8;                                  // two groups of four: even / odd chunks (the transform is a latency chain per chunk)
-constexpr int kC2XfGroup = 4;
-constexpr int kC2EpWarps = 8;                                  // two per TMEM lane quadrant: the epilogue is what a unit waits for
-constexpr int kC2Threads = (2 + kC2XfWarps + kC2EpWarps) * 32;
-constexpr size_t kC2Smem = (size_t)kC2Stages * kC2StageBytes + 1024 /* alignment */ + 512 /* barriers */ + (BLINK_CORR_DIAG == 3 ? 0 : kC2EpWarps * kCorrOutBytes);
-
-__device__ __forceinline__ uint32_t cluster_rank()
-{
-    uint32_t r;
-    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
-    return r;
-}
-__device__ __forceinline__ void cluster_sync_all()
-{
-    asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
-    asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
-}
-// shared::cluster address of the same variable in the leader CTA (rank 0 of the pair)
-__device__ __forceinline__ uint32_t leader_addr(const void *p)
-{
-    uint32_t r;
-    asm volatile("mapa.shared::cluster.u32 %0, %1, 0;" : "=r"(r) : "r"(smem_u32(p)));
-    return r;
-}
-__device__ __forceinline__ void mbar_arrive_leader(uint64_t *bar)
-{
-    // default semantics (release at CTA scope), as every cluster pipeline does: a cluster-scope release is a full memory barrier
-    // that waits for the thread's outstanding GLOBAL stores (measured: "membar" became the top stall reason, 18.4 instead of 6.x ms)
-    asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" ::"r"(leader_addr(bar)) : "memory");
-}
-__device__ __forceinline__ void mbar_wait_cluster(uint64_t *bar, uint32_t parity)
-{
-    asm volatile(
-        "{\n\t"
-        ".reg .pred p;\n\t"
-        "WAITC_%=:\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
-        "@p bra DONEC_%=;\n\t"
-        "bra WAITC_%=;\n\t"
-        "DONEC_%=:\n\t"
-        "}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
-}
-// tensor load whose completion is counted on the LEADER's barrier (either CTA of the pair may issue it)
-__device__ __forceinline__ void tma_load_4d_pair(void *smem_dst, const CUtensorMap *map, uint64_t *bar, int c0, int c1, int c2, int c3)
-{
-    asm volatile(
-        "cp.async.bulk.tensor.4d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];"
-        ::"r"(smem_u32(smem_dst)), "l"(map), "r"(leader_addr(bar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3)
-        : "memory");
-}
-__device__ __forceinline__ void tc_commit_pair(uint64_t *bar)      // arrives on `bar` of BOTH CTAs when the MMAs issued so far are done
-{
-    asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
-                 ::"r"(smem_u32(bar)), "h"((uint16_t)3) : "memory");
-}
-__device__ __forceinline__ void umma_i8_pair(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate)
-{
-    asm volatile(
-        "{\n\t"
-        ".reg .pred p;\n\t"
-        "setp.ne.b32 p, %4, 0;\n\t"
-        "tcgen05.mma.cta_group::2.kind::i8 [%0], %1, %2, %3, p;\n\t"
-        "}\n" ::"r"(tmem_d), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate) : "memory");
-}
-
-__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kC2Threads, 1)
-corr_pair_kernel(const CorrArgs a, const __grid_constant__ CUtensorMap tmap, const __grid_constant__ CUtensorMap tmap_tail)
-{
-    extern __shared__ __align__(16) unsigned char corr_smem[];
-    const uint32_t base = smem_u32(corr_smem);
-    unsigned char *tiles = corr_smem + (((base + 1023u) & ~1023u) - base);         // 1024-byte aligned stage ring
-    uint64_t *bars = reinterpret_cast<uint64_t *>(tiles + (size_t)kC2Stages * kC2StageBytes);
-    uint64_t *full_x = bars, *full_loc = bars + kC2Stages, *full_xf = bars + 2 * kC2Stages, *empty = bars + 3 * kC2Stages;
-    uint64_t *tmem_full = bars + 4 * kC2Stages, *tmem_empty = tmem_full + 2;
-    uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(tmem_empty + 2);
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const uint32_t r = cluster_rank();
-    const int cl = (int)(blockIdx.x >> 1), ncl = (int)(gridDim.x >> 1);
-    const int n_units = 2 * a.T * a.C;                          // (t, c, J), J fastest
-    const uint32_t tail_blk = (uint32_t)kC2Half * (uint32_t)a.tail_box;
-
-    if (threadIdx.x == 0) {
-        for (int s = 0; s < kC2Stages; ++s) {
-            mbar_init(&full_x[s], 1);                           // leader: its own arrive.expect_tx; bytes from both CTAs' loads
-            mbar_init(&full_loc[s], 1);
-            mbar_init(&full_xf[s], 2 * kC2XfGroup);           // leader: one arrival per transform warp of either CTA
-            mbar_init(&empty[s], 1);
-        }
-        for (int b = 0; b < 2; ++b) {
-            mbar_init(&tmem_full[b], 1);
-            mbar_init(&tmem_empty[b], 2 * kC2EpWarps);                  // leader: one arrival per epilogue warp of either CTA
-        }
-        fence_mbar_init();
-        tma_prefetch_desc(&tmap);
-        tma_prefetch_desc(&tmap_tail);
-    }
-    if (warp == 1) {                                            // TMEM: all 512 columns in both CTAs (two 128-lane x 256-column accumulators each)
-        asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)), "r"(512) : "memory");
-        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
-    }
-    tc_fence_before();
-    __syncthreads();
-    cluster_sync_all();                                         // both CTAs' barriers and TMEM exist before anything crosses over
-    tc_fence_after();
-    const uint32_t tmem_base = *tmem_slot;
-    const int chunks = a.n_avg * a.nk;
-
-    if (warp == 0) {
-        if (lane == 0) {
-            // ring position kept as (stage, phase) counters and the chunk loop nested (fine channel, chunk): no divisions in the
-            // single-thread loops -- the MMA issuer's ~300 dependent scalar instructions per chunk were the bound of the first version
-            uint32_t s = 0, ph = 0;
-            for (int u = cl; u < n_units; u += ncl) {
-                const int item = u >> 1, J = u & 1, c = item / a.T, t = item - c * a.T;
-                const int rowJ = J * kCorrTile + kC2Half * (int)r, rowO = (1 - J) * kCorrTile + kC2Half * (int)r;
-                for (int fi = 0; fi < a.n_avg; ++fi) {
-                    const int f = c * a.n_avg + fi;
-                    for (int kc = 0; kc < a.nk; ++kc) {
-                        mbar_wait_cluster(&empty[s], ph ^ 1u);
-                        unsigned char *st = tiles + (size_t)s * kC2StageBytes;
-                        const bool tail = kc == a.nk - 1;
-                        const CUtensorMap *map = tail ? &tmap_tail : &tmap;
-                        const uint32_t blk = tail ? tail_blk : (uint32_t)(kC2Half * kCorrChunk);
-                        mbar_expect_tx(&full_loc[s], blk);
-                        tma_load_4d(st + blk, map, &full_loc[s], kc * kCorrChunk, t, rowJ, f);
-                        if (r == 0) mbar_expect_tx(&full_x[s], 2 * blk);
-                        tma_load_4d_pair(st, map, &full_x[s], kc * kCorrChunk, t, rowO, f);
-                        if (++s == kC2Stages) { s = 0; ph ^= 1u; }
-                    }
-                }
-            }
-        }
-    } else if (warp == 1) {
-        if (lane == 0 && r == 0) {
-            // instruction descriptor: D = S32, A = B = signed 8 bit, both K-major, N = 256, M = 256 (128 rows per CTA)
-            const uint32_t idesc = (2u << 4) | (1u << 7) | (1u << 10) | ((256u >> 3) << 17) | ((256u >> 4) << 24);
-            const uint32_t tiles_s = smem_u32(tiles);
-            const uint64_t d128 = umma_desc_k(0u, 128u), dtail = umma_desc_k(0u, (uint32_t)a.tail_box);   // descriptors less the address
-            const uint32_t boff_tail = ((uint32_t)kC2Half * (uint32_t)a.tail_box) >> 4, boff = (uint32_t)(kC2Half * kCorrChunk) >> 4;
-            uint32_t s = 0, ph = 0, n = 0;
-            for (int u = cl; u < n_units; u += ncl, ++n) {
-                const uint32_t b = n & 1u;
-                mbar_wait_cluster(&tmem_empty[b], ((n >> 1) & 1u) ^ 1u);
-                tc_fence_after();
-                const uint32_t d = tmem_base + b * 256u;
-                uint32_t acc = 0;
-                for (int fi = 0; fi < a.n_avg; ++fi) {
-                    for (int kc = 0; kc < a.nk; ++kc) {
-                        mbar_wait_cluster(&full_x[s], ph);
-                        mbar_wait_cluster(&full_xf[s], ph);
-                        tc_fence_after();
-                        const uint32_t st16 = (tiles_s + s * (uint32_t)kC2StageBytes) >> 4;   // stage address in 16-byte units (< 2^14)
-                        if (kc != a.nk - 1) {
-                            const uint64_t adesc = d128 + st16, bdesc = adesc + boff;
-#pragma unroll
-                            for (int ks = 0; ks < 4; ++ks) { if (!(BLINK_CORR_DIAGX & 2)) umma_i8_pair(d, adesc + 2u * ks, bdesc + 2u * ks, idesc, acc); acc = 1u; }
-                        } else {
-                            const uint64_t adesc = dtail + st16, bdesc = adesc + boff_tail;
-                            for (int ks = 0; ks < a.last_ksteps; ++ks) { if (!(BLINK_CORR_DIAGX & 2)) umma_i8_pair(d, adesc + 2u * ks, bdesc + 2u * ks, idesc, acc); acc = 1u; }
-                        }
-                        tc_commit_pair(&empty[s]);
-                        if (++s == kC2Stages) { s = 0; ph ^= 1u; }
-                    }
-                }
-                tc_commit_pair(&tmem_full[b]);
-            }
-        }
-    } else if (warp < 2 + kC2XfWarps) {
-        constexpr int XT = kC2XfGroup * 32;                     // threads that share one chunk
-        const int grp = (warp - 2) / kC2XfGroup;                // group 0: chunks 0, 2, 4, ... of this CTA's sequence; group 1: the odd ones
-        const int tx = (threadIdx.x - 64) % XT;
-        auto xf = [](uint32_t w) {                              // bytes (r0, i0, r1, i1) -> (-i0, r0, -i1, r1), see corr_kernel
-            const uint32_t sw = __byte_perm(w, 0u, 0x2301);
-            const uint32_t neg = (~sw & 0x00FF00FFu) + 0x00010001u;
-            return (neg & 0x00FF00FFu) | (sw & 0xFF00FF00u);
-        };
-        static_assert(kC2Stages % 2 == 0, "a group's stages keep their parity");
-        uint32_t s = (uint32_t)grp, ph = 0;
-        int kc = grp % a.nk;
-        const long long total = (long long)((n_units - cl + ncl - 1) / ncl) * chunks;   // chunks this CTA sees
-        for (long long q = grp; q < total; q += 2) {
-            {
-                mbar_wait(&full_loc[s], ph);
-                const bool tail = kc == a.nk - 1;
-                kc += 2;
-                while (kc >= a.nk) kc -= a.nk;
-                const int nvec = (int)((tail ? tail_blk : (uint32_t)(kC2Half * kCorrChunk)) / 16u);
-                const uint4 *src = reinterpret_cast<const uint4 *>(tiles + (size_t)s * kC2StageBytes) + nvec;
-                uint4 *dst = const_cast<uint4 *>(src) + nvec;
-#ifndef BLINK_CORR_DIAGX
-#define BLINK_CORR_DIAGX 0
-#endif
-                if (BLINK_CORR_DIAGX & 1) {
-                } else if (nvec == 4 * XT) {
-                    uint4 v[4];
-#pragma unroll
-                    for (int m = 0; m < 4; ++m) v[m] = src[tx + m * XT];
-#pragma unroll
-                    for (int m = 0; m < 4; ++m) dst[tx + m * XT] = make_uint4(xf(v[m].x), xf(v[m].y), xf(v[m].z), xf(v[m].w));
-                } else {
-                    for (int i = tx; i < nvec; i += XT) {
-                        const uint4 v = src[i];
-                        dst[i] = make_uint4(xf(v.x), xf(v.y), xf(v.z), xf(v.w));
-                    }
-                }
-                fence_proxy_async();                            // generic-proxy writes -> the tensor core's async-proxy reads
-                __syncwarp();
-                if (lane == 0) mbar_arrive_leader(&full_xf[s]);
-                s += 2;
-                if (s >= kC2Stages) { s -= kC2Stages; ph ^= 1u; }
-            }
-        }
-    } else {
-        // sum / norm, correctly rounded (see corr_kernel), on (re, im) pairs with the packed fp32 instructions
-        const float2 nnrm2 = make_float2(-a.norm, -a.norm), rn2 = make_float2(a.rnorm, a.rnorm);
-        auto div_norm2 = [nnrm2, rn2](uint32_t vr, uint32_t vi) {
-            const float2 x = make_float2((float)(int)vr, (float)(int)vi);
-            float2 q = pk_mul(x, rn2);
-            q = pk_fma(pk_fma(nnrm2, q, x), rn2, q);
-            return pk_fma(pk_fma(nnrm2, q, x), rn2, q);
-        };
-        const int ew = warp - 2 - kC2XfWarps;                   // 0..7; warps 6..13 -> lane quadrants 2 3 0 1 2 3 0 1
-        const int q4 = warp & 3;                                // TMEM lane quadrant this warp may read
-        const int h = ew >> 2;                                  // which of the quadrant's two warps: column blocks h, h + 2
-        float2 *stage = reinterpret_cast<float2 *>(reinterpret_cast<unsigned char *>(bars) + 512 + (size_t)ew * kCorrOutBytes);
-        const size_t ntri = (size_t)a.A * (a.A + 1) / 2;
-        uint32_t n = 0;
-        for (int u = cl; u < n_units; u += ncl, ++n) {
-            const int item = u >> 1, J = u & 1, c = item / a.T, t = item - c * a.T;
-            const uint32_t b = n & 1u;
-            mbar_wait_cluster(&tmem_full[b], (n >> 1) & 1u);
-            tc_fence_after();
-            float2 *mat = a.vis + ((size_t)t * a.C + c) * ntri;
-            const int I = q4 < 2 ? 1 - J : J;                   // lanes 0..63: the other row tile, lanes 64..127: the diagonal tile
-            const int row0 = kC2Half * (int)r + 32 * (q4 & 1);  // first row of this warp inside its tile
-            if (I >= J) {
-                const int nblk = I == J ? (row0 >> 5) + 1 : 4;  // 32-column blocks at or below the diagonal for some row of this warp
-#ifndef BLINK_CORR_DIAG
-#define BLINK_CORR_DIAG 0
-#endif
-                for (int cj = h; cj < nblk && BLINK_CORR_DIAG != 3; cj += 2) {
-                    uint32_t re[32], im[32];
-                    const uint32_t taddr = tmem_base + ((uint32_t)(q4 * 32) << 16) + b * 256u + (uint32_t)(128 * (cj >> 1) + 32 * (cj & 1));
-                    tmem_ld32(taddr, re);
-                    tmem_ld32(taddr + 64u, im);
-                    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-                    // a lane holds 32 columns of ONE row; a warp writes 32 consecutive columns of a row: transpose through shared memory
-#pragma unroll
-                    for (int k = 0; k < 32; ++k) stage[lane * 33 + k] = div_norm2(re[k], im[k]);
-                    __syncwarp();
-                    const int gj = J * kCorrTile + cj * 32 + lane;
-                    const int gi0 = I * kCorrTile + row0;
-                    float2 *dst = mat + (size_t)gi0 * (gi0 + 1) / 2 + gj;   // row gi starts gi (gi + 1) / 2 entries in: +gi + 1 per row
-#pragma unroll 8
-                    for (int rr = 0; rr < 32; ++rr) {
-                        const int gi = gi0 + rr;
-                        if (gi < a.A && gj <= gi && BLINK_CORR_DIAG != 1) *dst = stage[rr * 33 + lane];
-                        dst += gi + 1;
-                    }
-                    __syncwarp();
-                }
-            }
-            tc_fence_before();
-            __syncwarp();
-            if (lane == 0) mbar_arrive_leader(&tmem_empty[b]);
-        }
-    }
-    tc_fence_before();
-    __syncthreads();
-    cluster_sync_all();                                         // no CTA leaves (or frees TMEM) while its peer may still signal it or run MMAs on it
-    if (warp == 1) {
-        tc_fence_after();
-        asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(512) : "memory");
-    }
-}
-
 }  // namespace blink
 
 using namespace blink;
@@ -626,10 +324,8 @@ extern "C" int blink_correlate(const int8_t *volt, int F, int A, int Ns, int n_t
     const int tail_bytes = kbytes - (a.nk - 1) * kCorrChunk;
     a.tail_box = tail_bytes <= 32 ? 32 : tail_bytes <= 64 ? 64 : 128;
     CUtensorMap tmap, tmap_tail;
-    // volt as bytes: [F][A][T][2 n_t], innermost first {2 n_t, T, A, F}; a box = 128 bytes x 1 interval x 128 (pairs: 64) inputs x 1 channel
-    const int path = option(BLINK_OPT_CORR_PATH);
-    const bool pair = a.n_tiles_side == 2 && path == 2;        // 129..256 inputs: CTA pairs (cta_group::2), measured slower: opt-in
-    const uint32_t box_rows = pair ? (uint32_t)kC2Half : (uint32_t)kCorrTile;
+    // volt as bytes: [F][A][T][2 n_t], innermost first {2 n_t, T, A, F}; a box = 128 bytes x 1 interval x 128 inputs x 1 channel
+    const uint32_t box_rows = (uint32_t)kCorrTile;
     const uint64_t dims[4] = {(uint64_t)kbytes, (uint64_t)a.T, (uint64_t)A, (uint64_t)F};
     const uint64_t strides[3] = {(uint64_t)kbytes, (uint64_t)Ns * 2, (uint64_t)A * Ns * 2};
     const uint32_t box[4] = {(uint32_t)kCorrChunk, 1u, box_rows, 1u};
@@ -640,21 +336,6 @@ extern "C" int blink_correlate(const int8_t *volt, int F, int A, int Ns, int n_t
         return BLINK_ERR_CUDA;
     }
     int ctas = sm_count() > 0 ? sm_count() : 148;
-    if (pair) {
-        BLINK_CUDA_TRY(cudaFuncSetAttribute(corr_pair_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kC2Smem));
-        int clusters = ctas / 2;
-        {   // persistent clusters: launch no more than can be resident at once
-            int maxc = 0;
-            cudaLaunchConfig_t q = {};
-            q.gridDim = dim3(2 * clusters); q.blockDim = dim3(kC2Threads); q.dynamicSmemBytes = kC2Smem;
-            if (cudaOccupancyMaxActiveClusters(&maxc, corr_pair_kernel, &q) == cudaSuccess && maxc > 0 && maxc < clusters) clusters = maxc;
-            (void)cudaGetLastError();
-        }
-        if (clusters > 2 * a.T * a.C) clusters = 2 * a.T * a.C;
-        corr_pair_kernel<<<2 * clusters, kC2Threads, kC2Smem, static_cast<cudaStream_t>(stream)>>>(a, tmap, tmap_tail);
-        BLINK_LAUNCH_CHECK("corr_pair_kernel");
-        return BLINK_OK;
-    }
     BLINK_CUDA_TRY(cudaFuncSetAttribute(corr_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kCorrSmem));
     if (ctas > a.n_units) ctas = a.n_units;
     corr_kernel<<<ctas, kCorrThreads, kCorrSmem, static_cast<cudaStream_t>(stream)>>>(a, tmap, tmap_tail);
