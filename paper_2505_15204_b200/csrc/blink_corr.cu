@@ -24,15 +24,28 @@
 
 namespace blink {
 
-constexpr int kCorrXfWarps = 8;                                  // warps that build the transformed rows
-constexpr int kCorrThreads = (2 + kCorrXfWarps + 4) * 32;
-constexpr int kCorrStages = 4;
+#ifndef BLINK_CORR_XF
+#define BLINK_CORR_XF 4
+#endif
+#ifndef BLINK_CORR_EP
+#define BLINK_CORR_EP 4
+#endif
+#ifndef BLINK_CORR_STAGES
+#define BLINK_CORR_STAGES 4
+#endif
+// measured on the one-second shape (profiles/r2_corr.md): 4 transform warps are as fast as 8; a ring of 3 stages (which is what
+// 8 epilogue warps' staging buffers leave room for) costs 12 %, and 8 epilogue warps on top of it give nothing back
+constexpr int kCorrXfWarps = BLINK_CORR_XF;                     // warps that build the transformed rows (a multiple of 4)
+constexpr int kCorrEpWarps = BLINK_CORR_EP;                     // epilogue warps: 4, or 8 = two per TMEM lane quadrant (column blocks h, h + 2)
+constexpr int kCorrThreads = (2 + kCorrXfWarps + kCorrEpWarps) * 32;
+constexpr int kCorrStages = BLINK_CORR_STAGES;
+static_assert(kCorrXfWarps % 4 == 0 && (kCorrEpWarps == 4 || kCorrEpWarps == 8), "epilogue warp w reads TMEM lane quadrant w % 4");
 constexpr int kCorrTile = 128;                                  // rows / columns of an output tile
 constexpr int kCorrChunk = 128;                                 // K bytes per stage row (64 complex samples) = swizzle span
 constexpr int kCorrRowsBytes = kCorrTile * kCorrChunk;          // 16 KB: 128 rows x 128 bytes
 constexpr int kCorrStageBytes = 3 * kCorrRowsBytes;             // X_I | X_J | b''_J
 constexpr int kCorrOutBytes = 32 * 33 * 8;                     // per epilogue warp: 32 x 32 complex64, rows padded to 33
-constexpr size_t kCorrSmem = (size_t)kCorrStages * kCorrStageBytes + 1024 /* alignment */ + 256 /* barriers */ + 4 * kCorrOutBytes;
+constexpr size_t kCorrSmem = (size_t)kCorrStages * kCorrStageBytes + 1024 /* alignment */ + 256 /* barriers */ + kCorrEpWarps * kCorrOutBytes;
 
 struct CorrArgs {
     int A, T, C, n_t, n_avg;
@@ -124,7 +137,7 @@ corr_kernel(const CorrArgs a, const __grid_constant__ CUtensorMap tmap, const __
         }
         for (int b = 0; b < 2; ++b) {
             mbar_init(&tmem_full[b], 1);
-            mbar_init(&tmem_empty[b], 128);
+            mbar_init(&tmem_empty[b], kCorrEpWarps * 32);
         }
         fence_mbar_init();
         tma_prefetch_desc(&tmap);
@@ -142,13 +155,12 @@ corr_kernel(const CorrArgs a, const __grid_constant__ CUtensorMap tmap, const __
 
     if (warp == 0) {
         if (lane == 0) {
-            uint32_t it = 0;
+            uint32_t s = 0, ph = 0;                             // ring position as (stage, phase) counters
             int t, c, I, J;
             for (int k = 0; corr_tile(a, k, t, c, I, J); ++k) {
                 for (int fi = 0; fi < a.n_avg; ++fi) {          // nested (fine channel, chunk): no divisions in the single-thread loops
                     const int f = c * a.n_avg + fi;
-                    for (int kc = 0; kc < a.nk; ++kc, ++it) {
-                        const uint32_t s = it % kCorrStages, ph = (it / kCorrStages) & 1u;
+                    for (int kc = 0; kc < a.nk; ++kc) {
                         mbar_wait(&empty[s], ph ^ 1u);
                         unsigned char *st = tiles + (size_t)s * kCorrStageBytes;
                         const bool tail = kc == a.nk - 1;
@@ -157,6 +169,7 @@ corr_kernel(const CorrArgs a, const __grid_constant__ CUtensorMap tmap, const __
                         mbar_expect_tx(&full_tma[s], I == J ? rows_bytes : 2 * rows_bytes);
                         tma_load_4d(st + kCorrRowsBytes, map, &full_tma[s], kc * kCorrChunk, t, J * kCorrTile, f);
                         if (I != J) tma_load_4d(st, map, &full_tma[s], kc * kCorrChunk, t, I * kCorrTile, f);
+                        if (++s == kCorrStages) { s = 0; ph ^= 1u; }
                     }
                 }
             }
@@ -165,7 +178,7 @@ corr_kernel(const CorrArgs a, const __grid_constant__ CUtensorMap tmap, const __
         if (lane == 0) {
             // instruction descriptor: D = S32 (2 << 4), A = B = signed 8 bit (1 << 7, 1 << 10), both K-major, N = 256, M = 128
             const uint32_t idesc = (2u << 4) | (1u << 7) | (1u << 10) | ((256u >> 3) << 17) | ((128u >> 4) << 24);
-            uint32_t it = 0, n = 0;
+            uint32_t s = 0, ph = 0, n = 0;
             int t, c, I, J;
             for (int k = 0; corr_tile(a, k, t, c, I, J); ++k, ++n) {
                 const uint32_t b = n & 1u;
@@ -174,8 +187,7 @@ corr_kernel(const CorrArgs a, const __grid_constant__ CUtensorMap tmap, const __
                 const uint32_t d = tmem_base + b * 256u;
                 uint32_t acc = 0;
                 for (int fi = 0; fi < a.n_avg; ++fi) {
-                    for (int kc = 0; kc < a.nk; ++kc, ++it) {
-                        const uint32_t s = it % kCorrStages, ph = (it / kCorrStages) & 1u;
+                    for (int kc = 0; kc < a.nk; ++kc) {
                         mbar_wait(&full_tma[s], ph);
                         mbar_wait(&full_xf[s], ph);
                         tc_fence_after();
@@ -189,6 +201,7 @@ corr_kernel(const CorrArgs a, const __grid_constant__ CUtensorMap tmap, const __
                             acc = 1u;
                         }
                         tc_commit(&empty[s]);
+                        if (++s == kCorrStages) { s = 0; ph ^= 1u; }
                     }
                 }
                 tc_commit(&tmem_full[b]);
@@ -205,11 +218,10 @@ corr_kernel(const CorrArgs a, const __grid_constant__ CUtensorMap tmap, const __
             const uint32_t neg = (~sw & 0x00FF00FFu) + 0x00010001u;
             return (neg & 0x00FF00FFu) | (sw & 0xFF00FF00u);
         };
-        uint32_t it = 0;
+        uint32_t s = 0, ph = 0;
         int t, c, I, J;
         for (int k = 0; corr_tile(a, k, t, c, I, J); ++k) {
-            for (int q = 0, kc = 0; q < chunks; ++q, ++it) {
-                const uint32_t s = it % kCorrStages, ph = (it / kCorrStages) & 1u;
+            for (int q = 0, kc = 0; q < chunks; ++q) {
                 mbar_wait(&full_tma[s], ph);
                 // (re, im) -> (-im, re), same (swizzled) slot of the block that follows X_J: the B operand is 256 rows in a row,
                 // so the transformed rows of a narrow tail block start right after its 128 x tail_box bytes
@@ -231,6 +243,7 @@ corr_kernel(const CorrArgs a, const __grid_constant__ CUtensorMap tmap, const __
                 }
                 fence_proxy_async();                            // generic-proxy writes -> the tensor core's async-proxy reads
                 mbar_arrive(&full_xf[s]);
+                if (++s == kCorrStages) { s = 0; ph ^= 1u; }
             }
         }
     } else {
@@ -246,7 +259,9 @@ corr_kernel(const CorrArgs a, const __grid_constant__ CUtensorMap tmap, const __
             return pk_fma(pk_fma(nnrm2, q, x), rn2, q);
         };
         const int q4 = warp & 3;                                // TMEM lane quadrant this warp may read
-        float2 *stage = reinterpret_cast<float2 *>(reinterpret_cast<unsigned char *>(tmem_slot + 4) + (size_t)(warp - 2 - kCorrXfWarps) * kCorrOutBytes);
+        const int ew = warp - 2 - kCorrXfWarps;                 // epilogue warp; with 8 of them, warps ew and ew + 4 share a quadrant
+        const int h = ew >> 2, hstep = kCorrEpWarps / 4;        // and take the 32-column blocks h, h + 2
+        float2 *stage = reinterpret_cast<float2 *>(reinterpret_cast<unsigned char *>(tmem_slot + 4) + (size_t)ew * kCorrOutBytes);
         const size_t ntri = (size_t)a.A * (a.A + 1) / 2;
         uint32_t n = 0;
         int t, c, I, J;
@@ -255,8 +270,8 @@ corr_kernel(const CorrArgs a, const __grid_constant__ CUtensorMap tmap, const __
             mbar_wait(&tmem_full[b], (n >> 1) & 1u);
             tc_fence_after();
             float2 *mat = a.vis + ((size_t)t * a.C + c) * ntri;
-            for (int cj = 0; cj < 4; ++cj) {
-                if (I == J && cj > q4) break;                   // above the diagonal for every row of this warp
+            const int nblk = I == J ? q4 + 1 : 4;               // 32-column blocks at or below the diagonal for some row of this warp
+            for (int cj = h; cj < nblk; cj += hstep) {
                 uint32_t re[32], im[32];
                 const uint32_t taddr = tmem_base + ((uint32_t)(q4 * 32) << 16) + b * 256u + (uint32_t)cj * 32u;
                 tmem_ld32(taddr, re);
