@@ -239,20 +239,55 @@ avg_scatter_runs_kernel(const AvgArgs a, const __grid_constant__ ScaleBlock sc, 
             atomicAdd(&g[mirror_of(cur, n)], make_float2(acc.x, -acc.y));
         }
     };
-#pragma unroll 4
-    for (int c = c0; c < c1; ++c) {
-        const int cell = cell_of(u, v, sc.s[c - a.c_base], n, h);
-        if (cell != cur) {
-            flush();
-            cur = cell;
-            acc = make_float2(0.f, 0.f);
+    // ncu: this kernel is bound by instruction issue (83 % issue-active, 75 thread instructions per sample at first, most of
+    // them 64-bit address arithmetic), not by its loads or atomics.  So: running pointers with 32-bit strides, and the cell is
+    // re-derived only when the rounded coordinates change -- the integer part of x + 1.5 * 2^23 sits in the mantissa of the sum
+    // (rint_rne), cell_of() is a function of these two sums alone, so equal bits = same cell, same range decision.
+    constexpr int kAvgAhead = 8;
+    const unsigned vs = (unsigned)a.P * (unsigned)a.B;          // elements between consecutive channels of one (t, p, b)
+    const float2 *vp = a.vis + ((size_t)(t * a.C + c0) * a.P + p) * a.B + b;
+    const float *wp = wq ? wq + ((size_t)t * a.C + c0) * a.B + b : winv + (size_t)t * a.C + c0;
+    const unsigned ws = wq ? (unsigned)a.B : 1u;
+    const float *sp = sc.s + (c0 - a.c_base);
+    int kx = 0x7fc00001, ky = 0x7fc00001;                       // bit patterns no valid sum has
+    auto step = [&](float s, float2 x, float w) {
+        const int bx = __float_as_int(__fadd_rn(__fmul_rn(u, s), 12582912.0f));
+        const int by = __float_as_int(__fadd_rn(__fmul_rn(v, s), 12582912.0f));
+        if (bx != kx || by != ky) {
+            kx = bx;
+            ky = by;
+            const int cell = cell_of(u, v, s, n, h);
+            if (cell != cur) {
+                flush();
+                cur = cell;
+                acc = make_float2(0.f, 0.f);
+            }
         }
         if (cur >= 0) {
-            const float w = wq ? __ldcs(wq + ((size_t)t * a.C + c) * a.B + b) : __ldg(winv + (size_t)t * a.C + c);
-            const float2 x = __ldcs(a.vis + ((size_t)(t * a.C + c) * a.P + p) * a.B + b);
             acc.x = fmaf(x.x, w, acc.x);
             acc.y = fmaf(x.y, w, acc.y);
         }
+    };
+    int c = c0;
+    for (; c + kAvgAhead <= c1; c += kAvgAhead) {
+        float2 x[kAvgAhead];
+        float w[kAvgAhead];
+#pragma unroll
+        for (int j = 0; j < kAvgAhead; ++j) {
+            x[j] = __ldcs(vp + (size_t)((unsigned)j * vs));
+            w[j] = wq ? __ldcs(wp + (size_t)((unsigned)j * ws)) : __ldg(wp + j);
+        }
+#pragma unroll
+        for (int j = 0; j < kAvgAhead; ++j) step(sp[j], x[j], w[j]);
+        vp += (size_t)(kAvgAhead * vs);
+        wp += (size_t)(kAvgAhead * ws);
+        sp += kAvgAhead;
+    }
+    for (; c < c1; ++c) {
+        step(*sp, __ldcs(vp), wq ? __ldcs(wp) : __ldg(wp));
+        vp += vs;
+        wp += ws;
+        ++sp;
     }
     flush();
 }
