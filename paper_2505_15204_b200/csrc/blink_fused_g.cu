@@ -117,6 +117,21 @@ __device__ __forceinline__ void fg_transform2(float2 *arr, const float2 *tw, int
     fg_stage<16, 75, false, true>(arr, tw + 16, tid, gsync, no_load, emit);
 }
 
+// the same with the last stage's outputs left in the arrays (natural order); ends with a group barrier
+template <class Sync, class Load>
+__device__ __forceinline__ void fg_transform2_inplace(float2 *arr, const float2 *tw, int tid, Sync gsync, Load load)
+{
+    auto no_load = [](int, int) { return make_float2(0.f, 0.f); };
+    auto no_emit = [](int, int, float2) {};
+    fg_stage<15, 1, true, false>(arr, tw, tid, gsync, load, no_emit);
+    fg_stage<5, 15, false, false>(arr, tw + 1, tid, gsync, no_load, no_emit);
+    fg_stage<16, 75, false, false>(arr, tw + 16, tid, gsync, no_load, no_emit);
+}
+
+#ifndef BLINK_FG_PAIRED_STORE
+#define BLINK_FG_PAIRED_STORE 1
+#endif
+
 __global__ void __launch_bounds__(FG_THREADS, 1)
 fused_g_kernel(const FusedArgs a, const __grid_constant__ ScaleBlock sc, const float2 *__restrict__ tw_full)
 {
@@ -274,10 +289,29 @@ fused_g_kernel(const FusedArgs a, const __grid_constant__ ScaleBlock sc, const f
                     }
                     return v;
                 };
+#if BLINK_FG_PAIRED_STORE
+                // The last stage leaves a thread with 16 outputs of ONE column; stored straight from the registers they are
+                // 8-byte pieces 4800 bytes apart (32 sectors per warp instruction, a quarter of each written).  Through the
+                // group's arrays instead: (HT[ky][u0], HT[ky][u0 + 1]) leaves as one 16-byte store, and the slots a thread
+                // reads are the slots it zeroes for the next unit (ncu: these stores were the kernel's top lg / mio throttle).
+                static_assert(FG_NT == 2, "paired stores want a column pair per group");
+                fg_transform2_inplace(arr, stw, tid, gsync, load);      // ends with a group barrier: outputs are in the arrays
+                {
+                    float4 *dst = reinterpret_cast<float4 *>(HT + u0);  // u0 even, H even: 16-byte aligned
+                    for (int ky = tid; ky < N; ky += FG_TG) {
+                        const float2 v0 = arr[ky], v1 = arr[FG_LD + ky];
+                        arr[ky] = make_float2(0.f, 0.f);
+                        arr[FG_LD + ky] = make_float2(0.f, 0.f);
+                        dst[(size_t)ky * (H / 2)] = make_float4(v0.x, v0.y, v1.x, v1.y);
+                    }
+                    if (uniform) for (int i = tid; i < FG_NT * (N / 2); i += FG_TG) cnt[i] = 0u;
+                }
+#else
                 auto emit = [&](int tr, int ky, float2 v) { HT[(size_t)ky * H + u0 + tr] = v; };
                 fg_transform2(arr, stw, tid, gsync, load, emit);
                 gsync();                                        // the last stage's reads are done: zero for the next unit
                 clear_group();
+#endif
             }
             if (p == 0) {
 #pragma unroll
