@@ -524,6 +524,9 @@ def main():
                    "h2d_bytes_per_step": int(vis_h.numel() * 8 + uvw_h.numel() * 4),
                    "d2h_bytes_per_step": int(img_h.numel() * 4 + wsum_h.numel() * 4),
                    "steps": e_steps, "ms_per_step": float(dt.item()) * 1e3,
+                   "d2h_gbs": float((img_h.numel() * 4 + wsum_h.numel() * 4) / float(dt.item()) / 1e9),
+                   "bound": "PCIe device->host: the images are 16x the visibilities; a pinned 2 GiB cudaMemcpy on the same kind of box "
+                            "measures 54.1 GB/s device->host alone (DESIGN.md 5.3)",
                    "api": "blink_image_host (pinned host buffers, per-timestep H2D/compute/D2H pipeline)"}
             del img_h, vis_h, ws_h
         except Exception as ex:  # report, never hide
