@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "libblinkimg.so")
 SOURCES = ["blink_api.cu", "blink_grid.cu", "blink_fft2d.cu", "blink_fused.cu", "blink_fused_conv.cu", "blink_image.cu", "blink_avg.cu", "blink_fftg.cu", "blink_fused_g.cu", "blink_corr.cu", "blink_noalloc.cu"]
-HEADERS = ["blink_common.cuh", "blink_fft.cuh", "blink_tma.cuh", "blink_fused_kernel.cuh", "blink_fftg.cuh", os.path.join("..", "..", "include", "blinkimg.h")]
+HEADERS = ["blink_common.cuh", "blink_fft.cuh", "blink_tma.cuh", "blink_fused_kernel.cuh", "blink_fftg.cuh", "blink_sort.cuh", os.path.join("..", "..", "include", "blinkimg.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "--fmad=true", "-Xptxas", "-v"]
 

@@ -11,6 +11,7 @@
 #include <algorithm>
 
 #include "blink_common.cuh"
+#include "blink_sort.cuh"
 
 namespace blink {
 
@@ -179,6 +180,31 @@ __global__ void __launch_bounds__(1024) avg_sortm_kernel(const float *__restrict
         }
     for (int i = threadIdx.x; i < B; i += 1024) sorted_m[(size_t)blockIdx.x * B + i] = key[i];
 }
+// the same with the keys in registers (blink_sort.cuh) for EPT * 512 < B <= EPT * 1024
+template <int EPT>
+__global__ void __launch_bounds__(1024) avg_sortm_regs_kernel(const float *__restrict__ uvw_m, int B, float *__restrict__ sorted_m)
+{
+    extern __shared__ float key_s[];
+    const float *uvw = uvw_m + (size_t)blockIdx.x * B * 3;
+    float key[EPT];
+    uint32_t val[EPT];
+#pragma unroll
+    for (int r = 0; r < EPT; ++r) {
+        const int i = r * 1024 + (int)threadIdx.x;
+        float k = __int_as_float(0x7f800000);                            // +inf: padding, NaN coordinates
+        if (i < B) {
+            const float u = uvw[3 * i], v = uvw[3 * i + 1];
+            if (u == u && v == v) k = fmaxf(fabsf(u), fabsf(v));
+        }
+        key[r] = k;
+        val[r] = 0u;
+    }
+    block_bitonic_sort<EPT, false>(key, val, key_s, nullptr);
+#pragma unroll
+    for (int r = 0; r < EPT; ++r) key_s[threadIdx.x * EPT + r] = key[r];
+    __syncthreads();
+    for (int i = threadIdx.x; i < B; i += 1024) sorted_m[(size_t)blockIdx.x * B + i] = key_s[i];
+}
 __global__ void avg_wsearch_kernel(const AvgArgs a, const __grid_constant__ ScaleBlock sc, const float *__restrict__ sorted_m,
                                    float *__restrict__ winv)
 {
@@ -214,6 +240,8 @@ __global__ void avg_winv_kernel(const AvgArgs a, float *__restrict__ winv)
 // baseline's cell moves slowly (the scale changes by 2.6e-4 per 40 kHz channel), so the thread keeps the
 // weighted sum of the current cell in registers and only touches the grid when the cell changes: ~20-60x fewer
 // atomics than one per sample.  Visibility reads stay coalesced (baseline is the fastest axis of vis).
+// WQ: per-sample weights wq [T*C][B] (uniform weighting) instead of one weight per (t,c) (natural: winv [T*C])
+template <bool WQ>
 __global__ void __launch_bounds__(kAvgThreads)
 avg_scatter_runs_kernel(const AvgArgs a, const __grid_constant__ ScaleBlock sc, const float *__restrict__ winv,
                         const float *__restrict__ wq, int t_lo,
@@ -246,8 +274,8 @@ avg_scatter_runs_kernel(const AvgArgs a, const __grid_constant__ ScaleBlock sc, 
     constexpr int kAvgAhead = 8;
     const unsigned vs = (unsigned)a.P * (unsigned)a.B;          // elements between consecutive channels of one (t, p, b)
     const float2 *vp = a.vis + ((size_t)(t * a.C + c0) * a.P + p) * a.B + b;
-    const float *wp = wq ? wq + ((size_t)t * a.C + c0) * a.B + b : winv + (size_t)t * a.C + c0;
-    const unsigned ws = wq ? (unsigned)a.B : 1u;
+    const float *wp = WQ ? wq + ((size_t)t * a.C + c0) * a.B + b : winv + (size_t)t * a.C + c0;
+    const unsigned ws = WQ ? (unsigned)a.B : 1u;
     const float *sp = sc.s + (c0 - a.c_base);
     int kx = 0x7fc00001, ky = 0x7fc00001;                       // bit patterns no valid sum has
     auto step = [&](float s, float2 x, float w) {
@@ -275,7 +303,8 @@ avg_scatter_runs_kernel(const AvgArgs a, const __grid_constant__ ScaleBlock sc, 
 #pragma unroll
         for (int j = 0; j < kAvgAhead; ++j) {
             x[j] = __ldcs(vp + (size_t)((unsigned)j * vs));
-            w[j] = wq ? __ldcs(wp + (size_t)((unsigned)j * ws)) : __ldg(wp + j);
+            if constexpr (WQ) w[j] = __ldcs(wp + (size_t)((unsigned)j * ws));
+            else w[j] = __ldg(wp + j);
         }
 #pragma unroll
         for (int j = 0; j < kAvgAhead; ++j) step(sp[j], x[j], w[j]);
@@ -284,7 +313,7 @@ avg_scatter_runs_kernel(const AvgArgs a, const __grid_constant__ ScaleBlock sc, 
         sp += kAvgAhead;
     }
     for (; c < c1; ++c) {
-        step(*sp, __ldcs(vp), wq ? __ldcs(wp) : __ldg(wp));
+        step(*sp, __ldcs(vp), WQ ? __ldcs(wp) : __ldg(wp));
         vp += vs;
         wp += ws;
         ++sp;
@@ -348,8 +377,16 @@ extern "C" int blink_image_avg(const blink_c64 *vis, const float *uvw_m, const d
         sorted_m = reinterpret_cast<float *>(static_cast<unsigned char *>(workspace) + gbytes + winv_bytes);
         int np2 = 1;
         while (np2 < B) np2 <<= 1;
-        BLINK_CUDA_TRY(cudaFuncSetAttribute(avg_sortm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, np2 * 4));
-        avg_sortm_kernel<<<T, 1024, (size_t)np2 * 4, st>>>(uvw_m, B, np2, sorted_m);
+        if (np2 == 8192) {
+            BLINK_CUDA_TRY(cudaFuncSetAttribute(avg_sortm_regs_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, np2 * 4));
+            avg_sortm_regs_kernel<8><<<T, 1024, (size_t)np2 * 4, st>>>(uvw_m, B, sorted_m);
+        } else if (np2 == 16384) {
+            BLINK_CUDA_TRY(cudaFuncSetAttribute(avg_sortm_regs_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, np2 * 4));
+            avg_sortm_regs_kernel<16><<<T, 1024, (size_t)np2 * 4, st>>>(uvw_m, B, sorted_m);
+        } else {
+            BLINK_CUDA_TRY(cudaFuncSetAttribute(avg_sortm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, np2 * 4));
+            avg_sortm_kernel<<<T, 1024, (size_t)np2 * 4, st>>>(uvw_m, B, np2, sorted_m);
+        }
         BLINK_LAUNCH_CHECK("avg_sortm_kernel");
     }
     float2 *grid = static_cast<float2 *>(workspace);
@@ -395,7 +432,7 @@ extern "C" int blink_image_avg(const blink_c64 *vis, const float *uvw_m, const d
                 const int nchunk = (nc + kAvgChunk - 1) / kAvgChunk, bblocks = (B + kAvgThreads - 1) / kAvgThreads;
                 const long long blocks = (long long)bblocks * nchunk * P * nt;
                 if (blocks > 0x7fffffffLL) return BLINK_ERR_UNSUPPORTED;
-                avg_scatter_runs_kernel<<<(unsigned)blocks, kAvgThreads, 0, st>>>(a, sc, nullptr, wq, t, c, nc, nchunk, bblocks);
+                avg_scatter_runs_kernel<true><<<(unsigned)blocks, kAvgThreads, 0, st>>>(a, sc, nullptr, wq, t, c, nc, nchunk, bblocks);
                 BLINK_LAUNCH_CHECK("avg_scatter_runs_kernel");
             }
         } else {
@@ -416,7 +453,7 @@ extern "C" int blink_image_avg(const blink_c64 *vis, const float *uvw_m, const d
             }
             const long long blocks = (long long)bblocks * nchunk * P * nt;
             if (blocks > 0x7fffffffLL) return BLINK_ERR_UNSUPPORTED;
-            avg_scatter_runs_kernel<<<(unsigned)blocks, kAvgThreads, 0, st>>>(a, sc, winv, nullptr, t, c, nc, nchunk, bblocks);
+            avg_scatter_runs_kernel<false><<<(unsigned)blocks, kAvgThreads, 0, st>>>(a, sc, winv, nullptr, t, c, nc, nchunk, bblocks);
             BLINK_LAUNCH_CHECK("avg_scatter_runs_kernel");
         }
         tc = end;
