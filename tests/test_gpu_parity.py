@@ -1015,3 +1015,33 @@ def test_volt_out_of_range(bk):
     v2.view(-1)[5] = -128
     with pytest.raises(bk.BlinkError):
         bk.blink_correlate(v2, 200, 4, check_range=True)
+
+
+@pytest.mark.parametrize("B,weighting", [(4097, 0), (8192, 1), (8193, 0), (14000, 0)])
+def test_presort_in_registers_edges(bk, oracle_mod, B, weighting):
+    # the per-timestep presorts run as register-resident bitonic networks (blink_sort.cuh) for 4097..16384 baselines: 8 or 16
+    # elements per thread.  Edges: almost all padding (4097), no padding (8192), one element over (8193), 16 per thread (14000); many EQUAL |u|
+    # (ties are ordered by index), u = +-same value (folded onto one key), NaN coordinates (sorted last with the padding).
+    # Observables: every nearest-cell index and W bit-exact, images within tolerance, through the fused kernel AND through
+    # blink_image_avg (whose weight sums come from its own sort by max(|u|, |v|) + binary search, option 1).
+    from paper_2505_15204_b200 import workloads
+    w = workloads.make_random(T=2, C=2, P=1, B=B, n_pix=256, weighting=weighting, seed=300 + B, device="cuda", fill=1.05)
+    cell_m = 299792458.0 / 150e6
+    w.uvw_m[0, 100:900, 0] = 7.25 * cell_m                         # 800 equal keys
+    w.uvw_m[0, 900:1300, 0] = -7.25 * cell_m                       # and 400 more with the other sign
+    w.uvw_m[1, ::7, 0] = 0.0                                       # many samples on the u = 0 column
+    w.uvw_m[0, 17, 0] = float("nan")
+    w.uvw_m[1, B - 1, 1] = float("nan")
+    bk.set_option(bk.OPT_IMAGE_PATH, 2)
+    try:
+        res = bk.blink_image(w.vis, w.uvw_m, w.freqs_hz, w.n_pix, w.pixscale_rad, weighting, want_cell_idx=True)
+        torch.cuda.synchronize()
+    finally:
+        bk.set_option(bk.OPT_IMAGE_PATH, 0)
+    _check_images(bk, w, res, oracle_mod)
+    assert np.array_equal(res["cell_idx"].cpu().numpy(), oracle_mod.cells(w.uvw_m.cpu().numpy(), w.freqs_hz, w.n_pix, w.pixscale_rad))
+    bk.set_option(bk.OPT_AVG_WSUM, 1)
+    try:
+        _check_avg(bk, oracle_mod, w, False)
+    finally:
+        bk.set_option(bk.OPT_AVG_WSUM, 0)
