@@ -240,6 +240,44 @@ bool grid_needs_global_counts(int B, int n_pix, int weighting)
     return weighting == BLINK_W_UNIFORM && B > chunk;
 }
 
+// Tiny batches (a single image, a handful of them): one CTA per (t,c) leaves the other SMs idle -- 52 of the 67 us of BASELINE
+// config 1 (one 256 x 256 image) were this gridder on ONE SM.  Natural weighting only: the grids are zeroed by a memset and every
+// (baseline, (t,c)) thread adds its sample and the conjugate with `red.global.add.v2.f32`; the in-range count of a (t,c) is
+// collected in its wsum slot as an integer (warp ballot + one atomic per warp) and turned into W = 2 count by a finishing kernel.
+__global__ void __launch_bounds__(256)
+grid_scatter_small_kernel(const GridArgs a, const __grid_constant__ ScaleBlock sc)
+{
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    const int tc = a.tc0 + blockIdx.y;
+    const int t = tc / a.C, c = tc - t * a.C;
+    const int n = a.n;
+    const size_t n2 = (size_t)n * n;
+    bool in = false;
+    if (b < a.B) {
+        const float *uvw = a.uvw_m + ((size_t)t * a.B + b) * 3;
+        const int cell = cell_of(uvw[0], uvw[1], sc.s[c - a.c_base], n, n / 2);
+        if (a.cell_idx) a.cell_idx[(size_t)tc * a.B + b] = cell;
+        if (cell >= 0) {
+            in = true;
+            const int mir = mirror_of(cell, n);
+            const int otc = tc - a.out_tc0;
+            for (int p = 0; p < a.P; ++p) {
+                const float2 v = __ldg(a.vis + ((size_t)tc * a.P + p) * a.B + b);
+                float2 *g = a.grid + ((size_t)otc * a.P + p) * n2;
+                atomicAdd(&g[cell], v);
+                atomicAdd(&g[mir], make_float2(v.x, -v.y));
+            }
+        }
+    }
+    const unsigned m = __ballot_sync(0xffffffffu, in);
+    if ((threadIdx.x & 31) == 0 && m) atomicAdd(reinterpret_cast<unsigned *>(a.wsum) + tc, (unsigned)__popc(m));
+}
+__global__ void grid_scatter_finish_kernel(float *wsum, int tc0, int ntc)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < ntc) wsum[tc0 + i] = (float)(2u * reinterpret_cast<const unsigned *>(wsum)[tc0 + i]);
+}
+
 int grid_range(const float2 *vis, const float *uvw_m, const double *freqs_hz, double pixscale_rad, int T, int C, int P,
                int B, int n_pix, int weighting, int tc0, int ntc, int out_tc0, float2 *grid, float *wsum,
                int32_t *cell_idx, uint32_t *counts, cudaStream_t st, bool half_only, int *row_extent)
@@ -261,6 +299,21 @@ int grid_range(const float2 *vis, const float *uvw_m, const double *freqs_hz, do
     if (a.n_chunks > 1 && weighting == BLINK_W_UNIFORM && counts == nullptr) return BLINK_ERR_WORKSPACE;
     a.half_only = (half_only && a.n_chunks == 1 && counts == nullptr) ? 1 : 0;
     a.row_extent = row_extent;
+    // tiny batches, natural weighting, nothing but the plain outputs asked for: scatter with global atomics over all SMs
+    const bool small = weighting == BLINK_W_NATURAL && counts == nullptr && !half_only && row_extent == nullptr &&
+                       ntc <= 16 && C <= 1024 && option(BLINK_OPT_GRID_CHUNK_B) == 0;
+    if (small) {
+        BLINK_CUDA_TRY(cudaMemsetAsync(grid + (size_t)(tc0 - out_tc0) * P * n2, 0, (size_t)ntc * P * n2 * sizeof(float2), st));
+        BLINK_CUDA_TRY(cudaMemsetAsync(wsum + tc0, 0, (size_t)ntc * sizeof(float), st));
+        ScaleBlock sc;
+        for (int k = 0; k < 1024; ++k) sc.s[k] = k < C ? scale_for(freqs_hz[k], n_pix, pixscale_rad) : 0.f;
+        a.tc0 = tc0; a.c_base = 0;
+        grid_scatter_small_kernel<<<dim3((unsigned)((B + 255) / 256), (unsigned)ntc), 256, 0, st>>>(a, sc);
+        BLINK_LAUNCH_CHECK("grid_scatter_small_kernel");
+        grid_scatter_finish_kernel<<<(ntc + 63) / 64, 64, 0, st>>>(wsum, tc0, ntc);
+        BLINK_LAUNCH_CHECK("grid_scatter_finish_kernel");
+        return BLINK_OK;
+    }
     const size_t smem = grid_smem_bytes(a.tile_cells, a.n_bands, a.chunk_b);
     BLINK_CUDA_TRY(cudaFuncSetAttribute(grid_tiles_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     // sub-ranges that stay inside one timestep's block of <= 1024 channels (scales travel as a kernel parameter)
