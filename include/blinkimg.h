@@ -54,7 +54,7 @@ enum {
  * A call reads the options of the thread that issues it, so a switch set by one thread never changes the route of a
  * call made by another; there is no process-wide mutable state besides the launch counter. */
 enum {
-    BLINK_OPT_IMAGE_PATH = 0,     /* [0] 0 = auto (fused where supported; batches of <= 8 Mi pixels take the unfused chain when the
+    BLINK_OPT_IMAGE_PATH = 0,     /* [0] 0 = auto (fused where supported; batches of <= 4 Mi pixels take the unfused chain when the
                                          workspace holds them), 1 = force unfused (grid -> rows -> columns), 2 = force fused */
     BLINK_OPT_FUSED_CTAS = 1,     /* [0] 0 = auto (one persistent CTA per SM), else CTAs for the fused kernel  */
     BLINK_OPT_GRID_CHUNK_B = 2,   /* [0] 0 = auto, else baselines per gridder chunk (tests the spill path)     */

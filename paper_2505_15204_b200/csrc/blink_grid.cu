@@ -301,7 +301,7 @@ int grid_range(const float2 *vis, const float *uvw_m, const double *freqs_hz, do
     a.row_extent = row_extent;
     // tiny batches, natural weighting, nothing but the plain outputs asked for: scatter with global atomics over all SMs
     const bool small = weighting == BLINK_W_NATURAL && counts == nullptr && !half_only && row_extent == nullptr &&
-                       ntc <= 16 && C <= 1024 && option(BLINK_OPT_GRID_CHUNK_B) == 0;
+                       ntc <= 128 && C <= 1024 && option(BLINK_OPT_GRID_CHUNK_B) == 0;
     if (small) {
         BLINK_CUDA_TRY(cudaMemsetAsync(grid + (size_t)(tc0 - out_tc0) * P * n2, 0, (size_t)ntc * P * n2 * sizeof(float2), st));
         BLINK_CUDA_TRY(cudaMemsetAsync(wsum + tc0, 0, (size_t)ntc * sizeof(float), st));

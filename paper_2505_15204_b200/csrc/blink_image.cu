@@ -37,11 +37,12 @@ static bool use_fused(int P, int B, int n_pix, int weighting)
     return fused_supported(P, B, n_pix, weighting);
 }
 
-// auto path only: batches of at most 8 Mi pixels (128 images of 256^2, 32 of 512^2, 8 of 1024^2, 2 of 2048^2: the measured
-// cross-over of the two paths on a B200) go through the unfused chain
+// auto path only: batches of at most 4 Mi pixels (64 images of 256^2, 16 of 512^2, 4 of 1024^2, 1 of 2048^2: the measured
+// cross-over of the two paths on a B200 -- e.g. 32 x 512^2: unfused 113 us, fused 91 us; 8 x 512^2: 44 / 89 us) go through
+// the unfused chain
 static bool small_batch(int ntc, int P, int n_pix)
 {
-    return option(BLINK_OPT_IMAGE_PATH) == 0 && (size_t)ntc * P * n_pix * n_pix <= ((size_t)8 << 20);
+    return option(BLINK_OPT_IMAGE_PATH) == 0 && (size_t)ntc * P * n_pix * n_pix <= ((size_t)4 << 20);
 }
 
 static int image_device(const float2 *vis, const float *uvw_m, const double *freqs_hz, int T, int C, int P, int B,

@@ -574,7 +574,7 @@ def test_more_than_1024_channels(bk, oracle_mod, path):
 
 
 def test_small_batch_auto_route(bk, oracle_mod):
-    """Auto path, batches of <= 8 Mi pixels: the unfused chain when the workspace holds the whole range (recommended
+    """Auto path, batches of <= 4 Mi pixels: the unfused chain when the workspace holds the whole range (recommended
     size), the fused kernel when it does not (minimum size); both against the oracle, indices and weight sums bit-exact."""
     from paper_2505_15204_b200 import workloads
     for weighting in (0, 1):
