@@ -63,8 +63,8 @@ def test_host_only_calls(so_path):
     rec, mn = bk.blink_workspace_bytes(bk.OP_IMAGE, 2, 768, 1, 8128, 1200, 0)
     sortb = 3 * (2 * 8128 * 4 + (-2 * 8128 * 4) % 256)
     assert mn == sortb + 9728 + 1200 * 600 * 8 and (rec - sortb - 9728) % (1200 * 600 * 8) == 0 and rec > mn
-    # small batches (<= 8 Mi pixels, auto path): the recommended size also holds the whole range for the unfused chain
-    for n, n_img in ((256, 128), (512, 32), (1024, 8), (2048, 2)):
+    # small batches (<= 4 Mi pixels, auto path): the recommended size also holds the whole range for the unfused chain
+    for n, n_img in ((256, 64), (512, 16), (1024, 4), (2048, 1)):
         rec, mn = bk.blink_workspace_bytes(bk.OP_IMAGE, 1, n_img, 1, 8128, n, 0)
         assert rec >= n_img * n * n * 8 and mn <= rec
 
