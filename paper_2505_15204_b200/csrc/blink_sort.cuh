@@ -4,8 +4,9 @@
 //   j <  EPT        stay inside a thread (compile-time register pairs),
 //   j <  32 EPT     exchange between lanes of a warp (shuffles),
 //   j >= 32 EPT     cross warps through shared memory (15 steps of 91 at 8192 elements; slot r * 1024 + tid: conflict-free).
-// The first version kept every element in shared memory and paid a CTA barrier for each of the 91 steps (0.107 ms per 8128
-// baselines; it was 4.5 % of config 2's step and 11 % of the averaged-image step).
+// The first version kept every element in shared memory and paid a CTA barrier for each of the 91 steps (0.108 ms per 8128
+// baselines, 4.5 % of config 2's step and 11 % of the averaged-image step; this one: 0.049 ms, bound by the ~6 M thread
+// instructions of the network itself).
 // Order: ascending in (key, value) -- a total order when the values are distinct indices, so padding (+inf, index >= B) stays last.
 #pragma once
 #include <stdint.h>
