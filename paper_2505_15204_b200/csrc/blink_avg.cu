@@ -15,7 +15,13 @@
 
 namespace blink {
 
+int presort_launch(const float *uvw_m, int T, int B, float *su, uint2 *svb, cudaStream_t st);      // blink_fused.cu
+size_t sort_bytes(int T, int B);
+
 constexpr int kAvgThreads = 256;
+// avg_grid_kernel: an item is a chain of returning L2 atomics per thread (ncu: 3 % issue-active, 133 us per (t,c) with 256 threads
+// at 10296 baselines = 40 samples per thread): 1024 threads keep four times as many of them in flight
+constexpr int kAvgGridThreads = 1024;
 
 struct AvgArgs {
     const float2 *vis; const float *uvw_m;
@@ -31,10 +37,10 @@ struct AvgArgs {
 // One persistent CTA per (t,c) item.  Sweep 1 finds the weight sum W of the item (natural: samples placed;
 // uniform: occupied cells, counted exactly as "first arrival" on a per-CTA count plane); sweep 2 adds every
 // sample times 1 / (n W) (uniform: also / count of its cell) to the combined grid of its output image.
-__global__ void __launch_bounds__(kAvgThreads)
+__global__ void __launch_bounds__(kAvgGridThreads)
 avg_grid_kernel(const AvgArgs a, const __grid_constant__ ScaleBlock sc)
 {
-    __shared__ int s_in[kAvgThreads / 32], s_first[kAvgThreads / 32];
+    __shared__ int s_in[kAvgGridThreads / 32], s_first[kAvgGridThreads / 32];
     const bool uniform = a.weighting == BLINK_W_UNIFORM;
     const int n = a.n, h = n / 2, B = a.B;
     const size_t n2 = (size_t)n * n;
@@ -46,7 +52,7 @@ avg_grid_kernel(const AvgArgs a, const __grid_constant__ ScaleBlock sc)
         const float *uvw = a.uvw_m + (size_t)t * B * 3;
         // ---- sweep 1: weight sum ---------------------------------------------------------------------
         int n_in = 0, n_first = 0;
-        for (int b = threadIdx.x; b < B; b += kAvgThreads) {
+        for (int b = threadIdx.x; b < B; b += kAvgGridThreads) {
             const int cell = cell_of(uvw[3 * b], uvw[3 * b + 1], s, n, h);
             if (cell >= 0) {
                 ++n_in;
@@ -65,19 +71,19 @@ avg_grid_kernel(const AvgArgs a, const __grid_constant__ ScaleBlock sc)
         __syncthreads();
         n_in = 0; n_first = 0;
 #pragma unroll
-        for (int k = 0; k < kAvgThreads / 32; ++k) { n_in += s_in[k]; n_first += s_first[k]; }
+        for (int k = 0; k < kAvgGridThreads / 32; ++k) { n_in += s_in[k]; n_first += s_first[k]; }
         const float W = uniform ? (float)n_first : (float)(2 * n_in);
         if (threadIdx.x == 0) a.wsum[tc] = W;
         // ---- sweep 2 ------------------------------------------------------------------------------------
         if (a.wq) {                                                     // fast route: only the per-sample weights; the
             const float wbase = W > 0.f ? a.inv_navg / W : 0.f;         // run-length scatter kernel does the adding
-            for (int b = threadIdx.x; b < B; b += kAvgThreads) {
+            for (int b = threadIdx.x; b < B; b += kAvgGridThreads) {
                 const int cell = cell_of(uvw[3 * b], uvw[3 * b + 1], s, n, h);
                 a.wq[(size_t)tc * B + b] = cell >= 0 ? wbase / (float)__ldcg(&cnt[cell]) : 0.f;
             }
         } else if (W > 0.f) {                                           // weighted scatter into the combined grids
             const float wbase = a.inv_navg / W;
-            for (int b = threadIdx.x; b < B; b += kAvgThreads) {
+            for (int b = threadIdx.x; b < B; b += kAvgGridThreads) {
                 const int cell = cell_of(uvw[3 * b], uvw[3 * b + 1], s, n, h);
                 if (cell < 0) continue;
                 const int mir = mirror_of(cell, n);
@@ -96,7 +102,7 @@ avg_grid_kernel(const AvgArgs a, const __grid_constant__ ScaleBlock sc)
         }
         if (uniform) {                                                  // leave the count plane clean for the next item
             __syncthreads();
-            for (int b = threadIdx.x; b < B; b += kAvgThreads) {
+            for (int b = threadIdx.x; b < B; b += kAvgGridThreads) {
                 const int cell = cell_of(uvw[3 * b], uvw[3 * b + 1], s, n, h);
                 if (cell >= 0) {
                     __stcg(&cnt[cell], 0u);
@@ -106,6 +112,94 @@ avg_grid_kernel(const AvgArgs a, const __grid_constant__ ScaleBlock sc)
             __threadfence();
         }
         __syncthreads();
+    }
+}
+
+// ---- uniform weighting, column route: per-sample weights WITHOUT count planes or global atomics ----------------------
+// avg_grid_kernel counts on a 4 N^2-byte plane per CTA with returning L2 atomics, a chain of round trips per thread (ncu: 3-6 %
+// issue-active, 0.54-0.80 of the 1.13-1.40 ms of a config-4 timestep).  With the baselines of a timestep sorted by |u| and folded
+// into the half plane u >= 0 (the fused kernels' presort: su = |u|, svb = {sign(u) v, b | conj << 31}), the samples of one grid
+// COLUMN are a contiguous range for every channel, so a warp counts a column in an N-entry shared-memory array, reads the counts
+// back for its samples and zeroes what it touched.  A half-plane cell's count is the full plane's count of that cell (a sample with
+// u < 0 sits on its conjugate's cell), column 0 takes the sample and its conjugate, and newly occupied cells count twice off the
+// axis (cell + mirror): W and every weight are exactly those of avg_grid_kernel.
+constexpr int kAvgColThreads = 256, kAvgColWarps = kAvgColThreads / 32;
+static size_t avg_col_smem(int n) { return ((size_t)(n / 2 + 2 + 3) / 4 * 4 + (size_t)kAvgColWarps * n) * sizeof(uint32_t); }
+__global__ void __launch_bounds__(kAvgColThreads)
+avg_uniform_cols_kernel(const AvgArgs a, const __grid_constant__ ScaleBlock sc, const float *__restrict__ su_all,
+                        const uint2 *__restrict__ svb_all)
+{
+    extern __shared__ uint32_t col_sm[];
+    __shared__ int s_first[kAvgColWarps];
+    const int n = a.n, H = n / 2, B = a.B;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    uint32_t *coff = col_sm;                                            // [H + 2]: first sorted sample of column u
+    uint32_t *cw = col_sm + (H + 2 + 3) / 4 * 4 + (size_t)warp * n;    // this warp's count column
+    const float lim = (float)(H - 1);
+    for (int i = threadIdx.x; i < kAvgColWarps * n; i += kAvgColThreads) col_sm[(H + 2 + 3) / 4 * 4 + i] = 0u;
+    for (int tc = a.tc0 + blockIdx.x; tc < a.tc0 + a.ntc; tc += gridDim.x) {
+        const int t = tc / a.C, c = tc - t * a.C;
+        const float s = sc.s[c - a.c_base];
+        const float *su = su_all + (size_t)t * B;
+        const uint2 *svb = svb_all + (size_t)t * B;
+        float *wq = a.wq + (size_t)tc * B;
+        auto col_of = [&](float x) -> int {
+            int i;
+            const float xr = rint_rne(__fmul_rn(x, s), i);
+            return (xr <= lim) ? i : H;                                 // NaN: H
+        };
+        __syncthreads();                                                // the previous item's readers of coff are done
+        for (int j = threadIdx.x; j <= B; j += kAvgColThreads) {
+            const int cj = j < B ? col_of(__ldg(su + j)) : H + 1;
+            const int cq = j > 0 ? col_of(__ldg(su + j - 1)) : -1;
+            for (int u = cq + 1; u <= cj; ++u) coff[u] = (uint32_t)j;
+        }
+        __syncthreads();
+        int n_first = 0;
+        for (int u = warp; u < H; u += kAvgColWarps) {
+            const int k0 = (int)coff[u], k1 = (int)coff[u + 1];
+            if (k0 == k1) continue;
+            for (int j = k0 + lane; j < k1; j += 32) {                  // count
+                int iv;
+                const float yr = rint_rne(__fmul_rn(__uint_as_float(__ldg(&svb[j].x)), s), iv);
+                if (fabsf(yr) <= lim) {
+                    n_first += (atomicAdd(&cw[iv + H], 1u) == 0u) ? (u == 0 ? 1 : 2) : 0;
+                    if (u == 0) n_first += atomicAdd(&cw[H - iv], 1u) == 0u;
+                }
+            }
+            __syncwarp();
+            for (int j = k0 + lane; j < k1; j += 32) {                  // read back: the count of every sample's cell, as a float
+                int iv;
+                const uint2 sq = __ldg(svb + j);
+                const float yr = rint_rne(__fmul_rn(__uint_as_float(sq.x), s), iv);
+                wq[sq.y & 0x7fffffffu] = fabsf(yr) <= lim ? (float)cw[iv + H] : 0.f;
+            }
+            __syncwarp();
+            for (int j = k0 + lane; j < k1; j += 32) {                  // leave the column clean
+                int iv;
+                const float yr = rint_rne(__fmul_rn(__uint_as_float(__ldg(&svb[j].x)), s), iv);
+                if (fabsf(yr) <= lim) {
+                    cw[iv + H] = 0u;
+                    if (u == 0) cw[H - iv] = 0u;
+                }
+            }
+            __syncwarp();
+        }
+        for (int j = (int)coff[H] + threadIdx.x; j < B; j += kAvgColThreads) wq[__ldg(&svb[j].y) & 0x7fffffffu] = 0.f;   // off the grid in u
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) n_first += __shfl_xor_sync(0xffffffffu, n_first, d);
+        if (lane == 0) s_first[warp] = n_first;
+        __syncthreads();                                                // also: every count of this item is in wq
+        n_first = 0;
+#pragma unroll
+        for (int k = 0; k < kAvgColWarps; ++k) n_first += s_first[k];
+        const float W = (float)n_first;
+        if (threadIdx.x == 0) a.wsum[tc] = W;
+        const float wbase = W > 0.f ? a.inv_navg / W : 0.f;
+        for (int b = threadIdx.x; b < B; b += kAvgColThreads) {
+            const float cnt = __ldcg(wq + b);                           // written by other warps of this CTA: read it from L2
+            wq[b] = cnt > 0.f ? wbase / cnt : 0.f;
+        }
     }
 }
 
@@ -338,6 +432,7 @@ size_t avg_workspace_bytes(int T, int C, int P, int B, int n_pix, int weighting,
         if (!minimum) planes = std::max<size_t>(1, std::min<size_t>(planes, ((size_t)2 << 30) / plane));
         b += planes * plane;
         if (!minimum) b += align_up((size_t)T * C * B * sizeof(float), 256);   // per-sample weights: the run-length scatter route
+        if (!minimum && B <= 16384) b += sort_bytes(T, B);                      // baselines sorted by |u|: the column route
     }
     return b;
 }
@@ -404,8 +499,26 @@ extern "C" int blink_image_avg(const blink_c64 *vis, const float *uvw_m, const d
             ctas = (int)std::min<size_t>((size_t)avg_max_planes(), avail / plane);
         }
     }
+    // uniform, column route: grid | per-sample weights | sorted baselines; no count planes
+    const float *col_su = nullptr;
+    const uint2 *col_svb = nullptr;
+    int col_ctas = 0;
+    if (uni && B <= 16384 && n_pix <= 4096 && option(BLINK_OPT_AVG_WSUM) != 2 &&
+        workspace_bytes >= gbytes + wq_bytes + sort_bytes(T, B)) {
+        unsigned char *wsp = static_cast<unsigned char *>(workspace) + gbytes;
+        wq = reinterpret_cast<float *>(wsp);
+        float *su = reinterpret_cast<float *>(wsp + wq_bytes);
+        uint2 *svb = reinterpret_cast<uint2 *>(wsp + wq_bytes + sort_bytes(T, B) / 3);
+        int rc2 = presort_launch(uvw_m, T, B, su, svb, st);
+        if (rc2 != BLINK_OK) return rc2;
+        col_su = su; col_svb = svb;
+        const size_t csm = avg_col_smem(n_pix);
+        BLINK_CUDA_TRY(cudaFuncSetAttribute(avg_uniform_cols_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)csm));
+        const int per_sm = (int)std::max<size_t>(1, std::min<size_t>(8, ((size_t)227 * 1024) / (csm + 1024)));
+        col_ctas = per_sm * (sm_count() > 0 ? sm_count() : 148);
+    }
     BLINK_CUDA_TRY(cudaMemsetAsync(grid, 0, gbytes, st));
-    if (uni) BLINK_CUDA_TRY(cudaMemsetAsync(cnt, 0, (size_t)ctas * plane, st));
+    if (uni && !col_su) BLINK_CUDA_TRY(cudaMemsetAsync(cnt, 0, (size_t)ctas * plane, st));
     const int n_out = (avg_time ? 1 : T) * P;
     int tc = 0;
     const int tc_end = T * C;
@@ -424,9 +537,15 @@ extern "C" int blink_image_avg(const blink_c64 *vis, const float *uvw_m, const d
         a.inv_navg = (float)(1.0 / (avg_time ? (double)T * C : (double)C));
         a.wq = wq;
         if (uni) {
-            const int gridx = a.ntc < ctas ? a.ntc : ctas;
-            avg_grid_kernel<<<gridx, kAvgThreads, 0, st>>>(a, sc);
-            BLINK_LAUNCH_CHECK("avg_grid_kernel");
+            if (col_su) {
+                const int gridx = a.ntc < col_ctas ? a.ntc : col_ctas;
+                avg_uniform_cols_kernel<<<gridx, kAvgColThreads, avg_col_smem(n_pix), st>>>(a, sc, col_su, col_svb);
+                BLINK_LAUNCH_CHECK("avg_uniform_cols_kernel");
+            } else {
+                const int gridx = a.ntc < ctas ? a.ntc : ctas;
+                avg_grid_kernel<<<gridx, kAvgGridThreads, 0, st>>>(a, sc);
+                BLINK_LAUNCH_CHECK("avg_grid_kernel");
+            }
             if (wq) {
                 const int nt = (C <= 1024) ? T : 1, nc = (C <= 1024) ? C : a.ntc;
                 const int nchunk = (nc + kAvgChunk - 1) / kAvgChunk, bblocks = (B + kAvgThreads - 1) / kAvgThreads;
