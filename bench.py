@@ -344,6 +344,29 @@ def main():
                    "algorithmic_bytes_per_step": bytes_a, "model": "n_img*8B + 12TB + T*P*4N^2 (vis + uvw read once, averaged images written)",
                    "hbm_gbs": bytes_a / (ms_a * 1e-3) / 1e9}
             del ws_a, img_a
+            # the same call with UNIFORM weighting on one timestep of BASELINE config 4 (768 channels x 4 planes of 2048^2,
+            # 10296 baselines): the column route of DESIGN.md 5.4 (per-sample weights by counting grid columns in shared memory)
+            if args.T is None and rank == 0:
+                w4 = workloads.make_config(4, device=dev, T=1)
+                T4, C4, P4, B4 = w4.vis.shape
+                rec4, _ = bk.blink_workspace_bytes(bk.OP_IMAGE_AVG, T4, C4, P4, B4, w4.n_pix, w4.weighting)
+                ws4 = torch.empty(max(rec4, 16), dtype=torch.uint8, device=dev)
+                img4 = torch.empty((T4 * P4, w4.n_pix, w4.n_pix), dtype=torch.float32, device=dev)
+                wsum4 = torch.empty((T4 * C4,), dtype=torch.float32, device=dev)
+                run4 = lambda: bk.blink_image_avg(w4.vis, w4.uvw_m, w4.freqs_hz, w4.n_pix, w4.pixscale_rad, w4.weighting,
+                                                  avg_time=False, image_avg=img4, workspace=ws4, wsum=wsum4)
+                for _ in range(args.warmup):
+                    run4()
+                e4 = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+                e4[0].record()
+                for _ in range(args.steps):
+                    run4()
+                e4[1].record()
+                torch.cuda.synchronize()
+                ms4 = e4[0].elapsed_time(e4[1]) / args.steps
+                avg["uniform_config4_one_timestep"] = {"ms_per_step": ms4, "images_in": T4 * C4 * P4, "images_out": T4 * P4,
+                                                        "gvis_per_s": T4 * C4 * P4 * B4 / (ms4 * 1e-3) / 1e9}
+                del w4, ws4, img4, wsum4
         except Exception as ex:  # report, never hide
             avg = {"error": str(ex)[:200]}
 
