@@ -151,7 +151,10 @@ int blink_image_host(const blink_c64 *vis_host, const float *uvw_m_host, const d
  * the samples are scattered, pre-multiplied by 1/(n W_tc) (uniform: also by 1/count of their cell), into one
  * combined uv grid per output image with global vector atomics, and only those grids are transformed.
  * Inputs as blink_grid; wsum out [T*C] as blink_image.  `workspace` >= blink_workspace_bytes(BLINK_OP_IMAGE_AVG)
- * (minimum via *min_bytes): the combined grids and, for uniform weighting, per-CTA count planes.
+ * (minimum via *min_bytes): the combined grids and, for uniform weighting, per-CTA count planes.  With the recommended
+ * size the per-sample weights [T*C][B] and the baselines sorted by |u| (12 bytes per (timestep, baseline)) fit as well, and
+ * uniform weighting takes the faster column route (counts per grid column in shared memory, no count planes) for
+ * n_pix <= 4096 and B <= 16384; results do not depend on the route.
  */
 int blink_image_avg(const blink_c64 *vis, const float *uvw_m, const double *freqs_hz,
                     int T, int C, int P, int B, int n_pix, double pixscale_rad, int weighting,
