@@ -133,7 +133,7 @@ bool fused_g_supported(int B, int n_pix);
 size_t fused_g_workspace_bytes(int T, int B, int ctas);
 int fused_g_image(const float2 *vis, const float *uvw_m, const double *freqs_hz, double pixscale_rad, int T, int C, int P, int B,
                   int weighting, int tc0, int ntc, float *image, float *wsum, int32_t *cell_idx, void *workspace,
-                  size_t workspace_bytes, cudaStream_t st, GainRef cal);
+                  size_t workspace_bytes, cudaStream_t st, GainRef cal, const ConvPoly *poly = nullptr, int R = 0, size_t extra = 0);
 
 // ------------------------------------------------------------------------------------------ host
 bool fused_supported(int P, int B, int n_pix, int weighting)

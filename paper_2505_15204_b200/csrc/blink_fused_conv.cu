@@ -15,6 +15,10 @@
 
 namespace blink {
 
+int fused_g_image(const float2 *vis, const float *uvw_m, const double *freqs_hz, double pixscale_rad, int T, int C, int P, int B,
+                  int weighting, int tc0, int ntc, float *image, float *wsum, int32_t *cell_idx, void *workspace,
+                  size_t workspace_bytes, cudaStream_t st, GainRef cal, const ConvPoly *poly, int R, size_t extra);      // blink_fused_g.cu
+
 bool fused_supported(int P, int B, int n_pix, int weighting);          // blink_fused.cu
 size_t fused_workspace_bytes(int T, int B, int n_pix, int ctas);
 int fused_default_ctas();
@@ -310,7 +314,7 @@ extern "C" int blink_image_conv(const blink_c64 *vis, const float *uvw_m, const 
     if (!size_supported(n_pix) || B > kMaxBaselines) return BLINK_ERR_UNSUPPORTED;
     rc = ensure_device();
     if (rc != BLINK_OK) return rc;
-    if (!is_pow2(n_pix) || !fused_supported(P, B, n_pix, BLINK_W_NATURAL)) {       // outside the fused kernel: the plain form
+    if (!(is_pow2(n_pix) || n_pix == 1200) || !fused_supported(P, B, n_pix, BLINK_W_NATURAL)) {   // outside the fused kernels: the plain form
         ConvPoly poly_u;
         conv_fit_taps(support, beta, &poly_u);
         return conv_unfused(reinterpret_cast<const float2 *>(vis), uvw_m, freqs_hz, T, C, P, B, n_pix, pixscale_rad, support, beta,
@@ -337,6 +341,8 @@ extern "C" int blink_image_conv(const blink_c64 *vis, const float *uvw_m, const 
         case 1024: return launch_conv<1024>(a, R, freqs_hz, pixscale_rad, workspace, workspace_bytes, st, &poly, extra);
         case 2048: return launch_conv<2048>(a, R, freqs_hz, pixscale_rad, workspace, workspace_bytes, st, &poly, extra);
         case 4096: return launch_conv<4096>(a, R, freqs_hz, pixscale_rad, workspace, workspace_bytes, st, &poly, extra);
+        case 1200: return fused_g_image(a.vis, uvw_m, freqs_hz, pixscale_rad, T, C, P, B, BLINK_W_NATURAL, 0, T * C, image, wsum, cell_idx,
+                                        workspace, workspace_bytes, st, GainRef(), &poly, R, extra);
         default: return BLINK_ERR_UNSUPPORTED;
     }
 }

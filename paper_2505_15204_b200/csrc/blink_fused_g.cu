@@ -132,8 +132,13 @@ __device__ __forceinline__ void fg_transform2_inplace(float2 *arr, const float2 
 #define BLINK_FG_PAIRED_STORE 1
 #endif
 
+// R > 0: convolutional gridding of support S = 2R + 1 (reading R16, blink_fused_kernel.cuh conv_one): a column pair
+// gathers every sorted sample whose support reaches it, the taps at columns <= 0 come back as the conjugate's mirrored taps, the
+// grid correction rides on the image store; natural weighting only
+template <int R>
 __global__ void __launch_bounds__(FG_THREADS, 1)
-fused_g_kernel(const FusedArgs a, const __grid_constant__ ScaleBlock sc, const float2 *__restrict__ tw_full)
+fused_g_kernel(const FusedArgs a, const __grid_constant__ ScaleBlock sc, const float2 *__restrict__ tw_full,
+               const __grid_constant__ ConvPoly cpoly)
 {
     constexpr int N = FG_N, H = FG_H;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -156,7 +161,7 @@ fused_g_kernel(const FusedArgs a, const __grid_constant__ ScaleBlock sc, const f
 
     float2 *HT = a.scratch + (size_t)blockIdx.x * N * H;         // [N ky][H u], transposed pass-1 output
     auto gsync = [g] { asm volatile("bar.sync %0, %1;" ::"r"(g + 1), "n"(FG_TG) : "memory"); };
-    const float lim = (float)(H - 1);
+    const float lim = (float)(H - 1 - R);                        // R > 0: the whole support of a sample stays on the grid (R16)
 
     // compact per-stage twiddle runs: stage with sub-transform length P reads W_N^(k N / (P R)), k < P
     for (int k = threadIdx.x; k < FG_TW; k += FG_THREADS) {
@@ -215,12 +220,12 @@ fused_g_kernel(const FusedArgs a, const __grid_constant__ ScaleBlock sc, const f
                     const int cj = j < B ? col_of(__ldg(su + j)) : H + 1;
                     const int cq = j > 0 ? col_of(__ldg(su + j - 1)) : -1;
                     for (int u = cq + 1; u <= cj; ++u) coff[u] = (uint32_t)j;
-                    if (cj >= H && cq < H) s_ncol = cq + 1;      // occupied columns are [0, cq]
+                    if (cj >= H && cq < H) s_ncol = cq + 1 + (cq >= 0 ? R : 0);   // occupied columns are [0, cq + R]
                 }
                 if (a.cell_idx) {
                     const float *uvw = a.uvw_m + (size_t)t * B * 3;
                     for (int b = threadIdx.x; b < B; b += FG_THREADS)
-                        a.cell_idx[(size_t)tc * B + b] = cell_of(uvw[3 * b], uvw[3 * b + 1], s, N, H);
+                        a.cell_idx[(size_t)tc * B + b] = cell_of(uvw[3 * b], uvw[3 * b + 1], s, N, H, R);
                 }
             }
             __syncthreads();                                    // (A)
@@ -272,10 +277,70 @@ fused_g_kernel(const FusedArgs a, const __grid_constant__ ScaleBlock sc, const f
                         ++my_in;
                     }
                 };
+                // convolutional gridding: sorted sample j seen from the column pair (u0, u0 + 1); transform index of row iv = iv mod N
+                auto conv_one = [&](int j) {
+                    if constexpr (R > 0) {
+                        constexpr int S = 2 * R + 1;
+                        int iu0, iv0;
+                        const float x = __fmul_rn(__ldg(su + j), s);
+                        const float xr = rint_rne(x, iu0);      // in range by construction of the sample range
+                        const uint2 sq = __ldg(svb + j);
+                        const float y = __fmul_rn(__uint_as_float(sq.x), s);
+                        const float yr = rint_rne(y, iv0);
+                        if (!(fabsf(yr) <= lim)) return;        // NaN fails
+                        const float fx = __fsub_rn(x, xr), fy = __fsub_rn(y, yr);
+                        float2 vv = visrow[sq.y & 0x7fffffffu];
+                        if (sq.y >> 31) vv.y = -vv.y;
+                        float wy[S];
+#pragma unroll
+                        for (int i = 0; i < S; ++i) {
+                            float w = cpoly.c[i][kConvTerms - 1];
+#pragma unroll
+                            for (int k = kConvTerms - 2; k >= 0; --k) w = fmaf(w, fy, cpoly.c[i][k]);
+                            wy[i] = w;
+                        }
+                        auto add_taps = [&](int tr, int row0, int dir, float ar, float ai) {
+#pragma unroll
+                            for (int i = 0; i < S; ++i) {
+                                const int row = row0 + dir * i;
+                                cell_add_take(&arr[tr * FG_LD + (row < 0 ? row + N : row)], make_float2(wy[i] * ar, wy[i] * ai));
+                            }
+                        };
+                        auto wx_of = [&](int jj) {
+                            float w = cpoly.c[jj][kConvTerms - 1];
+#pragma unroll
+                            for (int k = kConvTerms - 2; k >= 0; --k) w = fmaf(w, fx, cpoly.c[jj][k]);
+                            return w;
+                        };
+#pragma unroll
+                        for (int k = 0; k < 2; ++k) {
+                            const int u = u0 + k;
+                            const int jd = u - iu0;             // direct tap that lands in column u
+                            if (jd >= -R && jd <= R) {
+                                const float wx = wx_of(jd + R);
+                                add_taps(k, iv0 - R, 1, wx * vv.x, wx * vv.y);
+                                if (jd == 0) ++my_in;           // the sample's own column: counted once
+                            }
+                            const int jm = -u - iu0;            // tap at column -u, mirrored: conj(V) at row -(iv0 - R + i)
+                            if (jm >= -R) {
+                                const float wx = wx_of(jm + R);
+                                add_taps(k, -(iv0 - R), -1, wx * vv.x, -wx * vv.y);
+                            }
+                        }
+                    }
+                };
                 gsync();                                        // the arrays are zero (clear_group of the previous unit / image)
-                if (k0 + tid < k2) grid_one(sq_next, k0 + tid);
-                for (int j = k0 + tid + FG_TG; j < k2; j += FG_TG) grid_one(__ldg(svb + j), j);
-                sq_next = first_sample(cp + FG_G);              // lands while this unit is transformed
+                if constexpr (R == 0) {
+                    if (k0 + tid < k2) grid_one(sq_next, k0 + tid);
+                    for (int j = k0 + tid + FG_TG; j < k2; j += FG_TG) grid_one(__ldg(svb + j), j);
+                    sq_next = first_sample(cp + FG_G);          // lands while this unit is transformed
+                } else {
+                    // samples whose support reaches columns u0, u0 + 1: nearest columns [u0 - R, u0 + 1 + R] (the mirrored taps come
+                    // from nearest columns [0, R - u0], a subset); coff[H] = first sample beyond the range
+                    const int c0 = (int)coff[u0 > R ? u0 - R : 0], c2 = (int)coff[u0 + 2 + R < H ? u0 + 2 + R : H];
+                    for (int j = c0 + tid; j < c2; j += FG_TG) conv_one(j);
+                    (void)k0; (void)k1; (void)k2; (void)grid_one; (void)sq_next;
+                }
                 gsync();
                 auto load = [&](int tr, int n) -> float2 {      // a3: divide by the cell count (uniform weighting)
                     float2 v = arr[tr * FG_LD + n];
@@ -375,8 +440,14 @@ fused_g_kernel(const FusedArgs a, const __grid_constant__ ScaleBlock sc, const f
                     const int ky = ky0 + 2 * tr;
                     const int y0 = ky < H ? ky + H : ky - H, y1 = ky + 1 < H ? ky + 1 + H : ky + 1 - H;
                     const int x = j < H ? j + H : j - H;        // fftshift of both axes
-                    __stcs(img + (size_t)y0 * N + x, z.x * inv_w);
-                    __stcs(img + (size_t)y1 * N + x, z.y * inv_w);
+                    if constexpr (R == 0) {
+                        __stcs(img + (size_t)y0 * N + x, z.x * inv_w);
+                        __stcs(img + (size_t)y1 * N + x, z.y * inv_w);
+                    } else {                                    // grid correction 1 / (c(y) c(x)) rides on the same store
+                        const float tx = inv_w * __ldg(cpoly.inv_taper + x);
+                        __stcs(img + (size_t)y0 * N + x, z.x * (tx * __ldg(cpoly.inv_taper + y0)));
+                        __stcs(img + (size_t)y1 * N + x, z.y * (tx * __ldg(cpoly.inv_taper + y1)));
+                    }
                 };
                 auto after_first_reads = [&] {                  // runs right after the first stage's read -> write barrier
                     if (tid == 0 && unit + nbuf * FG_G < NU) request(unit + nbuf * FG_G, b);
@@ -401,18 +472,20 @@ int gfft_fill_twiddles(float2 *dst, int n, cudaStream_t st);      // blink_fftg.
 
 int fused_g_image(const float2 *vis, const float *uvw_m, const double *freqs_hz, double pixscale_rad, int T, int C, int P, int B,
                   int weighting, int tc0, int ntc, float *image, float *wsum, int32_t *cell_idx, void *workspace,
-                  size_t workspace_bytes, cudaStream_t st, GainRef cal)
+                  size_t workspace_bytes, cudaStream_t st, GainRef cal, const ConvPoly *poly, int R, size_t extra)
 {
+    // extra: bytes between the sort arrays and the twiddle table that the caller has filled (the conv taper table), 256-aligned
     const size_t per_cta = (size_t)FG_N * FG_H * sizeof(float2);
     const size_t twb = align_up((size_t)FG_N * sizeof(float2), 256);
-    const size_t sortb = sort_bytes(T, B);
+    const size_t sortb = sort_bytes(T, B) + extra;
+    if (R < 0 || R > 3 || (R > 0 && (!poly || weighting != BLINK_W_NATURAL))) return BLINK_ERR_INVALID_ARG;
     if (!workspace || (reinterpret_cast<uintptr_t>(workspace) & 255u) || workspace_bytes < sortb + twb + per_cta) return BLINK_ERR_WORKSPACE;
     int ctas = option(BLINK_OPT_FUSED_CTAS);
     if (ctas <= 0) ctas = fused_default_ctas();
     ctas = (int)std::min<size_t>((size_t)ctas, (workspace_bytes - sortb - twb) / per_cta);
     unsigned char *wsp = static_cast<unsigned char *>(workspace);
     float *su = reinterpret_cast<float *>(wsp);
-    uint2 *svb = reinterpret_cast<uint2 *>(wsp + sortb / 3);
+    uint2 *svb = reinterpret_cast<uint2 *>(wsp + (sortb - extra) / 3);
     float2 *tw = reinterpret_cast<float2 *>(wsp + sortb);
     float2 *scratch = reinterpret_cast<float2 *>(wsp + sortb + twb);
     int rc = presort_launch(uvw_m, T, B, su, svb, st);
@@ -420,7 +493,12 @@ int fused_g_image(const float2 *vis, const float *uvw_m, const double *freqs_hz,
     rc = gfft_fill_twiddles(tw, FG_N, st);
     if (rc != BLINK_OK) return rc;
     const size_t smem = FgSmem::bytes(B);
-    BLINK_CUDA_TRY(cudaFuncSetAttribute(fused_g_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    BLINK_CUDA_TRY(cudaFuncSetAttribute(fused_g_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    BLINK_CUDA_TRY(cudaFuncSetAttribute(fused_g_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    BLINK_CUDA_TRY(cudaFuncSetAttribute(fused_g_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    BLINK_CUDA_TRY(cudaFuncSetAttribute(fused_g_kernel<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    ConvPoly cpoly{};
+    if (poly) cpoly = *poly;
     FusedArgs base{};
     base.cal = cal;
     base.vis = vis; base.uvw_m = uvw_m; base.T = T; base.C = C; base.P = P; base.B = B; base.weighting = weighting;
@@ -431,7 +509,10 @@ int fused_g_image(const float2 *vis, const float *uvw_m, const double *freqs_hz,
                                   a.tc0 = s0; a.ntc = m; a.c_base = c_base;
                                   a.scratch = scratch; a.su = su; a.svb = svb;
                                   const int grid = m < ctas ? m : ctas;
-                                  fused_g_kernel<<<grid, FG_THREADS, smem, st>>>(a, sc, tw);
+                                  if (R == 0) fused_g_kernel<0><<<grid, FG_THREADS, smem, st>>>(a, sc, tw, cpoly);
+                                  else if (R == 1) fused_g_kernel<1><<<grid, FG_THREADS, smem, st>>>(a, sc, tw, cpoly);
+                                  else if (R == 2) fused_g_kernel<2><<<grid, FG_THREADS, smem, st>>>(a, sc, tw, cpoly);
+                                  else fused_g_kernel<3><<<grid, FG_THREADS, smem, st>>>(a, sc, tw, cpoly);
                                   BLINK_LAUNCH_CHECK("fused_g_kernel");
                                   return (int)BLINK_OK;
                               });

@@ -251,7 +251,7 @@ extern "C" int blink_workspace_bytes(int op, int T, int C, int P, int B, int n_p
             mn = avg_workspace_bytes(T, C, P, B, n_pix, weighting, true);
             break;
         case BLINK_OP_IMAGE_CONV: {
-            if (!is_pow2(n_pix) || !fused_supported(P, B, n_pix, BLINK_W_NATURAL)) {
+            if (!(is_pow2(n_pix) || n_pix == 1200) || !fused_supported(P, B, n_pix, BLINK_W_NATURAL)) {
                 rec = conv_unfused_workspace_bytes(T, C, P, n_pix, false);
                 mn = conv_unfused_workspace_bytes(T, C, P, n_pix, true);
                 break;

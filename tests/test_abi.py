@@ -116,10 +116,15 @@ def test_conv_argument_checks(so_path):
     rec, mn = bk.blink_workspace_bytes(bk.OP_IMAGE_CONV, 50, 768, 1, 8128, 512, 0)
     rec0, mn0 = bk.blink_workspace_bytes(bk.OP_IMAGE, 50, 768, 1, 8128, 512, 0)
     assert rec == rec0 + 2048 and mn == mn0 + 2048                        # + the 512-entry correction table
-    # outside the fused kernel (the paper's 1200, sides below 256): twiddles + correction table + counters + the chunk's grids
+    # the paper's 1200: the fused 1200 kernel's workspace + the 1200-entry correction table
     rec, mn = bk.blink_workspace_bytes(bk.OP_IMAGE_CONV, 2, 300, 1, 100, 1200, 0)
-    fixed = 9728 + 4864 + 2560
-    assert mn == fixed + 1200 * 1200 * 8 and rec == fixed + 256 * 1200 * 1200 * 8
+    rec0, mn0 = bk.blink_workspace_bytes(bk.OP_IMAGE, 2, 300, 1, 100, 1200, 0)
+    assert rec == rec0 + 4864 and mn == mn0 + 4864
+    # outside the fused kernels (sides below 256, other sides that are not a power of two): twiddles + correction table + counters +
+    # the chunk's grids
+    rec, mn = bk.blink_workspace_bytes(bk.OP_IMAGE_CONV, 2, 300, 1, 100, 240, 0)
+    fixed = 2048 + 1024 + 2560
+    assert mn == fixed + 240 * 240 * 8 and rec == fixed + 256 * 240 * 240 * 8
     rec, mn = bk.blink_workspace_bytes(bk.OP_IMAGE_CONV, 1, 1, 2, 100, 128, 0)
     assert rec == mn == 512 + 256 + 2 * 128 * 128 * 8
     with pytest.raises(bk.BlinkError):

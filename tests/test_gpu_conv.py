@@ -222,3 +222,33 @@ def test_conv_config3_full_size_sampled(bk, oracle_mod):
     peak = res["image"].reshape(T * C, -1).abs().amax(dim=1).double().cpu().numpy()
     assert np.max(np.abs(centre - want) / peak) <= TOL
     assert bool(torch.isfinite(res["image"]).all())
+
+
+@pytest.mark.parametrize("S", [3, 5, 7])
+def test_conv_fused_1200_axis_columns_and_collisions(bk, oracle_mod, S):
+    # the fused kernel of the paper's own side with a gridding kernel (R > 0 instantiations of fused_g_kernel): supports that
+    # straddle u = 0 (their taps at u < 0 come back as the conjugate's mirrored taps), samples on the u = 0 column and at DC,
+    # many samples in one cell, supports that touch the range limit exactly, u < 0 (folded), NaN, odd B (no bulk-copy prefetch)
+    from paper_2505_15204_b200 import workloads
+    n = 1200
+    w = workloads.make_random(T=1, C=2, P=2, B=2501, n_pix=n, weighting=0, seed=431 + S, device="cuda", fill=0.5)
+    cell_m = 299792458.0 / 150e6
+    r = S // 2
+    w.uvw_m[0, :400, 0] = 17.2 * cell_m
+    w.uvw_m[0, :400, 1] = -40.3 * cell_m
+    w.uvw_m[0, 400:500, 0] = -17.2 * cell_m                       # the same cells from the other half plane
+    w.uvw_m[0, 400:500, 1] = 40.3 * cell_m
+    w.uvw_m[0, 600:700, 0] = 0.0
+    w.uvw_m[0, 700:760, 0] = 0.0
+    w.uvw_m[0, 700:760, 1] = 0.0
+    for k, x in enumerate([-0.2, 0.3, -0.6, 0.7, 1.4, -1.5, 2.5, -2.6, 3.2, -3.49, 0.5, -0.5]):
+        w.uvw_m[0, 800 + 30 * k:830 + 30 * k, 0] = x * cell_m
+    lim = n // 2 - 1 - r
+    w.uvw_m[0, 1300:1320, 0] = lim * cell_m * 0.99999             # nearest column exactly at the limit (first channel)
+    w.uvw_m[0, 1320:1340, 1] = -lim * cell_m * 0.99999
+    w.uvw_m[0, 1340:1360, 0] = (lim + 0.6) * cell_m               # one cell beyond: dropped
+    w.uvw_m[0, 1400, 0] = float("nan")
+    w.uvw_m[0, 1401, 1] = float("nan")
+    res = bk.blink_image_conv(w.vis, w.uvw_m, w.freqs_hz, n, w.pixscale_rad, S, want_cell_idx=True)
+    torch.cuda.synchronize()
+    _check_conv(w, res, oracle_mod, S)
