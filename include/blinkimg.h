@@ -198,8 +198,8 @@ int blink_image_cal(const blink_c64 *vis, const float *uvw_m, const double *freq
  *   beta      <= 0 selects 2.34 * support; otherwise 1.7 * support <= beta <= 60 (the correction must stay positive
  *             over the whole image), else BLINK_ERR_INVALID_ARG
  *   cell_idx  out OPTIONAL [T][C][B]: the NEAREST cell (iv0+h)*N + (iu0+h) of every baseline, -1 if dropped
- * Runs in the fused kernel for n_pix a power of two in [256, 4096] and B <= 16384; every other supported side (32 .. 8192,
- * prime factors 2, 3, 5: the paper's 1200 and 8192 among them) takes the plain form -- taps scattered into full grids with
+ * Runs in the fused kernels for n_pix a power of two in [256, 4096] (B <= 16384) and for the paper's 1200 (B <= 15000); every
+ * other supported side (32 .. 8192, prime factors 2, 3, 5: 8192 among them) takes the plain form -- taps scattered into full grids with
  * global vector atomics, the unfused transform, one elementwise correction pass -- in chunks that fit the workspace.
  * `workspace` >= blink_workspace_bytes(BLINK_OP_IMAGE_CONV) minimum, 256-byte aligned.  Other arguments as blink_image.
  * The tap weights are evaluated as degree-11 polynomials in the offset, fitted on the host at every call;
