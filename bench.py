@@ -462,7 +462,25 @@ def main():
                      "frac_M4": m4 / (ms_p * 1e-3) / 1e9 / hbm_peak()[0], "model_speedup_M36": m36 / (ms_p * 1e-3) / 1e9 / hbm_peak()[0],
                      "paper_context": "PAPER.md Table 6 (L339-340), gridding + 2D FFT of 38400 images of 1200^2: 1.77 s on an H100 (cuFFT), "
                                       "7.09 s on an MI250X GCD (rocFFT); other machines: context, not a target"}
-            del ws_p, vis_p, uvw_p, img_p
+            # the same images with a Kaiser-Bessel gridding kernel (blink_image_conv inside the fused 1200 kernel)
+            S_p = args.conv_support
+            rec_c, _ = bk.blink_workspace_bytes(bk.OP_IMAGE_CONV, TP, C, P, B, NP, 0)
+            ws_c = torch.empty(max(rec_c, 16), dtype=torch.uint8, device=dev)
+            run_pc = lambda: bk.blink_image_conv(vis_p, uvw_p, w.freqs_hz, NP, 0.6 / NP, S_p, image=img_p, workspace=ws_c, wsum=wsum_p)
+            for _ in range(args.warmup):
+                run_pc()
+            barrier()
+            ec = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+            ec[0].record()
+            for _ in range(args.steps):
+                run_pc()
+            ec[1].record()
+            barrier()
+            ms_pc = torch.tensor([ec[0].elapsed_time(ec[1]) / args.steps], device=dev)
+            if world > 1:
+                dist.all_reduce(ms_pc, op=dist.ReduceOp.MAX)
+            paper["conv"] = {"api": f"blink_image_conv at n_pix = 1200, support {S_p}", "ms_per_run": float(ms_pc.item())}
+            del ws_p, ws_c, vis_p, uvw_p, img_p
         except Exception as ex:  # report, never hide
             paper = {"error": str(ex)[:200]}
 
