@@ -156,9 +156,42 @@ avg_uniform_cols_kernel(const AvgArgs a, const __grid_constant__ ScaleBlock sc, 
         }
         __syncthreads();
         int n_first = 0;
+        // a column holds a handful of samples (10296 baselines over ~700 occupied columns): the common case is ONE sample per lane,
+        // fetched once -- and one column ahead -- and kept in registers through the three steps (count, read back, clear); the first
+        // version re-read svb from L2 in each step and spent 0.18 ms per config-4 timestep waiting for those loads
+        auto fetch = [&](int u_, int &k0_, int &k1_) -> uint2 {
+            k0_ = k1_ = 0;
+            if (u_ < H) { k0_ = (int)coff[u_]; k1_ = (int)coff[u_ + 1]; }
+            return (k0_ + lane < k1_) ? __ldg(svb + k0_ + lane) : make_uint2(0u, 0u);
+        };
+        int k0n, k1n;
+        uint2 sqn = fetch(warp, k0n, k1n);
         for (int u = warp; u < H; u += kAvgColWarps) {
-            const int k0 = (int)coff[u], k1 = (int)coff[u + 1];
+            const int k0 = k0n, k1 = k1n;
+            const uint2 sq0 = sqn;
+            sqn = fetch(u + kAvgColWarps, k0n, k1n);
             if (k0 == k1) continue;
+            if (k1 - k0 <= 32) {
+                int iv = 0;
+                bool ok = false;
+                if (k0 + lane < k1) {
+                    const float yr = rint_rne(__fmul_rn(__uint_as_float(sq0.x), s), iv);
+                    ok = fabsf(yr) <= lim;
+                }
+                if (ok) {
+                    n_first += (atomicAdd(&cw[iv + H], 1u) == 0u) ? (u == 0 ? 1 : 2) : 0;
+                    if (u == 0) n_first += atomicAdd(&cw[H - iv], 1u) == 0u;
+                }
+                __syncwarp();
+                if (k0 + lane < k1) wq[sq0.y & 0x7fffffffu] = ok ? (float)cw[iv + H] : 0.f;
+                __syncwarp();
+                if (ok) {
+                    cw[iv + H] = 0u;
+                    if (u == 0) cw[H - iv] = 0u;
+                }
+                __syncwarp();
+                continue;
+            }
             for (int j = k0 + lane; j < k1; j += 32) {                  // count
                 int iv;
                 const float yr = rint_rne(__fmul_rn(__uint_as_float(__ldg(&svb[j].x)), s), iv);
