@@ -131,6 +131,7 @@ avg_uniform_cols_kernel(const AvgArgs a, const __grid_constant__ ScaleBlock sc, 
 {
     extern __shared__ uint32_t col_sm[];
     __shared__ int s_first[kAvgColWarps];
+    __shared__ int s_ncol;                                              // occupied columns are [0, s_ncol)
     const int n = a.n, H = n / 2, B = a.B;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     uint32_t *coff = col_sm;                                            // [H + 2]: first sorted sample of column u
@@ -153,20 +154,22 @@ avg_uniform_cols_kernel(const AvgArgs a, const __grid_constant__ ScaleBlock sc, 
             const int cj = j < B ? col_of(__ldg(su + j)) : H + 1;
             const int cq = j > 0 ? col_of(__ldg(su + j - 1)) : -1;
             for (int u = cq + 1; u <= cj; ++u) coff[u] = (uint32_t)j;
+            if (cj >= H && cq < H) s_ncol = cq + 1;                     // exactly one j sees the step off the grid
         }
         __syncthreads();
+        const int ncol = s_ncol;
         int n_first = 0;
         // a column holds a handful of samples (10296 baselines over ~700 occupied columns): the common case is ONE sample per lane,
         // fetched once -- and one column ahead -- and kept in registers through the three steps (count, read back, clear); the first
         // version re-read svb from L2 in each step and spent 0.18 ms per config-4 timestep waiting for those loads
         auto fetch = [&](int u_, int &k0_, int &k1_) -> uint2 {
             k0_ = k1_ = 0;
-            if (u_ < H) { k0_ = (int)coff[u_]; k1_ = (int)coff[u_ + 1]; }
+            if (u_ < ncol) { k0_ = (int)coff[u_]; k1_ = (int)coff[u_ + 1]; }
             return (k0_ + lane < k1_) ? __ldg(svb + k0_ + lane) : make_uint2(0u, 0u);
         };
         int k0n, k1n;
         uint2 sqn = fetch(warp, k0n, k1n);
-        for (int u = warp; u < H; u += kAvgColWarps) {
+        for (int u = warp; u < ncol; u += kAvgColWarps) {
             const int k0 = k0n, k1 = k1n;
             const uint2 sq0 = sqn;
             sqn = fetch(u + kAvgColWarps, k0n, k1n);
